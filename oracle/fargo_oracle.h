@@ -1,0 +1,88 @@
+/* fargo_oracle.h -- C interface of the CPU ORACLE.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may load this library.  It is a plain, slow, single
+ * threaded fp64 restatement of one full hydrodynamic update of the FARGO3D method, written from
+ * /root/reference/PAPER.md ("P:n" = line n of that file) with the readings listed in DESIGN.md.
+ * It shares no code with the CUDA path (paper_1602_02359_b200/csrc) and neither includes the other.
+ *
+ * Layout of every field passed through this interface: nz*ny*nx doubles, X (i) fastest, ACTIVE
+ * cells only; velocities on the LOWER face of the cell in their own direction.
+ */
+#ifndef FARGO_ORACLE_H
+#define FARGO_ORACLE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORC_CARTESIAN = 0, ORC_CYLINDRICAL = 1, ORC_SPHERICAL = 2 };  /* Tab. 1 */
+enum { ORC_ISOTHERMAL = 0, ORC_ADIABATIC = 1 };                      /* Eqs. 6, 7 */
+enum { ORC_PERIODIC = 0, ORC_OUTFLOW = 1, ORC_REFLECTING = 2 };
+
+/* stages of one full update, in the order of Fig. 2 (caption P:198); see oracle_step_until */
+enum {
+  ORC_ST_BC1 = 0, ORC_ST_VMEAN, ORC_ST_POT, ORC_ST_DT, ORC_ST_SRC_A, ORC_ST_SRC_B, ORC_ST_SRC_C,
+  ORC_ST_SRC_D, ORC_ST_BC2, ORC_ST_MOM, ORC_ST_SWEEP_X, ORC_ST_SWEEP_Y, ORC_ST_SWEEP_Z,
+  ORC_ST_ORB_FRAC, ORC_ST_ORB_SHIFT, ORC_ST_NEWVEL, ORC_ST_COUNT
+};
+
+typedef struct oracle_mesh {
+  int nx, ny, nz;            /* active cells; 1 = direction absent */
+  double xmin, xmax;         /* uniform in X */
+  const double* yedges;      /* ny+1 active edges, or NULL: uniform ymin + j*(ymax-ymin)/ny */
+  const double* zedges;      /* nz+1 active edges, or NULL */
+  double ymin, ymax, zmin, zmax;
+  int bc[3][2];              /* [direction][lower, upper] */
+  int nghost;                /* ghost layers, 3; 4 is accepted for the ghost-budget test */
+} oracle_mesh;
+
+typedef struct oracle_params {
+  double gamma, cfl, cvnr2, nu;
+  int fargo_on;
+  double omega_frame, gm_star, planet_mass, planet_r, planet_phi0, planet_omega, planet_eps;
+  double shear_c0, t_stop, dt_fixed;
+} oracle_params;
+
+typedef struct oracle_ctx oracle_ctx;
+
+int oracle_init(oracle_ctx** out, const oracle_mesh* mesh, int geometry, int eos, const oracle_params* p);
+int oracle_destroy(oracle_ctx* c);
+int oracle_set_fields(oracle_ctx* c, const double* rho, const double* e, const double* vx,
+                      const double* vy, const double* vz);
+int oracle_get_fields(oracle_ctx* c, double* rho, double* e, double* vx, double* vy, double* vz);
+int oracle_step(oracle_ctx* c, int n);
+int oracle_get_time(oracle_ctx* c, double* t, double* last_dt, long long* nsteps);
+
+/* Run the NEXT update only up to and including `stage`, leaving intermediates in place.  The state
+ * is then mid-step: inspect with oracle_get_array, do not call oracle_step afterwards. */
+int oracle_step_until(oracle_ctx* c, int stage);
+/* Run ONE stage on the arrays as they stand, with the current dt (oracle_set_dt overrides it). */
+int oracle_run_stage(oracle_ctx* c, int stage);
+int oracle_set_dt(oracle_ctx* c, double dt);
+/* Copy a named internal array INCLUDING ghosts (TX*TY*TZ doubles, or TY*TZ for "v0"/"nshift").
+ * names: rho e vx vy vz phi vxb vyb vzb vxc vyc vzc ec ed vxd vyd pxm pxp pym pyp pzm pzp v0 nshift */
+int oracle_get_array(oracle_ctx* c, const char* name, double* out);
+int oracle_set_array(oracle_ctx* c, const char* name, const double* in);
+int oracle_dims(oracle_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz);
+/* Geometry tables (Tab. 5): surfaces of the lower faces and inverse volume of cell (j,k),
+ * ghost-inclusive indices. */
+int oracle_geometry(oracle_ctx* c, int j, int k, double* sx, double* sy, double* sz, double* invv,
+                    double* lx, double* ly, double* lz);
+
+/* 1-D primitives used by the sweeps, exposed so that tests can pin them to the paper's formulas. */
+/* van Leer slopes a[m], m = 1..n-2, from cell values f and inverse centre distances
+ * invd[m] = 1/(c_m - c_{m-1}); a[0] = a[n-1] = 0. */
+void oracle_vanleer_slopes(int n, const double* f, const double* invd, double* a);
+/* Upwind star value on the lower face of cell m, m = 1..n-1 (Eq. 48). */
+void oracle_vanleer_star(int n, const double* f, const double* a, const double* len, const double* w,
+                         double dt, double* fstar);
+/* PPA star values on face i+1/2 of a periodic ring for a uniform shift of xi cells. */
+void oracle_ppa_star(int n, const double* f, double xi, double* fstar);
+/* PPA monotonised interface values fL, fR of a periodic ring (Eq. 71 + tests at P:484). */
+void oracle_ppa_interfaces(int n, const double* f, double* fl, double* fr);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

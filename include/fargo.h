@@ -1,0 +1,135 @@
+/* fargo.h -- C ABI of the B200-native FARGO3D hydrodynamic timestep library (libfargo_b200.so).
+ *
+ * One full hydrodynamic update of the method of Benitez-Llambay & Masset, "FARGO3D: a new GPU-oriented
+ * MHD code" (arXiv 1602.02359; "P:n" = line n of PAPER.md) on a structured staggered mesh, executed by
+ * hand-written CUDA kernels for sm_100a.  One update is the sequence of Fig. 2 (caption P:198):
+ *   ghost fill (cell 2) -> ring mean velocity (cell 3, Eq. 72) -> potential (cell 5)
+ *   -> CFL time step (cell 6, Eq. 59; shear limit Eq. 73)
+ *   -> source sub-steps 7a pressure/potential/centrifugal (Eqs. 27, 32-38, 53 P:245-280),
+ *      7b von Neumann-Richtmyer viscosity, 7c compression work,
+ *      7d viscous stress, 2-D cylindrical (App. B, Eqs. B2, B5 P:1160-1202)
+ *   -> ghost fill (cell 9) -> momenta (12a, Eqs. 49-50)
+ *   -> van Leer upwind sweeps X, Y, Z with consistent transport (12b-c, Eqs. 40-48)
+ *   -> orbital advection: PPA fractional sweep + integer ring shift (Eqs. 60-71)
+ *   -> new velocities (12d, Eq. 51).
+ * The readings taken where the paper is silent or garbled are listed in DESIGN.md.
+ *
+ * There is NO CPU fallback: every call that needs the device fails with FARGO_ECUDA when no CUDA
+ * device is usable.  Nothing throws across this boundary.  No global state: contexts are independent.
+ *
+ * FIELD LAYOUT for set/get: nz*ny*nx elements, X (index i) fastest, ACTIVE cells only, element type =
+ * the context's precision (double for 64, float for 32).  vx[i,j,k] is v_X on the LOWER X face of cell
+ * (i,j,k), vy on the lower Y face, vz on the lower Z face.  `e` is the internal energy
+ * density (adiabatic, Eq. 7) or the sound-speed field c_s (isothermal, Eq. 6).
+ * Directions are X,Y,Z = (x,y,z) | (phi,r,z) | (phi,r,theta) (Tab. 1).
+ *
+ * POINTERS: field pointers given to fargo_set_fields / fargo_get_fields may be HOST or DEVICE pointers
+ * (resolved with cudaPointerGetAttributes).  mesh/params structs and table pointers inside them are
+ * HOST memory, read during the call only.  `workspace` is DEVICE memory owned by the caller and must
+ * stay alive, untouched, until fargo_destroy.  `cuda_stream` is a cudaStream_t (NULL = legacy default).
+ */
+#ifndef FARGO_B200_H
+#define FARGO_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { FARGO_CARTESIAN = 0, FARGO_CYLINDRICAL = 1, FARGO_SPHERICAL = 2 }; /* Tab. 1 */
+enum { FARGO_ISOTHERMAL = 0, FARGO_ADIABATIC = 1 };                       /* Eqs. 6-7 */
+enum { FARGO_PERIODIC = 0, FARGO_OUTFLOW = 1, FARGO_REFLECTING = 2 };
+
+enum { FARGO_OK = 0, FARGO_EINVAL = -1, FARGO_ENOMEM = -2, FARGO_ECUDA = -3, FARGO_ESTATE = -4 };
+
+/* Stages of one update, for fargo_step_until (per-kernel parity checks).  A fused kernel is observable
+ * at the last stage it contains. */
+enum {
+  FARGO_ST_BC1 = 0, FARGO_ST_VMEAN, FARGO_ST_POT, FARGO_ST_DT, FARGO_ST_SRC_A, FARGO_ST_SRC_B,
+  FARGO_ST_SRC_C, FARGO_ST_SRC_D, FARGO_ST_BC2, FARGO_ST_MOM, FARGO_ST_SWEEP_X, FARGO_ST_SWEEP_Y,
+  FARGO_ST_SWEEP_Z, FARGO_ST_ORB_FRAC, FARGO_ST_ORB_SHIFT, FARGO_ST_NEWVEL, FARGO_ST_COUNT
+};
+
+typedef struct fargo_mesh {
+  int nx, ny, nz;          /* active cells per direction; 1 = direction absent */
+  double xmin, xmax;       /* X is uniform */
+  const double* yedges;    /* HOST, ny+1 active cell edges, or NULL: uniform ymin + j*(ymax-ymin)/ny */
+  const double* zedges;    /* HOST, nz+1 active cell edges, or NULL */
+  double ymin, ymax, zmin, zmax;
+  int bc[3][2];            /* [direction][lower, upper]; X periodic => ghost-free wrapped X,
+                              X non-periodic => 3 ghost layers in X too (reading G20) */
+} fargo_mesh;
+
+typedef struct fargo_params {
+  double gamma;            /* adiabatic index (Eq. 7) */
+  double cfl;              /* Courant number C of Eq. 59 (0.44) */
+  double cvnr2;            /* C_q^2 of the artificial viscosity (reading G8; 2) */
+  double nu;               /* constant kinematic viscosity, 0 = off (App. B) */
+  int fargo_on;            /* orbital advection (section 3.5.1); needs periodic X */
+  double omega_frame;      /* Omega_f (ignored in Cartesian geometry) */
+  double gm_star;          /* G M of the central star (0 = none) */
+  double planet_mass;      /* G m_p of the planet on a fixed circular orbit in the midplane (0 = none) */
+  double planet_r, planet_phi0, planet_omega, planet_eps;   /* orbit radius, azimuth at t=0, angular
+                              speed in the inertial frame, Plummer smoothing length (reading G12) */
+  double shear_c0;         /* C_0 of Eq. 73 (0.5; reading G10) */
+  double t_stop;           /* > 0: the step that would pass t_stop is clipped to land on it and later
+                              steps are no-ops (reading G21); <= 0: none */
+  double dt_fixed;         /* > 0: overrides the CFL time step */
+  int precision;           /* 64 (double) or 32 (float) */
+  int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (default path);
+                              0: plain stream launches */
+  void* workspace;         /* DEVICE memory, >= fargo_workspace_bytes(), 256-byte aligned; caller-owned */
+  size_t workspace_bytes;
+  void* cuda_stream;       /* cudaStream_t on which every kernel and copy of this context is enqueued */
+} fargo_params;
+
+typedef struct fargo_ctx fargo_ctx;
+
+/* Bytes of device workspace a context for (mesh, geometry, eos, params) needs.  0 on invalid input.
+ * Does not touch the device. */
+size_t fargo_workspace_bytes(const fargo_mesh* mesh, int geometry, int eos, const fargo_params* p);
+
+/* Validate, build the Tab. 5 geometric coefficient tables and the trigonometric tables
+ * on the host, upload them, carve the workspace.  On failure *out = NULL and a negative code is
+ * returned; fargo_last_error(NULL) then describes the most recent init failure of this thread. */
+int fargo_init(fargo_ctx** out, const fargo_mesh* mesh, int geometry, int eos, const fargo_params* p);
+int fargo_destroy(fargo_ctx* c);
+
+/* Load the five fields (layout above).  vy / vz may be NULL when that direction is absent.
+ * Resets t = 0 and the step count.  Host pointers are copied through the context's stream. */
+int fargo_set_fields(fargo_ctx* c, const void* rho, const void* e, const void* vx, const void* vy,
+                     const void* vz);
+/* Synchronise the stream and copy the active cells out (any pointer may be NULL = skip).  No
+ * boundary fill is applied first. */
+int fargo_get_fields(fargo_ctx* c, void* rho, void* e, void* vx, void* vy, void* vz);
+
+/* Enqueue n full updates on the stream.  No host synchronisation inside (except when the planet
+ * moves in the frame, planet_omega != omega_frame, where the host needs t once per update). */
+int fargo_step(fargo_ctx* c, int n);
+
+/* Synchronise and read the clock: simulated time, last time step, number of updates done. */
+int fargo_get_time(fargo_ctx* c, double* t, double* last_dt, long long* nsteps);
+
+/* Number of kernels launched (or replayed through graphs) by this context since fargo_init. */
+long long fargo_kernel_launches(const fargo_ctx* c);
+
+/* ---- inspection, for per-stage parity tests ---------------------------------------------------- */
+/* Run the NEXT update up to and including `stage`; the state is then mid-step (only
+ * fargo_get_array / fargo_dims / fargo_destroy / fargo_set_fields are valid afterwards). */
+int fargo_step_until(fargo_ctx* c, int stage);
+/* Ghost-inclusive extents and ghost counts of the device arrays. */
+int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz);
+/* Copy a named ghost-inclusive array (TZ*TY*TX elements of the context's precision, X fastest,
+ * unpadded; TZ*TY for "v0") to HOST memory.  Names: rho e vx vy vz phi vxb vyb vzb vxc vyc vzc ec ed
+ * vxd vyd pxm pxp pym pyp pzm pzp trho te v0.  pxm..pzp, trho, te refer to the transported set written
+ * by the most recent transport pass.  Which names hold defined data depends on the stage reached. */
+int fargo_get_array(fargo_ctx* c, const char* name, void* out);
+
+/* Message for the last error of `c` (or of the last failed fargo_init on this thread when c == NULL). */
+const char* fargo_last_error(const fargo_ctx* c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,212 @@
+"""ctypes binding of libfargo_b200.so (include/fargo.h): argument marshalling only.
+
+Every step of the hydrodynamic update runs in the CUDA kernels of csrc/; this module allocates the
+device workspace as one torch.uint8 tensor, hands over the current torch CUDA stream, and converts
+numpy / torch arrays to pointers.  There is no CPU fallback: without the built library or without a
+CUDA device, construction raises.  Nothing here imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+_DP = C.POINTER(C.c_double)
+STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2", "MOM",
+          "SWEEP_X", "SWEEP_Y", "SWEEP_Z", "ORB_FRAC", "ORB_SHIFT", "NEWVEL"]
+EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
+           "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
+           "fargo_get_array", "fargo_last_error"]
+
+
+class FargoMesh(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("xmin", C.c_double), ("xmax", C.c_double),
+                ("yedges", _DP), ("zedges", _DP),
+                ("ymin", C.c_double), ("ymax", C.c_double), ("zmin", C.c_double), ("zmax", C.c_double),
+                ("bc", (C.c_int * 2) * 3)]
+
+
+class FargoParams(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("cfl", C.c_double), ("cvnr2", C.c_double), ("nu", C.c_double),
+                ("fargo_on", C.c_int),
+                ("omega_frame", C.c_double), ("gm_star", C.c_double), ("planet_mass", C.c_double),
+                ("planet_r", C.c_double), ("planet_phi0", C.c_double), ("planet_omega", C.c_double),
+                ("planet_eps", C.c_double),
+                ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double),
+                ("precision", C.c_int), ("use_graph", C.c_int),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load():
+    """Load (building first if the sources are newer) the C-ABI library and declare its signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp = C.c_void_p
+    L.fargo_workspace_bytes.argtypes = [C.POINTER(FargoMesh), C.c_int, C.c_int, C.POINTER(FargoParams)]
+    L.fargo_workspace_bytes.restype = C.c_size_t
+    L.fargo_init.argtypes = [C.POINTER(vp), C.POINTER(FargoMesh), C.c_int, C.c_int, C.POINTER(FargoParams)]
+    L.fargo_destroy.argtypes = [vp]
+    L.fargo_set_fields.argtypes = [vp] + [vp] * 5
+    L.fargo_get_fields.argtypes = [vp] + [vp] * 5
+    L.fargo_step.argtypes = [vp, C.c_int]
+    L.fargo_get_time.argtypes = [vp, _DP, _DP, C.POINTER(C.c_longlong)]
+    L.fargo_kernel_launches.argtypes = [vp]
+    L.fargo_kernel_launches.restype = C.c_longlong
+    L.fargo_step_until.argtypes = [vp, C.c_int]
+    L.fargo_dims.argtypes = [vp] + [C.POINTER(C.c_int)] * 6
+    L.fargo_get_array.argtypes = [vp, C.c_char_p, vp]
+    L.fargo_last_error.argtypes = [vp]
+    L.fargo_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _ptr(a) -> Optional[int]:
+    """Raw address of a numpy array (host) or a torch tensor (host or device); None passes through."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return a.data_ptr()
+
+
+class Fargo:
+    """One simulation context on the current CUDA device.
+
+    `mesh` / `params` are the plain dataclasses of workloads.py (any objects with the same attributes).
+    """
+
+    def __init__(self, mesh, geometry: int, eos: int, params, precision: int = 64, use_graph: bool = True,
+                 device: Optional[str] = None):
+        import torch
+        L = load()
+        if not torch.cuda.is_available():
+            raise RuntimeError("fargo_b200 needs a CUDA device (there is no CPU fallback)")
+        self._torch = torch
+        self.device = torch.device(device or "cuda:%d" % torch.cuda.current_device())
+        self.dtype = np.float64 if precision == 64 else np.float32
+        self.tdtype = torch.float64 if precision == 64 else torch.float32
+        self._ye = np.ascontiguousarray(mesh.yedges, dtype=np.float64)
+        self._ze = np.ascontiguousarray(mesh.zedges, dtype=np.float64)
+        m = FargoMesh()
+        m.nx, m.ny, m.nz = mesh.nx, mesh.ny, mesh.nz
+        m.xmin, m.xmax = mesh.xmin, mesh.xmax
+        m.yedges = self._ye.ctypes.data_as(_DP)
+        m.zedges = self._ze.ctypes.data_as(_DP)
+        m.ymin, m.ymax = float(self._ye[0]), float(self._ye[-1])
+        m.zmin, m.zmax = float(self._ze[0]), float(self._ze[-1])
+        for d in range(3):
+            for s in range(2):
+                m.bc[d][s] = mesh.bc[d][s]
+        p = FargoParams()
+        for name in ("gamma", "cfl", "cvnr2", "nu", "fargo_on", "omega_frame", "gm_star", "planet_mass", "planet_r",
+                     "planet_phi0", "planet_omega", "planet_eps", "shear_c0", "t_stop", "dt_fixed"):
+            setattr(p, name, getattr(params, name))
+        p.precision = precision
+        p.use_graph = 1 if use_graph else 0
+        nbytes = L.fargo_workspace_bytes(C.byref(m), geometry, eos, C.byref(p))
+        if nbytes == 0:
+            raise ValueError("fargo_workspace_bytes rejected the mesh / parameters")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            off = (-base) % 256
+            self.stream = torch.cuda.current_stream(self.device)
+            p.workspace = base + off
+            p.workspace_bytes = nbytes
+            p.cuda_stream = self.stream.cuda_stream
+            self._h = C.c_void_p()
+            rc = L.fargo_init(C.byref(self._h), C.byref(m), geometry, eos, C.byref(p))
+        if rc != 0:
+            raise RuntimeError("fargo_init failed (%d): %s" % (rc, L.fargo_last_error(None).decode()))
+        self.shape = (mesh.nz, mesh.ny, mesh.nx)
+        self.ncells = mesh.nx * mesh.ny * mesh.nz
+        self.hasy, self.hasz = mesh.ny > 1, mesh.nz > 1
+        d = [C.c_int() for _ in range(6)]
+        L.fargo_dims(self._h, *[C.byref(x) for x in d])
+        self.TX, self.TY, self.TZ, self.ngx, self.ngy, self.ngz = [x.value for x in d]
+
+    # -- lifetime ------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            load().fargo_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise RuntimeError("%s failed (%d): %s" % (what, rc, load().fargo_last_error(self._h).decode()))
+
+    # -- the four calls of the north star ---------------------------------------------------------
+    def set_fields(self, rho, e, vx, vy=None, vz=None):
+        """Host numpy arrays or torch tensors (host or device) of the context's precision, shape (nz, ny, nx)."""
+        arrs = []
+        for a in (rho, e, vx, vy, vz):
+            if isinstance(a, np.ndarray):
+                a = np.ascontiguousarray(a, dtype=self.dtype)
+            elif a is not None:
+                a = a.to(self.tdtype).contiguous()
+            if a is not None:
+                n = a.size if isinstance(a, np.ndarray) else a.numel()
+                assert n == self.ncells, "field size does not match the mesh"
+            arrs.append(a)
+        self._keep = arrs
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_set_fields(self._h, *[_ptr(a) for a in arrs]), "fargo_set_fields")
+
+    def step(self, n: int = 1):
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_step(self._h, int(n)), "fargo_step")
+
+    def get_fields(self, out=None):
+        """Returns (rho, e, vx, vy, vz) as host numpy arrays, or fills `out` (5 arrays / tensors / None)."""
+        if out is None:
+            out = [np.empty(self.shape, dtype=self.dtype) for _ in range(5)]
+            if not self.hasy:
+                out[3][...] = 0
+            if not self.hasz:
+                out[4][...] = 0
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_get_fields(self._h, *[_ptr(a) for a in out]), "fargo_get_fields")
+        return tuple(out)
+
+    def time(self):
+        t, dt, n = C.c_double(), C.c_double(), C.c_longlong()
+        self._check(load().fargo_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n)), "fargo_get_time")
+        return t.value, dt.value, n.value
+
+    def kernel_launches(self) -> int:
+        return int(load().fargo_kernel_launches(self._h))
+
+    # -- inspection ----------------------------------------------------------------------------------
+    def step_until(self, stage: str):
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_step_until(self._h, STAGES.index(stage)), "fargo_step_until")
+
+    def array(self, name: str) -> np.ndarray:
+        ring = name in ("v0", "nshift")
+        out = np.empty((self.TZ, self.TY) if ring else (self.TZ, self.TY, self.TX), dtype=self.dtype)
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_get_array(self._h, name.encode(), out.ctypes.data), "fargo_get_array")
+        return out

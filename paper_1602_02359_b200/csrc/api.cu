@@ -1,0 +1,518 @@
+// api.cu -- the C ABI of include/fargo.h: context, workspace carving, field I/O and the step scheduler
+// that enqueues the fixed kernel sequence of one update (Fig. 2, caption P:198) on one CUDA stream,
+// with the time step and the clock resident on the device.  With use_graph the sequence of one update
+// is captured once into a CUDA graph and replayed (small meshes are launch-bound).
+// Product code: nothing here includes, links or calls anything under oracle/.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/fargo.h"
+#include "kernels.h"
+#include "tables.h"
+
+namespace fg {
+
+template <typename T> void sweep_setup();   // k_transport.cu: opt-in shared memory sizes
+
+static thread_local std::string g_init_error;
+
+struct CtxBase {
+  virtual ~CtxBase() {}
+  std::string err;
+  int precision = 64;
+  virtual int set_fields(const void*, const void*, const void*, const void*, const void*) = 0;
+  virtual int get_fields(void*, void*, void*, void*, void*) = 0;
+  virtual int step(int n) = 0;
+  virtual int step_until(int stage) = 0;
+  virtual int get_time(double*, double*, long long*) = 0;
+  virtual int get_array(const char*, void*) = 0;
+  virtual void dims(int*, int*, int*, int*, int*, int*) const = 0;
+  long long launches = 0;
+};
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {   // sizes shared by fargo_workspace_bytes and fargo_init
+  int nx, ny, nz, ngx, ngy, ngz, TX, TY, TZ;
+  long long pitch, plane, narr;
+  bool xwrap, hasx, hasy, hasz, has_pot, visc, fargo, adi;
+  int n3d;             // number of 3-D arrays
+  size_t table_elems;  // total 1-D table elements (each table padded to 32 elements)
+  size_t bytes(size_t es) const {
+    size_t b = 256;                                              // Ctl
+    b += align_up(table_elems * es, 256);                        // tables
+    b += 2 * align_up((size_t)TY * TZ * es, 256);                // v0, nshift
+    b += (size_t)n3d * align_up((size_t)narr * es, 256);
+    return b;
+  }
+};
+
+static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, const fargo_params* p, std::string& err) {
+  if (!m || !p) { err = "null mesh or params"; return false; }
+  if (m->nx < 1 || m->ny < 1 || m->nz < 1) { err = "mesh extents must be >= 1"; return false; }
+  if (geometry < 0 || geometry > 2) { err = "unknown geometry"; return false; }
+  if (eos < 0 || eos > 1) { err = "unknown equation of state"; return false; }
+  if (p->precision != 64 && p->precision != 32) { err = "precision must be 64 or 32"; return false; }
+  for (int dd = 0; dd < 3; ++dd)
+    for (int s = 0; s < 2; ++s)
+      if (m->bc[dd][s] < 0 || m->bc[dd][s] > 2) { err = "unknown boundary kind"; return false; }
+  if (!(m->xmax > m->xmin)) { err = "xmax must exceed xmin"; return false; }
+  L.nx = m->nx; L.ny = m->ny; L.nz = m->nz;
+  L.hasx = m->nx > 1; L.hasy = m->ny > 1; L.hasz = m->nz > 1;
+  if (!L.hasx && !L.hasy && !L.hasz) { err = "at least one direction must have more than one cell"; return false; }
+  L.xwrap = m->bc[0][0] == FARGO_PERIODIC;
+  if (p->fargo_on && !(L.xwrap && L.hasx)) { err = "orbital advection needs a periodic X axis (P:728)"; return false; }
+  const int ng = 3;
+  L.ngx = (L.hasx && !L.xwrap) ? ng : 0;
+  L.ngy = L.hasy ? ng : 0;
+  L.ngz = L.hasz ? ng : 0;
+  L.TX = L.nx + 2 * L.ngx; L.TY = L.ny + 2 * L.ngy; L.TZ = L.nz + 2 * L.ngz;
+  L.pitch = (long long)align_up((size_t)L.TX, 16);
+  L.plane = L.pitch * L.TY;
+  L.narr = L.plane * L.TZ;
+  L.has_pot = geometry != FARGO_CARTESIAN && (p->gm_star != 0.0 || p->planet_mass != 0.0);
+  L.visc = p->nu > 0.0 && geometry == FARGO_CYLINDRICAL && L.hasx && L.hasy && !L.hasz && L.xwrap;
+  L.fargo = p->fargo_on != 0;
+  L.adi = eos == FARGO_ADIABATIC;
+  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16;
+  const size_t pad = 32;
+  auto t1 = [&](int n) { return align_up((size_t)n, pad); };
+  L.table_elems = 7 * t1(L.TY + 1) + 10 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 4 * t1(L.TZ + 1) + 2 * t1(L.TX);
+  return true;
+}
+
+template <typename T>
+struct Sim : CtxBase {
+  Layout L;
+  Dev<T> d;
+  State<T> st;
+  T *phi = nullptr, *v0 = nullptr, *nshift = nullptr;
+  T* pool[16];
+  Ctl* ctl = nullptr;
+  fargo_params prm;
+  int geometry, eos;
+  cudaStream_t stream = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  int launches_per_step = 0;
+  bool midstep = false, have_fields = false, pot_static = true, pot_valid = false;
+  std::map<std::string, T*> dbg;
+  // transport plan
+  int npass = 0, pass_kind[4];   // 0,1,2 = sweep direction, 3 = orbital
+  int nq = 0, slots[8];
+
+  ~Sim() override { if (gexec) cudaGraphExecDestroy(gexec); }
+
+  bool ck(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    char buf[256];
+    snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    err = buf;
+    return false;
+  }
+
+  T* set_arr(int s, int slot /* -1 = rho, 0 = e, 1..6 momenta */) { return pool[s * 8 + 1 + slot]; }
+
+  int init(const fargo_mesh* m, int geo, int eos_, const fargo_params* p) {
+    geometry = geo; eos = eos_; prm = *p;
+    stream = (cudaStream_t)p->cuda_stream;
+    int ndev = 0;
+    if (!ck(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev < 1) {
+      if (err.empty()) err = "no CUDA device";
+      return FARGO_ECUDA;
+    }
+    const size_t need = L.bytes(sizeof(T));
+    if (!p->workspace || p->workspace_bytes < need) { err = "workspace missing or too small"; return FARGO_ENOMEM; }
+    if (((uintptr_t)p->workspace) % 256) { err = "workspace must be 256-byte aligned"; return FARGO_EINVAL; }
+    cudaPointerAttributes at;
+    if (!ck(cudaPointerGetAttributes(&at, p->workspace), "cudaPointerGetAttributes(workspace)")) return FARGO_ECUDA;
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) {
+      err = "workspace is not device memory";
+      return FARGO_EINVAL;
+    }
+
+    // ---- host tables (fp64, libm) ----
+    const double dx = (m->xmax - m->xmin) / (double)m->nx;
+    std::vector<double> ye = ghosted_edges(m->yedges, L.ny, L.ngy, m->ymin, m->ymax);
+    std::vector<double> ze = ghosted_edges(m->zedges, L.nz, L.ngz, m->zmin, m->zmax);
+    for (size_t n = 1; n < ye.size(); ++n) if (!(ye[n] > ye[n - 1])) { err = "yedges must increase"; return FARGO_EINVAL; }
+    for (size_t n = 1; n < ze.size(); ++n) if (!(ze[n] > ze[n - 1])) { err = "zedges must increase"; return FARGO_EINVAL; }
+    HostTables ht;
+    build_tables(ht, geo, L.TX, L.TY, L.TZ, L.ngx, m->xmin, dx, ye, ze);
+
+    // ---- carve the workspace ----
+    unsigned char* base = (unsigned char*)p->workspace;
+    size_t off = 0;
+    ctl = (Ctl*)base; off += 256;
+    T* tab = (T*)(base + off);
+    std::vector<T> htab(L.table_elems, T(0));
+    size_t tpos = 0;
+    auto put = [&](const std::vector<double>& v) -> const T* {
+      const T* dev = tab + tpos;
+      for (size_t n = 0; n < v.size(); ++n) htab[tpos + n] = (T)v[n];
+      tpos += align_up(v.size(), 32);
+      return dev;
+    };
+    memset(&d, 0, sizeof d);
+    d.ye = put(ht.ye); d.yc = put(ht.yc); d.inv_ye = put(ht.inv_ye); d.inv_yc = put(ht.inv_yc);
+    d.LY = put(ht.LY); d.invLY = put(ht.invLY); d.invDY = put(ht.invDY);
+    d.sxj = put(ht.sxj); d.syj = put(ht.syj); d.szj = put(ht.szj); d.invVj = put(ht.invVj);
+    d.Rxj = put(ht.Rxj); d.invRxj = put(ht.invRxj); d.LXj = put(ht.LXj); d.invLXj = put(ht.invLXj);
+    d.Rzj = put(ht.Rzj); d.invRzj = put(ht.invRzj);
+    d.zc = put(ht.zc); d.dz = put(ht.dz); d.invdz = put(ht.invdz); d.invdzc = put(ht.invdzc);
+    d.sxk = put(ht.sxk); d.syk = put(ht.syk); d.inv_syk = put(ht.inv_syk); d.szk = put(ht.szk);
+    d.Rxk = put(ht.Rxk); d.invRxk = put(ht.invRxk);
+    d.sin_zc = put(ht.sin_zc); d.cos_zc = put(ht.cos_zc); d.sin_ze = put(ht.sin_ze); d.cot_ze = put(ht.cot_ze);
+    d.cos_xc = put(ht.cos_xc); d.sin_xc = put(ht.sin_xc);
+    if (tpos > L.table_elems) { err = "internal: table area overflow"; return FARGO_EINVAL; }
+    off += align_up(L.table_elems * sizeof(T), 256);
+    const size_t ringb = align_up((size_t)L.TY * L.TZ * sizeof(T), 256);
+    v0 = (T*)(base + off); off += ringb;
+    nshift = (T*)(base + off); off += ringb;
+    const size_t arrb = align_up((size_t)L.narr * sizeof(T), 256);
+    auto arr = [&]() { T* a = (T*)(base + off); off += arrb; return a; };
+    st.rho = arr(); st.e = arr(); st.vx = arr(); st.vy = arr(); st.vz = arr();
+    if (L.has_pot) phi = arr();
+    for (int n = 0; n < 16; ++n) pool[n] = arr();
+    if (off > p->workspace_bytes) { err = "internal: workspace overflow"; return FARGO_ENOMEM; }
+
+    if (!ck(cudaMemsetAsync(base, 0, off, stream), "cudaMemsetAsync(workspace)")) return FARGO_ECUDA;
+    if (!ck(cudaMemcpyAsync(tab, htab.data(), L.table_elems * sizeof(T), cudaMemcpyHostToDevice, stream),
+            "upload tables")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "init sync")) return FARGO_ECUDA;
+
+    // ---- device descriptor ----
+    d.nx = L.nx; d.ny = L.ny; d.nz = L.nz; d.ngx = L.ngx; d.ngy = L.ngy; d.ngz = L.ngz;
+    d.TX = L.TX; d.TY = L.TY; d.TZ = L.TZ; d.pitch = L.pitch; d.plane = L.plane; d.narr = L.narr;
+    d.geometry = geo; d.eos = eos_;
+    d.xwrap = L.xwrap; d.hasx = L.hasx; d.hasy = L.hasy; d.hasz = L.hasz;
+    d.fargo = L.fargo; d.has_pot = L.has_pot; d.visc = L.visc;
+    for (int a = 0; a < 3; ++a) for (int s = 0; s < 2; ++s) d.bc[a][s] = m->bc[a][s];
+    d.dx = (T)dx; d.invdx = (T)(1.0 / dx);
+    d.gamma = (T)p->gamma; d.gm1 = (T)(p->gamma - 1.0); d.gg1 = (T)(p->gamma * (p->gamma - 1.0));
+    d.cfl = (T)p->cfl; d.cvnr2 = (T)p->cvnr2; d.nu = (T)p->nu;
+    d.omega = (T)p->omega_frame; d.om_eff = geo == FARGO_CARTESIAN ? T(0) : (T)p->omega_frame;
+    d.shear_c0 = (T)p->shear_c0;
+    d.c3 = (T)(4.0 * p->cvnr2); d.c4 = (T)(4.0 * p->nu);
+    d.t_stop = p->t_stop; d.dt_fixed = p->dt_fixed;
+    d.ctl = ctl;
+    pot_static = !(L.has_pot && p->planet_mass != 0.0 && p->planet_omega != p->omega_frame);
+
+    // ---- transport plan: X, Y, Z sweeps (reading G14), then orbital advection ----
+    npass = 0;
+    if (L.hasx) pass_kind[npass++] = 0;
+    if (L.hasy) pass_kind[npass++] = 1;
+    if (L.hasz) pass_kind[npass++] = 2;
+    if (L.fargo) pass_kind[npass++] = 3;
+    nq = 0;
+    if (L.adi) slots[nq++] = 0;
+    if (L.hasx) { slots[nq++] = 1; slots[nq++] = 2; }
+    if (L.hasy) { slots[nq++] = 3; slots[nq++] = 4; }
+    if (L.hasz) { slots[nq++] = 5; slots[nq++] = 6; }
+    sweep_setup<T>();
+    return FARGO_OK;
+  }
+
+  // ---- field I/O --------------------------------------------------------------------------------------
+  static bool on_device(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+  }
+
+  int set_fields(const void* rho, const void* e, const void* vx, const void* vy, const void* vz) override {
+    if (!rho || !e || !vx) { err = "rho, e and vx are required"; return FARGO_EINVAL; }
+    if ((L.hasy && !vy) || (L.hasz && !vz)) { err = "vy / vz required when that direction is present"; return FARGO_EINVAL; }
+    const size_t nact = (size_t)L.nx * L.ny * L.nz;
+    // ghost-inclusive arrays start from zero, as every intermediate does
+    unsigned char* a0 = (unsigned char*)st.rho;
+    unsigned char* a1 = (unsigned char*)pool[15] + align_up((size_t)L.narr * sizeof(T), 256);
+    if (!ck(cudaMemsetAsync(a0, 0, (size_t)(a1 - a0), stream), "cudaMemsetAsync(fields)")) return FARGO_ECUDA;
+    if (!ck(cudaMemsetAsync(ctl, 0, sizeof(Ctl), stream), "cudaMemsetAsync(ctl)")) return FARGO_ECUDA;
+    const void* src[5] = {rho, e, vx, L.hasy ? vy : nullptr, L.hasz ? vz : nullptr};
+    T* dst[5] = {st.rho, st.e, st.vx, st.vy, st.vz};
+    T* staging = pool[15];   // dead between updates
+    for (int f = 0; f < 5; ++f) {
+      if (!src[f]) continue;
+      const T* dev = (const T*)src[f];
+      if (!on_device(src[f])) {
+        if (!ck(cudaMemcpyAsync(staging, src[f], nact * sizeof(T), cudaMemcpyHostToDevice, stream), "H2D field"))
+          return FARGO_ECUDA;
+        dev = staging;
+      }
+      launches += launch_scatter<T>(d, dev, dst[f], stream);
+    }
+    if (!ck(cudaMemsetAsync(staging, 0, (size_t)L.narr * sizeof(T), stream), "cudaMemsetAsync(staging)")) return FARGO_ECUDA;
+    pot_valid = false;
+    if (!ck(cudaGetLastError(), "set_fields launch")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "set_fields sync")) return FARGO_ECUDA;
+    have_fields = true; midstep = false;
+    return FARGO_OK;
+  }
+
+  int get_fields(void* rho, void* e, void* vx, void* vy, void* vz) override {
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step (fargo_step_until)"; return FARGO_ESTATE; }
+    const size_t nact = (size_t)L.nx * L.ny * L.nz;
+    void* dstp[5] = {rho, e, vx, L.hasy ? vy : nullptr, L.hasz ? vz : nullptr};
+    const T* srcp[5] = {st.rho, st.e, st.vx, st.vy, st.vz};
+    int nstage = 0;
+    for (int f = 0; f < 5; ++f) {
+      if (!dstp[f]) continue;
+      if (on_device(dstp[f])) {
+        launches += launch_gather<T>(d, srcp[f], (T*)dstp[f], stream);
+      } else {
+        T* staging = pool[8 + (nstage++ % 8)];   // set B is dead between updates
+        launches += launch_gather<T>(d, srcp[f], staging, stream);
+        if (!ck(cudaMemcpyAsync(dstp[f], staging, nact * sizeof(T), cudaMemcpyDeviceToHost, stream), "D2H field"))
+          return FARGO_ECUDA;
+      }
+    }
+    if (!ck(cudaGetLastError(), "get_fields launch")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "get_fields sync")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
+  int get_time(double* t, double* last_dt, long long* ns) override {
+    Ctl h;
+    if (!ck(cudaMemcpyAsync(&h, ctl, sizeof h, cudaMemcpyDeviceToHost, stream), "read clock")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "clock sync")) return FARGO_ECUDA;
+    if (t) *t = h.t;
+    if (last_dt) *last_dt = h.dt;
+    if (ns) *ns = h.nsteps;
+    return FARGO_OK;
+  }
+
+  // ---- one update --------------------------------------------------------------------------------------
+  int field_mask(bool with_rho, bool with_e) const {
+    int mk = F_VX;
+    if (with_rho) mk |= F_RHO;
+    if (with_e) mk |= F_E;
+    if (L.hasy) mk |= F_VY;
+    if (L.hasz) mk |= F_VZ;
+    return mk;
+  }
+
+  int potential(double t) {
+    const double phip = prm.planet_phi0 + (prm.planet_omega - prm.omega_frame) * t;
+    const double xp = prm.planet_r * std::cos(phip), yp = prm.planet_r * std::sin(phip);
+    const double eps2 = prm.planet_eps * prm.planet_eps;
+    return launch_potential<T>(d, phi, (T)prm.gm_star, (T)prm.planet_mass, (T)xp, (T)yp, (T)eps2, stream);
+  }
+
+  // Enqueue the kernels of one update up to and including `until` (-1 = all).  Returns the launch count.
+  int enqueue_update(int until, bool capturing) {
+    int n = 0;
+    dbg.clear();
+    dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
+    dbg["phi"] = phi; dbg["v0"] = v0;
+    n += launch_bc<T>(d, st, field_mask(true, true), stream);                        // cell 2
+    if (until == FARGO_ST_BC1) return n;
+    if (L.fargo) n += launch_vmean<T>(d, st.vx, v0, stream);                         // cell 3
+    if (until == FARGO_ST_VMEAN) return n;
+    if (L.has_pot && (!pot_valid || !pot_static)) {                                  // cell 5
+      double t = 0.0;
+      if (!pot_static && !capturing) { get_time(&t, nullptr, nullptr); }
+      n += potential(t);
+      pot_valid = true;
+    }
+    if (until == FARGO_ST_POT) return n;
+    const T* v0p = L.fargo ? v0 : nullptr;
+    n += launch_dt<T>(d, st, v0p, stream);                                           // cell 6
+    if (until == FARGO_ST_DT) return n;
+    // source step: intermediates live in transport set B (idle until the second pass)
+    T *vxb = set_arr(1, 0), *vyb = set_arr(1, 1), *vzb = set_arr(1, 2), *ec = set_arr(1, 3);
+    n += launch_source_a<T>(d, st, phi, vxb, vyb, vzb, stream);                      // cell 7a
+    dbg["vxb"] = vxb; dbg["vyb"] = vyb; dbg["vzb"] = vzb;
+    if (until == FARGO_ST_SRC_A) return n;
+    T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
+    if (L.visc) { vxc = set_arr(1, 4); vyc = set_arr(1, 5); }
+    n += launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream);        // cell 7b
+    dbg["vxc"] = vxc; dbg["vyc"] = vyc; dbg["vzc"] = vzc; dbg["ec"] = L.adi ? ec : st.e;
+    dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
+    if (until == FARGO_ST_SRC_B) return n;
+    if (L.adi) n += launch_source_c<T>(d, vxc, vyc, vzc, ec, st.e, stream);          // cell 7c
+    dbg["ed"] = st.e;
+    if (until == FARGO_ST_SRC_C) return n;
+    if (L.visc)                                                                      // cell 7d
+      n += launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream);
+    dbg["vxd"] = st.vx; dbg["vyd"] = st.vy;
+    dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
+    if (until == FARGO_ST_SRC_D) return n;
+    n += launch_bc<T>(d, st, field_mask(false, L.adi), stream);                      // cell 9
+    if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
+    // transport: pass p reads set (p-1)%2 (the state on the first pass) and writes set p%2; the last pass
+    // writes rho and e straight back into the state arrays, so one update leaves every array where it
+    // started and the same captured graph serves every update.
+    for (int p = 0; p < npass; ++p) {
+      const bool first = p == 0, last = p == npass - 1;
+      const int ds = p % 2, ss = 1 - ds;
+      SweepArgs<T> a;
+      memset(&a, 0, sizeof a);
+      a.st = st;
+      a.first = first ? 1 : 0;
+      a.v0 = (pass_kind[p] == 0 || pass_kind[p] == 3) ? v0p : nullptr;
+      a.nq = nq;
+      const bool to_state = last && !first;
+      a.srho = first ? st.rho : set_arr(ss, -1);
+      a.drho = to_state ? st.rho : set_arr(ds, -1);
+      for (int q = 0; q < nq; ++q) {
+        a.slot[q] = slots[q];
+        a.sq[q] = first ? nullptr : set_arr(ss, slots[q]);
+        a.dq[q] = (to_state && slots[q] == 0) ? st.e : set_arr(ds, slots[q]);
+      }
+      if (pass_kind[p] == 3) n += launch_orbital<T>(d, a, nshift, stream);
+      else n += launch_sweep<T>(d, a, pass_kind[p], stream);
+      static const char* names[7] = {"te", "pxm", "pxp", "pym", "pyp", "pzm", "pzp"};
+      dbg["trho"] = a.drho;
+      for (int q = 0; q < nq; ++q) dbg[names[slots[q]]] = a.dq[q];
+      if (last && first) {   // single pass: bring rho and e home
+        n += launch_copy<T>(d, set_arr(ds, -1), st.rho, stream);
+        if (L.adi) n += launch_copy<T>(d, set_arr(ds, 0), st.e, stream);
+      }
+      const int stage_of[4] = {FARGO_ST_SWEEP_X, FARGO_ST_SWEEP_Y, FARGO_ST_SWEEP_Z, FARGO_ST_ORB_SHIFT};
+      if (until == stage_of[pass_kind[p]]) return n;
+      if (pass_kind[p] == 3 && until == FARGO_ST_ORB_FRAC) return n;
+    }
+    if (until >= FARGO_ST_SWEEP_X && until < FARGO_ST_NEWVEL) return n;   // stage absent in this setup
+    const int ls = (npass - 1) % 2;
+    QSet<T> S;
+    S.rho = st.rho;
+    for (int q = 0; q < 7; ++q) S.q[q] = set_arr(ls, q);
+    n += launch_newvel<T>(d, st.rho, S, st, stream);                                 // cell 12d
+    n += launch_advance(ctl, prm.t_stop, stream);
+    return n;
+  }
+
+  int step(int nsteps) override {
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step (fargo_step_until)"; return FARGO_ESTATE; }
+    if (nsteps < 0) { err = "negative step count"; return FARGO_EINVAL; }
+    if (nsteps == 0) return FARGO_OK;
+    const bool graph_ok = prm.use_graph && pot_static;
+    int s = 0;
+    if (graph_ok) {
+      if (!gexec) {
+        if (L.has_pot && !pot_valid) { launches += potential(0.0); pot_valid = true; }   // keep it out of the graph
+        cudaGraph_t g = nullptr;
+        if (!ck(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal), "begin capture")) return FARGO_ECUDA;
+        launches_per_step = enqueue_update(-1, true);
+        if (!ck(cudaStreamEndCapture(stream, &g), "end capture")) return FARGO_ECUDA;
+        if (!ck(cudaGraphInstantiate(&gexec, g, 0), "graph instantiate")) { cudaGraphDestroy(g); return FARGO_ECUDA; }
+        cudaGraphDestroy(g);
+      }
+      for (; s < nsteps; ++s)
+        if (!ck(cudaGraphLaunch(gexec, stream), "graph launch")) return FARGO_ECUDA;
+      launches += (long long)launches_per_step * nsteps;
+    } else {
+      for (; s < nsteps; ++s) launches += enqueue_update(-1, false);
+    }
+    if (!ck(cudaGetLastError(), "step launch")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
+  int step_until(int stage) override {
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    if (stage < 0 || stage >= FARGO_ST_COUNT) { err = "unknown stage"; return FARGO_EINVAL; }
+    launches += enqueue_update(stage == FARGO_ST_NEWVEL ? -1 : stage, false);
+    midstep = stage != FARGO_ST_NEWVEL;
+    if (!ck(cudaGetLastError(), "step_until launch")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "step_until sync")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
+  void dims(int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) const override {
+    if (tx) *tx = L.TX; if (ty) *ty = L.TY; if (tz) *tz = L.TZ;
+    if (ngx) *ngx = L.ngx; if (ngy) *ngy = L.ngy; if (ngz) *ngz = L.ngz;
+  }
+
+  int get_array(const char* name, void* out) override {
+    if (!name || !out) { err = "null argument"; return FARGO_EINVAL; }
+    if (dbg.empty()) {
+      dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
+      dbg["phi"] = phi; dbg["v0"] = v0;
+    }
+    dbg["nshift"] = nshift;
+    auto it = dbg.find(name);
+    if (it == dbg.end() || !it->second) { err = std::string("array not available at this stage: ") + name; return FARGO_EINVAL; }
+    if (!ck(cudaStreamSynchronize(stream), "get_array sync")) return FARGO_ECUDA;
+    const std::string nm(name);
+    if (nm == "v0" || nm == "nshift") {
+      if (!ck(cudaMemcpy(out, it->second, (size_t)L.TY * L.TZ * sizeof(T), cudaMemcpyDeviceToHost), "D2H ring array"))
+        return FARGO_ECUDA;
+      return FARGO_OK;
+    }
+    const size_t n = (size_t)L.TX * L.TY * L.TZ;
+    T* tmp = nullptr;
+    if (!ck(cudaMalloc(&tmp, n * sizeof(T)), "cudaMalloc(debug)")) return FARGO_ENOMEM;
+    launches += launch_unpad<T>(d, it->second, tmp, stream);
+    bool ok = ck(cudaMemcpyAsync(out, tmp, n * sizeof(T), cudaMemcpyDeviceToHost, stream), "D2H array") &&
+              ck(cudaStreamSynchronize(stream), "get_array sync");
+    cudaFree(tmp);
+    return ok ? FARGO_OK : FARGO_ECUDA;
+  }
+};
+
+}  // namespace fg
+
+// ---- C ABI ---------------------------------------------------------------------------------------------
+struct fargo_ctx { fg::CtxBase* impl; };
+
+extern "C" {
+
+size_t fargo_workspace_bytes(const fargo_mesh* mesh, int geometry, int eos, const fargo_params* p) {
+  fg::Layout L;
+  std::string err;
+  if (!fg::make_layout(L, mesh, geometry, eos, p, err)) return 0;
+  return L.bytes(p->precision == 32 ? sizeof(float) : sizeof(double));
+}
+
+int fargo_init(fargo_ctx** out, const fargo_mesh* mesh, int geometry, int eos, const fargo_params* p) {
+  if (!out) { fg::g_init_error = "null output pointer"; return FARGO_EINVAL; }
+  *out = nullptr;
+  fg::Layout L;
+  if (!fg::make_layout(L, mesh, geometry, eos, p, fg::g_init_error)) return FARGO_EINVAL;
+  int rc;
+  fg::CtxBase* impl;
+  if (p->precision == 32) {
+    auto* s = new fg::Sim<float>(); s->L = L; s->precision = 32; rc = s->init(mesh, geometry, eos, p); impl = s;
+  } else {
+    auto* s = new fg::Sim<double>(); s->L = L; s->precision = 64; rc = s->init(mesh, geometry, eos, p); impl = s;
+  }
+  if (rc != FARGO_OK) { fg::g_init_error = impl->err; delete impl; return rc; }
+  *out = new fargo_ctx{impl};
+  return FARGO_OK;
+}
+
+int fargo_destroy(fargo_ctx* c) {
+  if (!c) return FARGO_EINVAL;
+  delete c->impl;
+  delete c;
+  return FARGO_OK;
+}
+
+int fargo_set_fields(fargo_ctx* c, const void* rho, const void* e, const void* vx, const void* vy, const void* vz) {
+  return c ? c->impl->set_fields(rho, e, vx, vy, vz) : FARGO_EINVAL;
+}
+int fargo_get_fields(fargo_ctx* c, void* rho, void* e, void* vx, void* vy, void* vz) {
+  return c ? c->impl->get_fields(rho, e, vx, vy, vz) : FARGO_EINVAL;
+}
+int fargo_step(fargo_ctx* c, int n) { return c ? c->impl->step(n) : FARGO_EINVAL; }
+int fargo_get_time(fargo_ctx* c, double* t, double* last_dt, long long* nsteps) {
+  return c ? c->impl->get_time(t, last_dt, nsteps) : FARGO_EINVAL;
+}
+long long fargo_kernel_launches(const fargo_ctx* c) { return c ? c->impl->launches : 0; }
+int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }
+int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) {
+  if (!c) return FARGO_EINVAL;
+  c->impl->dims(tx, ty, tz, ngx, ngy, ngz);
+  return FARGO_OK;
+}
+int fargo_get_array(fargo_ctx* c, const char* name, void* out) { return c ? c->impl->get_array(name, out) : FARGO_EINVAL; }
+const char* fargo_last_error(const fargo_ctx* c) { return c ? c->impl->err.c_str() : fg::g_init_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,194 @@
+// k_dt.cu -- ring mean velocity (Fig. 2 cell 3, Eq. 72), potential (cell 5, reading G12), CFL time
+// step (cell 6, Eq. 59) with the FARGO shear limit (Eq. 73), and the clock.
+// The time step is reduced wholly on the device (warp shuffles -> one atomic max per block -> a
+// one-block finishing kernel): the paper finishes it on the CPU and names that its one bottleneck.
+#include "kernels.h"
+
+namespace fg {
+
+// ---- cell 3: v0_jk = (max_i vx + min_i vx)/2, one warp per ring, ghost rings included --------------
+template <typename T>
+__global__ void k_vmean(const Dev<T> d, const T* __restrict__ vx, T* __restrict__ v0) {
+  if (d.ctl->done) return;
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  const int nring = d.TY * d.TZ;
+  if (warp >= nring) return;
+  const int j = warp % d.TY, k = warp / d.TY;
+  const T* row = vx + d.id(d.ngx, j, k);
+  T lo = row[0], hi = lo;
+  for (int i = lane; i < d.nx; i += 32) {
+    const T v = row[i];
+    lo = rmin(lo, v); hi = rmax(hi, v);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo = rmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    hi = rmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+  }
+  if (lane == 0) v0[warp] = T(0.5) * (hi + lo);
+}
+
+template <typename T>
+int launch_vmean(const Dev<T>& d, const T* vx, T* v0, cudaStream_t s) {
+  const int nring = d.TY * d.TZ;
+  k_vmean<T><<<(nring + 7) / 8, 256, 0, s>>>(d, vx, v0);
+  return 1;
+}
+
+// ---- cell 5: Phi = -GM/|x| - G m_p / sqrt(|x - x_p|^2 + eps^2) at cell centres ----------------------
+// Trigonometry comes from host tables only (no device transcendental).
+template <typename T>
+__global__ void k_potential(const Dev<T> d, T* __restrict__ phi, const T gm_star, const T gm_planet, const T xp,
+                            const T yp, const T eps2) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= d.TX) return;
+  T R, z, r;
+  if (d.geometry == GEO_SPH) { R = d.yc[j] * d.sin_zc[k]; z = d.yc[j] * d.cos_zc[k]; r = d.yc[j]; }
+  else { R = d.yc[j]; z = d.zc[k]; r = rsqrt_ieee(R * R + z * z); }
+  const T x = R * d.cos_xc[i], y = R * d.sin_xc[i];
+  T p = -(gm_star / r);
+  if (gm_planet != T(0)) {
+    const T ddx = x - xp, ddy = y - yp;
+    const T d2 = ((ddx * ddx + ddy * ddy) + z * z) + eps2;
+    p = p - gm_planet / rsqrt_ieee(d2);
+  }
+  phi[d.id(i, j, k)] = p;
+}
+
+template <typename T>
+int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2, cudaStream_t s) {
+  dim3 b(128), g((d.TX + 127) / 128, d.TY, d.TZ);
+  k_potential<T><<<g, b, 0, s>>>(d, phi, gm_star, gm_planet, xp, yp, eps2);
+  return 1;
+}
+
+// ---- cell 6 ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long to_bits(double v) { return (unsigned long long)__double_as_longlong(v); }
+__device__ __forceinline__ unsigned long long to_bits(float v) { return (unsigned long long)__float_as_uint(v); }
+template <typename T> __device__ __forceinline__ T from_bits(unsigned long long b);
+template <> __device__ __forceinline__ double from_bits<double>(unsigned long long b) { return __longlong_as_double((long long)b); }
+template <> __device__ __forceinline__ float from_bits<float>(unsigned long long b) { return __uint_as_float((unsigned)b); }
+
+// Per active cell: sum over the processes of Eq. 59 of the squared inverse time steps, each inverse
+// time step being the max over the directions present ("dt_i = min_j dt_ij").  max is exact,
+// so the block/grid reduction order does not matter: dt is bit-reproducible.
+template <typename T>
+__global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T> st, const T* __restrict__ v0) {
+  if (d.ctl->done) return;
+  const int nrow = d.ny * d.nz;
+  T m2 = T(0);
+  for (int row = blockIdx.x; row < nrow; row += gridDim.x) {
+    const int j = d.ngy + row % d.ny, k = d.ngz + row / d.ny;
+    const T ilx = d.invLX(j, k), ily = d.invLY[j], ilz = d.invLZ(j, k);
+    T ilmax = T(0);
+    if (d.hasx) ilmax = rmax(ilmax, ilx);
+    if (d.hasy) ilmax = rmax(ilmax, ily);
+    if (d.hasz) ilmax = rmax(ilmax, ilz);
+    const T il2 = ilmax * ilmax;
+    const T I4 = d.c4 * il2;
+    const T I4sq = I4 * I4;
+    const T vm = v0 ? v0[d.rid(j, k)] : T(0);
+    for (int ia = threadIdx.x; ia < d.nx; ia += blockDim.x) {
+      const int i = d.ngx + ia;
+      const long long l = d.id(i, j, k);
+      const T cs2 = (d.eos == EOS_ADI) ? (d.gg1 * st.e[l]) / st.rho[l] : st.e[l] * st.e[l];
+      const T I1sq = cs2 * il2;
+      T I2 = T(0), I3 = T(0);
+      if (d.hasx) {
+        const T a = st.vx[l], b = st.vx[d.id(d.xw(i + 1), j, k)];
+        I2 = rmax(I2, rabs(T(0.5) * (a + b) - vm) * ilx);
+        I3 = rmax(I3, rabs(b - a) * ilx);
+      }
+      if (d.hasy) {
+        const T a = st.vy[l], b = st.vy[l + d.pitch];
+        I2 = rmax(I2, rabs(T(0.5) * (a + b)) * ily);
+        I3 = rmax(I3, rabs(b - a) * ily);
+      }
+      if (d.hasz) {
+        const T a = st.vz[l], b = st.vz[l + d.plane];
+        I2 = rmax(I2, rabs(T(0.5) * (a + b)) * ilz);
+        I3 = rmax(I3, rabs(b - a) * ilz);
+      }
+      I3 = d.c3 * I3;
+      const T Isq = ((I1sq + I2 * I2) + I3 * I3) + I4sq;
+      m2 = rmax(m2, Isq);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+  __shared__ T sm[8];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m2;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    m2 = threadIdx.x < (blockDim.x >> 5) ? sm[threadIdx.x] : T(0);
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+    if (threadIdx.x == 0) atomicMax(&d.ctl->m2bits, to_bits(m2));   // non-negative: bit order = value order
+  }
+}
+
+// One block: shear limit over the active rings (Eq. 73 with V_X = v0_jk), Courant factor, overrides.
+template <typename T>
+__global__ void __launch_bounds__(256) k_dt_finish(const Dev<T> d, const T* __restrict__ v0) {
+  Ctl* c = d.ctl;
+  if (c->done) return;
+  T s = T(0);
+  if (d.fargo) {
+    const int nyp = d.ny - 1;
+    const int n = nyp > 0 ? nyp * d.nz : 0;
+    for (int r = threadIdx.x; r < n; r += blockDim.x) {
+      const int j = d.ngy + r % nyp, k = d.ngz + r / nyp;
+      s = rmax(s, rabs(v0[d.rid(j, k)] * d.invLX(j, k) - v0[d.rid(j + 1, k)] * d.invLX(j + 1, k)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s = rmax(s, __shfl_xor_sync(0xffffffffu, s, o));
+  }
+  __shared__ T sm[8];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) s = rmax(s, sm[w]);
+    const T M2 = from_bits<T>(c->m2bits);
+    T dt = T(1) / rsqrt_ieee(M2);
+    if (d.fargo && s > T(0)) dt = rmin(dt, d.shear_c0 / s);
+    dt = d.cfl * dt;
+    double dtd = (double)dt;
+    if (d.dt_fixed > 0.0) dtd = (double)(T)d.dt_fixed;
+    int clipped = 0;
+    if (d.t_stop > 0.0 && c->t + dtd >= d.t_stop) { dtd = (double)(T)(d.t_stop - c->t); clipped = 1; }
+    c->dt = dtd;
+    c->clipped = clipped;
+    c->m2bits = 0ull;
+  }
+}
+
+template <typename T>
+int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s) {
+  const int nrow = d.ny * d.nz;
+  const int grid = nrow < 148 * 8 ? nrow : 148 * 8;
+  k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0);
+  k_dt_finish<T><<<1, 256, 0, s>>>(d, v0);
+  return 2;
+}
+
+// The clock: t <- t + dt (or exactly t_stop on a clipped step); afterwards every kernel is a no-op.
+__global__ void k_advance(Ctl* c, const double t_stop) {
+  if (c->done) return;
+  c->t = c->clipped ? t_stop : c->t + c->dt;
+  c->nsteps += 1;
+  if (t_stop > 0.0 && c->t >= t_stop) c->done = 1;
+}
+int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s) {
+  k_advance<<<1, 1, 0, s>>>(ctl, t_stop);
+  return 1;
+}
+
+#define INST(T)                                                                              \
+  template int launch_vmean<T>(const Dev<T>&, const T*, T*, cudaStream_t);                   \
+  template int launch_potential<T>(const Dev<T>&, T*, T, T, T, T, T, cudaStream_t);          \
+  template int launch_dt<T>(const Dev<T>&, const State<T>&, const T*, cudaStream_t);
+INST(double)
+INST(float)
+#undef INST
+
+}  // namespace fg

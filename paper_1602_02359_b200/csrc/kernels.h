@@ -1,0 +1,59 @@
+// kernels.h -- launchers of the CUDA kernels of one hydrodynamic update (host-callable, templated
+// on the arithmetic type, instantiated for double and float in the k_*.cu files).
+// Every launcher enqueues on `s` and returns the number of kernels it launched.
+#pragma once
+#include "common.cuh"
+
+namespace fg {
+
+enum { F_RHO = 1, F_E = 2, F_VX = 4, F_VY = 8, F_VZ = 16 };
+
+// cells 2 / 9: ghost fill of the fields in `mask`, X then Y then Z
+template <typename T> int launch_bc(const Dev<T>& d, const State<T>& st, int mask, cudaStream_t s);
+// cell 3: v0_jk = (max_i vx + min_i vx)/2 (Eq. 72)
+template <typename T> int launch_vmean(const Dev<T>& d, const T* vx, T* v0, cudaStream_t s);
+// cell 5: potential of the star and the planet at cell centres; cphi, sphi = cos, sin of the planet's azimuth
+template <typename T> int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2,
+                                           cudaStream_t s);
+// cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
+template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s);
+// cell 7a: st -> vb[3]
+template <typename T> int launch_source_a(const Dev<T>& d, const State<T>& st, const T* phi, T* vxb, T* vyb, T* vzb,
+                                          cudaStream_t s);
+// cell 7b: (rho, e, vb) -> vc[3], ec
+template <typename T> int launch_source_b(const Dev<T>& d, const State<T>& st, const T* vxb, const T* vyb,
+                                          const T* vzb, T* vxc, T* vyc, T* vzc, T* ec, cudaStream_t s);
+// cell 7c: (vc, ec) -> ed
+template <typename T> int launch_source_c(const Dev<T>& d, const T* vxc, const T* vyc, const T* vzc, const T* ec,
+                                          T* ed, cudaStream_t s);
+// cell 7d (2-D cylindrical): (rho, vc) -> vd, with the stress tensor in tpp, trr, tpr
+template <typename T> int launch_source_d(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, T* tpp, T* trr,
+                                          T* tpr, T* vxd, T* vyd, cudaStream_t s);
+
+// cells 12a-12c: one directional sweep.  first != 0: the momenta are formed from the state (12a fused).
+template <typename T> struct SweepArgs {
+  State<T> st;        // state: e and velocities for the momenta (first pass); the frozen face velocities
+  const T* srho;      // density read by this pass (the state's on the first pass)
+  T* drho;            // density written by this pass
+  const T* sq[8];     // the nq transported quantities read (compacted; unused on the first pass)
+  T* dq[8];           // ... and written
+  const T* v0;        // ring mean velocity or nullptr
+  int nq;             // transported quantities besides rho (<= 7)
+  int slot[8];        // what each one is: 0 = e, 1..6 = pxm pxp pym pyp pzm pzp
+  int first;
+};
+template <typename T> int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s);
+// orbital advection: PPA fractional sweep (Eq. 70) with the integer shift (Eq. 69) folded into the store index
+template <typename T> int launch_orbital(const Dev<T>& d, const SweepArgs<T>& a, T* nshift_out, cudaStream_t s);
+// cell 12d: Eq. 51; then the clock advances
+template <typename T> int launch_newvel(const Dev<T>& d, const T* rho, const QSet<T>& set, const State<T>& st,
+                                        cudaStream_t s);
+template <typename T> int launch_copy(const Dev<T>& d, const T* src, T* dst, cudaStream_t s);
+int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s);
+
+// active cells <-> ghosted, padded device layout
+template <typename T> int launch_scatter(const Dev<T>& d, const T* active, T* full, cudaStream_t s);
+template <typename T> int launch_gather(const Dev<T>& d, const T* full, T* active, cudaStream_t s);
+template <typename T> int launch_unpad(const Dev<T>& d, const T* full, T* out, cudaStream_t s);
+
+}  // namespace fg

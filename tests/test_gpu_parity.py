@@ -1,0 +1,243 @@
+"""GPU parity: the CUDA path (through the C ABI of include/fargo.h) against the CPU oracle, element by
+element, on the same seeded inputs.  Bar (BASELINE.json north_star):
+    rel_f = max_active |gpu_f - oracle_f| / max_active |oracle_f|  <= 1e-10 (fp64), <= 1e-4 (fp32),
+and the time step, which is a max/min reduction and therefore exact, must be BIT-equal.
+Both sides keep automatic FMA contraction off and follow one operation order,
+so in practice the fp64 fields come out bit-identical; the tests assert the contract's tolerance and
+print the observed difference.
+"""
+import numpy as np
+import pytest
+
+import gpu_cases as G
+from oracle.binding import Oracle
+from paper_1602_02359_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-10
+TOL32 = 1e-4
+
+
+def _gpu(w, precision=64, use_graph=True):
+    from paper_1602_02359_b200 import Fargo
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=precision, use_graph=use_graph)
+    g.set_fields(*w.fields())
+    return g
+
+
+def _oracle(w):
+    o = Oracle(w.mesh, w.geometry, w.eos, w.params)
+    o.set_fields(*w.fields())
+    return o
+
+
+def _rel(a, b):
+    d = float(np.max(np.abs(a.astype(np.float64) - b)))
+    s = float(np.max(np.abs(b)))
+    return d / s if s > 0 else d
+
+
+def _diff_report(name, a, b):
+    d = np.abs(a.astype(np.float64) - b)
+    idx = np.unravel_index(int(np.argmax(d)), d.shape)
+    return "%s: rel %.3e, max|d| %.3e at %s (gpu %.17g, oracle %.17g), %d / %d elements differ" % (
+        name, _rel(a, b), float(d.max()), idx, float(a[idx]), float(b[idx]), int((d > 0).sum()), d.size)
+
+
+# ---------------------------------------------------------------- per-stage parity (fp64) -------------
+def _stage_arrays(w, stage):
+    """(gpu name, oracle name) pairs holding defined data once `stage` has run."""
+    adi = w.eos == W.ADIABATIC
+    hx, hy, hz = w.mesh.nx > 1, w.mesh.ny > 1, w.mesh.nz > 1
+    vel = [("vx", "vx")] + ([("vy", "vy")] if hy else []) + ([("vz", "vz")] if hz else [])
+    mom = ([("pxm", "pxm"), ("pxp", "pxp")] if hx else []) + ([("pym", "pym"), ("pyp", "pyp")] if hy else []) + \
+          ([("pzm", "pzm"), ("pzp", "pzp")] if hz else [])
+    tr = [("trho", "rho")] + ([("te", "e")] if adi else []) + mom
+    visc = w.params.nu > 0 and w.geometry == W.CYLINDRICAL and hx and hy and not hz
+    sfx = lambda s: ([("vx" + s, "vx" + s)] if hx else []) + ([("vy" + s, "vy" + s)] if hy else []) + \
+        ([("vz" + s, "vz" + s)] if hz else [])
+    return {
+        "BC1": [("rho", "rho"), ("e", "e")] + vel,
+        "VMEAN": [("v0", "v0")] if w.params.fargo_on else [],
+        "POT": [("phi", "phi")] if (w.geometry != W.CARTESIAN and (w.params.gm_star or w.params.planet_mass)) else [],
+        "DT": [],
+        "SRC_A": sfx("b"),
+        "SRC_B": sfx("c") + ([("ec", "ec")] if adi else []),
+        "SRC_C": [("ed", "ed")] if adi else [],
+        "SRC_D": [("vxd", "vxd"), ("vyd", "vyd")] if visc else [],
+        "BC2": [("rho", "rho"), ("e", "e")] + vel,
+        "SWEEP_X": tr if hx else [],
+        "SWEEP_Y": tr if hy else [],
+        "SWEEP_Z": tr if hz else [],
+        "ORB_SHIFT": (tr + [("nshift", "nshift")]) if w.params.fargo_on else [],
+    }[stage]
+
+
+STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2", "SWEEP_X", "SWEEP_Y", "SWEEP_Z",
+          "ORB_SHIFT"]
+
+
+@pytest.mark.parametrize("make", G.ALL, ids=[m.__name__ for m in G.ALL])
+def test_stage_by_stage(make):
+    """Every kernel alone: run both sides up to each stage of Fig. 2 and compare the arrays it wrote,
+    ghost zones included (both sides compute wherever the stencil fits and pass the input through elsewhere)."""
+    w = make()
+    bad = []
+    for stage in STAGES:
+        pairs = _stage_arrays(w, stage)
+        if not pairs and stage != "DT":
+            continue
+        o, g = _oracle(w), _gpu(w, use_graph=False)
+        o.step_until(stage)
+        g.step_until(stage)
+        if stage == "DT":
+            dt_o, dt_g = o.time()[1], g.time()[1]
+            if dt_o != dt_g:
+                bad.append("DT: gpu %.17g oracle %.17g" % (dt_g, dt_o))
+        for gn, on in pairs:
+            a, b = g.array(gn), o.array(on)
+            if _rel(a, b) > TOL64 or not np.isfinite(a).all():
+                bad.append(stage + " " + _diff_report(gn, a, b))
+        g.close(); o.close()
+    assert not bad, "\n".join(bad)
+
+
+@pytest.mark.parametrize("make", G.ALL, ids=[m.__name__ for m in G.ALL])
+@pytest.mark.parametrize("use_graph", [False, True], ids=["stream", "graph"])
+def test_multi_step(make, use_graph):
+    """Several full updates (graph replay and plain launches): fields within 1e-10, clock bit-equal."""
+    w = make()
+    o, g = _oracle(w), _gpu(w, use_graph=use_graph)
+    o.step(w.nsteps)
+    g.step(w.nsteps)
+    to, tg = o.time(), g.time()
+    assert tg[2] == to[2]
+    assert tg[0] == to[0] and tg[1] == to[1], "clock differs: gpu %r oracle %r" % (tg, to)
+    fo, fg = o.get_fields(), g.get_fields()
+    bad = []
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), fg, fo):
+        r = _rel(a, b)
+        print("%s %s rel %.3e" % (w.name, name, r))
+        if r > TOL64 or not np.isfinite(a).all():
+            bad.append(_diff_report(name, a, b))
+    assert not bad, "\n".join(bad)
+    assert g.kernel_launches() > 0
+
+
+# ---------------------------------------------------------------- the five configs ---------------------
+def _run_config(w, nsteps, precision=64, tol=TOL64):
+    o, g = _oracle(w), _gpu(w, precision=precision)
+    o.step(nsteps)
+    g.step(nsteps)
+    fo, fg = o.get_fields(), g.get_fields()
+    rels = {}
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), fg, fo):
+        assert np.isfinite(a).all(), name
+        rels[name] = _rel(a, b)
+    print(w.name, "steps", o.time()[2], "t", o.time()[0], {k: "%.2e" % v for k, v in rels.items()})
+    assert max(rels.values()) <= tol, rels
+    return o, g
+
+
+def test_config1_sound_wave():
+    """Config 1: 32^3 linear sound wave, 200 steps; also the phase speed against the closed form."""
+    w = W.sound_wave()
+    o, g = _run_config(w, 200)
+    assert g.time() == o.time()
+    rho = g.get_fields()[0]
+    m = w.mesh
+    psi = 2 * np.pi * (m.xc()[None, None, :] + m.yc()[None, :, None] + m.zc()[:, None, None])
+    a, b = np.sum((rho - 1) * np.cos(psi)), np.sum((rho - 1) * np.sin(psi))
+    phase = np.arctan2(b, a) % (2 * np.pi)
+    expect = (2 * np.pi * np.sqrt(3.0) * 1.0 * g.time()[0]) % (2 * np.pi)
+    dphi = (phase - expect + np.pi) % (2 * np.pi) - np.pi
+    assert abs(dphi) < 0.005 * 2 * np.pi * np.sqrt(3.0) * g.time()[0], (phase, expect)
+
+
+def test_config2_sod():
+    """Config 2: Sod tube 512x4x4 to t = 0.2 (outflow X = ghosted X axis)."""
+    w = W.sod()
+    o, g = _run_config(w, 2000)
+    assert g.time() == o.time() and g.time()[0] == 0.2
+
+
+def test_config3_disk2d():
+    """Config 3: 768x256 cylindrical isothermal disk, planet, viscosity, FARGO; 500 steps."""
+    w = W.disk2d()
+    _run_config(w, 500)
+
+
+def test_config4_disk3d_reduced():
+    """Config 4 at a size the oracle finishes in seconds (192x64x16, same recipe); the full size is
+    checked by test_full_size.py on sampled rings."""
+    w = W.disk3d(192, 64, 16)
+    _run_config(w, 30)
+
+
+def test_config5_noise_box_64():
+    w = W.noise_box(64)
+    _run_config(w, 50)
+
+
+def test_config5_noise_box_64_fp32():
+    """fp32 build against the fp64 oracle: <= 1e-4."""
+    w = W.noise_box(64)
+    _run_config(w, 50, precision=32, tol=TOL32)
+
+
+# ---------------------------------------------------------------- edge cases -----------------------------
+def test_uniform_state_is_preserved():
+    w = W.noise_box(shape3=(40, 8, 8))
+    w.rho[...] = 1.0; w.vx[...] = 0.25; w.vy[...] = -0.5; w.vz[...] = 0.125
+    g = _gpu(w)
+    g.step(5)
+    rho, e, vx, vy, vz = g.get_fields()
+    assert np.all(rho == 1.0) and np.all(e == w.e) and np.all(vx == 0.25) and np.all(vy == -0.5) and np.all(vz == 0.125)
+
+
+def test_set_get_roundtrip_and_device_pointers():
+    """fargo_get_fields(fargo_set_fields(x)) == x bit for bit (the checkpoint path), host and device pointers."""
+    import torch
+    w = G.cart_adi_mixed_bc()
+    g = _gpu(w)
+    for a, b in zip(g.get_fields(), w.fields()):
+        assert np.array_equal(a, b)
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in w.fields()]
+    g.set_fields(*dev)
+    out = [torch.empty_like(t) for t in dev]
+    g.get_fields(out)
+    for a, b in zip(out, dev):
+        assert torch.equal(a, b)
+
+
+def test_t_stop_makes_later_steps_noops():
+    w = G.sod_small()
+    o, g = _oracle(w), _gpu(w)
+    o.step(60); g.step(60)
+    assert g.time() == o.time() and g.time()[0] == 0.05
+    f1 = g.get_fields()
+    g.step(3)
+    for a, b in zip(g.get_fields(), f1):
+        assert np.array_equal(a, b)
+
+
+def test_exact_integer_shift():
+    """delta v = 0 and v0 dt / LX an exact integer: the ring is rotated bit for bit."""
+    import math
+    nphi, nr = 64, 8
+    bc = ((W.PERIODIC,) * 2, (W.REFLECTING,) * 2, (W.PERIODIC,) * 2)
+    mesh = W.Mesh(nphi, nr, 1, 0.0, 2.0 * math.pi, W.uedges(1.0, 2.0, nr), np.array([-0.5, 0.5]), bc)
+    prm = W.Params(fargo_on=1, dt_fixed=0.25)
+    shape = (1, nr, nphi)
+    r = mesh.yc()[None, :, None] * np.ones(shape)
+    rho = 1.0 + 0.3 * W.uniform_pm1(0, nr * nphi).reshape(shape)
+    cs = np.full(shape, 1e-3)
+    nsh = np.array([3, -2, 5, 0, 1, -7, 64, 2])[None, :, None]
+    vx = nsh * (mesh.dx * r) / prm.dt_fixed * np.ones(shape)
+    w = W.Workload("shift", mesh, W.CYLINDRICAL, W.ISOTHERMAL, prm, rho, cs, vx, np.zeros(shape), None, 1)
+    g, o = _gpu(w, use_graph=False), _oracle(w)
+    g.step_until("ORB_SHIFT"); o.step_until("ORB_SHIFT")
+    got, ref = g.array("trho"), o.array("rho")
+    assert np.array_equal(g.array("nshift"), o.array("nshift"))
+    assert np.array_equal(got, ref)

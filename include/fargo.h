@@ -77,7 +77,8 @@ typedef struct fargo_params {
                               steps are no-ops (reading G21); <= 0: none */
   double dt_fixed;         /* > 0: overrides the CFL time step */
   int precision;           /* 64 (double) or 32 (float) */
-  int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (default path);
+  int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (needs a non-default
+                              cuda_stream; on the legacy default stream it falls back to plain launches);
                               0: plain stream launches */
   void* workspace;         /* DEVICE memory, >= fargo_workspace_bytes(), 256-byte aligned; caller-owned */
   size_t workspace_bytes;

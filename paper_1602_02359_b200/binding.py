@@ -127,6 +127,10 @@ class Fargo:
             base = self.workspace.data_ptr()
             off = (-base) % 256
             self.stream = torch.cuda.current_stream(self.device)
+            if self.stream.cuda_stream == 0:
+                # the legacy default stream cannot be captured into a CUDA graph: give the context its own
+                self.stream = torch.cuda.Stream(self.device)
+                torch.cuda.current_stream(self.device).synchronize()
             p.workspace = base + off
             p.workspace_bytes = nbytes
             p.cuda_stream = self.stream.cuda_stream
@@ -173,6 +177,7 @@ class Fargo:
             arrs.append(a)
         self._keep = arrs
         with self._torch.cuda.device(self.device):
+            self._torch.cuda.current_stream(self.device).synchronize()   # device inputs made on another stream
             self._check(load().fargo_set_fields(self._h, *[_ptr(a) for a in arrs]), "fargo_set_fields")
 
     def step(self, n: int = 1):

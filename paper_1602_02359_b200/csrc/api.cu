@@ -392,7 +392,8 @@ struct Sim : CtxBase {
     if (midstep) { err = "context is mid-step (fargo_step_until)"; return FARGO_ESTATE; }
     if (nsteps < 0) { err = "negative step count"; return FARGO_EINVAL; }
     if (nsteps == 0) return FARGO_OK;
-    const bool graph_ok = prm.use_graph && pot_static;
+    // the legacy default stream cannot be captured: plain launches there
+    const bool graph_ok = prm.use_graph && pot_static && stream != nullptr;
     int s = 0;
     if (graph_ok) {
       if (!gexec) {

@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the full hydrodynamic update on B200 (BASELINE.json metric: fp64 cell
+updates/s per HD step on 1 B200; achieved HBM GB/s vs peak).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (ghost fill, dt reduction, source sub-steps, X/Y/Z sweeps,
+orbital advection where on, new velocities) over the whole synthetic mesh.  Prints ONE JSON line.
+  value      cells * K / device time of fargo_step(K) (CUDA events on the context's stream, max over ranks),
+             inputs resident in HBM, one CUDA-graph replay per step;
+  e2e        same metric through the public API with pinned HOST buffers: every step does
+             fargo_set_fields (H2D) + fargo_step(1) + fargo_get_fields (D2H) inside the timed region;
+  roofline   the launcher with the largest share of the step, timed live with per-launch CUDA events
+             (fargo_profile) in a second region of K steps: algorithmic bytes / mean launch duration
+             against the measured copy bandwidth of MEASURED_PEAKS.json;
+  kernels    the same for every launcher (share of the step, GB/s), step_roofline for the whole update;
+  cpu_baseline  the CPU oracle, as it stands, single thread, on a bounded sample of the same recipe.
+With --gpus N > 1 (torchrun) every rank runs an independent replica of the workload ("replicas only",
+DESIGN.md section 8(e)): no data-path collective; value = N * cells * K / max-over-ranks time.
+--impl reference times the CPU oracle (there is no reference implementation to install: the reference
+is a paper), on rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1602_02359_b200 import workloads as W  # noqa: E402
+
+METRIC = "fp64 cell updates/s per HD step"
+UNIT = "cell updates/s"
+
+
+# ---------------------------------------------------------------------------------- workloads -------
+def make_workload(name: str):
+    """(workload, bounded oracle sample of the same recipe, description of the sample)."""
+    if name.startswith("noise"):
+        n = int(name[5:])
+        sample = W.noise_box(shape3=(n, min(n, 64), min(n, 64)))
+        return W.noise_box(n), sample, "same recipe on a %dx%dx%d slab" % (n, min(n, 64), min(n, 64))
+    if name == "disk3d":
+        return W.disk3d(), W.disk3d(1536, 32, 16), "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
+    if name == "disk2d":
+        return W.disk2d(), W.disk2d(), "the whole 768x256 mesh"
+    if name == "sound":
+        return W.sound_wave(), W.sound_wave(), "the whole 32^3 mesh"
+    if name == "sod":
+        return W.sod(), W.sod(), "the whole 512x4x4 mesh"
+    raise SystemExit("unknown workload " + name)
+
+
+CONFIG_OF = {"noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
+
+
+def algorithmic_reals(w):
+    """Reals (read + written) per ACTIVE cell that each launcher must move if every array it touches
+    crosses HBM exactly once, and the fused-plan total of SURVEY.md 8(d.3)."""
+    nd = sum(1 for n in (w.mesh.nx, w.mesh.ny, w.mesh.nz) if n > 1)
+    adi = w.eos == W.ADIABATIC
+    pot = w.geometry != W.CARTESIAN and (w.params.gm_star != 0 or w.params.planet_mass != 0)
+    nq = (1 if adi else 0) + 2 * nd
+    visc = w.params.nu > 0
+    k = {
+        "vmean": 1,
+        "dt": (2 if adi else 1) + nd,
+        "source_a": (2 + nd + (1 if pot else 0)) + nd,
+        "source_b": (1 + (1 if adi else 0) + nd) + (nd + (1 if adi else 0)),
+        "source_c": (nd + 1) + 1,
+        "source_d": (3 + 3) + (3 + 3 + 2),
+        "first_sweep": (1 + (1 if adi else 0) + nd) + (1 + nq),
+        "sweep": (1 + nq + 1) + (1 + nq),
+        "orbital": (1 + nq) + (1 + nq),
+        "newvel": (1 + 2 * nd) + nd,
+    }
+    if not adi:
+        k["source_c"] = 0
+    if not visc:
+        k["source_d"] = 0
+    # fused plan of SURVEY.md 8(d.3): dt, one source pass, one pass per direction, orbital, Eq. 51 folded
+    state_r = (2 if adi else 1) + nd                                  # rho, e (adiabatic), velocities
+    fused = state_r                                                   # dt
+    fused += (state_r + (1 if pot else 0)) + (nd + (1 if adi else 0))   # source: state (+ phi) -> e', v'
+    npass = nd + (1 if w.params.fargo_on else 0)
+    for p in range(npass):
+        reads = state_r if p == 0 else (1 + nq + 1)                   # first pass forms the momenta on the fly
+        writes = (1 + nq) if p < npass - 1 else (1 + (1 if adi else 0) + nd)   # last pass ends with Eq. 51
+        fused += reads + writes
+    return k, fused
+
+
+# ---------------------------------------------------------------------------------- clocks ----------
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md, clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.lines, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (copy, read+write bytes)"
+    except Exception:
+        return 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+# ---------------------------------------------------------------------------------- reference arm ---
+def oracle_rate(sample, steps, warmup):
+    from oracle.binding import Oracle
+    o = Oracle(sample.mesh, sample.geometry, sample.eos, sample.params)
+    o.set_fields(*sample.fields())
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return sample.mesh.ncells * steps / dt, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w, sample, desc = make_workload(args.workload)
+    steps = max(1, min(args.steps, max(1, int(40e6 // sample.mesh.ncells))))   # bound the whole run to minutes
+    warm = min(args.warmup, 1)
+    rate, dt = oracle_rate(sample, steps, warm)
+    out = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / steps * (w.mesh.ncells / sample.mesh.ncells),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "baseline_config": CONFIG_OF[args.workload],
+                   "note": "CPU oracle (plain C++, one thread) timed on %d step(s) of a bounded sample; ms_per_step is "
+                           "scaled to the full mesh" % steps},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+# ---------------------------------------------------------------------------------- our arm ---------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1602_02359_b200 import Fargo
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if world == 1:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    w, sample, sample_desc = make_workload(args.workload)
+    prec = 32 if args.fp32 else 64
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=prec)
+    es = 8 if prec == 64 else 4
+    ncell = w.mesh.ncells
+    tdt = torch.float64 if prec == 64 else torch.float32
+    host_in = [None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(tdt).pin_memory() for a in w.fields()]
+    g.set_fields(*host_in)
+    K, Wm = args.steps, max(args.warmup, 3)
+
+    # ---- region 1: device-resident throughput (graph replay) ----
+    g.step(Wm)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = g.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    g.step(K)
+    e1.record(g.stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    launches = g.kernel_launches() - l0
+    value = world * ncell * K / (ms * 1e-3)
+
+    # ---- region 2: per-launcher CUDA-event timing (plain launches) ----
+    g.profile(True)
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record(g.stream)
+    g.step(K)
+    e3.record(g.stream)
+    rep = g.profile_report()
+    g.profile(False)
+    ms_prof = e2.elapsed_time(e3)
+    reals, fused_reals = algorithmic_reals(w)
+    peak, peak_src = measured_peak()
+    total_ms = sum(v[1] for v in rep.values())
+    kernels = {}
+    first_sweep = next((n for n in ("sweep_x", "sweep_y", "sweep_z") if n in rep), None)
+    for name, (nk, tms) in rep.items():
+        key = "first_sweep" if name == first_sweep else ("sweep" if name.startswith("sweep") else name)
+        r = reals.get(key, 0)
+        calls = K * (2 if name == "bc" else 1)
+        per_launch_ms = tms / calls
+        gbs = (r * es * ncell / (per_launch_ms * 1e-3) / 1e9) if r else None
+        kernels[name] = {"share": tms / total_ms, "ms_per_launch": per_launch_ms, "kernels": nk // calls,
+                         "algorithmic_bytes_per_cell": r * es, "achieved_gbs": gbs,
+                         "frac": (gbs / peak) if gbs else None}
+    dom = max((n for n in kernels if kernels[n]["achieved_gbs"]), key=lambda n: kernels[n]["share"])
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_cell"] * ncell,
+                "ms_per_launch": kernels[dom]["ms_per_launch"], "share_of_step": kernels[dom]["share"]}
+    step_gbs = fused_reals * es * ncell / (ms / K * 1e-3) / 1e9
+    step_roofline = {"algorithmic_bytes_per_cell_fused_plan": fused_reals * es,
+                     "algorithmic_bytes_per_cell_as_built": sum(
+                         reals["first_sweep" if n == first_sweep else ("sweep" if n.startswith("sweep") else n)] * es
+                         for n in rep if n in reals or n.startswith("sweep")),
+                     "achieved_gbs_vs_fused_plan": step_gbs, "frac_of_measured_peak": step_gbs / peak,
+                     "frac_of_nominal_8TBs": step_gbs / 8000.0, "ms_per_step_profiled": ms_prof / K}
+
+    # ---- region 3: end to end through the public API with pinned host buffers ----
+    ke = max(1, min(K, args.e2e_steps))
+    if args.no_e2e:
+        ke = 0
+    e2e = None
+    if ke > 0:
+        host_out = [None if a is None else torch.empty_like(a).pin_memory() for a in host_in]
+        cur = host_in
+        g.set_fields(*cur); g.step(1); g.get_fields(host_out)   # warm the path once
+        barrier()
+        e4, e5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e4.record(g.stream)
+        for _ in range(ke):
+            g.set_fields(*cur)
+            g.step(1)
+            g.get_fields(host_out)
+            cur = host_out
+        e5.record(g.stream)
+        barrier()
+        ms_e2e = max_over_ranks(e4.elapsed_time(e5))
+        nfield = sum(1 for a in host_in if a is not None)
+        e2e = {"value": world * ncell * ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nfield * ncell * es,
+               "d2h_bytes_per_step": nfield * ncell * es, "steps": ke, "ms_per_step": ms_e2e / ke}
+
+    # ---- CPU baseline: the oracle as it stands, one thread, bounded sample (rank 0, N = 1) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nst = max(1, int(20e6 // sample.mesh.ncells))
+        rate, _ = oracle_rate(sample, nst, 0)
+        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "%s, %d step(s), single thread, %d host cores present" % (sample_desc, nst, os.cpu_count())}
+
+    if rank == 0:
+        out = {
+            "metric": METRIC if prec == 64 else METRIC.replace("fp64", "fp32"), "value": value, "unit": UNIT,
+            "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
+            "config": {"workload": w.name, "baseline_config": CONFIG_OF[args.workload], "cells": ncell,
+                       "state_bytes": 5 * ncell * es, "l2": "inputs larger than L2" if 5 * ncell * es > 4 * 126e6
+                       else "working set fits L2: launch/latency-bound, HBM fraction not meaningful",
+                       "parallelism": "replicas x%d" % world if world > 1 else "1 GPU, whole mesh resident in HBM",
+                       "launch": "one CUDA graph replay per step"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "step_roofline": step_roofline, "kernels": kernels, "cpu_baseline": cpu,
+        }
+        print(json.dumps(out))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="noise512", choices=sorted(CONFIG_OF))
+    ap.add_argument("--fp32", action="store_true", help="the optional fp32 build (config 5)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer region (short runs under ncu)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -127,6 +127,15 @@ int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy
  * by the most recent transport pass.  Which names hold defined data depends on the stage reached. */
 int fargo_get_array(fargo_ctx* c, const char* name, void* out);
 
+/* ---- measurement ------------------------------------------------------------------------------------- */
+/* enable != 0: from now on fargo_step uses plain launches and brackets every kernel launcher with a CUDA
+ * event pair on the context's stream; enable == 0: stop and drop the record.  Either way the record restarts. */
+int fargo_profile(fargo_ctx* c, int enable);
+/* Synchronise, then write one text line per launcher into HOST buffer `buf` (len bytes):
+ * "<name> <kernel launches> <total milliseconds>\n".  Names: bc vmean potential dt source_a source_b source_c
+ * source_d sweep_x sweep_y sweep_z orbital newvel advance. */
+int fargo_profile_report(fargo_ctx* c, char* buf, size_t len);
+
 /* Message for the last error of `c` (or of the last failed fargo_init on this thread when c == NULL). */
 const char* fargo_last_error(const fargo_ctx* c);
 

@@ -20,7 +20,7 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
           "SWEEP_X", "SWEEP_Y", "SWEEP_Z", "ORB_FRAC", "ORB_SHIFT", "NEWVEL"]
 EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
-           "fargo_get_array", "fargo_last_error"]
+           "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report"]
 
 
 class FargoMesh(C.Structure):
@@ -70,6 +70,8 @@ def load():
     L.fargo_step_until.argtypes = [vp, C.c_int]
     L.fargo_dims.argtypes = [vp] + [C.POINTER(C.c_int)] * 6
     L.fargo_get_array.argtypes = [vp, C.c_char_p, vp]
+    L.fargo_profile.argtypes = [vp, C.c_int]
+    L.fargo_profile_report.argtypes = [vp, C.c_char_p, C.c_size_t]
     L.fargo_last_error.argtypes = [vp]
     L.fargo_last_error.restype = C.c_char_p
     _lib = L
@@ -203,6 +205,20 @@ class Fargo:
 
     def kernel_launches(self) -> int:
         return int(load().fargo_kernel_launches(self._h))
+
+    # -- measurement -------------------------------------------------------------------------------
+    def profile(self, enable: bool = True):
+        self._check(load().fargo_profile(self._h, 1 if enable else 0), "fargo_profile")
+
+    def profile_report(self) -> dict:
+        """{launcher name: (kernel launches, total ms)} since profile(True), CUDA-event timed on the stream."""
+        buf = C.create_string_buffer(1 << 14)
+        self._check(load().fargo_profile_report(self._h, buf, len(buf)), "fargo_profile_report")
+        out = {}
+        for line in buf.value.decode().splitlines():
+            name, n, ms = line.split()
+            out[name] = (int(n), float(ms))
+        return out
 
     # -- inspection ----------------------------------------------------------------------------------
     def step_until(self, stage: str):

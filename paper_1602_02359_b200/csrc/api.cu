@@ -31,6 +31,8 @@ struct CtxBase {
   virtual int get_time(double*, double*, long long*) = 0;
   virtual int get_array(const char*, void*) = 0;
   virtual void dims(int*, int*, int*, int*, int*, int*) const = 0;
+  virtual int profile(int enable) = 0;
+  virtual int profile_report(char* buf, size_t len) = 0;
   long long launches = 0;
 };
 
@@ -100,11 +102,60 @@ struct Sim : CtxBase {
   int launches_per_step = 0;
   bool midstep = false, have_fields = false, pot_static = true, pot_valid = false;
   std::map<std::string, T*> dbg;
+  // per-kernel CUDA-event timing (fargo_profile): one event pair per launcher call, on the context's stream
+  struct Span { const char* name; cudaEvent_t a, b; int nk; };
+  bool prof = false;
+  std::vector<Span> spans;
   // transport plan
   int npass = 0, pass_kind[4];   // 0,1,2 = sweep direction, 3 = orbital
   int nq = 0, slots[8];
 
-  ~Sim() override { if (gexec) cudaGraphExecDestroy(gexec); }
+  ~Sim() override {
+    if (gexec) cudaGraphExecDestroy(gexec);
+    for (auto& sp : spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+  }
+
+  // run one launcher, bracketed by events when profiling
+  template <typename F> int timed(const char* name, F&& f) {
+    if (!prof) return f();
+    Span sp{name, nullptr, nullptr, 0};
+    cudaEventCreate(&sp.a); cudaEventCreate(&sp.b);
+    cudaEventRecord(sp.a, stream);
+    sp.nk = f();
+    cudaEventRecord(sp.b, stream);
+    spans.push_back(sp);
+    return sp.nk;
+  }
+
+  int profile(int enable) override {
+    for (auto& sp : spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+    spans.clear();
+    prof = enable != 0;
+    return FARGO_OK;
+  }
+
+  int profile_report(char* buf, size_t len) override {
+    if (!buf || len == 0) { err = "null buffer"; return FARGO_EINVAL; }
+    if (!ck(cudaStreamSynchronize(stream), "profile sync")) return FARGO_ECUDA;
+    std::map<std::string, std::pair<long long, double>> acc;   // name -> (kernel launches, total ms)
+    std::vector<std::string> order;
+    for (auto& sp : spans) {
+      float ms = 0.f;
+      if (!ck(cudaEventElapsedTime(&ms, sp.a, sp.b), "cudaEventElapsedTime")) return FARGO_ECUDA;
+      if (!acc.count(sp.name)) order.push_back(sp.name);
+      acc[sp.name].first += sp.nk;
+      acc[sp.name].second += ms;
+    }
+    std::string out;
+    char line[160];
+    for (auto& nm : order) {
+      snprintf(line, sizeof line, "%s %lld %.6f\n", nm.c_str(), acc[nm].first, acc[nm].second);
+      out += line;
+    }
+    if (out.size() + 1 > len) { err = "profile buffer too small"; return FARGO_EINVAL; }
+    memcpy(buf, out.c_str(), out.size() + 1);
+    return FARGO_OK;
+  }
 
   bool ck(cudaError_t e, const char* what) {
     if (e == cudaSuccess) return true;
@@ -309,40 +360,40 @@ struct Sim : CtxBase {
     dbg.clear();
     dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
     dbg["phi"] = phi; dbg["v0"] = v0;
-    n += launch_bc<T>(d, st, field_mask(true, true), stream);                        // cell 2
+    n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(true, true), stream); });                        // cell 2
     if (until == FARGO_ST_BC1) return n;
-    if (L.fargo) n += launch_vmean<T>(d, st.vx, v0, stream);                         // cell 3
+    if (L.fargo) n += timed("vmean", [&] { return launch_vmean<T>(d, st.vx, v0, stream); });                         // cell 3
     if (until == FARGO_ST_VMEAN) return n;
     if (L.has_pot && (!pot_valid || !pot_static)) {                                  // cell 5
       double t = 0.0;
       if (!pot_static && !capturing) { get_time(&t, nullptr, nullptr); }
-      n += potential(t);
+      n += timed("potential", [&] { return potential(t); });
       pot_valid = true;
     }
     if (until == FARGO_ST_POT) return n;
     const T* v0p = L.fargo ? v0 : nullptr;
-    n += launch_dt<T>(d, st, v0p, stream);                                           // cell 6
+    n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream); });                                           // cell 6
     if (until == FARGO_ST_DT) return n;
     // source step: intermediates live in transport set B (idle until the second pass)
     T *vxb = set_arr(1, 0), *vyb = set_arr(1, 1), *vzb = set_arr(1, 2), *ec = set_arr(1, 3);
-    n += launch_source_a<T>(d, st, phi, vxb, vyb, vzb, stream);                      // cell 7a
+    n += timed("source_a", [&] { return launch_source_a<T>(d, st, phi, vxb, vyb, vzb, stream); });                      // cell 7a
     dbg["vxb"] = vxb; dbg["vyb"] = vyb; dbg["vzb"] = vzb;
     if (until == FARGO_ST_SRC_A) return n;
     T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
     if (L.visc) { vxc = set_arr(1, 4); vyc = set_arr(1, 5); }
-    n += launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream);        // cell 7b
+    n += timed("source_b", [&] { return launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream); });        // cell 7b
     dbg["vxc"] = vxc; dbg["vyc"] = vyc; dbg["vzc"] = vzc; dbg["ec"] = L.adi ? ec : st.e;
     dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
     if (until == FARGO_ST_SRC_B) return n;
-    if (L.adi) n += launch_source_c<T>(d, vxc, vyc, vzc, ec, st.e, stream);          // cell 7c
+    if (L.adi) n += timed("source_c", [&] { return launch_source_c<T>(d, vxc, vyc, vzc, ec, st.e, stream); });          // cell 7c
     dbg["ed"] = st.e;
     if (until == FARGO_ST_SRC_C) return n;
     if (L.visc)                                                                      // cell 7d
-      n += launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream);
+      n += timed("source_d", [&] { return launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream); });
     dbg["vxd"] = st.vx; dbg["vyd"] = st.vy;
     dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
     if (until == FARGO_ST_SRC_D) return n;
-    n += launch_bc<T>(d, st, field_mask(false, L.adi), stream);                      // cell 9
+    n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(false, L.adi), stream); });                      // cell 9
     if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
     // transport: pass p reads set (p-1)%2 (the state on the first pass) and writes set p%2; the last pass
     // writes rho and e straight back into the state arrays, so one update leaves every array where it
@@ -364,8 +415,9 @@ struct Sim : CtxBase {
         a.sq[q] = first ? nullptr : set_arr(ss, slots[q]);
         a.dq[q] = (to_state && slots[q] == 0) ? st.e : set_arr(ds, slots[q]);
       }
-      if (pass_kind[p] == 3) n += launch_orbital<T>(d, a, nshift, stream);
-      else n += launch_sweep<T>(d, a, pass_kind[p], stream);
+      static const char* pnames[4] = {"sweep_x", "sweep_y", "sweep_z", "orbital"};
+      if (pass_kind[p] == 3) n += timed(pnames[3], [&] { return launch_orbital<T>(d, a, nshift, stream); });
+      else n += timed(pnames[pass_kind[p]], [&] { return launch_sweep<T>(d, a, pass_kind[p], stream); });
       static const char* names[7] = {"te", "pxm", "pxp", "pym", "pyp", "pzm", "pzp"};
       dbg["trho"] = a.drho;
       for (int q = 0; q < nq; ++q) dbg[names[slots[q]]] = a.dq[q];
@@ -382,8 +434,8 @@ struct Sim : CtxBase {
     QSet<T> S;
     S.rho = st.rho;
     for (int q = 0; q < 7; ++q) S.q[q] = set_arr(ls, q);
-    n += launch_newvel<T>(d, st.rho, S, st, stream);                                 // cell 12d
-    n += launch_advance(ctl, prm.t_stop, stream);
+    n += timed("newvel", [&] { return launch_newvel<T>(d, st.rho, S, st, stream); });                                 // cell 12d
+    n += timed("advance", [&] { return launch_advance(ctl, prm.t_stop, stream); });
     return n;
   }
 
@@ -393,7 +445,7 @@ struct Sim : CtxBase {
     if (nsteps < 0) { err = "negative step count"; return FARGO_EINVAL; }
     if (nsteps == 0) return FARGO_OK;
     // the legacy default stream cannot be captured: plain launches there
-    const bool graph_ok = prm.use_graph && pot_static && stream != nullptr;
+    const bool graph_ok = prm.use_graph && pot_static && stream != nullptr && !prof;
     int s = 0;
     if (graph_ok) {
       if (!gexec) {
@@ -514,6 +566,8 @@ int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy
   return FARGO_OK;
 }
 int fargo_get_array(fargo_ctx* c, const char* name, void* out) { return c ? c->impl->get_array(name, out) : FARGO_EINVAL; }
+int fargo_profile(fargo_ctx* c, int enable) { return c ? c->impl->profile(enable) : FARGO_EINVAL; }
+int fargo_profile_report(fargo_ctx* c, char* buf, size_t len) { return c ? c->impl->profile_report(buf, len) : FARGO_EINVAL; }
 const char* fargo_last_error(const fargo_ctx* c) { return c ? c->impl->err.c_str() : fg::g_init_error.c_str(); }
 
 }  // extern "C"

@@ -398,13 +398,19 @@ struct Sim : CtxBase {
     // transport: pass p reads set (p-1)%2 (the state on the first pass) and writes set p%2; the last pass
     // writes rho and e straight back into the state arrays, so one update leaves every array where it
     // started and the same captured graph serves every update.
+    if (!L.hasx) {   // no X sweep to fuse 12a into: store the momenta once, in the set the first pass reads
+      QSet<T> S;
+      S.rho = nullptr;
+      for (int q = 0; q < 7; ++q) S.q[q] = set_arr(1, q);
+      n += timed("momenta", [&] { return launch_momenta<T>(d, st, S, stream); });
+    }
     for (int p = 0; p < npass; ++p) {
       const bool first = p == 0, last = p == npass - 1;
       const int ds = p % 2, ss = 1 - ds;
       SweepArgs<T> a;
       memset(&a, 0, sizeof a);
       a.st = st;
-      a.first = first ? 1 : 0;
+      a.first = (first && L.hasx) ? 1 : 0;   // 12a fused into the X sweep
       a.v0 = (pass_kind[p] == 0 || pass_kind[p] == 3) ? v0p : nullptr;
       a.nq = nq;
       const bool to_state = last && !first;
@@ -412,7 +418,8 @@ struct Sim : CtxBase {
       a.drho = to_state ? st.rho : set_arr(ds, -1);
       for (int q = 0; q < nq; ++q) {
         a.slot[q] = slots[q];
-        a.sq[q] = first ? nullptr : set_arr(ss, slots[q]);
+        if (first) a.sq[q] = L.hasx ? nullptr : (slots[q] == 0 ? st.e : set_arr(1, slots[q]));
+        else a.sq[q] = set_arr(ss, slots[q]);
         a.dq[q] = (to_state && slots[q] == 0) ? st.e : set_arr(ds, slots[q]);
       }
       static const char* pnames[4] = {"sweep_x", "sweep_y", "sweep_z", "orbital"};

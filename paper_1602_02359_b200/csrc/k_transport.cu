@@ -7,19 +7,16 @@
 //
 // One sweep = ONE kernel: divide-by-rho, slope, star value, flux and update of rho and of every
 // transported quantity are fused, so each field is read once and written once per direction
-// (the paper runs ~4 kernels per field per direction).  A thread block owns a tile of
-// BM cells along the sweep axis (2 halo cells per side, recomputed) by BX cells along X; cell values,
-// slopes and fluxes are exchanged between neighbouring threads through shared memory.
+// (the paper runs ~4 kernels per field per direction).  No shared memory, no barriers:
+//   X sweep  : one lane per cell, a warp owns 32 consecutive cells of a row (2 halo cells per side,
+//              recomputed); neighbours' values, slopes and fluxes travel by warp shuffles.  On the
+//              first pass the momenta are formed from the state in registers (12a fused).
+//   Y/Z sweep: one thread per (i, line) marches along the sweep axis with a three-cell register
+//              window; threads of a warp sit side by side along X, so every load and store is a
+//              coalesced row segment.  The next row is loaded while the current one is reduced.
 #include "kernels.h"
 
 namespace fg {
-
-constexpr int QB = 4;   // quantities processed together (shared memory = 3 * QB * tile * sizeof(T))
-
-template <int DIR> struct Tile;
-template <> struct Tile<0> { static constexpr int BX = 1, BM = 256; };
-template <> struct Tile<1> { static constexpr int BX = 16, BM = 32; };
-template <> struct Tile<2> { static constexpr int BX = 16, BM = 32; };
 
 // van Leer slope per unit length; zero unless both one-sided differences have the same sign (reading G4)
 template <typename T>
@@ -33,199 +30,270 @@ __device__ __forceinline__ T vl_slope(const T fm, const T f0, const T fp, const 
   return flat ? T(0) : a;
 }
 
-template <typename T, int DIR>
-__global__ void __launch_bounds__(Tile<DIR>::BX * Tile<DIR>::BM)
-k_sweep(const Dev<T> d, const SweepArgs<T> A) {
-  constexpr int BX = Tile<DIR>::BX, BM = Tile<DIR>::BM, NT = BX * BM, INNER = BM - 4;
+template <typename T> __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <typename T> __device__ __forceinline__ T shfl_dn1(T v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+// ---- 12a alone: only when X is absent, so that the first sweep (Y or Z) can read a stored set ----------
+template <typename T>
+__global__ void __launch_bounds__(128) k_momenta(const Dev<T> d, const State<T> st, const QSet<T> S) {
   if (d.ctl->done) return;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* const sf = reinterpret_cast<T*>(smem_raw);   // [QB][NT] cell values q
-  T* const sa = sf + QB * NT;                     // [QB][NT] slopes
-  T* const sF = sa + QB * NT;                     // [QB][NT] fluxes through the lower face
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= d.TX) return;
+  const long long l = d.id(i, j, k);
+  const T r0 = st.rho[l], rz = d.Rzj[j];
+  if (d.hasy) {
+    const T v = st.vy[l];
+    const T vp = j + 1 < d.TY ? st.vy[l + d.pitch] : v;
+    S.q[3][l] = r0 * v;
+    S.q[4][l] = r0 * vp;
+  }
+  if (d.hasz) {
+    const T v = st.vz[l];
+    const T vp = k + 1 < d.TZ ? st.vz[l + d.plane] : v;
+    S.q[5][l] = r0 * (rz * v);
+    S.q[6][l] = r0 * (rz * vp);
+  }
+}
 
-  const int tx = DIR == 0 ? 0 : threadIdx.x;
-  const int tm = DIR == 0 ? threadIdx.x : threadIdx.y;
-  const int sidx = tm * BX + tx;
-  const int T_line = DIR == 0 ? d.TX : DIR == 1 ? d.TY : d.TZ;
-  const bool wrap = DIR == 0 && d.xwrap;
+template <typename T>
+int launch_momenta(const Dev<T>& d, const State<T>& st, const QSet<T>& S, cudaStream_t s) {
+  dim3 b(128), g((d.TX + 127) / 128, d.TY, d.TZ);
+  k_momenta<T><<<g, b, 0, s>>>(d, st, S);
+  return 1;
+}
 
-  // position of this thread's cell: m along the sweep axis (wrapped in a periodic X), line (i | j, k)
-  const int m_unwrapped = (DIR == 0 ? blockIdx.x : blockIdx.y) * INNER - 2 + tm;
-  int m = m_unwrapped;
-  if (wrap) { m %= d.nx; if (m < 0) m += d.nx; }
-  int i, j, k;
-  if (DIR == 0) { i = m; j = blockIdx.y; k = blockIdx.z; }
-  else if (DIR == 1) { i = blockIdx.x * BX + tx; j = m; k = blockIdx.z; }
-  else { i = blockIdx.x * BX + tx; j = blockIdx.z; k = m; }
-  const bool valid = (m >= 0 && m < T_line) && (i < d.TX);
-  // cells this thread writes: the tile's interior, once (the last X tile may run past the row)
-  const bool inner = valid && tm >= 2 && tm < BM - 2 && m_unwrapped < T_line;
-  const bool upd = inner && (wrap || (m >= 2 && m < T_line - 2));   // cells the sweep updates; others pass through
+// ---- X sweep ------------------------------------------------------------------------------------------
+constexpr int XW = 8;         // warps (rows) per block
+constexpr int XIN = 28;       // interior cells per warp
+
+template <typename T, int NQ, bool FIRST>
+__global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const SweepArgs<T> A) {
+  if (d.ctl->done) return;
+  const int lane = threadIdx.x;
+  const int j = blockIdx.y * XW + threadIdx.y, k = blockIdx.z;
+  if (j >= d.TY) return;   // whole warps leave together
+  const bool wrap = d.xwrap != 0;
+  const int iu = blockIdx.x * XIN - 2 + lane;   // un-wrapped cell index
+  int i = iu;
+  if (wrap) { i %= d.nx; if (i < 0) i += d.nx; }
+  const bool valid = i >= 0 && i < d.TX;
+  const bool inner = valid && lane >= 2 && lane < 30 && iu < d.TX;
+  const bool upd = inner && (wrap || (i >= 2 && i < d.TX - 2));
 
   const T dt = (T)d.ctl->dt;
-  long long l = 0;
-  T w = T(0), r0 = T(1), ir = T(1), Sm = T(0), dtiv = T(0), invd0 = T(0), invdp = T(0), hup = T(0), hdn = T(0);
+  const T len = d.LX(j, k), invd = d.invLX(j, k), Sm = d.Sx(j, k), dtiv = dt * d.invV(j, k);
+  const long long l = valid ? d.id(i, j, k) : d.id(0, j, k);
+
+  T Q[NQ], r0 = T(1), w = T(0);
   if (valid) {
-    l = d.id(i, j, k);
-    T len0, lenm;
-    if (DIR == 0) {
-      len0 = lenm = d.LX(j, k);
-      invd0 = invdp = d.invLX(j, k);
-      Sm = d.Sx(j, k);
-      w = A.st.vx[l];
-      if (A.v0) w = w - A.v0[d.rid(j, k)];   // residual velocity under orbital advection
-    } else if (DIR == 1) {
-      const int jm = j > 0 ? j - 1 : 0, jp = j + 1 < d.TY ? j + 1 : j;
-      len0 = d.LY[j]; lenm = d.LY[jm];
-      invd0 = d.invDY[j]; invdp = d.invDY[jp];
-      Sm = d.Sy(j, k);
-      w = A.st.vy[l];
-    } else {
-      const int km = k > 0 ? k - 1 : 0, kp = k + 1 < d.TZ ? k + 1 : k;
-      len0 = d.LZ(j, k); lenm = d.LZ(j, km);
-      invd0 = d.invDZ(j, k); invdp = d.invDZ(j, kp);
-      Sm = d.Sz(j, k);
-      w = A.st.vz[l];
-    }
-    dtiv = dt * d.invV(j, k);
-    const T wdt = w * dt;
-    hup = (lenm - wdt) * T(0.5);   // Eq. 48, upwind cell m-1
-    hdn = (len0 + wdt) * T(0.5);   // Eq. 48, upwind cell m
     r0 = A.srho[l];
-    ir = T(1) / r0;
+    w = A.st.vx[l];
   }
-  const bool up = w >= T(0);   // reading G3: ties go to the first branch
-
-  // momenta of Tab. 2 from the state (12a), only on the first pass
-  T mom[7] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
-  if (A.first && valid) {
-    const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, rz = d.Rzj[j];
-    mom[0] = d.eos == EOS_ADI ? A.st.e[l] : T(0);
-    if (d.hasx) {
-      const T v = A.st.vx[l];
-      const bool ipok = d.xwrap || i + 1 < d.TX;
-      const T vp = ipok ? A.st.vx[d.id(d.xw(i + 1), j, k)] : v;
-      mom[1] = r0 * (rx * v + rx2om);
-      mom[2] = r0 * (rx * vp + rx2om);
+  if (FIRST) {
+    // momenta of Tab. 2 from the state (12a)
+    T mom[7] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    T wp = shfl_dn1(w);
+    if (valid) {
+      if (lane == 31) wp = (d.xwrap || i + 1 < d.TX) ? A.st.vx[d.id(d.xw(i + 1), j, k)] : w;
+      else if (!d.xwrap && i + 1 >= d.TX) wp = w;
+      const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, rz = d.Rzj[j];
+      if (d.eos == EOS_ADI) mom[0] = A.st.e[l];
+      mom[1] = r0 * (rx * w + rx2om);
+      mom[2] = r0 * (rx * wp + rx2om);
+      if (d.hasy) {
+        const T v = A.st.vy[l];
+        const T vp = j + 1 < d.TY ? A.st.vy[l + d.pitch] : v;
+        mom[3] = r0 * v;
+        mom[4] = r0 * vp;
+      }
+      if (d.hasz) {
+        const T v = A.st.vz[l];
+        const T vp = k + 1 < d.TZ ? A.st.vz[l + d.plane] : v;
+        mom[5] = r0 * (rz * v);
+        mom[6] = r0 * (rz * vp);
+      }
     }
-    if (d.hasy) {
-      const T v = A.st.vy[l];
-      const T vp = j + 1 < d.TY ? A.st.vy[l + d.pitch] : v;
-      mom[3] = r0 * v;
-      mom[4] = r0 * vp;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+      const int sl = A.slot[q];
+      T v = mom[0];
+#pragma unroll
+      for (int s = 1; s < 7; ++s) v = (sl == s) ? mom[s] : v;
+      Q[q] = v;
     }
-    if (d.hasz) {
-      const T v = A.st.vz[l];
-      const T vp = k + 1 < d.TZ ? A.st.vz[l + d.plane] : v;
-      mom[5] = r0 * (rz * v);
-      mom[6] = r0 * (rz * vp);
-    }
+  } else {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) Q[q] = valid ? A.sq[q][l] : T(0);
   }
+  if (A.v0) w = w - A.v0[d.rid(j, k)];   // residual velocity under orbital advection
+  const bool up = w >= T(0);              // reading G3: ties go to the first branch
+  const T wdt = w * dt;
+  const T hup = (len - wdt) * T(0.5), hdn = (len + wdt) * T(0.5);   // Eq. 48
+  const T ir = T(1) / r0;
 
-  // ---- density first: its mass flux F = w rho* S multiplies every other star value ----------------
-  T Fr0;   // mass flux through this cell's lower face
+  // density: its mass flux F = w rho* S multiplies every other star value
+  T Fr;
   {
-    sf[sidx] = r0;
-    __syncthreads();
-    T a = T(0);
-    if (tm >= 1 && tm < BM - 1) a = vl_slope(sf[sidx - BX], r0, sf[sidx + BX], invd0, invdp);
-    sa[sidx] = a;
-    __syncthreads();
-    T rs = r0;
-    if (tm >= 1) rs = up ? sf[sidx - BX] + sa[sidx - BX] * hup : r0 - a * hdn;
-    Fr0 = (w * rs) * Sm;
-    sF[sidx] = Fr0;
-    __syncthreads();
-    if (inner) {
-      T* out = A.drho;
-      out[l] = upd ? r0 - dtiv * (sF[sidx + BX] - Fr0) : r0;
-    }
+    const T fm = shfl_up1(r0), fp = shfl_dn1(r0);
+    const T a = vl_slope(fm, r0, fp, invd, invd);
+    const T am = shfl_up1(a);
+    const T rs = up ? fm + am * hup : r0 - a * hdn;
+    Fr = (w * rs) * Sm;
+    const T Fp = shfl_dn1(Fr);
+    if (inner) A.drho[l] = upd ? r0 - dtiv * (Fp - Fr) : r0;
   }
-
-  // ---- the other quantities, QB at a time -------------------------------------------------------------
 #pragma unroll
-  for (int b0 = 0; b0 < 8; b0 += QB) {   // compile-time batch offsets: the pointer lists stay in the parameter bank
-    if (b0 >= A.nq) break;
-    T Q[QB], f[QB], a[QB], FQ[QB];
-#pragma unroll
-    for (int u = 0; u < QB; ++u) {
-      Q[u] = T(0);
-      if (b0 + u < A.nq && valid) {
-        const int sl = A.slot[b0 + u];
-        if (A.first) {
-          // select from the small per-thread momentum set without dynamic register indexing
-          T v = mom[0];
-#pragma unroll
-          for (int s = 1; s < 7; ++s) v = (sl == s) ? mom[s] : v;
-          Q[u] = v;
-        } else {
-          Q[u] = A.sq[b0 + u][l];
-        }
-      }
-      f[u] = Q[u] * ir;
-    }
-    __syncthreads();   // previous batch has finished reading sf / sa / sF
-#pragma unroll
-    for (int u = 0; u < QB; ++u) sf[u * NT + sidx] = f[u];
-    __syncthreads();
-#pragma unroll
-    for (int u = 0; u < QB; ++u) {
-      a[u] = T(0);
-      if (tm >= 1 && tm < BM - 1) a[u] = vl_slope(sf[u * NT + sidx - BX], f[u], sf[u * NT + sidx + BX], invd0, invdp);
-      sa[u * NT + sidx] = a[u];
-    }
-    __syncthreads();
-#pragma unroll
-    for (int u = 0; u < QB; ++u) {
-      T fs = f[u];
-      if (tm >= 1) fs = up ? sf[u * NT + sidx - BX] + sa[u * NT + sidx - BX] * hup : f[u] - a[u] * hdn;
-      FQ[u] = Fr0 * fs;
-      sF[u * NT + sidx] = FQ[u];
-    }
-    __syncthreads();
-    if (inner) {
-#pragma unroll
-      for (int u = 0; u < QB; ++u) {
-        if (b0 + u < A.nq) {
-          T* out = A.dq[b0 + u];
-          out[l] = upd ? Q[u] - dtiv * (sF[u * NT + sidx + BX] - FQ[u]) : Q[u];
-        }
-      }
-    }
+  for (int q = 0; q < NQ; ++q) {
+    const T f = Q[q] * ir;
+    const T fm = shfl_up1(f), fp = shfl_dn1(f);
+    const T a = vl_slope(fm, f, fp, invd, invd);
+    const T am = shfl_up1(a);
+    const T fs = up ? fm + am * hup : f - a * hdn;
+    const T F = Fr * fs;
+    const T Fp = shfl_dn1(F);
+    if (inner) A.dq[q][l] = upd ? Q[q] - dtiv * (Fp - F) : Q[q];
   }
 }
 
-template <typename T, int DIR>
-static size_t sweep_smem() { return (size_t)3 * QB * Tile<DIR>::BX * Tile<DIR>::BM * sizeof(T); }
+// ---- Y / Z sweep: register marching -----------------------------------------------------------------------
+constexpr int MTHREADS = 128;
 
-// Opt in to more than 48 KB of dynamic shared memory; called once per context, outside graph capture.
-template <typename T>
-void sweep_setup() {
-  cudaFuncSetAttribute(k_sweep<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<T, 0>());
-  cudaFuncSetAttribute(k_sweep<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<T, 1>());
-  cudaFuncSetAttribute(k_sweep<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<T, 2>());
-  cudaGetLastError();
+template <typename T, int DIR, int NQ>
+__global__ void __launch_bounds__(MTHREADS) k_sweep_march(const Dev<T> d, const SweepArgs<T> A, const int CH) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * MTHREADS + threadIdx.x;
+  if (i >= d.TX) return;
+  const int line = blockIdx.y;                       // k for the Y sweep, j for the Z sweep
+  const int TL = DIR == 1 ? d.TY : d.TZ;
+  const int c0 = blockIdx.z * CH, c1 = (c0 + CH < TL) ? c0 + CH : TL;   // cells this thread writes: [c0, c1)
+  const long long str = DIR == 1 ? d.pitch : d.plane;
+  const long long base = DIR == 1 ? d.id(i, 0, line) : d.id(i, line, 0);
+  const T* __restrict__ vel = DIR == 1 ? A.st.vy : A.st.vz;
+  const T dt = (T)d.ctl->dt;
+  // per-line geometry factors (Tab. 5 products)
+  const T gS = DIR == 1 ? d.syk[line] : d.szj[line];          // S = s^j s^k
+  const T gV = DIR == 1 ? d.inv_syk[line] : d.invVj[line];    // 1/V = invVj / syk
+  const T gL = DIR == 1 ? T(1) : d.Rzj[line];                 // LZ = dz R_z
+  const T gD = DIR == 1 ? T(1) : d.invRzj[line];
+  const T* __restrict__ tS = DIR == 1 ? d.syj : d.szk;
+  const T* __restrict__ tV = DIR == 1 ? d.invVj : d.inv_syk;
+  const T* __restrict__ tL = DIR == 1 ? d.LY : d.dz;
+  const T* __restrict__ tD = DIR == 1 ? d.invDY : d.invdzc;
+
+  // window: suffix 2 = cell r-2, 1 = cell r-1, 0 = cell r (just arrived), n = cell r+1 (in flight)
+  T Q2[NQ + 1], Q1[NQ + 1], f2[NQ + 1], f1[NQ + 1], a2[NQ + 1], F2[NQ + 1];
+#pragma unroll
+  for (int q = 0; q <= NQ; ++q) { Q2[q] = Q1[q] = f2[q] = f1[q] = a2[q] = F2[q] = T(0); }
+  T len2 = T(0), len1 = T(0), invd1 = T(0), w1 = T(0), S1 = T(0), dtiv2 = T(0), dtiv1 = T(0);
+
+  T Qn[NQ + 1], wn = T(0);
+  auto load_row = [&](const int r) {
+    if (r >= 0 && r < TL) {
+      const long long l = base + (long long)r * str;
+      Qn[NQ] = A.srho[l];
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) Qn[q] = A.sq[q][l];
+      wn = vel[l];
+    } else {
+      Qn[NQ] = T(1);
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) Qn[q] = T(0);
+      wn = T(0);
+    }
+  };
+  load_row(c0 - 2);
+#pragma unroll 1
+  for (int r = c0 - 2; r < c1 + 2; ++r) {
+    // row r has arrived in Qn; start the loads of row r+1 at once
+    T Q0[NQ + 1], f0[NQ + 1];
+#pragma unroll
+    for (int q = 0; q <= NQ; ++q) Q0[q] = Qn[q];
+    const T w0 = wn;
+    if (r + 1 < c1 + 2) load_row(r + 1);
+    const int rc = r < 0 ? 0 : (r >= TL ? TL - 1 : r);
+    const T len0 = DIR == 1 ? tL[rc] : tL[rc] * gL;
+    const T invd0 = DIR == 1 ? tD[rc] : tD[rc] * gD;
+    const T S0 = DIR == 1 ? tS[rc] * gS : gS * tS[rc];
+    const T dtiv0 = dt * (DIR == 1 ? tV[rc] * gV : gV * tV[rc]);
+    const T ir = T(1) / Q0[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) f0[q] = Q0[q] * ir;
+    f0[NQ] = Q0[NQ];
+    const int s = r - c0;   // stage of the pipeline (uniform over the block)
+    T a1[NQ + 1], F1[NQ + 1];
+#pragma unroll
+    for (int q = 0; q <= NQ; ++q) { a1[q] = T(0); F1[q] = T(0); }
+    if (s >= 0) {   // slopes of cell r-1
+#pragma unroll
+      for (int q = 0; q <= NQ; ++q) a1[q] = vl_slope(f2[q], f1[q], f0[q], invd1, invd0);
+    }
+    if (s >= 1) {   // fluxes through the lower face of cell r-1 (Eq. 48, Eqs. 45-47)
+      const bool up = w1 >= T(0);
+      const T wdt = w1 * dt;
+      const T hup = (len2 - wdt) * T(0.5), hdn = (len1 + wdt) * T(0.5);
+      const T rs = up ? f2[NQ] + a2[NQ] * hup : f1[NQ] - a1[NQ] * hdn;
+      const T Fr = (w1 * rs) * S1;
+      F1[NQ] = Fr;
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) {
+        const T fs = up ? f2[q] + a2[q] * hup : f1[q] - a1[q] * hdn;
+        F1[q] = Fr * fs;
+      }
+    }
+    if (s >= 2) {   // update (or pass through) cell r-2
+      const int m = r - 2;
+      const bool upd = m >= 2 && m < TL - 2;
+      const long long l = base + (long long)m * str;
+      A.drho[l] = upd ? Q2[NQ] - dtiv2 * (F1[NQ] - F2[NQ]) : Q2[NQ];
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) A.dq[q][l] = upd ? Q2[q] - dtiv2 * (F1[q] - F2[q]) : Q2[q];
+    }
+#pragma unroll
+    for (int q = 0; q <= NQ; ++q) { Q2[q] = Q1[q]; Q1[q] = Q0[q]; f2[q] = f1[q]; f1[q] = f0[q]; a2[q] = a1[q]; F2[q] = F1[q]; }
+    len2 = len1; len1 = len0; invd1 = invd0; w1 = w0; S1 = S0; dtiv2 = dtiv1; dtiv1 = dtiv0;
+  }
 }
-template void sweep_setup<double>();
-template void sweep_setup<float>();
 
-template <typename T, int DIR>
-static int launch_sweep_dir(const Dev<T>& d, const SweepArgs<T>& a, cudaStream_t s) {
-  constexpr int BX = Tile<DIR>::BX, BM = Tile<DIR>::BM, INNER = BM - 4;
-  dim3 b, g;
-  if (DIR == 0) { b = dim3(BM); g = dim3((d.TX + INNER - 1) / INNER, d.TY, d.TZ); }
-  else if (DIR == 1) { b = dim3(BX, BM); g = dim3((d.TX + BX - 1) / BX, (d.TY + INNER - 1) / INNER, d.TZ); }
-  else { b = dim3(BX, BM); g = dim3((d.TX + BX - 1) / BX, (d.TZ + INNER - 1) / INNER, d.TY); }
-  k_sweep<T, DIR><<<g, b, sweep_smem<T, DIR>(), s>>>(d, a);
+template <typename T, int NQ>
+static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s) {
+  if (dir == 0) {
+    dim3 b(32, XW), g((d.TX + XIN - 1) / XIN, (d.TY + XW - 1) / XW, d.TZ);
+    if (a.first) k_sweep_x<T, NQ, true><<<g, b, 0, s>>>(d, a);
+    else k_sweep_x<T, NQ, false><<<g, b, 0, s>>>(d, a);
+    return 1;
+  }
+  const int TL = dir == 1 ? d.TY : d.TZ, lines = dir == 1 ? d.TZ : d.TY;
+  // chunk the sweep axis so that the grid fills the machine a few times over, but keep chunks long
+  // (each one re-reads 4 rows of halo)
+  const long long cols = (long long)((d.TX + MTHREADS - 1) / MTHREADS) * lines;
+  int nch = (int)((148LL * 16 * 4 + cols - 1) / cols);
+  if (nch < 1) nch = 1;
+  int CH = (TL + nch - 1) / nch;
+  if (CH < 32) CH = 32;
+  if (CH > TL) CH = TL;
+  nch = (TL + CH - 1) / CH;
+  dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);
+  if (dir == 1) k_sweep_march<T, 1, NQ><<<g, b, 0, s>>>(d, a, CH);
+  else k_sweep_march<T, 2, NQ><<<g, b, 0, s>>>(d, a, CH);
   return 1;
 }
 
 template <typename T>
 int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s) {
-  if (dir == 0) return launch_sweep_dir<T, 0>(d, a, s);
-  if (dir == 1) return launch_sweep_dir<T, 1>(d, a, s);
-  return launch_sweep_dir<T, 2>(d, a, s);
+  switch (a.nq) {
+    case 2: return launch_sweep_nq<T, 2>(d, a, dir, s);
+    case 3: return launch_sweep_nq<T, 3>(d, a, dir, s);
+    case 4: return launch_sweep_nq<T, 4>(d, a, dir, s);
+    case 5: return launch_sweep_nq<T, 5>(d, a, dir, s);
+    case 6: return launch_sweep_nq<T, 6>(d, a, dir, s);
+    case 7: return launch_sweep_nq<T, 7>(d, a, dir, s);
+    default: return 0;
+  }
 }
+
+template <typename T> void sweep_setup() {}
+template void sweep_setup<double>();
+template void sweep_setup<float>();
 
 // ---- 12d: new velocities from the transported left/right momenta (Eq. 51), active cells ----------------
 template <typename T>
@@ -260,6 +328,7 @@ int launch_newvel(const Dev<T>& d, const T* rho, const QSet<T>& set, const State
 }
 
 #define INST(T)                                                                                    \
+  template int launch_momenta<T>(const Dev<T>&, const State<T>&, const QSet<T>&, cudaStream_t);   \
   template int launch_sweep<T>(const Dev<T>&, const SweepArgs<T>&, int, cudaStream_t);             \
   template int launch_newvel<T>(const Dev<T>&, const T*, const QSet<T>&, const State<T>&, cudaStream_t);
 INST(double)

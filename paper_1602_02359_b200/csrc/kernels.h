@@ -43,6 +43,8 @@ template <typename T> struct SweepArgs {
   int first;
 };
 template <typename T> int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s);
+// cell 12a alone (only when X is absent): momenta of the Y and Z directions into S.q[3..6]
+template <typename T> int launch_momenta(const Dev<T>& d, const State<T>& st, const QSet<T>& S, cudaStream_t s);
 // orbital advection: PPA fractional sweep (Eq. 70) with the integer shift (Eq. 69) folded into the store index
 template <typename T> int launch_orbital(const Dev<T>& d, const SweepArgs<T>& a, T* nshift_out, cudaStream_t s);
 // cell 12d: Eq. 51; then the clock advances

@@ -157,6 +157,30 @@ def measured_peak():
         return 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
 
 
+# ---------------------------------------------------------------------------------- ranks -----------
+def rank_barrier(world: int):
+    """Barrier over the process group (no-op for one process)."""
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def rank_max(ms: float, world: int, device: str) -> float:
+    """Max over ranks of a device-measured time: the slowest replica defines the job's time."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(cells_per_rank: int, steps: int, world: int, ms: float) -> float:
+    """Replicas only: every rank updates its own mesh, value = all cells / max time."""
+    return world * cells_per_rank * steps / (ms * 1e-3)
+
+
 # ---------------------------------------------------------------------------------- reference arm ---
 def oracle_rate(sample, steps, warmup):
     from oracle.binding import Oracle
@@ -207,16 +231,11 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        rank_barrier(world)
         torch.cuda.synchronize()
 
     def max_over_ranks(ms):
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return rank_max(ms, world, "cuda")
 
     w, sample, sample_desc = make_workload(args.workload)
     prec = 32 if args.fp32 else 64
@@ -242,7 +261,7 @@ def run_ours(args):
     clocks = sampler.stop()
     ms = max_over_ranks(e0.elapsed_time(e1))
     launches = g.kernel_launches() - l0
-    value = world * ncell * K / (ms * 1e-3)
+    value = whole_job_rate(ncell, K, world, ms)
 
     # ---- region 2: per-launcher CUDA-event timing (plain launches) ----
     g.profile(True)
@@ -301,7 +320,7 @@ def run_ours(args):
         barrier()
         ms_e2e = max_over_ranks(e4.elapsed_time(e5))
         nfield = sum(1 for a in host_in if a is not None)
-        e2e = {"value": world * ncell * ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nfield * ncell * es,
+        e2e = {"value": whole_job_rate(ncell, ke, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": nfield * ncell * es,
                "d2h_bytes_per_step": nfield * ncell * es, "steps": ke, "ms_per_step": ms_e2e / ke}
 
     # ---- CPU baseline: the oracle as it stands, one thread, bounded sample (rank 0, N = 1) ----

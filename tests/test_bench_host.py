@@ -1,0 +1,73 @@
+"""Host-side logic of bench.py for N > 1 ("replicas only"), on CPU with a world-size-2
+gloo group: max-over-ranks timing, whole-job aggregation, and the reference arm under a 2-rank launch
+(rank 0 alone runs and prints; the other rank exits 0 without work)."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+bench.rank_barrier(world)
+ms = bench.rank_max(10.0 + 5.0 * rank, world, "cpu")       # rank 1 is the slow replica
+rate = bench.whole_job_rate(1000, 4, world, ms)
+print("RESULT %d %.6f %.6f" % (rank, ms, rate), flush=True)
+dist.destroy_process_group()
+"""
+
+
+def _torchrun(args, port):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port)] + args
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    return subprocess.run(cmd, cwd=ROOT, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, timeout=300)
+
+
+def test_max_over_ranks_and_whole_job_rate_gloo_world2(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT))
+    r = _torchrun([str(script)], 29611)
+    assert r.returncode == 0, r.stderr[-2000:]
+    res = sorted(ln.split()[1:] for ln in r.stdout.splitlines() if ln.startswith("RESULT"))
+    assert len(res) == 2
+    for rank, ms, rate in res:
+        assert float(ms) == 15.0                       # every rank sees the slowest replica's time
+        assert float(rate) == pytest.approx(2 * 1000 * 4 / 15e-3)
+
+
+def test_single_rank_helpers_need_no_process_group():
+    sys.path.insert(0, ROOT)
+    import bench
+    bench.rank_barrier(1)
+    assert bench.rank_max(3.5, 1, "cpu") == 3.5
+    assert bench.whole_job_rate(10, 2, 1, 4.0) == pytest.approx(5000.0)
+
+
+def test_reference_arm_two_ranks_prints_one_line():
+    r = _torchrun(["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--workload",
+                   "sound"], 29612)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    out = json.loads(lines[0])
+    assert out["impl"] == "reference" and out["n_gpus"] == 2 and out["value"] > 0
+    assert out["cpu_baseline"]["kind"] == "oracle" and out["e2e"]["h2d_bytes_per_step"] == 0
+    assert out["unit"] == "cell updates/s" and out["higher_is_better"] is True
+
+
+def test_algorithmic_bytes_match_design_table():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1602_02359_b200 import workloads as W
+    reals, fused = bench.algorithmic_reals(W.noise_box(shape3=(8, 8, 8)))
+    assert 8 * reals["first_sweep"] == 104 and 8 * reals["sweep"] == 136 and 8 * reals["newvel"] == 80
+    assert 8 * fused == 464                                   # SURVEY.md 8(d.3), 3-D adiabatic, no FARGO

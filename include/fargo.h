@@ -136,6 +136,12 @@ int fargo_profile(fargo_ctx* c, int enable);
  * source_d momenta sweep_x sweep_y sweep_z orbital newvel advance. */
 int fargo_profile_report(fargo_ctx* c, char* buf, size_t len);
 
+/* Self-test of the branch-free fp64 division the kernels use in place of a / b (csrc/common.cuh, rdiv;
+ * DESIGN.md "rounding"): out[n] = rdiv(a[n], b[n]) for n elements; a, b, out are DEVICE pointers to
+ * doubles, `cuda_stream` a cudaStream_t (NULL = default stream).  Synchronises before returning.
+ * Returns FARGO_OK or FARGO_ECUDA / FARGO_EINVAL (no context: message not retrievable). */
+int fargo_selftest_div(const double* a, const double* b, double* out, long long n, void* cuda_stream);
+
 /* Message for the last error of `c` (or of the last failed fargo_init on this thread when c == NULL). */
 const char* fargo_last_error(const fargo_ctx* c);
 

@@ -20,7 +20,7 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
           "SWEEP_X", "SWEEP_Y", "SWEEP_Z", "ORB_FRAC", "ORB_SHIFT", "NEWVEL"]
 EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
-           "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report"]
+           "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div"]
 
 
 class FargoMesh(C.Structure):
@@ -73,6 +73,8 @@ def load():
     L.fargo_profile.argtypes = [vp, C.c_int]
     L.fargo_profile_report.argtypes = [vp, C.c_char_p, C.c_size_t]
     L.fargo_last_error.argtypes = [vp]
+    L.fargo_selftest_div.argtypes = [vp, vp, vp, C.c_longlong, vp]
+    L.fargo_selftest_div.restype = C.c_int
     L.fargo_last_error.restype = C.c_char_p
     _lib = L
     return L
@@ -231,3 +233,16 @@ class Fargo:
         with self._torch.cuda.device(self.device):
             self._check(load().fargo_get_array(self._h, name.encode(), out.ctypes.data), "fargo_get_array")
         return out
+
+
+def selftest_div(a, b):
+    """out = rdiv(a, b) elementwise on the GPU (torch.float64 CUDA tensors): the kernels' division."""
+    import torch
+    assert a.is_cuda and b.is_cuda and a.dtype == torch.float64 and b.dtype == torch.float64 and a.numel() == b.numel()
+    a, b = a.contiguous(), b.contiguous()
+    out = torch.empty_like(a)
+    torch.cuda.synchronize()
+    rc = load().fargo_selftest_div(a.data_ptr(), b.data_ptr(), out.data_ptr(), a.numel(), None)
+    if rc != 0:
+        raise RuntimeError("fargo_selftest_div failed with code %d" % rc)
+    return out

@@ -183,6 +183,16 @@ int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s) {
   return 1;
 }
 
+__global__ void k_selftest_div(const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ out,
+                               const long long n) {
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x)
+    out[m] = rdiv(a[m], b[m]);
+}
+int launch_selftest_div(const double* a, const double* b, double* out, long long n, cudaStream_t s) {
+  k_selftest_div<<<148 * 8, 256, 0, s>>>(a, b, out, n);
+  return 1;
+}
+
 #define INST(T)                                                                              \
   template int launch_vmean<T>(const Dev<T>&, const T*, T*, cudaStream_t);                   \
   template int launch_potential<T>(const Dev<T>&, T*, T, T, T, T, T, cudaStream_t);          \

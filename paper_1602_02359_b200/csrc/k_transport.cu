@@ -26,7 +26,7 @@ __device__ __forceinline__ T vl_slope(const T fm, const T f0, const T fp, const 
   const T pr = dm * dp;
   const bool flat = pr <= T(0);
   const T den = flat ? T(1) : dm + dp;   // keeps the division on its fast path when the slope is dropped
-  const T a = (T(2) * pr) / den;
+  const T a = rdiv(T(2) * pr, den);
   return flat ? T(0) : a;
 }
 
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
   const bool up = w >= T(0);              // reading G3: ties go to the first branch
   const T wdt = w * dt;
   const T hup = (len - wdt) * T(0.5), hdn = (len + wdt) * T(0.5);   // Eq. 48
-  const T ir = T(1) / r0;
+  const T ir = rdiv(T(1), r0);
 
   // density: its mass flux F = w rho* S multiplies every other star value
   T Fr;
@@ -155,14 +155,183 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
   }
 }
 
-// ---- Y / Z sweep: register marching -----------------------------------------------------------------------
+// ---- X sweep, two cells per lane ---------------------------------------------------------------------------
+// A warp owns 64 consecutive cells of a row: lane L holds cells (t0 - 2 + 2L, +1) as one 16-byte vector
+// per array.  Lanes 0 and 31 are the two-cell halo (recomputed, never stored), so a tile advances by 60
+// cells.  Per quantity only four values cross lanes (f and the slope from the left, f and the flux from
+// the right); everything else stays in registers.  The quantity list is fixed at compile time
+// (e | pxm pxp | pym pyp | pzm pzp, Tab. 2) and the momenta are formed from the state on the fly (12a).
+// Needs an even nx when X wraps (a pair never straddles the seam); odd rings take k_sweep_x.
+template <typename T> struct Pair;
+template <> struct Pair<double> { using type = double2; };
+template <> struct Pair<float> { using type = float2; };
+
+constexpr int X2W = 4;          // warps (rows) per block
+constexpr int X2IN = 60;        // interior cells per warp
+
+template <typename T>
+__device__ __forceinline__ void ld_pair(const T* __restrict__ p, T& a, T& b) {
+  const typename Pair<T>::type v = *reinterpret_cast<const typename Pair<T>::type*>(p);
+  a = v.x; b = v.y;
+}
+template <typename T>
+__device__ __forceinline__ void st_pair(T* __restrict__ p, const T a, const T b) {
+  typename Pair<T>::type v; v.x = a; v.y = b;
+  *reinterpret_cast<typename Pair<T>::type*>(p) = v;
+}
+
+template <typename T, bool ADI, bool HASY, bool HASZ, bool WRAP>
+__global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const SweepArgs<T> A) {
+  constexpr int NQ = (ADI ? 1 : 0) + 2 + (HASY ? 2 : 0) + (HASZ ? 2 : 0);
+  if (d.ctl->done) return;
+  const int lane = threadIdx.x;
+  const int j = blockIdx.y * X2W + threadIdx.y, k = blockIdx.z;
+  if (j >= d.TY) return;   // whole warps leave together
+  const int iu = blockIdx.x * X2IN - 2 + 2 * lane;   // un-wrapped index of this lane's first cell
+  int i = iu;
+  bool have = true;
+  if (WRAP) { i %= d.nx; if (i < 0) i += d.nx; }
+  else have = iu >= 0 && iu < d.TX;   // the second cell of the pair may be row padding (never stored)
+  const long long row = d.id(0, j, k);
+  const long long l = row + (have ? i : 0);
+
+  const T dt = (T)d.ctl->dt;
+  const T len = d.LX(j, k), invd = d.invLX(j, k), Sm = d.Sx(j, k), dtiv = dt * d.invV(j, k);
+
+  // ---- loads: everything this lane needs, issued up front ----
+  T r[2] = {T(1), T(1)}, w[2] = {T(0), T(0)}, en[2] = {T(0), T(0)};
+  T vy0[2] = {T(0), T(0)}, vy1[2] = {T(0), T(0)}, vz0[2] = {T(0), T(0)}, vz1[2] = {T(0), T(0)};
+  if (have) {
+    ld_pair(A.srho + l, r[0], r[1]);
+    ld_pair(A.st.vx + l, w[0], w[1]);
+    if (ADI) ld_pair(A.st.e + l, en[0], en[1]);
+    if (HASY) {
+      ld_pair(A.st.vy + l, vy0[0], vy0[1]);
+      if (j + 1 < d.TY) ld_pair(A.st.vy + l + d.pitch, vy1[0], vy1[1]);
+      else { vy1[0] = vy0[0]; vy1[1] = vy0[1]; }
+    }
+    if (HASZ) {
+      ld_pair(A.st.vz + l, vz0[0], vz0[1]);
+      if (k + 1 < d.TZ) ld_pair(A.st.vz + l + d.plane, vz1[0], vz1[1]);
+      else { vz1[0] = vz0[0]; vz1[1] = vz0[1]; }
+    }
+  }
+  // velocity on the upper face of the pair's second cell: the right neighbour's first, one extra load on lane 31
+  T wn = shfl_dn1(w[0]);
+  if (lane == 31 && have) {
+    if (WRAP) { int ip = i + 2; if (ip >= d.nx) ip -= d.nx; wn = A.st.vx[row + ip]; }
+    else if (i + 2 < d.TX) wn = A.st.vx[row + i + 2];
+  }
+  if (!WRAP) {   // the last cell of a ghosted row has no upper neighbour: its own face value stands in
+    if (i + 2 >= d.TX) wn = w[1];
+    if (i + 1 >= d.TX) w[1] = w[0];
+  }
+
+  // ---- 12a: the momenta of Tab. 2 ----
+  T Q[NQ][2];
+  {
+    const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, rz = d.Rzj[j];
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const T wp = c == 0 ? w[1] : wn;
+      int q = 0;
+      if (ADI) Q[q++][c] = en[c];
+      Q[q++][c] = r[c] * (rx * w[c] + rx2om);
+      Q[q++][c] = r[c] * (rx * wp + rx2om);
+      if (HASY) { Q[q++][c] = r[c] * vy0[c]; Q[q++][c] = r[c] * vy1[c]; }
+      if (HASZ) { Q[q++][c] = r[c] * (rz * vz0[c]); Q[q++][c] = r[c] * (rz * vz1[c]); }
+    }
+  }
+  if (A.v0) { const T vm = A.v0[d.rid(j, k)]; w[0] = w[0] - vm; w[1] = w[1] - vm; }   // residual velocity
+  bool up[2];
+  T hup[2], hdn[2], ir[2];
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    up[c] = w[c] >= T(0);                 // reading G3
+    const T wdt = w[c] * dt;
+    hup[c] = (len - wdt) * T(0.5); hdn[c] = (len + wdt) * T(0.5);   // Eq. 48
+    ir[c] = rdiv(T(1), r[c]);
+  }
+  const bool store = lane >= 1 && lane <= 30 && (WRAP ? iu < d.nx : have);
+
+  // ---- density: its mass flux multiplies every other star value ----
+  T Fr[2];
+  {
+    const T fl = shfl_up1(r[1]), fr = shfl_dn1(r[0]);
+    const T a0 = vl_slope(fl, r[0], r[1], invd, invd);
+    const T a1 = vl_slope(r[0], r[1], fr, invd, invd);
+    const T al = shfl_up1(a1);
+    const T s0 = up[0] ? fl + al * hup[0] : r[0] - a0 * hdn[0];
+    const T s1 = up[1] ? r[0] + a0 * hup[1] : r[1] - a1 * hdn[1];
+    Fr[0] = (w[0] * s0) * Sm;
+    Fr[1] = (w[1] * s1) * Sm;
+    const T Fn = shfl_dn1(Fr[0]);
+    if (store) {
+      const T o0 = r[0] - dtiv * (Fr[1] - Fr[0]), o1 = r[1] - dtiv * (Fn - Fr[1]);
+      if (WRAP) st_pair(A.drho + l, o0, o1);
+      else {
+        A.drho[l] = (i >= 2 && i < d.TX - 2) ? o0 : r[0];
+        if (i + 1 < d.TX) A.drho[l + 1] = (i + 1 >= 2 && i + 1 < d.TX - 2) ? o1 : r[1];
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) {
+    const T f0 = Q[q][0] * ir[0], f1 = Q[q][1] * ir[1];
+    const T fl = shfl_up1(f1), fr = shfl_dn1(f0);
+    const T a0 = vl_slope(fl, f0, f1, invd, invd);
+    const T a1 = vl_slope(f0, f1, fr, invd, invd);
+    const T al = shfl_up1(a1);
+    const T s0 = up[0] ? fl + al * hup[0] : f0 - a0 * hdn[0];
+    const T s1 = up[1] ? f0 + a0 * hup[1] : f1 - a1 * hdn[1];
+    const T F0 = Fr[0] * s0, F1 = Fr[1] * s1;
+    const T Fn = shfl_dn1(F0);
+    if (store) {
+      const T o0 = Q[q][0] - dtiv * (F1 - F0), o1 = Q[q][1] - dtiv * (Fn - F1);
+      if (WRAP) st_pair(A.dq[q] + l, o0, o1);
+      else {
+        A.dq[q][l] = (i >= 2 && i < d.TX - 2) ? o0 : Q[q][0];
+        if (i + 1 < d.TX) A.dq[q][l + 1] = (i + 1 >= 2 && i + 1 < d.TX - 2) ? o1 : Q[q][1];
+      }
+    }
+  }
+}
+
+// ---- Y / Z sweep: marching with an asynchronous shared-memory ring -----------------------------------------
+// One thread per (i, line) marches along the sweep axis; threads of a warp sit side by side along X, so
+// every access is a coalesced row segment.  Rows are fetched RD rows ahead with cp.async into a ring of
+// RS slots that is private to each thread (no barrier: a thread reads only what it copied itself), which
+// keeps ~RD * (NQ+2) * 8 B per thread in flight without holding them in registers.  The ring also keeps
+// rows r-1 and r-2, so the un-divided quantities of the cell being updated are re-read from shared
+// memory instead of living in registers.  The row loop is unrolled by two so that the two-row window of
+// q = Q / rho rotates by renaming.
 constexpr int MTHREADS = 128;
+constexpr int RD = 5;            // rows in flight
+constexpr int RS = 8;            // ring slots (>= RD + 3), a power of two
+
+template <typename T> struct CpAsync;
+template <> struct CpAsync<double> {
+  static __device__ __forceinline__ void go(unsigned dst, const double* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+  }
+};
+template <> struct CpAsync<float> {
+  static __device__ __forceinline__ void go(unsigned dst, const float* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+  }
+};
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <typename T, int DIR, int NQ>
-__global__ void __launch_bounds__(MTHREADS) k_sweep_march(const Dev<T> d, const SweepArgs<T> A, const int CH) {
+__global__ void __launch_bounds__(MTHREADS) k_sweep_ring(const Dev<T> d, const SweepArgs<T> A, const int CH) {
+  constexpr int NA = NQ + 2;   // rho, NQ quantities, the face velocity
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* const ring = reinterpret_cast<T*>(smem_raw) + threadIdx.x;   // element (slot, array) at (slot*NA + array)*MTHREADS
   if (d.ctl->done) return;
-  const int i = blockIdx.x * MTHREADS + threadIdx.x;
-  if (i >= d.TX) return;
+  int i = blockIdx.x * MTHREADS + threadIdx.x;
+  const bool live = i < d.TX;
+  if (!live) i = d.TX - 1;                            // idle lanes shadow the last column and store nothing
   const int line = blockIdx.y;                       // k for the Y sweep, j for the Z sweep
   const int TL = DIR == 1 ? d.TY : d.TZ;
   const int c0 = blockIdx.z * CH, c1 = (c0 + CH < TL) ? c0 + CH : TL;   // cells this thread writes: [c0, c1)
@@ -180,101 +349,125 @@ __global__ void __launch_bounds__(MTHREADS) k_sweep_march(const Dev<T> d, const 
   const T* __restrict__ tL = DIR == 1 ? d.LY : d.dz;
   const T* __restrict__ tD = DIR == 1 ? d.invDY : d.invdzc;
 
-  // window: suffix 2 = cell r-2, 1 = cell r-1, 0 = cell r (just arrived), n = cell r+1 (in flight)
-  T Q2[NQ + 1], Q1[NQ + 1], f2[NQ + 1], f1[NQ + 1], a2[NQ + 1], F2[NQ + 1];
+  const unsigned ring_s = (unsigned)__cvta_generic_to_shared(ring);
+  const int nrow = (c1 - c0) + 4;                    // rows c0-2 .. c1+1, numbered n = 0 .. nrow-1
+  auto fetch = [&](const int n) {                    // row n -> slot n & (RS-1); rows off the array are clamped
+    if (n < nrow) {
+      int r = c0 - 2 + n;
+      r = r < 0 ? 0 : (r >= TL ? TL - 1 : r);
+      const long long l = base + (long long)r * str;
+      const unsigned dst = ring_s + (unsigned)(((n & (RS - 1)) * NA) * MTHREADS * sizeof(T));
+      CpAsync<T>::go(dst, A.srho + l);
 #pragma unroll
-  for (int q = 0; q <= NQ; ++q) { Q2[q] = Q1[q] = f2[q] = f1[q] = a2[q] = F2[q] = T(0); }
+      for (int q = 0; q < NQ; ++q) CpAsync<T>::go(dst + (unsigned)((1 + q) * MTHREADS * sizeof(T)), A.sq[q] + l);
+      CpAsync<T>::go(dst + (unsigned)((NQ + 1) * MTHREADS * sizeof(T)), vel + l);
+    }
+    cp_commit();                                     // one group per row, empty past the end
+  };
+#pragma unroll
+  for (int n = 0; n < RD; ++n) fetch(n);
+
+  // window (index 0 = rho, 1..NQ = quantities): fA/fB hold q of rows r-2 / r-1 in turn, a2 the slope of
+  // cell r-2, F2 the flux through the lower face of cell r-2
+  T fA[NQ + 1], fB[NQ + 1], a2[NQ + 1], F2[NQ + 1];
+#pragma unroll
+  for (int q = 0; q <= NQ; ++q) { fA[q] = fB[q] = a2[q] = F2[q] = T(0); }
   T len2 = T(0), len1 = T(0), invd1 = T(0), w1 = T(0), S1 = T(0), dtiv2 = T(0), dtiv1 = T(0);
 
-  T Qn[NQ + 1], wn = T(0);
-  auto load_row = [&](const int r) {
-    if (r >= 0 && r < TL) {
-      const long long l = base + (long long)r * str;
-      Qn[NQ] = A.srho[l];
-#pragma unroll
-      for (int q = 0; q < NQ; ++q) Qn[q] = A.sq[q][l];
-      wn = vel[l];
-    } else {
-      Qn[NQ] = T(1);
-#pragma unroll
-      for (int q = 0; q < NQ; ++q) Qn[q] = T(0);
-      wn = T(0);
-    }
-  };
-  load_row(c0 - 2);
-#pragma unroll 1
-  for (int r = c0 - 2; r < c1 + 2; ++r) {
-    // row r has arrived in Qn; start the loads of row r+1 at once
-    T Q0[NQ + 1], f0[NQ + 1];
-#pragma unroll
-    for (int q = 0; q <= NQ; ++q) Q0[q] = Qn[q];
-    const T w0 = wn;
-    if (r + 1 < c1 + 2) load_row(r + 1);
+  // one row: f2 (in: q of row r-2; out: q of row r), f1 (q of row r-1)
+  auto row_step = [&](const int n, T (&f2)[NQ + 1], T (&f1)[NQ + 1]) {
+    fetch(n + RD);
+    cp_wait<RD>();                                   // row n has landed
+    const int r = c0 - 2 + n;
+    const T* cur = ring + ((n & (RS - 1)) * NA) * MTHREADS;
+    const T* old = ring + (((n - 2) & (RS - 1)) * NA) * MTHREADS;   // row r-2 (the cell being updated)
     const int rc = r < 0 ? 0 : (r >= TL ? TL - 1 : r);
     const T len0 = DIR == 1 ? tL[rc] : tL[rc] * gL;
     const T invd0 = DIR == 1 ? tD[rc] : tD[rc] * gD;
     const T S0 = DIR == 1 ? tS[rc] * gS : gS * tS[rc];
     const T dtiv0 = dt * (DIR == 1 ? tV[rc] * gV : gV * tV[rc]);
-    const T ir = T(1) / Q0[NQ];
-#pragma unroll
-    for (int q = 0; q < NQ; ++q) f0[q] = Q0[q] * ir;
-    f0[NQ] = Q0[NQ];
-    const int s = r - c0;   // stage of the pipeline (uniform over the block)
-    T a1[NQ + 1], F1[NQ + 1];
-#pragma unroll
-    for (int q = 0; q <= NQ; ++q) { a1[q] = T(0); F1[q] = T(0); }
-    if (s >= 0) {   // slopes of cell r-1
-#pragma unroll
-      for (int q = 0; q <= NQ; ++q) a1[q] = vl_slope(f2[q], f1[q], f0[q], invd1, invd0);
-    }
-    if (s >= 1) {   // fluxes through the lower face of cell r-1 (Eq. 48, Eqs. 45-47)
-      const bool up = w1 >= T(0);
-      const T wdt = w1 * dt;
-      const T hup = (len2 - wdt) * T(0.5), hdn = (len1 + wdt) * T(0.5);
-      const T rs = up ? f2[NQ] + a2[NQ] * hup : f1[NQ] - a1[NQ] * hdn;
-      const T Fr = (w1 * rs) * S1;
-      F1[NQ] = Fr;
-#pragma unroll
-      for (int q = 0; q < NQ; ++q) {
-        const T fs = up ? f2[q] + a2[q] * hup : f1[q] - a1[q] * hdn;
-        F1[q] = Fr * fs;
-      }
-    }
-    if (s >= 2) {   // update (or pass through) cell r-2
-      const int m = r - 2;
-      const bool upd = m >= 2 && m < TL - 2;
-      const long long l = base + (long long)m * str;
-      A.drho[l] = upd ? Q2[NQ] - dtiv2 * (F1[NQ] - F2[NQ]) : Q2[NQ];
-#pragma unroll
-      for (int q = 0; q < NQ; ++q) A.dq[q][l] = upd ? Q2[q] - dtiv2 * (F1[q] - F2[q]) : Q2[q];
+    const T w0 = cur[(NQ + 1) * MTHREADS];
+    const T rho0 = cur[0];
+    const T ir = rdiv(T(1), rho0);
+    // face between cells r-2 and r-1 (Eq. 48, Eqs. 45-47)
+    const bool up = w1 >= T(0);
+    const T wdt = w1 * dt;
+    const T hup = (len2 - wdt) * T(0.5), hdn = (len1 + wdt) * T(0.5);
+    const int m = r - 2;
+    const bool wr = n >= 4 && live;
+    const bool upd = m >= 2 && m < TL - 2;
+    const long long lo = base + (long long)m * str;
+    T Fr;
+    {
+      const T f0 = rho0;
+      const T a1 = vl_slope(f2[0], f1[0], f0, invd1, invd0);
+      const T rs = up ? f2[0] + a2[0] * hup : f1[0] - a1 * hdn;
+      Fr = (w1 * rs) * S1;
+      if (wr) { const T Qo = old[0]; A.drho[lo] = upd ? Qo - dtiv2 * (Fr - F2[0]) : Qo; }
+      f2[0] = f0; a2[0] = a1; F2[0] = Fr;
     }
 #pragma unroll
-    for (int q = 0; q <= NQ; ++q) { Q2[q] = Q1[q]; Q1[q] = Q0[q]; f2[q] = f1[q]; f1[q] = f0[q]; a2[q] = a1[q]; F2[q] = F1[q]; }
+    for (int q = 1; q <= NQ; ++q) {
+      const T f0 = cur[q * MTHREADS] * ir;
+      const T a1 = vl_slope(f2[q], f1[q], f0, invd1, invd0);
+      const T fs = up ? f2[q] + a2[q] * hup : f1[q] - a1 * hdn;
+      const T F1 = Fr * fs;
+      if (wr) { const T Qo = old[q * MTHREADS]; A.dq[q - 1][lo] = upd ? Qo - dtiv2 * (F1 - F2[q]) : Qo; }
+      f2[q] = f0; a2[q] = a1; F2[q] = F1;
+    }
     len2 = len1; len1 = len0; invd1 = invd0; w1 = w0; S1 = S0; dtiv2 = dtiv1; dtiv1 = dtiv0;
+  };
+#pragma unroll 1
+  for (int n = 0; n < nrow; n += 2) {
+    row_step(n, fA, fB);
+    if (n + 1 < nrow) row_step(n + 1, fB, fA);
   }
+  cp_wait<0>();
+}
+
+template <typename T, bool ADI, bool HASY, bool HASZ>
+static int launch_x2(const Dev<T>& d, const SweepArgs<T>& a, cudaStream_t s) {
+  const int span = d.xwrap ? d.nx : d.TX;
+  dim3 b(32, X2W), g((span + X2IN - 1) / X2IN, (d.TY + X2W - 1) / X2W, d.TZ);
+  if (d.xwrap) k_sweep_x2<T, ADI, HASY, HASZ, true><<<g, b, 0, s>>>(d, a);
+  else k_sweep_x2<T, ADI, HASY, HASZ, false><<<g, b, 0, s>>>(d, a);
+  return 1;
 }
 
 template <typename T, int NQ>
 static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s) {
-  if (dir == 0) {
+  if (dir == 0) {   // the X sweep is always the first pass: 12a is fused into it
+    if (!d.xwrap || d.nx % 2 == 0) {
+      const int key = (d.eos == EOS_ADI ? 4 : 0) | (d.hasy ? 2 : 0) | (d.hasz ? 1 : 0);
+      switch (key) {
+        case 0: return launch_x2<T, false, false, false>(d, a, s);
+        case 1: return launch_x2<T, false, false, true>(d, a, s);
+        case 2: return launch_x2<T, false, true, false>(d, a, s);
+        case 3: return launch_x2<T, false, true, true>(d, a, s);
+        case 4: return launch_x2<T, true, false, false>(d, a, s);
+        case 5: return launch_x2<T, true, false, true>(d, a, s);
+        case 6: return launch_x2<T, true, true, false>(d, a, s);
+        default: return launch_x2<T, true, true, true>(d, a, s);
+      }
+    }
     dim3 b(32, XW), g((d.TX + XIN - 1) / XIN, (d.TY + XW - 1) / XW, d.TZ);
-    if (a.first) k_sweep_x<T, NQ, true><<<g, b, 0, s>>>(d, a);
-    else k_sweep_x<T, NQ, false><<<g, b, 0, s>>>(d, a);
+    k_sweep_x<T, NQ, true><<<g, b, 0, s>>>(d, a);
     return 1;
   }
   const int TL = dir == 1 ? d.TY : d.TZ, lines = dir == 1 ? d.TZ : d.TY;
-  // chunk the sweep axis so that the grid fills the machine a few times over, but keep chunks long
+  // chunk the sweep axis so that the grid fills the machine several times over, but keep chunks long
   // (each one re-reads 4 rows of halo)
   const long long cols = (long long)((d.TX + MTHREADS - 1) / MTHREADS) * lines;
-  int nch = (int)((148LL * 16 * 4 + cols - 1) / cols);
+  int nch = (int)((148LL * 3 * 6 + cols - 1) / cols);
   if (nch < 1) nch = 1;
   int CH = (TL + nch - 1) / nch;
   if (CH < 32) CH = 32;
   if (CH > TL) CH = TL;
   nch = (TL + CH - 1) / CH;
   dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);
-  if (dir == 1) k_sweep_march<T, 1, NQ><<<g, b, 0, s>>>(d, a, CH);
-  else k_sweep_march<T, 2, NQ><<<g, b, 0, s>>>(d, a, CH);
+  const size_t sm = (size_t)RS * (NQ + 2) * MTHREADS * sizeof(T);
+  if (dir == 1) k_sweep_ring<T, 1, NQ><<<g, b, sm, s>>>(d, a, CH);
+  else k_sweep_ring<T, 2, NQ><<<g, b, sm, s>>>(d, a, CH);
   return 1;
 }
 
@@ -291,7 +484,15 @@ int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s
   }
 }
 
-template <typename T> void sweep_setup() {}
+template <typename T, int NQ> static void ring_attr() {
+  const int sm = RS * (NQ + 2) * MTHREADS * (int)sizeof(T);
+  cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+  cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+}
+template <typename T> void sweep_setup() {
+  ring_attr<T, 2>(); ring_attr<T, 3>(); ring_attr<T, 4>(); ring_attr<T, 5>(); ring_attr<T, 6>(); ring_attr<T, 7>();
+}
+
 template void sweep_setup<double>();
 template void sweep_setup<float>();
 

@@ -52,6 +52,8 @@ template <typename T> int launch_newvel(const Dev<T>& d, const T* rho, const QSe
                                         cudaStream_t s);
 template <typename T> int launch_copy(const Dev<T>& d, const T* src, T* dst, cudaStream_t s);
 int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s);
+// out[n] = rdiv(a[n], b[n]): the kernels' branch-free division, exposed for its self-test
+int launch_selftest_div(const double* a, const double* b, double* out, long long n, cudaStream_t s);
 
 // active cells <-> ghosted, padded device layout
 template <typename T> int launch_scatter(const Dev<T>& d, const T* active, T* full, cudaStream_t s);

@@ -241,3 +241,31 @@ def test_exact_integer_shift():
     got, ref = g.array("trho"), o.array("rho")
     assert np.array_equal(g.array("nshift"), o.array("nshift"))
     assert np.array_equal(got, ref)
+
+
+def test_division_is_correctly_rounded():
+    """The kernels' branch-free division (csrc/common.cuh rdiv) against IEEE division on the host: bit-equal on
+    2^24 random operand pairs spanning 2^+-400 in each operand plus a set of hard cases."""
+    import torch
+    from paper_1602_02359_b200.binding import selftest_div
+    rng = np.random.default_rng(20260211)
+    n = 1 << 24
+    def draw():
+        m = rng.uniform(1.0, 2.0, n)
+        e = rng.integers(-400, 400, n)
+        s = rng.choice([-1.0, 1.0], n)
+        return s * np.ldexp(m, e)
+    a, b = draw(), draw()
+    # hard cases: quotients next to rounding boundaries, equal operands, powers of two, zero numerators
+    k = np.arange(1, 4097, dtype=np.float64)
+    a[:4096] = k; b[:4096] = 3.0
+    a[4096:8192] = 1.0; b[4096:8192] = 1.0 + k * 2.0 ** -52
+    a[8192:12288] = 1.0 + k * 2.0 ** -52; b[8192:12288] = 1.0 + (k + 1) * 2.0 ** -52
+    a[12288:16384] = 0.0
+    a[16384:20480] = b[16384:20480]
+    b[20480:24576] = 6.0
+    got = selftest_div(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda()).cpu().numpy()
+    ref = a / b
+    bad = np.nonzero(got != ref)[0]
+    assert bad.size == 0, "first mismatch: %r / %r -> gpu %r host %r (%d of %d)" % (
+        a[bad[0]], b[bad[0]], got[bad[0]], ref[bad[0]], bad.size, n)

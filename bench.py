@@ -76,7 +76,7 @@ def algorithmic_reals(w):
         "dt": (2 if adi else 1) + nd,
         "source_a": (2 + nd + (1 if pot else 0)) + nd,
         "source_b": (1 + (1 if adi else 0) + nd) + (nd + (1 if adi else 0)),
-        "source_c": (nd + 1) + 1,
+        "source_bc": (2 + nd) + (nd + 1),
         "source_d": (3 + 3) + (3 + 3 + 2),
         "first_sweep": (1 + (1 if adi else 0) + nd) + (1 + nq),
         "sweep": (1 + nq + 1) + (1 + nq),
@@ -84,7 +84,9 @@ def algorithmic_reals(w):
         "newvel": (1 + 2 * nd) + nd,
     }
     if not adi:
-        k["source_c"] = 0
+        k["source_bc"] = 0
+    else:
+        k["source_b"] = 0
     if not visc:
         k["source_d"] = 0
     # fused plan of SURVEY.md 8(d.3): dt, one source pass, one pass per direction, orbital, Eq. 51 folded

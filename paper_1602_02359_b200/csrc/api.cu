@@ -381,13 +381,13 @@ struct Sim : CtxBase {
     if (until == FARGO_ST_SRC_A) return n;
     T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
     if (L.visc) { vxc = set_arr(1, 4); vyc = set_arr(1, 5); }
-    n += timed("source_b", [&] { return launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream); });        // cell 7b
-    dbg["vxc"] = vxc; dbg["vyc"] = vyc; dbg["vzc"] = vzc; dbg["ec"] = L.adi ? ec : st.e;
+    // adiabatic: 7b and 7c run as ONE kernel (e_c is never stored); compared with the oracle at stage SRC_C
+    if (L.adi) n += timed("source_bc", [&] { return launch_source_bc<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, st.e, stream); });
+    else n += timed("source_b", [&] { return launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream); });   // cell 7b
+    dbg["vxc"] = vxc; dbg["vyc"] = vyc; dbg["vzc"] = vzc; dbg["ec"] = nullptr;
     dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
-    if (until == FARGO_ST_SRC_B) return n;
-    if (L.adi) n += timed("source_c", [&] { return launch_source_c<T>(d, vxc, vyc, vzc, ec, st.e, stream); });          // cell 7c
     dbg["ed"] = st.e;
-    if (until == FARGO_ST_SRC_C) return n;
+    if (until == FARGO_ST_SRC_B || until == FARGO_ST_SRC_C) return n;
     if (L.visc)                                                                      // cell 7d
       n += timed("source_d", [&] { return launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream); });
     dbg["vxd"] = st.vx; dbg["vyd"] = st.vy;

@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
     for (int ia = threadIdx.x; ia < d.nx; ia += blockDim.x) {
       const int i = d.ngx + ia;
       const long long l = d.id(i, j, k);
-      const T cs2 = (d.eos == EOS_ADI) ? (d.gg1 * st.e[l]) / st.rho[l] : st.e[l] * st.e[l];
+      const T cs2 = (d.eos == EOS_ADI) ? rdiv(d.gg1 * st.e[l], st.rho[l]) : st.e[l] * st.e[l];
       const T I1sq = cs2 * il2;
       T I2 = T(0), I3 = T(0);
       if (d.hasx) {

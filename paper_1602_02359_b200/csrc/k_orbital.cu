@@ -33,7 +33,7 @@ __device__ __forceinline__ T ppa_star_upper(const T f, const int tm, const bool 
   s_dm[tm] = dm;
   __syncthreads();
   T fr = f;
-  if (tm < OBM - 1) fr = (f + T(0.5) * (s_f[tm + 1] - f)) - (s_dm[tm + 1] - dm) / T(6);   // Eq. 71
+  if (tm < OBM - 1) fr = (f + T(0.5) * (s_f[tm + 1] - f)) - rdiv(s_dm[tm + 1] - dm, T(6));   // Eq. 71
   s_fu[tm] = fr;
   __syncthreads();
   T fl = tm >= 1 ? s_fu[tm - 1] : f;
@@ -41,7 +41,7 @@ __device__ __forceinline__ T ppa_star_upper(const T f, const int tm, const bool 
   else {
     const T D = fr - fl;
     const T C = f - T(0.5) * (fl + fr);
-    const T DC = D * C, D26 = (D * D) / T(6);
+    const T DC = D * C, D26 = rdiv(D * D, T(6));
     if (DC > D26) fl = T(3) * f - T(2) * fr;
     else if (-D26 > DC) fr = T(3) * f - T(2) * fl;
   }
@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(OBM) k_orbital(const Dev<T> d, const SweepArgs
   const long long l = row + i, lo = row + io;
 
   const T r0 = A.srho[l];
-  const T ir = T(1) / r0;
+  const T ir = rdiv(T(1), r0);
   const T rs = ppa_star_upper(r0, tm, fwd, x, x1x, s_f, s_dm, s_fu, s_fl, s_fr);
   const T Fr = xi * rs;   // mass through face i+1/2 per unit of (LX Sx)
   s_F[tm] = Fr;

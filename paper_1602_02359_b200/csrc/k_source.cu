@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
     if (d.xwrap || i >= 1) {   // Eq. 53: density on the face = arithmetic mean
       const long long lm = d.id(d.xw(i - 1), j, k);
       const T il = d.invLX(j, k);
-      const T wf = (T(2) * il) / (r0 + rho[lm]);
+      const T wf = rdiv(T(2) * il, r0 + rho[lm]);
       T acc = wf * (p0 - pressure(d, rho, e, lm));
       if (d.has_pot) acc = acc + (f0 - phi[lm]) * il;
       v = vx[l] - dt * acc;
@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
     if (j >= 1 && (!curv || ipok) && (!(sph && d.hasz) || k + 1 < d.TZ)) {
       const long long lm = l - d.pitch;
       const T il = d.invDY[j];
-      const T wf = (T(2) * il) / (r0 + rho[lm]);
+      const T wf = rdiv(T(2) * il, r0 + rho[lm]);
       T acc = wf * (p0 - pressure(d, rho, e, lm));
       if (d.has_pot) acc = acc + (f0 - phi[lm]) * il;
       v = vy[l] - dt * acc;
@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
     if (k >= 1 && (!sph || ipok)) {
       const long long lm = l - d.plane;
       const T il = d.invDZ(j, k);
-      const T wf = (T(2) * il) / (r0 + rho[lm]);
+      const T wf = rdiv(T(2) * il, r0 + rho[lm]);
       T acc = wf * (p0 - pressure(d, rho, e, lm));
       if (d.has_pot) acc = acc + (f0 - phi[lm]) * il;
       v = vz[l] - dt * acc;
@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(128) k_source_b(const Dev<T> d, const State<T>
       const long long lm = d.id(d.xw(i - 1), j, k);
       const T rm = rho[lm];
       const T qm = qvisc(cq2, rm, v0 - vxb[lm]);   // q of the lower neighbour: its dv = v0 - vb[lm]
-      const T wf = (T(2) * d.invLX(j, k)) / (r0 + rm);
+      const T wf = rdiv(T(2) * d.invLX(j, k), r0 + rm);
       v = v0 - dt * (wf * (q - qm));
     }
     vxc[l] = v;
@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(128) k_source_b(const Dev<T> d, const State<T>
       const long long lm = l - d.pitch;
       const T rm = rho[lm];
       const T qm = qvisc(cq2, rm, v0 - vyb[lm]);
-      const T wf = (T(2) * d.invDY[j]) / (r0 + rm);
+      const T wf = rdiv(T(2) * d.invDY[j], r0 + rm);
       v = v0 - dt * (wf * (q - qm));
     }
     vyc[l] = v;
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(128) k_source_b(const Dev<T> d, const State<T>
       const long long lm = l - d.plane;
       const T rm = rho[lm];
       const T qm = qvisc(cq2, rm, v0 - vzb[lm]);
-      const T wf = (T(2) * d.invDZ(j, k)) / (r0 + rm);
+      const T wf = rdiv(T(2) * d.invDZ(j, k), r0 + rm);
       v = v0 - dt * (wf * (q - qm));
     }
     vzc[l] = v;
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(128) k_source_c(const Dev<T> d, const T* __res
     if (d.hasz) tz = vzc[l + d.plane] * d.Sz(j, k + 1) - vzc[l] * d.Sz(j, k);
     const T D = d.invV(j, k) * ((tx + ty) + tz);
     const T a = hd * D;
-    v = (ec[l] * (T(1) - a)) / (T(1) + a);
+    v = rdiv(ec[l] * (T(1) - a), T(1) + a);
   }
   ed[l] = v;
 }
@@ -200,6 +200,112 @@ template <typename T>
 int launch_source_c(const Dev<T>& d, const T* vxc, const T* vyc, const T* vzc, const T* ec, T* ed, cudaStream_t s) {
   dim3 b(128), g((d.TX + 127) / 128, d.TY, d.TZ);
   k_source_c<T><<<g, b, 0, s>>>(d, vxc, vyc, vzc, ec, ed);
+  return 1;
+}
+
+// ---- 7b + 7c fused (adiabatic) ----------------------------------------------------------------------------
+// e_d of a cell needs v_c on its six faces, and v_c on a face needs q on both sides of it, so per direction
+// the thread forms q at m-1, m, m+1 from v_b at m-1 .. m+2 and v_c at m and m+1: one extra q and one extra
+// division per direction against the two separate kernels, in exchange for never writing e_c and never
+// re-reading v_c (9 reals per cell instead of 14).  Every expression is the one k_source_b / k_source_c
+// evaluate for the same face, so the results are bit-identical to the two-kernel sequence.
+template <typename T>
+struct FaceBC { T vc0, vc1, heat; };   // v_c on the lower and upper face of the cell, q dv / L of the cell
+
+// one direction: vb[] = v_b at m-1, m, m+1, m+2; rr[] = rho at m-1, m, m+1; have* say which exist;
+// il0 / il1 = inverse centre distance across the lower / upper face; ilc = inverse cell width
+template <typename T>
+__device__ __forceinline__ FaceBC<T> face_bc(const T cq2, const T dt, const T vbm, const T vb0, const T vb1,
+                                             const T vb2, const T rm, const T r0, const T r1, const bool has_m,
+                                             const bool has_1, const bool has_2, const T il0, const T il1,
+                                             const T ilc) {
+  FaceBC<T> o;
+  T dv = T(0), q = T(0);
+  if (has_1) { dv = vb1 - vb0; q = qvisc(cq2, r0, dv); }
+  o.vc0 = vb0;
+  if (has_m) {
+    const T qm = qvisc(cq2, rm, vb0 - vbm);
+    const T wf = rdiv(T(2) * il0, r0 + rm);
+    o.vc0 = vb0 - dt * (wf * (q - qm));
+  }
+  o.vc1 = vb1;
+  if (has_1) {   // the upper face: what k_source_b computes at the upper neighbour
+    T q1 = T(0);
+    if (has_2) q1 = qvisc(cq2, r1, vb2 - vb1);
+    const T wf = rdiv(T(2) * il1, r1 + r0);
+    o.vc1 = vb1 - dt * (wf * (q1 - q));
+  }
+  o.heat = (q * dv) * ilc;
+  return o;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) k_source_bc(const Dev<T> d, const State<T> st, const T* __restrict__ vxb,
+                                                   const T* __restrict__ vyb, const T* __restrict__ vzb,
+                                                   T* __restrict__ vxc, T* __restrict__ vyc, T* __restrict__ vzc,
+                                                   T* __restrict__ ed) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= d.TX) return;
+  const T dt = (T)d.ctl->dt, cq2 = d.cvnr2;
+  const long long l = d.id(i, j, k);
+  const T* __restrict__ rho = st.rho;
+  const T r0 = rho[l];
+  T heat = T(0), tx = T(0), ty = T(0), tz = T(0);
+  bool ok = true;
+  if (d.hasx) {
+    const bool w = d.xwrap != 0;
+    const bool hm = w || i >= 1, h1 = w || i + 1 < d.TX, h2 = w || i + 2 < d.TX;
+    const long long row = l - i;
+    const long long lm = row + d.xw(i - 1), l1 = row + d.xw(i + 1), l2 = row + d.xw(i + 2);
+    const T il = d.invLX(j, k);
+    const FaceBC<T> f = face_bc<T>(cq2, dt, hm ? vxb[lm] : T(0), vxb[l], h1 ? vxb[l1] : T(0), h2 ? vxb[l2] : T(0),
+                                   hm ? rho[lm] : T(0), r0, h1 ? rho[l1] : T(0), hm, h1, h2, il, il, il);
+    vxc[l] = f.vc0;
+    heat = f.heat;
+    ok = ok && h1;
+    tx = (f.vc1 - f.vc0) * d.Sx(j, k);
+  }
+  if (d.hasy) {
+    const bool hm = j >= 1, h1 = j + 1 < d.TY, h2 = j + 2 < d.TY;
+    const long long p = d.pitch;
+    const FaceBC<T> f = face_bc<T>(cq2, dt, hm ? vyb[l - p] : T(0), vyb[l], h1 ? vyb[l + p] : T(0),
+                                   h2 ? vyb[l + 2 * p] : T(0), hm ? rho[l - p] : T(0), r0, h1 ? rho[l + p] : T(0), hm,
+                                   h1, h2, d.invDY[j], h1 ? d.invDY[j + 1] : T(0), d.invLY[j]);
+    vyc[l] = f.vc0;
+    heat = heat + f.heat;
+    ok = ok && h1;
+    if (h1) ty = f.vc1 * d.Sy(j + 1, k) - f.vc0 * d.Sy(j, k);
+  } else {
+    heat = heat + T(0);
+  }
+  if (d.hasz) {
+    const bool hm = k >= 1, h1 = k + 1 < d.TZ, h2 = k + 2 < d.TZ;
+    const long long p = d.plane;
+    const FaceBC<T> f = face_bc<T>(cq2, dt, hm ? vzb[l - p] : T(0), vzb[l], h1 ? vzb[l + p] : T(0),
+                                   h2 ? vzb[l + 2 * p] : T(0), hm ? rho[l - p] : T(0), r0, h1 ? rho[l + p] : T(0), hm,
+                                   h1, h2, d.invDZ(j, k), h1 ? d.invDZ(j, k + 1) : T(0), d.invLZ(j, k));
+    vzc[l] = f.vc0;
+    heat = heat + f.heat;
+    ok = ok && h1;
+    if (h1) tz = f.vc1 * d.Sz(j, k + 1) - f.vc0 * d.Sz(j, k);
+  }
+  const T ec = st.e[l] - dt * heat;   // heating -q_d dv_d / Delta_d (G19)
+  T v = ec;
+  if (ok) {
+    const T hd = (T(0.5) * dt) * d.gm1;
+    const T D = d.invV(j, k) * ((tx + ty) + tz);
+    const T a = hd * D;
+    v = rdiv(ec * (T(1) - a), T(1) + a);
+  }
+  ed[l] = v;
+}
+
+template <typename T>
+int launch_source_bc(const Dev<T>& d, const State<T>& st, const T* vxb, const T* vyb, const T* vzb, T* vxc, T* vyc,
+                     T* vzc, T* ed, cudaStream_t s) {
+  dim3 b(128), g((d.TX + 127) / 128, d.TY, d.TZ);
+  k_source_bc<T><<<g, b, 0, s>>>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ed);
   return 1;
 }
 
@@ -252,13 +358,13 @@ __global__ void __launch_bounds__(128) k_visc_force(const Dev<T> d, const T* __r
     {   // B5, azimuthal: (1/r^2) d_r(r^2 tau_phi_r) + (1/r) d_phi tau_phi_phi
       const T a = (((y1 * y1) * tpr[ljp] - (y0 * y0) * tpr[l]) * (d.inv_yc[j] * d.inv_yc[j])) * d.invLY[j];
       const T b = (tpp[l] - tpp[lim]) * il;
-      ox = vx[l] - dt * ((T(2) / (rho[l] + rho[lim])) * (a + b));
+      ox = vx[l] - dt * (rdiv(T(2), rho[l] + rho[lim]) * (a + b));
     }
     if (j >= 2) {   // B5, radial: (1/r) d_r(r tau_rr) + (1/r) d_phi tau_r_phi - tau_phi_phi / r
       const T a = ((d.yc[j] * trr[l] - d.yc[j - 1] * trr[ljm]) * d.inv_ye[j]) * d.invDY[j];
       const T b = (tpr[lip] - tpr[l]) * ilf;
       const T dd = (T(0.5) * (tpp[l] + tpp[ljm])) * d.inv_ye[j];
-      oy = vy[l] - dt * ((T(2) / (rho[l] + rho[ljm])) * ((a + b) - dd));
+      oy = vy[l] - dt * (rdiv(T(2), rho[l] + rho[ljm]) * ((a + b) - dd));
     }
   }
   vxd[l] = ox; vyd[l] = oy;
@@ -274,6 +380,8 @@ int launch_source_d(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, T
 }
 
 #define INST(T)                                                                                                      \
+  template int launch_source_bc<T>(const Dev<T>&, const State<T>&, const T*, const T*, const T*, T*, T*, T*, T*,     \
+                                   cudaStream_t);                                                                    \
   template int launch_source_a<T>(const Dev<T>&, const State<T>&, const T*, T*, T*, T*, cudaStream_t);               \
   template int launch_source_b<T>(const Dev<T>&, const State<T>&, const T*, const T*, const T*, T*, T*, T*, T*,      \
                                   cudaStream_t);                                                                     \

@@ -488,6 +488,8 @@ template <typename T, int NQ> static void ring_attr() {
   const int sm = RS * (NQ + 2) * MTHREADS * (int)sizeof(T);
   cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+  cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
 }
 template <typename T> void sweep_setup() {
   ring_attr<T, 2>(); ring_attr<T, 3>(); ring_attr<T, 4>(); ring_attr<T, 5>(); ring_attr<T, 6>(); ring_attr<T, 7>();
@@ -509,15 +511,15 @@ __global__ void __launch_bounds__(128) k_newvel(const Dev<T> d, const T* __restr
   if (d.hasx) {
     const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, irx = d.invRx(j, k);
     const long long lm = d.id(d.xw(i - 1), j, k);
-    st.vx[l] = ((S.q[2][lm] + S.q[1][l]) / (rho[lm] + r0) - rx2om) * irx;
+    st.vx[l] = (rdiv(S.q[2][lm] + S.q[1][l], rho[lm] + r0) - rx2om) * irx;
   }
   if (d.hasy) {
     const long long lm = l - d.pitch;
-    st.vy[l] = (S.q[4][lm] + S.q[3][l]) / (rho[lm] + r0);
+    st.vy[l] = rdiv(S.q[4][lm] + S.q[3][l], rho[lm] + r0);
   }
   if (d.hasz) {
     const long long lm = l - d.plane;
-    st.vz[l] = ((S.q[6][lm] + S.q[5][l]) / (rho[lm] + r0)) * d.invRzj[j];
+    st.vz[l] = rdiv(S.q[6][lm] + S.q[5][l], rho[lm] + r0) * d.invRzj[j];
   }
 }
 

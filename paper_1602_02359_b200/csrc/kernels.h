@@ -23,6 +23,9 @@ template <typename T> int launch_source_a(const Dev<T>& d, const State<T>& st, c
 // cell 7b: (rho, e, vb) -> vc[3], ec
 template <typename T> int launch_source_b(const Dev<T>& d, const State<T>& st, const T* vxb, const T* vyb,
                                           const T* vzb, T* vxc, T* vyc, T* vzc, T* ec, cudaStream_t s);
+// cells 7b + 7c fused (adiabatic): (rho, e, vb) -> vc[3], ed; ed may alias st.e (each thread reads only its own e)
+template <typename T> int launch_source_bc(const Dev<T>& d, const State<T>& st, const T* vxb, const T* vyb,
+                                           const T* vzb, T* vxc, T* vyc, T* vzc, T* ed, cudaStream_t s);
 // cell 7c: (vc, ec) -> ed
 template <typename T> int launch_source_c(const Dev<T>& d, const T* vxc, const T* vyc, const T* vzc, const T* ec,
                                           T* ed, cudaStream_t s);

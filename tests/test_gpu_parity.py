@@ -63,8 +63,9 @@ def _stage_arrays(w, stage):
         "POT": [("phi", "phi")] if (w.geometry != W.CARTESIAN and (w.params.gm_star or w.params.planet_mass)) else [],
         "DT": [],
         "SRC_A": sfx("b"),
-        "SRC_B": sfx("c") + ([("ec", "ec")] if adi else []),
-        "SRC_C": [("ed", "ed")] if adi else [],
+        # adiabatic: 7b and 7c are one kernel (e_c is never stored): compared at the last stage it contains
+        "SRC_B": [] if adi else sfx("c"),
+        "SRC_C": (sfx("c") + [("ed", "ed")]) if adi else [],
         "SRC_D": [("vxd", "vxd"), ("vyd", "vyd")] if visc else [],
         "BC2": [("rho", "rho"), ("e", "e")] + vel,
         "SWEEP_X": tr if hx else [],

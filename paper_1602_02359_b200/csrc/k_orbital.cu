@@ -98,8 +98,151 @@ __global__ void __launch_bounds__(OBM) k_orbital(const Dev<T> d, const SweepArgs
   }
 }
 
+// ---- two cells per lane, no shared memory, no barriers -----------------------------------------------------
+// A warp owns 64 consecutive cells of one ring: lane L holds tile positions t = 2L, 2L+1 as one 16-byte
+// vector per array.  The PPA chain (difference -> monotonised slope -> interface value -> limiter -> star
+// value -> flux difference) needs 3 cells to the left and 3 to the right of a stored cell (the upwind cell of
+// its upper face may be the next one); positions 4 .. 59 are stored (56 per warp), lanes 0, 1, 30 and 31
+// are recomputed halo.  Per quantity five values cross
+// lanes by shuffle (two more when xi < 0); the quantities are independent, so their chains interleave.
+// Every expression is the one of k_orbital above: results are bit-identical.  Needs an even nx.
+constexpr int O2W = 4;          // warps (rings) per block
+constexpr int O2IN = 56;        // cells stored per warp
+
+template <typename T> __device__ __forceinline__ T o_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <typename T> __device__ __forceinline__ T o_dn1(T v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+template <typename T>
+__device__ __forceinline__ T ppa_mono(const T fm, const T f, const T fp, bool& flat) {
+  const T a = f - fm, b = fp - f;
+  const T dd = T(0.5) * (fp - fm);
+  flat = a * b <= T(0);
+  const T mm = rmin(rmin(T(2) * rabs(a), T(2) * rabs(b)), rabs(dd));
+  const T dm = dd < T(0) ? -mm : mm;
+  return flat ? T(0) : dm;
+}
+
+template <typename T>
+__device__ __forceinline__ void ppa_limit(const T f, const bool flat, T& fl, T& fr) {   // the three tests of P:484
+  const T D = fr - fl;
+  const T C = f - T(0.5) * (fl + fr);
+  const T DC = D * C, D26 = rdiv(D * D, T(6));
+  const T fl2 = T(3) * f - T(2) * fr, fr2 = T(3) * f - T(2) * fl;
+  const bool c1 = DC > D26, c2 = -D26 > DC;
+  const T ol = flat ? f : (c1 ? fl2 : fl);
+  const T orr = flat ? f : (c1 ? fr : (c2 ? fr2 : fr));
+  fl = ol; fr = orr;
+}
+
+// star values on the upper faces of the lane's two cells (reading G15: x = |xi| in both branches)
+template <typename T>
+__device__ __forceinline__ void ppa_pair(const T fA, const T fB, const bool fwd, const T x, const T x1x, T& sA,
+                                         T& sB) {
+  const T fm = o_up1(fB);        // position t-1
+  const T fn = o_dn1(fA);        // position t+2
+  bool flatA, flatB;
+  const T dmA = ppa_mono(fm, fA, fB, flatA), dmB = ppa_mono(fA, fB, fn, flatB);
+  const T dmn = o_dn1(dmA);
+  const T fuA = (fA + T(0.5) * (fB - fA)) - rdiv(dmB - dmA, T(6));   // Eq. 71, un-limited
+  const T fuB = (fB + T(0.5) * (fn - fB)) - rdiv(dmn - dmB, T(6));
+  T flA = o_up1(fuB), frA = fuA, flB = fuA, frB = fuB;
+  ppa_limit(fA, flatA, flA, frA);
+  ppa_limit(fB, flatB, flB, frB);
+  if (fwd) {   // warp-uniform: the whole ring moves one way
+    sA = (frA + x * (fA - frA)) + x1x * ((T(2) * fA - frA) - flA);
+    sB = (frB + x * (fB - frB)) + x1x * ((T(2) * fB - frB) - flB);
+  } else {
+    const T fln = o_dn1(flA), frn = o_dn1(frA);
+    sA = (flB + x * (fB - flB)) + x1x * ((T(2) * fB - frB) - flB);
+    sB = (fln + x * (fn - fln)) + x1x * ((T(2) * fn - frn) - fln);
+  }
+}
+
+template <typename T> struct OPair;
+template <> struct OPair<double> { using type = double2; };
+template <> struct OPair<float> { using type = float2; };
+
+template <typename T, int NQ>
+__global__ void __launch_bounds__(32 * O2W) k_orbital2(const Dev<T> d, const SweepArgs<T> A, T* __restrict__ nshift_out) {
+  if (d.ctl->done) return;
+  using P2 = typename OPair<T>::type;
+  const int lane = threadIdx.x;
+  const int n = d.nx, ntile = (n + O2IN - 1) / O2IN;
+  const int tile = blockIdx.x % ntile;   // 1-D grid: tiles of a ring are neighbours in launch order
+  const int ring = (blockIdx.x / ntile) * O2W + threadIdx.y;
+  if (ring >= d.TY * d.TZ) return;   // whole warps leave together
+  const int j = ring % d.TY, k = ring / d.TY;
+  const int iu = tile * O2IN - 4 + 2 * lane;   // un-wrapped index of the lane's first cell (even)
+  int i = iu % n; if (i < 0) i += n;
+
+  const T dt = (T)d.ctl->dt;
+  const T s = (A.v0[ring] * dt) * d.invLX(j, k);
+  const T N = floor(s + T(0.5));
+  const T xi = s - N;
+  const T g = (d.LX(j, k) * d.Sx(j, k)) * d.invV(j, k);
+  const bool fwd = xi >= T(0);
+  const T x = rabs(xi), x1x = x * (T(1) - x);
+  const long long Nl = (long long)N;
+  const int sh = (int)(((Nl % n) + n) % n);
+  if (nshift_out && tile == 0 && lane == 0) nshift_out[ring] = N;
+  int io = i + sh; if (io >= n) io -= n;
+  int io1 = io + 1; if (io1 >= n) io1 -= n;
+  const long long row = d.id(0, j, k);
+  const long long l = row + i;
+  const bool stA = lane >= 2 && lane <= 29 && iu < n, stB = stA && iu + 1 < n;
+  const bool vec = (sh & 1) == 0;   // even shift: the pair stays 16-byte aligned
+
+  // loads, all up front
+  const P2 r2 = *reinterpret_cast<const P2*>(A.srho + l);
+  P2 Q2[NQ];
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) Q2[q] = *reinterpret_cast<const P2*>(A.sq[q] + l);
+
+  const T irA = rdiv(T(1), r2.x), irB = rdiv(T(1), r2.y);
+  T sA, sB;
+  ppa_pair<T>(r2.x, r2.y, fwd, x, x1x, sA, sB);
+  const T FrA = xi * sA, FrB = xi * sB;   // mass through the upper face per unit of (LX Sx)
+  {
+    const T Fm = o_up1(FrB);
+    const T oA = r2.x - g * (FrA - Fm), oB = r2.y - g * (FrB - FrA);
+    if (stA) {
+      if (vec && stB) { P2 o; o.x = oA; o.y = oB; *reinterpret_cast<P2*>(A.drho + row + io) = o; }
+      else { A.drho[row + io] = oA; if (stB) A.drho[row + io1] = oB; }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) {
+    ppa_pair<T>(Q2[q].x * irA, Q2[q].y * irB, fwd, x, x1x, sA, sB);
+    const T FA = FrA * sA, FB = FrB * sB;
+    const T Fm = o_up1(FB);
+    const T oA = Q2[q].x - g * (FA - Fm), oB = Q2[q].y - g * (FB - FA);
+    if (stA) {
+      if (vec && stB) { P2 o; o.x = oA; o.y = oB; *reinterpret_cast<P2*>(A.dq[q] + row + io) = o; }
+      else { A.dq[q][row + io] = oA; if (stB) A.dq[q][row + io1] = oB; }
+    }
+  }
+}
+
+template <typename T, int NQ>
+static int launch_orbital2(const Dev<T>& d, const SweepArgs<T>& a, T* nshift_out, cudaStream_t s) {
+  dim3 b(32, O2W), g((unsigned)(((d.nx + O2IN - 1) / O2IN) * ((d.TY * d.TZ + O2W - 1) / O2W)));
+  k_orbital2<T, NQ><<<g, b, 0, s>>>(d, a, nshift_out);
+  return 1;
+}
+
 template <typename T>
 int launch_orbital(const Dev<T>& d, const SweepArgs<T>& a, T* nshift_out, cudaStream_t s) {
+  if (d.nx % 2 == 0) {
+    switch (a.nq) {
+      case 2: return launch_orbital2<T, 2>(d, a, nshift_out, s);
+      case 3: return launch_orbital2<T, 3>(d, a, nshift_out, s);
+      case 4: return launch_orbital2<T, 4>(d, a, nshift_out, s);
+      case 5: return launch_orbital2<T, 5>(d, a, nshift_out, s);
+      case 6: return launch_orbital2<T, 6>(d, a, nshift_out, s);
+      case 7: return launch_orbital2<T, 7>(d, a, nshift_out, s);
+      default: break;
+    }
+  }
   dim3 b(OBM), g((d.nx + OIN - 1) / OIN, d.TY, d.TZ);
   k_orbital<T><<<g, b, 0, s>>>(d, a, nshift_out);
   return 1;

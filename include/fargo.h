@@ -138,7 +138,8 @@ int fargo_profile_report(fargo_ctx* c, char* buf, size_t len);
 
 /* Self-test of the branch-free fp64 division the kernels use in place of a / b (csrc/common.cuh, rdiv;
  * DESIGN.md "rounding"): out[n] = rdiv(a[n], b[n]) for n elements; a, b, out are DEVICE pointers to
- * doubles, `cuda_stream` a cudaStream_t (NULL = default stream).  Synchronises before returning.
+ * doubles, `cuda_stream` a cudaStream_t (NULL = default stream).  b == NULL selects the kernels' division by
+ * the constant six (rdiv6): out[n] = a[n] / 6.  Synchronises before returning.
  * Returns FARGO_OK or FARGO_ECUDA / FARGO_EINVAL (no context: message not retrievable). */
 int fargo_selftest_div(const double* a, const double* b, double* out, long long n, void* cuda_stream);
 

@@ -235,14 +235,18 @@ class Fargo:
         return out
 
 
-def selftest_div(a, b):
-    """out = rdiv(a, b) elementwise on the GPU (torch.float64 CUDA tensors): the kernels' division."""
+def selftest_div(a, b=None):
+    """out = rdiv(a, b) elementwise on the GPU (torch.float64 CUDA tensors): the kernels' division; b = None
+    selects their division by the constant six (rdiv6)."""
     import torch
-    assert a.is_cuda and b.is_cuda and a.dtype == torch.float64 and b.dtype == torch.float64 and a.numel() == b.numel()
-    a, b = a.contiguous(), b.contiguous()
+    assert a.is_cuda and a.dtype == torch.float64
+    a = a.contiguous()
+    if b is not None:
+        assert b.is_cuda and b.dtype == torch.float64 and a.numel() == b.numel()
+        b = b.contiguous()
     out = torch.empty_like(a)
     torch.cuda.synchronize()
-    rc = load().fargo_selftest_div(a.data_ptr(), b.data_ptr(), out.data_ptr(), a.numel(), None)
+    rc = load().fargo_selftest_div(a.data_ptr(), None if b is None else b.data_ptr(), out.data_ptr(), a.numel(), None)
     if rc != 0:
         raise RuntimeError("fargo_selftest_div failed with code %d" % rc)
     return out

@@ -126,7 +126,7 @@ template <typename T>
 __device__ __forceinline__ void ppa_limit(const T f, const bool flat, T& fl, T& fr) {   // the three tests of P:484
   const T D = fr - fl;
   const T C = f - T(0.5) * (fl + fr);
-  const T DC = D * C, D26 = rdiv(D * D, T(6));
+  const T DC = D * C, D26 = rdiv6(D * D);
   const T fl2 = T(3) * f - T(2) * fr, fr2 = T(3) * f - T(2) * fl;
   const bool c1 = DC > D26, c2 = -D26 > DC;
   const T ol = flat ? f : (c1 ? fl2 : fl);
@@ -143,8 +143,8 @@ __device__ __forceinline__ void ppa_pair(const T fA, const T fB, const bool fwd,
   bool flatA, flatB;
   const T dmA = ppa_mono(fm, fA, fB, flatA), dmB = ppa_mono(fA, fB, fn, flatB);
   const T dmn = o_dn1(dmA);
-  const T fuA = (fA + T(0.5) * (fB - fA)) - rdiv(dmB - dmA, T(6));   // Eq. 71, un-limited
-  const T fuB = (fB + T(0.5) * (fn - fB)) - rdiv(dmn - dmB, T(6));
+  const T fuA = (fA + T(0.5) * (fB - fA)) - rdiv6(dmB - dmA);   // Eq. 71, un-limited
+  const T fuB = (fB + T(0.5) * (fn - fB)) - rdiv6(dmn - dmB);
   T flA = o_up1(fuB), frA = fuA, flB = fuA, frB = fuB;
   ppa_limit(fA, flatA, flA, frA);
   ppa_limit(fB, flatB, flB, frB);

@@ -270,3 +270,10 @@ def test_division_is_correctly_rounded():
     bad = np.nonzero(got != ref)[0]
     assert bad.size == 0, "first mismatch: %r / %r -> gpu %r host %r (%d of %d)" % (
         a[bad[0]], b[bad[0]], got[bad[0]], ref[bad[0]], bad.size, n)
+    # the division by the constant six of the PPA step (rdiv6): same operands, plus multiples of 6 +- 1 ulp
+    a[:4096] = 6.0 * k; a[4096:8192] = np.nextafter(6.0 * k, np.inf); a[8192:12288] = np.nextafter(6.0 * k, -np.inf)
+    got6 = selftest_div(torch.from_numpy(a).cuda()).cpu().numpy()
+    ref6 = a / 6.0
+    bad = np.nonzero(got6 != ref6)[0]
+    assert bad.size == 0, "rdiv6 first mismatch: %r / 6 -> gpu %r host %r (%d of %d)" % (
+        a[bad[0]], got6[bad[0]], ref6[bad[0]], bad.size, n)

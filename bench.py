@@ -74,6 +74,7 @@ def algorithmic_reals(w):
     k = {
         "vmean": 1,
         "dt": (2 if adi else 1) + nd,
+        "source": ((2 if adi else 1) + nd + (1 if pot else 0)) + (nd + (1 if adi else 0)),
         "source_a": (2 + nd + (1 if pot else 0)) + nd,
         "source_b": (1 + (1 if adi else 0) + nd) + (nd + (1 if adi else 0)),
         "source_bc": (2 + nd) + (nd + 1),

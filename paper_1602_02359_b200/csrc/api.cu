@@ -5,6 +5,7 @@
 // Product code: nothing here includes, links or calls anything under oracle/.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <string>
@@ -80,7 +81,7 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.visc = p->nu > 0.0 && geometry == FARGO_CYLINDRICAL && L.hasx && L.hasy && !L.hasz && L.xwrap;
   L.fargo = p->fargo_on != 0;
   L.adi = eos == FARGO_ADIABATIC;
-  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16;
+  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4;   // state, Phi, two transport sets, the source step's output
   const size_t pad = 32;
   auto t1 = [&](int n) { return align_up((size_t)n, pad); };
   L.table_elems = 7 * t1(L.TY + 1) + 10 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 4 * t1(L.TZ + 1) + 2 * t1(L.TX);
@@ -94,6 +95,8 @@ struct Sim : CtxBase {
   State<T> st;
   T *phi = nullptr, *v0 = nullptr, *nshift = nullptr;
   T* pool[16];
+  T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
+  bool fuse_source = false;
   Ctl* ctl = nullptr;
   fargo_params prm;
   int geometry, eos;
@@ -228,6 +231,7 @@ struct Sim : CtxBase {
     st.rho = arr(); st.e = arr(); st.vx = arr(); st.vy = arr(); st.vz = arr();
     if (L.has_pot) phi = arr();
     for (int n = 0; n < 16; ++n) pool[n] = arr();
+    for (int n = 0; n < 4; ++n) alt[n] = arr();
     if (off > p->workspace_bytes) { err = "internal: workspace overflow"; return FARGO_ENOMEM; }
 
     if (!ck(cudaMemsetAsync(base, 0, off, stream), "cudaMemsetAsync(workspace)")) return FARGO_ECUDA;
@@ -264,6 +268,7 @@ struct Sim : CtxBase {
     if (L.hasy) { slots[nq++] = 3; slots[nq++] = 4; }
     if (L.hasz) { slots[nq++] = 5; slots[nq++] = 6; }
     sweep_setup<T>();
+    fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE");
     return FARGO_OK;
   }
 
@@ -280,7 +285,7 @@ struct Sim : CtxBase {
     const size_t nact = (size_t)L.nx * L.ny * L.nz;
     // ghost-inclusive arrays start from zero, as every intermediate does
     unsigned char* a0 = (unsigned char*)st.rho;
-    unsigned char* a1 = (unsigned char*)pool[15] + align_up((size_t)L.narr * sizeof(T), 256);
+    unsigned char* a1 = (unsigned char*)alt[3] + align_up((size_t)L.narr * sizeof(T), 256);
     if (!ck(cudaMemsetAsync(a0, 0, (size_t)(a1 - a0), stream), "cudaMemsetAsync(fields)")) return FARGO_ECUDA;
     if (!ck(cudaMemsetAsync(ctl, 0, sizeof(Ctl), stream), "cudaMemsetAsync(ctl)")) return FARGO_ECUDA;
     const void* src[5] = {rho, e, vx, L.hasy ? vy : nullptr, L.hasz ? vz : nullptr};
@@ -374,27 +379,36 @@ struct Sim : CtxBase {
     const T* v0p = L.fargo ? v0 : nullptr;
     n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream); });                                           // cell 6
     if (until == FARGO_ST_DT) return n;
+    State<T> s2 = st;   // the state the transport step reads: e and v after the source step
+    if (fuse_source && until < 0) {
+      // cells 7a-7c in one pass; it reads neighbours of the state, so its output goes to arrays of its own
+      if (L.adi) s2.e = alt[0];
+      s2.vx = alt[1]; s2.vy = alt[2]; s2.vz = alt[3];
+      n += timed("source", [&] { return launch_source_fused<T>(d, st, phi, s2, stream); });
+      n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                    // cell 9
+    } else {
     // source step: intermediates live in transport set B (idle until the second pass)
-    T *vxb = set_arr(1, 0), *vyb = set_arr(1, 1), *vzb = set_arr(1, 2), *ec = set_arr(1, 3);
-    n += timed("source_a", [&] { return launch_source_a<T>(d, st, phi, vxb, vyb, vzb, stream); });                      // cell 7a
-    dbg["vxb"] = vxb; dbg["vyb"] = vyb; dbg["vzb"] = vzb;
-    if (until == FARGO_ST_SRC_A) return n;
-    T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
-    if (L.visc) { vxc = set_arr(1, 4); vyc = set_arr(1, 5); }
-    // adiabatic: 7b and 7c run as ONE kernel (e_c is never stored); compared with the oracle at stage SRC_C
-    if (L.adi) n += timed("source_bc", [&] { return launch_source_bc<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, st.e, stream); });
-    else n += timed("source_b", [&] { return launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream); });   // cell 7b
-    dbg["vxc"] = vxc; dbg["vyc"] = vyc; dbg["vzc"] = vzc; dbg["ec"] = nullptr;
-    dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
-    dbg["ed"] = st.e;
-    if (until == FARGO_ST_SRC_B || until == FARGO_ST_SRC_C) return n;
-    if (L.visc)                                                                      // cell 7d
-      n += timed("source_d", [&] { return launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream); });
-    dbg["vxd"] = st.vx; dbg["vyd"] = st.vy;
-    dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
-    if (until == FARGO_ST_SRC_D) return n;
-    n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(false, L.adi), stream); });                      // cell 9
-    if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
+      T *vxb = set_arr(1, 0), *vyb = set_arr(1, 1), *vzb = set_arr(1, 2), *ec = set_arr(1, 3);
+      n += timed("source_a", [&] { return launch_source_a<T>(d, st, phi, vxb, vyb, vzb, stream); });                      // cell 7a
+      dbg["vxb"] = vxb; dbg["vyb"] = vyb; dbg["vzb"] = vzb;
+      if (until == FARGO_ST_SRC_A) return n;
+      T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
+      if (L.visc) { vxc = set_arr(1, 4); vyc = set_arr(1, 5); }
+      // adiabatic: 7b and 7c run as ONE kernel (e_c is never stored); compared with the oracle at stage SRC_C
+      if (L.adi) n += timed("source_bc", [&] { return launch_source_bc<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, st.e, stream); });
+      else n += timed("source_b", [&] { return launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream); });   // cell 7b
+      dbg["vxc"] = vxc; dbg["vyc"] = vyc; dbg["vzc"] = vzc; dbg["ec"] = nullptr;
+      dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
+      dbg["ed"] = st.e;
+      if (until == FARGO_ST_SRC_B || until == FARGO_ST_SRC_C) return n;
+      if (L.visc)                                                                      // cell 7d
+        n += timed("source_d", [&] { return launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream); });
+      dbg["vxd"] = st.vx; dbg["vyd"] = st.vy;
+      dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
+      if (until == FARGO_ST_SRC_D) return n;
+      n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(false, L.adi), stream); });                      // cell 9
+      if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
+    }
     // transport: pass p reads set (p-1)%2 (the state on the first pass) and writes set p%2; the last pass
     // writes rho and e straight back into the state arrays, so one update leaves every array where it
     // started and the same captured graph serves every update.
@@ -409,7 +423,7 @@ struct Sim : CtxBase {
       const int ds = p % 2, ss = 1 - ds;
       SweepArgs<T> a;
       memset(&a, 0, sizeof a);
-      a.st = st;
+      a.st = s2;
       a.first = (first && L.hasx) ? 1 : 0;   // 12a fused into the X sweep
       a.v0 = (pass_kind[p] == 0 || pass_kind[p] == 3) ? v0p : nullptr;
       a.nq = nq;

@@ -324,7 +324,7 @@ __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_grou
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <typename T, int DIR, int NQ>
-__global__ void __launch_bounds__(MTHREADS) k_sweep_ring(const Dev<T> d, const SweepArgs<T> A, const int CH) {
+__global__ void __launch_bounds__(MTHREADS, 3) k_sweep_ring(const Dev<T> d, const SweepArgs<T> A, const int CH) {
   constexpr int NA = NQ + 2;   // rho, NQ quantities, the face velocity
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* const ring = reinterpret_cast<T*>(smem_raw) + threadIdx.x;   // element (slot, array) at (slot*NA + array)*MTHREADS
@@ -374,6 +374,13 @@ __global__ void __launch_bounds__(MTHREADS) k_sweep_ring(const Dev<T> d, const S
   for (int q = 0; q <= NQ; ++q) { fA[q] = fB[q] = a2[q] = F2[q] = T(0); }
   T len2 = T(0), len1 = T(0), invd1 = T(0), w1 = T(0), S1 = T(0), dtiv2 = T(0), dtiv1 = T(0);
 
+  T nL, nD, nS, nV;   // table entries of the next row to be reduced
+  {
+    const int r0 = c0 - 2;
+    const int rc = r0 < 0 ? 0 : (r0 >= TL ? TL - 1 : r0);
+    nL = tL[rc]; nD = tD[rc]; nS = tS[rc]; nV = tV[rc];
+  }
+
   // one row: f2 (in: q of row r-2; out: q of row r), f1 (q of row r-1)
   auto row_step = [&](const int n, T (&f2)[NQ + 1], T (&f1)[NQ + 1]) {
     fetch(n + RD);
@@ -381,11 +388,17 @@ __global__ void __launch_bounds__(MTHREADS) k_sweep_ring(const Dev<T> d, const S
     const int r = c0 - 2 + n;
     const T* cur = ring + ((n & (RS - 1)) * NA) * MTHREADS;
     const T* old = ring + (((n - 2) & (RS - 1)) * NA) * MTHREADS;   // row r-2 (the cell being updated)
-    const int rc = r < 0 ? 0 : (r >= TL ? TL - 1 : r);
-    const T len0 = DIR == 1 ? tL[rc] : tL[rc] * gL;
-    const T invd0 = DIR == 1 ? tD[rc] : tD[rc] * gD;
-    const T S0 = DIR == 1 ? tS[rc] * gS : gS * tS[rc];
-    const T dtiv0 = dt * (DIR == 1 ? tV[rc] * gV : gV * tV[rc]);
+    // geometry of row r was fetched one row ago (a load consumed in the row it is issued in costs a full
+    // L1 round trip per row: profiles/r01e); fetch row r+1's now
+    const T len0 = DIR == 1 ? nL : nL * gL;
+    const T invd0 = DIR == 1 ? nD : nD * gD;
+    const T S0 = DIR == 1 ? nS * gS : gS * nS;
+    const T dtiv0 = dt * (DIR == 1 ? nV * gV : gV * nV);
+    {
+      const int rn = r + 1;
+      const int rc = rn < 0 ? 0 : (rn >= TL ? TL - 1 : rn);
+      nL = tL[rc]; nD = tD[rc]; nS = tS[rc]; nV = tV[rc];
+    }
     const T w0 = cur[(NQ + 1) * MTHREADS];
     const T rho0 = cur[0];
     const T ir = rdiv(T(1), rho0);

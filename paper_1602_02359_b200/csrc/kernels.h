@@ -29,6 +29,10 @@ template <typename T> int launch_source_bc(const Dev<T>& d, const State<T>& st, 
 // cell 7c: (vc, ec) -> ed
 template <typename T> int launch_source_c(const Dev<T>& d, const T* vxc, const T* vyc, const T* vzc, const T* ec,
                                           T* ed, cudaStream_t s);
+// cells 7a-7c in ONE pass (3-D meshes, wrapped X with an even nx, no viscosity): st -> out.{e, vx, vy, vz}
+template <typename T> bool source_fused_ok(const Dev<T>& d);
+template <typename T> int launch_source_fused(const Dev<T>& d, const State<T>& st, const T* phi, const State<T>& out,
+                                              cudaStream_t s);
 // cell 7d (2-D cylindrical): (rho, vc) -> vd, with the stress tensor in tpp, trr, tpr
 template <typename T> int launch_source_d(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, T* tpp, T* trr,
                                           T* tpr, T* vxd, T* vyd, cudaStream_t s);

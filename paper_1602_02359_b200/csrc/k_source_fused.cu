@@ -9,8 +9,11 @@
 // Work decomposition (no shared memory, no barriers):
 //   X : a warp owns 64 consecutive cells of a row, two per lane (16-byte vector accesses); v_b, q and v_c of
 //       the X faces cross lanes by shuffle; lanes 0 and 31 are recomputed halo (60 cells stored per warp).
-//   Z : the thread marches along Z; v_b, q, v_c of the Z faces and the rho / P / e of the two planes behind
-//       the leading one live in registers.  Plane m = n - 2 is finished when plane n has been read.
+//   Z : the thread marches along Z; v_b, q, v_c of the Z faces live in registers.  Plane m = n - 2 is finished
+//       when plane n has been read.  The thread's own row (rho, e, v [, Phi]) is fetched SF_RD planes ahead with
+//       16-byte cp.async into a ring of SF_RS slots private to the thread (no barrier: a thread reads only what
+//       it copied itself); the ring also keeps planes n-1 and n-2, so nothing of the state is carried in
+//       registers.
 //   Y : v_b of the Y faces of rows j-1 .. j+2 is recomputed from the neighbour rows' state (served by L1/L2:
 //       the four warps of a block are four consecutive rows); one division per recomputed face.
 // Every expression is the one k_source_a / k_source_b / k_source_c evaluate for the same face or cell, in the
@@ -49,9 +52,20 @@ __device__ __forceinline__ T eos_p(const T gm1, const T e, const T rho) {   // E
 
 constexpr int SFW = 4;        // warps (consecutive rows) per block
 constexpr int SFIN = 60;      // cells stored per warp
+constexpr int SF_RD = 3;      // planes in flight
+constexpr int SF_RS = 6;      // ring slots (>= SF_RD + 3: planes n-2 .. n+SF_RD)
 
-template <typename T, int GEO, bool ADI, bool POT>
-__global__ void __launch_bounds__(32 * SFW) k_source_fused(const Dev<T> d, const State<T> st, const T* __restrict__ phi,
+__device__ __forceinline__ void sf_cp_pair(unsigned dst, const double* src) {   // one pair of cells
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void sf_cp_pair(unsigned dst, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void sf_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void sf_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename T, int GEO, bool ADI, bool POT, bool RING>
+__global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, const State<T> st, const T* __restrict__ phi,
                                                            const State<T> out, const int CH) {
   constexpr bool CURV = GEO != GEO_CART, SPH = GEO == GEO_SPH;
   constexpr int NV = ADI ? 4 : 3;   // Y faces whose v_b is needed: rows j-1 .. j-2+NV (7c needs v_c on the upper face too)
@@ -85,19 +99,57 @@ __global__ void __launch_bounds__(32 * SFW) k_source_fused(const Dev<T> d, const
   const T sxj = d.sxj[j], syj0 = d.syj[j], syj1 = d.syj[j + 1], szj = d.szj[j], invVj = d.invVj[j];
   const T ycj = d.yc[j], iycj = d.inv_yc[j];
 
-  // state carried along Z: index 1 = plane n-1, 2 = plane n-2
-  const V2<T> one = {T(1), T(1)}, zero = {T(0), T(0)};
-  V2<T> r1 = one, r2 = one, p1 = zero, p2 = zero, e1 = zero, e2 = zero, f1 = zero, f2 = zero;
-  V2<T> vbz1 = zero, wfz1 = zero, qz2 = zero, hz2 = zero, vcz2 = zero, vx1 = zero;
+  // ring of the thread's own row: slot s, array a at ((s * NAO + a) * 128 + tid) pairs; arrays: rho e vz vx vy [Phi]
+  constexpr int NAO = POT ? 6 : 5;
+  using P2 = typename SPair<T>::type;
+  extern __shared__ __align__(16) unsigned char sf_smem[];
+  const int tid = threadIdx.y * 32 + lane;
+  P2* const ring = reinterpret_cast<P2*>(sf_smem) + tid;
+  const unsigned ring_s = (unsigned)__cvta_generic_to_shared(ring);
+  const int nlast = m1 + 1;
+  auto fetch = [&](const int n) {
+    if (!RING) return;
+    if (n <= nlast) {
+      const long long l = base + (long long)n * P;
+      const unsigned dst = ring_s + (unsigned)(((n % SF_RS) * NAO) * 128 * sizeof(P2));
+      sf_cp_pair(dst, rho + l);
+      sf_cp_pair(dst + (unsigned)(1 * 128 * sizeof(P2)), en + l);
+      sf_cp_pair(dst + (unsigned)(2 * 128 * sizeof(P2)), vz + l);
+      sf_cp_pair(dst + (unsigned)(3 * 128 * sizeof(P2)), vx + l);
+      sf_cp_pair(dst + (unsigned)(4 * 128 * sizeof(P2)), vy + l);
+      if (POT) sf_cp_pair(dst + (unsigned)(5 * 128 * sizeof(P2)), phi + l);
+    }
+    sf_commit();   // one group per plane, empty past the end
+  };
+  auto own = [&](const int n, const int a) -> V2<T> {
+    if (!RING) {   // curvilinear meshes read many neighbour rows: they keep the whole L1 instead of a ring
+      const T* const arr = a == 0 ? rho : a == 1 ? en : a == 2 ? vz : a == 3 ? vx : a == 4 ? vy : phi;
+      return ldv(arr + base + (long long)n * P);
+    }
+    const P2 v = ring[((n % SF_RS) * NAO + a) * 128];
+    V2<T> o; o.a = v.x; o.b = v.y; return o;
+  };
+#pragma unroll
+  for (int q = 0; q < SF_RD; ++q) fetch(m0 - 2 + q);
+
+  // carried along Z (index 1 = plane n-1, 2 = plane n-2): only what was computed, the state is in the ring
+  const V2<T> zero = {T(0), T(0)};
+  V2<T> vbz1 = zero, wfz1 = zero, qz2 = zero, hz2 = zero, vcz2 = zero;
 
 #pragma unroll 1
   for (int n = m0 - 2; n <= m1 + 1; ++n) {
+    fetch(n + SF_RD);
+    if (RING) sf_wait<SF_RD>();   // plane n has landed
     // ---- leading plane n: v_b, q, v_c of the Z faces -------------------------------------------------------
-    const long long ln = base + (long long)n * P;
-    const V2<T> rn = ldv(rho + ln), en_ = ldv(en + ln), vzn = ldv(vz + ln);
-    V2<T> fn = zero, vxn = zero;
-    if (POT) fn = ldv(phi + ln);
-    if (SPH) vxn = ldv(vx + ln);
+    const bool warm = n > m0 - 2;   // plane n-1 is in the ring
+    const V2<T> rn = own(n, 0), en_ = own(n, 1), vzn = own(n, 2);
+    const V2<T> r1 = warm ? own(n - 1, 0) : rn, e1 = warm ? own(n - 1, 1) : en_;
+    V2<T> fn = zero, f1 = zero, vxn = zero, vx1 = zero;
+    if (POT) { fn = own(n, 5); f1 = warm ? own(n - 1, 5) : fn; }
+    if (SPH) { vxn = own(n, 3); vx1 = warm ? own(n - 1, 3) : vxn; }
+    V2<T> p1;
+    p1.a = eos_p<T, ADI>(gm1, e1.a, r1.a);
+    p1.b = eos_p<T, ADI>(gm1, e1.b, r1.b);
     V2<T> pn;
     pn.a = eos_p<T, ADI>(gm1, en_.a, rn.a);
     pn.b = eos_p<T, ADI>(gm1, en_.b, rn.b);
@@ -130,11 +182,15 @@ __global__ void __launch_bounds__(32 * SFW) k_source_fused(const Dev<T> d, const
       // ---- plane m = n - 2: X and Y faces, then the cell ---------------------------------------------------
       const int m = n - 2;
       const long long lm = base + (long long)m * P;
+      const V2<T> r2 = own(m, 0), e2 = own(m, 1), f2 = POT ? own(m, 5) : zero;
+      V2<T> p2;
+      p2.a = eos_p<T, ADI>(gm1, e2.a, r2.a);
+      p2.b = eos_p<T, ADI>(gm1, e2.b, r2.b);
       V2<T> rr[NV + 1], pp[NV + 1], ff[NV + 1], vyr[NV + 1], vxr[NV + 1], vz0[NV + 1], vz1[NV + 1];
 #pragma unroll
       for (int t = 0; t <= NV; ++t) {
         const long long lr = lm + (long long)(t - 2) * R;
-        if (t == 2) { rr[t] = r2; pp[t] = p2; ff[t] = f2; }
+        if (t == 2) { rr[t] = r2; pp[t] = p2; ff[t] = f2; }   // own row: from the ring
         else {
           rr[t] = ldv(rho + lr);
           const V2<T> ee = ldv(en + lr);
@@ -142,10 +198,10 @@ __global__ void __launch_bounds__(32 * SFW) k_source_fused(const Dev<T> d, const
           pp[t].b = eos_p<T, ADI>(gm1, ee.b, rr[t].b);
           ff[t] = POT ? ldv(phi + lr) : zero;
         }
-        vyr[t] = t >= 1 ? ldv(vy + lr) : zero;
-        vxr[t] = (CURV || t == 2) ? ldv(vx + lr) : zero;
-        vz0[t] = SPH ? ldv(vz + lr) : zero;
-        vz1[t] = SPH ? ldv(vz + lr + P) : zero;
+        vyr[t] = t == 2 ? own(m, 4) : (t >= 1 ? ldv(vy + lr) : zero);
+        vxr[t] = t == 2 ? own(m, 3) : (CURV ? ldv(vx + lr) : zero);
+        vz0[t] = SPH ? (t == 2 ? own(m, 2) : ldv(vz + lr)) : zero;
+        vz1[t] = SPH ? (t == 2 ? own(m + 1, 2) : ldv(vz + lr + P)) : zero;
       }
       const T il = invLXj * d.invRxk[m];
       // ---- X faces ----
@@ -240,9 +296,9 @@ __global__ void __launch_bounds__(32 * SFW) k_source_fused(const Dev<T> d, const
       }
     }
     // ---- shift the Z window ----
-    r2 = r1; r1 = rn; p2 = p1; p1 = pn; e2 = e1; e1 = en_; f2 = f1; f1 = fn;
-    vbz1 = vbz; wfz1 = wfz; qz2 = qz1; hz2 = hz1; vcz2 = vcz1; vx1 = vxn;
+    vbz1 = vbz; wfz1 = wfz; qz2 = qz1; hz2 = hz1; vcz2 = vcz1;
   }
+  if (RING) sf_wait<0>();
 }
 
 template <typename T>
@@ -261,8 +317,17 @@ static int launch_sf(const Dev<T>& d, const State<T>& st, const T* phi, const St
   if (CH > d.nz) CH = d.nz;
   nch = (d.nz + CH - 1) / CH;
   dim3 b(32, SFW), g(ntile, nrow, nch);
-  if (d.has_pot) k_source_fused<T, GEO, ADI, true><<<g, b, 0, s>>>(d, st, phi, out, CH);
-  else k_source_fused<T, GEO, ADI, false><<<g, b, 0, s>>>(d, st, phi, out, CH);
+  constexpr bool RING = GEO == GEO_CART;
+  const size_t pair = 2 * sizeof(T);
+  if (d.has_pot) {
+    const int sm = RING ? (int)(SF_RS * 6 * 128 * pair) : 0;
+    if (RING) cudaFuncSetAttribute(k_source_fused<T, GEO, ADI, true, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+    k_source_fused<T, GEO, ADI, true, RING><<<g, b, sm, s>>>(d, st, phi, out, CH);
+  } else {
+    const int sm = RING ? (int)(SF_RS * 5 * 128 * pair) : 0;
+    if (RING) cudaFuncSetAttribute(k_source_fused<T, GEO, ADI, false, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+    k_source_fused<T, GEO, ADI, false, RING><<<g, b, sm, s>>>(d, st, phi, out, CH);
+  }
   return 1;
 }
 

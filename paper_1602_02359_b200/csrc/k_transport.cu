@@ -321,6 +321,13 @@ template <> struct CpAsync<float> {
   }
 };
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// a load the compiler may not sink towards its use (volatile asm keeps its place among the cp.async statements)
+__device__ __forceinline__ double ld_pinned(const double* p) {
+  double v; asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ float ld_pinned(const float* p) {
+  float v; asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v;
+}
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <typename T, int DIR, int NQ>
@@ -383,22 +390,23 @@ __global__ void __launch_bounds__(MTHREADS, 3) k_sweep_ring(const Dev<T> d, cons
 
   // one row: f2 (in: q of row r-2; out: q of row r), f1 (q of row r-1)
   auto row_step = [&](const int n, T (&f2)[NQ + 1], T (&f1)[NQ + 1]) {
-    fetch(n + RD);
-    cp_wait<RD>();                                   // row n has landed
     const int r = c0 - 2 + n;
-    const T* cur = ring + ((n & (RS - 1)) * NA) * MTHREADS;
-    const T* old = ring + (((n - 2) & (RS - 1)) * NA) * MTHREADS;   // row r-2 (the cell being updated)
-    // geometry of row r was fetched one row ago (a load consumed in the row it is issued in costs a full
-    // L1 round trip per row: profiles/r01e); fetch row r+1's now
-    const T len0 = DIR == 1 ? nL : nL * gL;
-    const T invd0 = DIR == 1 ? nD : nD * gD;
-    const T S0 = DIR == 1 ? nS * gS : gS * nS;
-    const T dtiv0 = dt * (DIR == 1 ? nV * gV : gV * nV);
+    // geometry of row r was fetched one row ago (a load consumed in the row it is issued in costs a full L1
+    // round trip per row: profiles/r01e); row r+1's is fetched here, pinned ahead of the wait below
+    const T cL = nL, cD = nD, cS = nS, cV = nV;
     {
       const int rn = r + 1;
       const int rc = rn < 0 ? 0 : (rn >= TL ? TL - 1 : rn);
-      nL = tL[rc]; nD = tD[rc]; nS = tS[rc]; nV = tV[rc];
+      nL = ld_pinned(tL + rc); nD = ld_pinned(tD + rc); nS = ld_pinned(tS + rc); nV = ld_pinned(tV + rc);
     }
+    fetch(n + RD);
+    cp_wait<RD>();                                   // row n has landed
+    const T* cur = ring + ((n & (RS - 1)) * NA) * MTHREADS;
+    const T* old = ring + (((n - 2) & (RS - 1)) * NA) * MTHREADS;   // row r-2 (the cell being updated)
+    const T len0 = DIR == 1 ? cL : cL * gL;
+    const T invd0 = DIR == 1 ? cD : cD * gD;
+    const T S0 = DIR == 1 ? cS * gS : gS * cS;
+    const T dtiv0 = dt * (DIR == 1 ? cV * gV : gV * cV);
     const T w0 = cur[(NQ + 1) * MTHREADS];
     const T rho0 = cur[0];
     const T ir = rdiv(T(1), rho0);

@@ -62,6 +62,7 @@ __device__ __forceinline__ void sf_cp_pair(unsigned dst, const float* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ void sf_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void sf_prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 template <int N> __device__ __forceinline__ void sf_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <typename T, int GEO, bool ADI, bool POT, bool RING>
@@ -139,6 +140,20 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
 #pragma unroll 1
   for (int n = m0 - 2; n <= m1 + 1; ++n) {
     fetch(n + SF_RD);
+    if (n + 1 >= m0 + 2 && n + 1 <= nlast) {   // next plane's neighbour rows: into L1 while this plane is reduced
+      const long long lq = base + (long long)(n - 1) * P;
+#pragma unroll
+      for (int t = 0; t <= NV; ++t) {
+        if (t == 2) continue;
+        const long long lr = lq + (long long)(t - 2) * R;
+        sf_prefetch_l1(rho + lr);
+        sf_prefetch_l1(en + lr);
+        if (POT) sf_prefetch_l1(phi + lr);
+        if (t >= 1) sf_prefetch_l1(vy + lr);
+        if (CURV) sf_prefetch_l1(vx + lr);
+        if (SPH) { sf_prefetch_l1(vz + lr); sf_prefetch_l1(vz + lr + P); }
+      }
+    }
     if (RING) sf_wait<SF_RD>();   // plane n has landed
     // ---- leading plane n: v_b, q, v_c of the Z faces -------------------------------------------------------
     const bool warm = n > m0 - 2;   // plane n-1 is in the ring

@@ -127,6 +127,84 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
   }
 }
 
+// ---- cell 6, 3-D meshes with a wrapped X axis and an even nx: two cells per lane ----------------------------
+// A warp owns a ring (j,k) and walks it 64 cells at a time with 16-byte loads; the upper X face of the pair is
+// the next lane's first cell (lane 31 reads it).  Same expressions, in the same order, as k_dt_cells; the
+// reduction is a max, so the result is bit-equal whatever the order.
+template <typename T> struct DPair;
+template <> struct DPair<double> { using type = double2; };
+template <> struct DPair<float> { using type = float2; };
+
+template <typename T, bool ADI>
+__global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T> st, const T* __restrict__ v0) {
+  if (d.ctl->done) return;
+  using P2 = typename DPair<T>::type;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int nrow = d.ny * d.nz, nwarp = gridDim.x * (blockDim.x >> 5);
+  const int nx = d.nx;
+  T m2 = T(0);
+  for (int row = blockIdx.x * (blockDim.x >> 5) + wib; row < nrow; row += nwarp) {
+    const int j = d.ngy + row % d.ny, k = d.ngz + row / d.ny;
+    const T ilx = d.invLX(j, k), ily = d.invLY[j], ilz = d.invLZ(j, k);
+    const T ilmax = rmax(rmax(rmax(T(0), ilx), ily), ilz);
+    const T il2 = ilmax * ilmax;
+    const T I4 = d.c4 * il2;
+    const T I4sq = I4 * I4;
+    const T vm = v0 ? v0[d.rid(j, k)] : T(0);
+    const long long base = d.id(0, j, k);
+    for (int i0 = 0; i0 < nx; i0 += 64) {
+      const int i = i0 + 2 * lane;
+      const bool live = i < nx;
+      const long long l = base + (live ? i : 0);
+      const P2 r = *reinterpret_cast<const P2*>(st.rho + l);
+      const P2 e = *reinterpret_cast<const P2*>(st.e + l);
+      const P2 ax = *reinterpret_cast<const P2*>(st.vx + l);
+      const P2 ay = *reinterpret_cast<const P2*>(st.vy + l);
+      const P2 by = *reinterpret_cast<const P2*>(st.vy + l + d.pitch);
+      const P2 az = *reinterpret_cast<const P2*>(st.vz + l);
+      const P2 bz = *reinterpret_cast<const P2*>(st.vz + l + d.plane);
+      T nxt = __shfl_down_sync(0xffffffffu, ax.x, 1);
+      if (lane == 31 || i + 2 >= nx) { const int ip = i + 2 >= nx ? i + 2 - nx : i + 2; nxt = st.vx[base + (live ? ip : 0)]; }
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const T rho = c ? r.y : r.x, en = c ? e.y : e.x;
+        const T cs2 = ADI ? rdiv(d.gg1 * en, rho) : en * en;
+        const T I1sq = cs2 * il2;
+        T I2 = T(0), I3 = T(0);
+        {
+          const T a = c ? ax.y : ax.x, b = c ? nxt : ax.y;
+          I2 = rmax(I2, rabs(T(0.5) * (a + b) - vm) * ilx);
+          I3 = rmax(I3, rabs(b - a) * ilx);
+        }
+        {
+          const T a = c ? ay.y : ay.x, b = c ? by.y : by.x;
+          I2 = rmax(I2, rabs(T(0.5) * (a + b)) * ily);
+          I3 = rmax(I3, rabs(b - a) * ily);
+        }
+        {
+          const T a = c ? az.y : az.x, b = c ? bz.y : bz.x;
+          I2 = rmax(I2, rabs(T(0.5) * (a + b)) * ilz);
+          I3 = rmax(I3, rabs(b - a) * ilz);
+        }
+        I3 = d.c3 * I3;
+        const T Isq = ((I1sq + I2 * I2) + I3 * I3) + I4sq;
+        if (live) m2 = rmax(m2, Isq);
+      }
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+  __shared__ T sm[8];
+  if (lane == 0) sm[wib] = m2;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    m2 = threadIdx.x < (blockDim.x >> 5) ? sm[threadIdx.x] : T(0);
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+    if (threadIdx.x == 0) atomicMax(&d.ctl->m2bits, to_bits(m2));
+  }
+}
+
 // One block: shear limit over the active rings (Eq. 73 with V_X = v0_jk), Courant factor, overrides.
 template <typename T>
 __global__ void __launch_bounds__(256) k_dt_finish(const Dev<T> d, const T* __restrict__ v0) {
@@ -166,7 +244,13 @@ template <typename T>
 int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s) {
   const int nrow = d.ny * d.nz;
   const int grid = nrow < 148 * 8 ? nrow : 148 * 8;
-  k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0);
+  if (d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0) {
+    const int g2 = nrow < 148 * 8 * 8 ? (nrow + 7) / 8 : 148 * 8;
+    if (d.eos == EOS_ADI) k_dt_cells2<T, true><<<g2, 256, 0, s>>>(d, st, v0);
+    else k_dt_cells2<T, false><<<g2, 256, 0, s>>>(d, st, v0);
+  } else {
+    k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0);
+  }
   k_dt_finish<T><<<1, 256, 0, s>>>(d, v0);
   return 2;
 }

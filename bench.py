@@ -60,6 +60,14 @@ def make_workload(name: str):
     raise SystemExit("unknown workload " + name)
 
 
+# DRAM bytes per ACTIVE cell per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one
+# `--set full` capture at the bench's own size; profiles/r01f_fused_source.md names the command).  None = not captured.
+NCU_TRAFFIC_B_PER_CELL = {
+    "noise512": {"dt": 41.4, "source": 90.2, "sweep_x": 106.1, "sweep_y": 139.5, "sweep_z": 139.5, "newvel": 79.9},
+    "disk3d": {"vmean": 8.5, "dt": 33.0, "source": 77.2, "sweep_x": 95.1, "sweep_y": 127.2, "sweep_z": 127.2,
+               "orbital": 118.2, "newvel": 82.6},
+}
+
 CONFIG_OF = {"noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
@@ -291,7 +299,10 @@ def run_ours(args):
                          "frac": (gbs / peak) if gbs else None}
     dom = max((n for n in kernels if kernels[n]["achieved_gbs"]), key=lambda n: kernels[n]["share"])
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                "frac": kernels[dom]["frac"],
+                "traffic": (NCU_TRAFFIC_B_PER_CELL.get(args.workload, {}).get(dom) or 0) * ncell * (es / 8) or None,
+                "traffic_source": "ncu --set full, profiles/r01f_fused_source.md (bytes per cell x cells)",
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_cell"] * ncell,
                 "ms_per_launch": kernels[dom]["ms_per_launch"], "share_of_step": kernels[dom]["share"]}
     step_gbs = fused_reals * es * ncell / (ms / K * 1e-3) / 1e9

@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T
 
 // One block: shear limit over the active rings (Eq. 73 with V_X = v0_jk), Courant factor, overrides.
 template <typename T>
-__global__ void __launch_bounds__(256) k_dt_finish(const Dev<T> d, const T* __restrict__ v0) {
+__global__ void __launch_bounds__(1024) k_dt_finish(const Dev<T> d, const T* __restrict__ v0) {
   Ctl* c = d.ctl;
   if (c->done) return;
   T s = T(0);
@@ -221,11 +221,11 @@ __global__ void __launch_bounds__(256) k_dt_finish(const Dev<T> d, const T* __re
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s = rmax(s, __shfl_xor_sync(0xffffffffu, s, o));
   }
-  __shared__ T sm[8];
+  __shared__ T sm[32];
   if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int w = 1; w < 8; ++w) s = rmax(s, sm[w]);
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) s = rmax(s, sm[w]);
     const T M2 = from_bits<T>(c->m2bits);
     T dt = T(1) / rsqrt_ieee(M2);
     if (d.fargo && s > T(0)) dt = rmin(dt, d.shear_c0 / s);
@@ -251,7 +251,7 @@ int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s) 
   } else {
     k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0);
   }
-  k_dt_finish<T><<<1, 256, 0, s>>>(d, v0);
+  k_dt_finish<T><<<1, 1024, 0, s>>>(d, v0);
   return 2;
 }
 

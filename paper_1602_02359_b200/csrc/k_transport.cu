@@ -305,7 +305,11 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
 // rows r-1 and r-2, so the un-divided quantities of the cell being updated are re-read from shared
 // memory instead of living in registers.  The row loop is unrolled by two so that the two-row window of
 // q = Q / rho rotates by renaming.
-constexpr int MTHREADS = 128;
+#ifndef FG_MTHREADS
+#define FG_MTHREADS 128
+#define FG_MBLOCKS 3
+#endif
+constexpr int MTHREADS = FG_MTHREADS;
 constexpr int RD = 5;            // rows in flight
 constexpr int RS = 8;            // ring slots (>= RD + 3), a power of two
 
@@ -331,7 +335,7 @@ __device__ __forceinline__ float ld_pinned(const float* p) {
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <typename T, int DIR, int NQ>
-__global__ void __launch_bounds__(MTHREADS, 3) k_sweep_ring(const Dev<T> d, const SweepArgs<T> A, const int CH) {
+__global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T> d, const SweepArgs<T> A, const int CH) {
   constexpr int NA = NQ + 2;   // rho, NQ quantities, the face velocity
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* const ring = reinterpret_cast<T*>(smem_raw) + threadIdx.x;   // element (slot, array) at (slot*NA + array)*MTHREADS

@@ -21,6 +21,29 @@ def cart_adi_periodic(nx=37, ny=29, nz=11, nsteps=6):
     return w
 
 
+def cart_adi_periodic_even(nx=130, ny=29, nz=37, nsteps=5):
+    """Even wrapped nx: the path bench.py times (two-cell X sweep, fused source pass, two-cell dt) at a size that
+    spans three 60-cell warp tiles with a ragged tail, a row count that is no multiple of the block's 4 rows and
+    strong compressions so that 7b fires."""
+    w = W.noise_box(shape3=(nx, ny, nz), nsteps=nsteps)
+    w.e = w.e * (1.0 + _noise(w.e.shape, 1, 0.3))
+    w.vx, w.vy, w.vz = (6.0 * v for v in (w.vx, w.vy, w.vz))
+    return w
+
+
+def cart_iso_periodic(nx=66, ny=10, nz=9, nsteps=5):
+    """Isothermal Cartesian box (the `e` slot carries c_s): the fused source pass without 7c."""
+    w = W.noise_box(shape3=(nx, ny, nz), nsteps=nsteps)
+    cs = 0.8 * (1.0 + _noise(w.e.shape, 1, 0.2))
+    return W.Workload("cart_iso_periodic", w.mesh, W.CARTESIAN, W.ISOTHERMAL, W.Params(gamma=1.4), w.rho, cs,
+                      4.0 * w.vx, 4.0 * w.vy, 4.0 * w.vz, nsteps)
+
+
+def sph3d_iso_fargo_odd(nphi=45, nr=20, nth=10, nsteps=5):
+    """Odd ring length: the one-cell-per-lane X sweep, the shared-memory orbital kernel and the unfused source."""
+    return W.disk3d(nphi, nr, nth, nsteps)
+
+
 def cart_adi_mixed_bc(nx=70, ny=9, nz=40, nsteps=5):
     """Non-periodic X (ghosted X), reflecting Y, outflow/reflecting Z; strong compressions so 7b fires."""
     bc = ((R, O), (R, R), (O, R))
@@ -116,5 +139,5 @@ def nonuniform_cyl2d(nphi=50, nr=36, nsteps=6):
     return W.Workload("nonuniform_cyl2d", mesh, W.CYLINDRICAL, W.ISOTHERMAL, prm, rho, cs, vx, vy, None, nsteps)
 
 
-ALL = [cart_adi_periodic, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
+ALL = [cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
        sph3d_adi_nofargo, x_only_1d, yz_only_2d, nonuniform_cyl2d]

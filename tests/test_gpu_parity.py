@@ -126,6 +126,26 @@ def test_multi_step(make, use_graph):
     assert g.kernel_launches() > 0
 
 
+FUSED = [G.cart_adi_periodic_even, G.cart_iso_periodic, G.sph3d_iso_fargo, G.cyl3d_adi_fargo, G.sph3d_adi_nofargo]
+
+
+@pytest.mark.parametrize("make", FUSED, ids=[m.__name__ for m in FUSED])
+def test_fused_source_equals_the_kernel_sequence(make, monkeypatch):
+    """The one-pass source step (k_source_fused) against the 7a -> 7b -> 7c kernels it replaces (selected with
+    FARGO_UNFUSED_SOURCE, read at fargo_init): bit-identical fields after several updates, and both within the bar
+    of the oracle (test_multi_step)."""
+    w = make()
+    g1 = _gpu(w)
+    monkeypatch.setenv("FARGO_UNFUSED_SOURCE", "1")
+    g2 = _gpu(w)
+    monkeypatch.delenv("FARGO_UNFUSED_SOURCE")
+    g1.step(w.nsteps); g2.step(w.nsteps)
+    assert g1.time() == g2.time()
+    assert g1.kernel_launches() < g2.kernel_launches()      # the fused path really is the one that ran
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), g1.get_fields(), g2.get_fields()):
+        assert np.array_equal(a, b), _diff_report(name, a, b)
+
+
 # ---------------------------------------------------------------- the five configs ---------------------
 def _run_config(w, nsteps, precision=64, tol=TOL64):
     o, g = _oracle(w), _gpu(w, precision=precision)

@@ -91,6 +91,7 @@ def algorithmic_reals(w):
         "sweep": (1 + nq + 1) + (1 + nq),
         "orbital": (1 + nq) + (1 + nq),
         "newvel": (1 + 2 * nd) + nd,
+        "newvel_dt": (1 + 2 * nd + (1 if adi else 0)) + nd,
     }
     if not adi:
         k["source_bc"] = 0
@@ -284,6 +285,8 @@ def run_ours(args):
     g.profile(False)
     ms_prof = e2.elapsed_time(e3)
     reals, fused_reals = algorithmic_reals(w)
+    if "newvel_dt" in rep:
+        reals["dt"] = 0   # only the one-block finish is left of the dt pass: its bytes moved into newvel_dt
     peak, peak_src = measured_peak()
     total_ms = sum(v[1] for v in rep.values())
     kernels = {}

@@ -133,7 +133,7 @@ int fargo_get_array(fargo_ctx* c, const char* name, void* out);
 int fargo_profile(fargo_ctx* c, int enable);
 /* Synchronise, then write one text line per launcher into HOST buffer `buf` (len bytes):
  * "<name> <kernel launches> <total milliseconds>\n".  Names: bc vmean potential dt source_a source_b source_bc
- * source (7a-7c in one pass) source_d momenta sweep_x sweep_y sweep_z orbital newvel advance. */
+ * source (7a-7c in one pass) source_d momenta sweep_x sweep_y sweep_z orbital newvel newvel_dt (Eq. 51 + the next update's per-cell CFL rate) advance. */
 int fargo_profile_report(fargo_ctx* c, char* buf, size_t len);
 
 /* Self-test of the branch-free fp64 division the kernels use in place of a / b (csrc/common.cuh, rdiv;

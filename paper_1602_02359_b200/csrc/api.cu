@@ -97,6 +97,8 @@ struct Sim : CtxBase {
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
   bool fuse_source = false;
+  bool fuse_dt = false;   // Eq. 51 and the next update's per-cell CFL rate in one kernel (k_newvel_dt)
+  bool dt_ready = false;  // ctl->m2bits holds the running max for the coming update
   Ctl* ctl = nullptr;
   fargo_params prm;
   int geometry, eos;
@@ -269,6 +271,7 @@ struct Sim : CtxBase {
     if (L.hasz) { slots[nq++] = 5; slots[nq++] = 6; }
     sweep_setup<T>();
     fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE");
+    fuse_dt = newvel_dt_ok<T>(d) && !getenv("FARGO_UNFUSED_DT");
     return FARGO_OK;
   }
 
@@ -303,6 +306,7 @@ struct Sim : CtxBase {
     }
     if (!ck(cudaMemsetAsync(staging, 0, (size_t)L.narr * sizeof(T), stream), "cudaMemsetAsync(staging)")) return FARGO_ECUDA;
     pot_valid = false;
+    dt_ready = false;
     if (!ck(cudaGetLastError(), "set_fields launch")) return FARGO_ECUDA;
     if (!ck(cudaStreamSynchronize(stream), "set_fields sync")) return FARGO_ECUDA;
     have_fields = true; midstep = false;
@@ -377,7 +381,11 @@ struct Sim : CtxBase {
     }
     if (until == FARGO_ST_POT) return n;
     const T* v0p = L.fargo ? v0 : nullptr;
-    n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream); });                                           // cell 6
+    {                                                                                // cell 6
+      const int mode = (fuse_dt && dt_ready) ? DT_FINISH : DT_BOTH;
+      n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream, mode); });
+      dt_ready = false;   // k_dt_finish consumed and cleared the running max
+    }
     if (until == FARGO_ST_DT) return n;
     State<T> s2 = st;   // the state the transport step reads: e and v after the source step
     if (fuse_source && until < 0) {
@@ -455,7 +463,12 @@ struct Sim : CtxBase {
     QSet<T> S;
     S.rho = st.rho;
     for (int q = 0; q < 7; ++q) S.q[q] = set_arr(ls, q);
-    n += timed("newvel", [&] { return launch_newvel<T>(d, st.rho, S, st, stream); });                                 // cell 12d
+    if (fuse_dt) {                                                                   // cell 12d (+ cell 6 of the next update)
+      n += timed("newvel_dt", [&] { return launch_newvel_dt<T>(d, st.rho, st.e, S, st, stream); });
+      dt_ready = true;
+    } else {
+      n += timed("newvel", [&] { return launch_newvel<T>(d, st.rho, S, st, stream); });
+    }
     n += timed("advance", [&] { return launch_advance(ctl, prm.t_stop, stream); });
     return n;
   }
@@ -468,6 +481,13 @@ struct Sim : CtxBase {
     // the legacy default stream cannot be captured: plain launches there
     const bool graph_ok = prm.use_graph && pot_static && stream != nullptr && !prof;
     int s = 0;
+    if (graph_ok && fuse_dt && !dt_ready) {
+      // the captured sequence relies on the previous update's k_newvel_dt for the per-cell CFL rate: the first
+      // update after fargo_set_fields gets it from the dt pass, after the ghost fill it reads through
+      launches += launch_bc<T>(d, st, field_mask(true, true), stream);
+      launches += launch_dt<T>(d, st, nullptr, stream, DT_CELLS);
+      dt_ready = true;
+    }
     if (graph_ok) {
       if (!gexec) {
         if (L.has_pot && !pot_valid) { launches += potential(0.0); pot_valid = true; }   // keep it out of the graph

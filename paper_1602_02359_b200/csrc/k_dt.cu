@@ -63,12 +63,6 @@ int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp
 }
 
 // ---- cell 6 ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned long long to_bits(double v) { return (unsigned long long)__double_as_longlong(v); }
-__device__ __forceinline__ unsigned long long to_bits(float v) { return (unsigned long long)__float_as_uint(v); }
-template <typename T> __device__ __forceinline__ T from_bits(unsigned long long b);
-template <> __device__ __forceinline__ double from_bits<double>(unsigned long long b) { return __longlong_as_double((long long)b); }
-template <> __device__ __forceinline__ float from_bits<float>(unsigned long long b) { return __uint_as_float((unsigned)b); }
-
 // Per active cell: sum over the processes of Eq. 59 of the squared inverse time steps, each inverse
 // time step being the max over the directions present ("dt_i = min_j dt_ij").  max is exact,
 // so the block/grid reduction order does not matter: dt is bit-reproducible.
@@ -241,9 +235,13 @@ __global__ void __launch_bounds__(1024) k_dt_finish(const Dev<T> d, const T* __r
 }
 
 template <typename T>
-int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s) {
+int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode) {
   const int nrow = d.ny * d.nz;
   const int grid = nrow < 148 * 8 ? nrow : 148 * 8;
+  if (mode == DT_FINISH) {   // the per-cell max was accumulated by k_newvel_dt at the end of the previous update
+    k_dt_finish<T><<<1, 1024, 0, s>>>(d, v0);
+    return 1;
+  }
   if (d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0) {
     const int g2 = nrow < 148 * 8 * 8 ? (nrow + 7) / 8 : 148 * 8;
     if (d.eos == EOS_ADI) k_dt_cells2<T, true><<<g2, 256, 0, s>>>(d, st, v0);
@@ -251,6 +249,7 @@ int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s) 
   } else {
     k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0);
   }
+  if (mode == DT_CELLS) return 1;
   k_dt_finish<T><<<1, 1024, 0, s>>>(d, v0);
   return 2;
 }
@@ -280,7 +279,7 @@ int launch_selftest_div(const double* a, const double* b, double* out, long long
 #define INST(T)                                                                              \
   template int launch_vmean<T>(const Dev<T>&, const T*, T*, cudaStream_t);                   \
   template int launch_potential<T>(const Dev<T>&, T*, T, T, T, T, T, cudaStream_t);          \
-  template int launch_dt<T>(const Dev<T>&, const State<T>&, const T*, cudaStream_t);
+  template int launch_dt<T>(const Dev<T>&, const State<T>&, const T*, cudaStream_t, int);
 INST(double)
 INST(float)
 #undef INST

@@ -555,10 +555,89 @@ int launch_newvel(const Dev<T>& d, const T* rho, const QSet<T>& set, const State
   return 1;
 }
 
+// ---- 12d + cell 6 of the NEXT update: Eq. 51, then the CFL rate of the new state -------------------------------
+// Meshes without orbital advection, X wrapped, Y and Z periodic.  The cell's new velocities are stored as k_newvel
+// stores them; the velocities on its three upper faces are re-formed from the neighbours' momenta (one division
+// each), with the index the periodic ghost fill of the next update would copy from, and the per-cell rate of
+// Eq. 59 (same expressions as k_dt_cells) goes into the running max that k_dt_finish of the next update turns into
+// dt.  The dt pass (40 B per cell) disappears; newvel reads e in addition (88 B per cell instead of 80 + 40).
+template <typename T, bool ADI>
+__global__ void __launch_bounds__(128) k_newvel_dt(const Dev<T> d, const T* __restrict__ rho, const T* __restrict__ en,
+                                                   const QSet<T> S, const State<T> st) {
+  if (d.ctl->done) return;
+  const int ia = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = ia < d.nx;
+  const int i = live ? ia : 0, j = d.ngy + blockIdx.y, k = d.ngz + blockIdx.z;
+  const long long row = d.id(0, j, k), l = row + i;
+  const long long lxm = row + (i == 0 ? d.nx - 1 : i - 1), lxp = row + (i + 1 == d.nx ? 0 : i + 1);
+  // upper neighbours in Y and Z: where the periodic ghost fill takes the face value from
+  const int jp = j + 1 == d.ngy + d.ny ? d.ngy : j + 1, kp = k + 1 == d.ngz + d.nz ? d.ngz : k + 1;
+  const long long lyp = d.id(i, jp, k), lzp = d.id(i, j, kp);
+  const T r0 = rho[l];
+  const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, irx = d.invRx(j, k), irz = d.invRzj[j];
+  // Eq. 51 on the three lower faces (stored) ...
+  const T ax = (rdiv(S.q[2][lxm] + S.q[1][l], rho[lxm] + r0) - rx2om) * irx;
+  const T ay = rdiv(S.q[4][l - d.pitch] + S.q[3][l], rho[l - d.pitch] + r0);
+  const T az = rdiv(S.q[6][l - d.plane] + S.q[5][l], rho[l - d.plane] + r0) * irz;
+  // ... and on the three upper faces: the neighbours' own values.  X: the next lane's (re-formed at the end of the
+  // warp and of the ring); Y, Z: re-formed from this cell's and the upper neighbour's momenta, or, on the last active
+  // row / plane, at the index the periodic ghost fill copies from
+  T bx = __shfl_down_sync(0xffffffffu, ax, 1);
+  if ((threadIdx.x & 31) == 31 || i + 1 >= d.nx) bx = (rdiv(S.q[2][l] + S.q[1][lxp], r0 + rho[lxp]) - rx2om) * irx;
+  const bool wy = jp != j + 1, wz = kp != k + 1;   // uniform over the block
+  const T by = rdiv((wy ? S.q[4][lyp - d.pitch] : S.q[4][l]) + S.q[3][lyp], (wy ? rho[lyp - d.pitch] : r0) + rho[lyp]);
+  const T bz = rdiv((wz ? S.q[6][lzp - d.plane] : S.q[6][l]) + S.q[5][lzp], (wz ? rho[lzp - d.plane] : r0) + rho[lzp]) * irz;
+  if (live) { st.vx[l] = ax; st.vy[l] = ay; st.vz[l] = az; }
+  // Eq. 59 for the new state
+  const T ilx = d.invLX(j, k), ily = d.invLY[j], ilz = d.invLZ(j, k);
+  const T ilmax = rmax(rmax(rmax(T(0), ilx), ily), ilz);
+  const T il2 = ilmax * ilmax;
+  const T I4 = d.c4 * il2;
+  const T e0 = en[l];
+  const T cs2 = ADI ? rdiv(d.gg1 * e0, r0) : e0 * e0;
+  const T I1sq = cs2 * il2;
+  T I2 = T(0), I3 = T(0);
+  I2 = rmax(I2, rabs(T(0.5) * (ax + bx)) * ilx);
+  I3 = rmax(I3, rabs(bx - ax) * ilx);
+  I2 = rmax(I2, rabs(T(0.5) * (ay + by)) * ily);
+  I3 = rmax(I3, rabs(by - ay) * ily);
+  I2 = rmax(I2, rabs(T(0.5) * (az + bz)) * ilz);
+  I3 = rmax(I3, rabs(bz - az) * ilz);
+  I3 = d.c3 * I3;
+  T m2 = live ? ((I1sq + I2 * I2) + I3 * I3) + I4 * I4 : T(0);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+  __shared__ T sm[4];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m2;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    m2 = rmax(rmax(sm[0], sm[1]), rmax(sm[2], sm[3]));
+    // a million blocks, one address: only a block that raises the running max pays for the atomic
+    const unsigned long long b = to_bits(m2);
+    if (b > *(volatile unsigned long long*)&d.ctl->m2bits) atomicMax(&d.ctl->m2bits, b);
+  }
+}
+
+template <typename T>
+bool newvel_dt_ok(const Dev<T>& d) {
+  return d.hasx && d.hasy && d.hasz && d.xwrap && !d.fargo && d.bc[1][0] == BC_PERIODIC && d.bc[1][1] == BC_PERIODIC &&
+         d.bc[2][0] == BC_PERIODIC && d.bc[2][1] == BC_PERIODIC;
+}
+
+template <typename T>
+int launch_newvel_dt(const Dev<T>& d, const T* rho, const T* en, const QSet<T>& set, const State<T>& st, cudaStream_t s) {
+  dim3 b(128), g((d.nx + 127) / 128, d.ny, d.nz);
+  if (d.eos == EOS_ADI) k_newvel_dt<T, true><<<g, b, 0, s>>>(d, rho, en, set, st);
+  else k_newvel_dt<T, false><<<g, b, 0, s>>>(d, rho, en, set, st);
+  return 1;
+}
+
 #define INST(T)                                                                                    \
   template int launch_momenta<T>(const Dev<T>&, const State<T>&, const QSet<T>&, cudaStream_t);   \
   template int launch_sweep<T>(const Dev<T>&, const SweepArgs<T>&, int, cudaStream_t);             \
-  template int launch_newvel<T>(const Dev<T>&, const T*, const QSet<T>&, const State<T>&, cudaStream_t);
+  template int launch_newvel<T>(const Dev<T>&, const T*, const QSet<T>&, const State<T>&, cudaStream_t);       \
+  template bool newvel_dt_ok<T>(const Dev<T>&);                                                              \
+  template int launch_newvel_dt<T>(const Dev<T>&, const T*, const T*, const QSet<T>&, const State<T>&, cudaStream_t);
 INST(double)
 INST(float)
 #undef INST

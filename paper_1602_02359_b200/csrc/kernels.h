@@ -16,7 +16,8 @@ template <typename T> int launch_vmean(const Dev<T>& d, const T* vx, T* v0, cuda
 template <typename T> int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2,
                                            cudaStream_t s);
 // cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
-template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s);
+enum { DT_BOTH = 0, DT_FINISH = 1, DT_CELLS = 2 };   // per-cell max + finish | finish only | per-cell max only
+template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode = DT_BOTH);
 // cell 7a: st -> vb[3]
 template <typename T> int launch_source_a(const Dev<T>& d, const State<T>& st, const T* phi, T* vxb, T* vyb, T* vzb,
                                           cudaStream_t s);
@@ -57,6 +58,11 @@ template <typename T> int launch_orbital(const Dev<T>& d, const SweepArgs<T>& a,
 // cell 12d: Eq. 51; then the clock advances
 template <typename T> int launch_newvel(const Dev<T>& d, const T* rho, const QSet<T>& set, const State<T>& st,
                                         cudaStream_t s);
+// cell 12d fused with cell 6 of the next update (no orbital advection, X wrapped, Y and Z periodic): Eq. 51, then the
+// per-cell rate of Eq. 59 for the new state into ctl->m2bits; launch_dt(..., DT_FINISH) finishes it
+template <typename T> bool newvel_dt_ok(const Dev<T>& d);
+template <typename T> int launch_newvel_dt(const Dev<T>& d, const T* rho, const T* e, const QSet<T>& set, const State<T>& st,
+                                           cudaStream_t s);
 template <typename T> int launch_copy(const Dev<T>& d, const T* src, T* dst, cudaStream_t s);
 int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s);
 // out[n] = rdiv(a[n], b[n]): the kernels' branch-free division, exposed for its self-test

@@ -148,14 +148,14 @@ __device__ __forceinline__ void ppa_pair(const T fA, const T fB, const bool fwd,
   T flA = o_up1(fuB), frA = fuA, flB = fuA, frB = fuB;
   ppa_limit(fA, flatA, flA, frA);
   ppa_limit(fB, flatB, flB, frB);
-  if (fwd) {   // warp-uniform: the whole ring moves one way
-    sA = (frA + x * (fA - frA)) + x1x * ((T(2) * fA - frA) - flA);
-    sB = (frB + x * (fB - frB)) + x1x * ((T(2) * fB - frB) - flB);
-  } else {
-    const T fln = o_dn1(flA), frn = o_dn1(frA);
-    sA = (flB + x * (fB - flB)) + x1x * ((T(2) * fB - frB) - flB);
-    sB = (fln + x * (fn - fln)) + x1x * ((T(2) * fn - frn) - fln);
-  }
+  // the upwind cell of a face is the cell itself (xi >= 0) or the next one; selected without a branch so that the
+  // chains of the different quantities stay in one basic block and interleave
+  const T fln = o_dn1(flA), frn = o_dn1(frA);
+  const T uA = fwd ? fA : fB, ulA = fwd ? flA : flB, urA = fwd ? frA : frB;
+  const T uB = fwd ? fB : fn, ulB = fwd ? flB : fln, urB = fwd ? frB : frn;
+  const T eA = fwd ? urA : ulA, eB = fwd ? urB : ulB;
+  sA = (eA + x * (uA - eA)) + x1x * ((T(2) * uA - urA) - ulA);
+  sB = (eB + x * (uB - eB)) + x1x * ((T(2) * uB - urB) - ulB);
 }
 
 template <typename T> struct OPair;

@@ -205,10 +205,9 @@ __global__ void __launch_bounds__(32 * O2W) k_orbital2(const Dev<T> d, const Swe
   {
     const T Fm = o_up1(FrB);
     const T oA = r2.x - g * (FrA - Fm), oB = r2.y - g * (FrB - FrA);
-    if (stA) {
-      if (vec && stB) { P2 o; o.x = oA; o.y = oB; *reinterpret_cast<P2*>(A.drho + row + io) = o; }
-      else { A.drho[row + io] = oA; if (stB) A.drho[row + io1] = oB; }
-    }
+    st2_if(A.drho + row + io, oA, oB, vec && stB);
+    st_if(A.drho + row + io, oA, stA && !(vec && stB));
+    st_if(A.drho + row + io1, oB, stB && !vec);
   }
 #pragma unroll
   for (int q = 0; q < NQ; ++q) {
@@ -216,10 +215,9 @@ __global__ void __launch_bounds__(32 * O2W) k_orbital2(const Dev<T> d, const Swe
     const T FA = FrA * sA, FB = FrB * sB;
     const T Fm = o_up1(FB);
     const T oA = Q2[q].x - g * (FA - Fm), oB = Q2[q].y - g * (FB - FA);
-    if (stA) {
-      if (vec && stB) { P2 o; o.x = oA; o.y = oB; *reinterpret_cast<P2*>(A.dq[q] + row + io) = o; }
-      else { A.dq[q][row + io] = oA; if (stB) A.dq[q][row + io1] = oB; }
-    }
+    st2_if(A.dq[q] + row + io, oA, oB, vec && stB);
+    st_if(A.dq[q] + row + io, oA, stA && !(vec && stB));
+    st_if(A.dq[q] + row + io1, oB, stB && !vec);
   }
 }
 

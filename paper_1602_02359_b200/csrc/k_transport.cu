@@ -266,12 +266,12 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
     Fr[0] = (w[0] * s0) * Sm;
     Fr[1] = (w[1] * s1) * Sm;
     const T Fn = shfl_dn1(Fr[0]);
-    if (store) {
+    {
       const T o0 = r[0] - dtiv * (Fr[1] - Fr[0]), o1 = r[1] - dtiv * (Fn - Fr[1]);
-      if (WRAP) st_pair(A.drho + l, o0, o1);
+      if (WRAP) st2_if(A.drho + l, o0, o1, store);
       else {
-        A.drho[l] = (i >= 2 && i < d.TX - 2) ? o0 : r[0];
-        if (i + 1 < d.TX) A.drho[l + 1] = (i + 1 >= 2 && i + 1 < d.TX - 2) ? o1 : r[1];
+        st_if(A.drho + l, (i >= 2 && i < d.TX - 2) ? o0 : r[0], store);
+        st_if(A.drho + l + 1, (i + 1 >= 2 && i + 1 < d.TX - 2) ? o1 : r[1], store && i + 1 < d.TX);
       }
     }
   }
@@ -286,12 +286,12 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
     const T s1 = up[1] ? f0 + a0 * hup[1] : f1 - a1 * hdn[1];
     const T F0 = Fr[0] * s0, F1 = Fr[1] * s1;
     const T Fn = shfl_dn1(F0);
-    if (store) {
+    {
       const T o0 = Q[q][0] - dtiv * (F1 - F0), o1 = Q[q][1] - dtiv * (Fn - F1);
-      if (WRAP) st_pair(A.dq[q] + l, o0, o1);
+      if (WRAP) st2_if(A.dq[q] + l, o0, o1, store);
       else {
-        A.dq[q][l] = (i >= 2 && i < d.TX - 2) ? o0 : Q[q][0];
-        if (i + 1 < d.TX) A.dq[q][l + 1] = (i + 1 >= 2 && i + 1 < d.TX - 2) ? o1 : Q[q][1];
+        st_if(A.dq[q] + l, (i >= 2 && i < d.TX - 2) ? o0 : Q[q][0], store);
+        st_if(A.dq[q] + l + 1, (i + 1 >= 2 && i + 1 < d.TX - 2) ? o1 : Q[q][1], store && i + 1 < d.TX);
       }
     }
   }
@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
       const T a1 = vl_slope(f2[0], f1[0], f0, invd1, invd0);
       const T rs = up ? f2[0] + a2[0] * hup : f1[0] - a1 * hdn;
       Fr = (w1 * rs) * S1;
-      if (wr) { const T Qo = old[0]; A.drho[lo] = upd ? Qo - dtiv2 * (Fr - F2[0]) : Qo; }
+      { const T Qo = old[0]; st_if(A.drho + lo, upd ? Qo - dtiv2 * (Fr - F2[0]) : Qo, wr); }
       f2[0] = f0; a2[0] = a1; F2[0] = Fr;
     }
 #pragma unroll
@@ -437,7 +437,7 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
       const T a1 = vl_slope(f2[q], f1[q], f0, invd1, invd0);
       const T fs = up ? f2[q] + a2[q] * hup : f1[q] - a1 * hdn;
       const T F1 = Fr * fs;
-      if (wr) { const T Qo = old[q * MTHREADS]; A.dq[q - 1][lo] = upd ? Qo - dtiv2 * (F1 - F2[q]) : Qo; }
+      { const T Qo = old[q * MTHREADS]; st_if(A.dq[q - 1] + lo, upd ? Qo - dtiv2 * (F1 - F2[q]) : Qo, wr); }
       f2[q] = f0; a2[q] = a1; F2[q] = F1;
     }
     len2 = len1; len1 = len0; invd1 = invd0; w1 = w0; S1 = S0; dtiv2 = dtiv1; dtiv1 = dtiv0;

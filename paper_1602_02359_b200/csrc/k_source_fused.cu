@@ -285,11 +285,9 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
         }
       }
       // ---- the cell: 7b heating, 7c compression (readings G8, G19) ----
-      if (store) {
-        stv(out.vx + lm, vcx.a, vcx.b);
-        stv(out.vy + lm, vcy.a, vcy.b);
-        stv(out.vz + lm, vcz2.a, vcz2.b);
-      }
+      st2_if(out.vx + lm, vcx.a, vcx.b, store);
+      st2_if(out.vy + lm, vcy.a, vcy.b, store);
+      st2_if(out.vz + lm, vcz2.a, vcz2.b, store);
       if (ADI) {
         const T ilZ = d.invdz[m] * invRzj;
         const T Sz0 = szj * d.szk[m], Sz1 = szj * d.szk[m + 1];
@@ -307,7 +305,7 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
           const T a = hd * D;
           ed[c] = rdiv(ec * (T(1) - a), T(1) + a);
         }
-        if (store) stv(out.e + lm, ed[0], ed[1]);
+        st2_if(out.e + lm, ed[0], ed[1], store);
       }
     }
     // ---- shift the Z window ----

@@ -26,7 +26,7 @@ extern "C" int oracle_init(oracle_ctx** out, const oracle_mesh* m, int geometry,
   orc_build_tables(*c, *m);
   const size_t n = c->ncell();
   for (vec* f : {&c->rho, &c->e, &c->vx, &c->vy, &c->vz, &c->phi, &c->vxb, &c->vyb, &c->vzb, &c->vxc, &c->vyc,
-                 &c->vzc, &c->ec, &c->ed, &c->vxd, &c->vyd, &c->pxm, &c->pxp, &c->pym, &c->pyp, &c->pzm, &c->pzp})
+                 &c->vzc, &c->ec, &c->ed, &c->vxd, &c->vyd, &c->vzd, &c->pxm, &c->pxp, &c->pym, &c->pyp, &c->pzm, &c->pzp})
     f->assign(n, 0.0);
   c->v0.assign((size_t)c->TY * c->TZ, 0.0);
   c->nshift.assign((size_t)c->TY * c->TZ, 0.0);
@@ -91,8 +91,8 @@ static void full_update(oracle_ctx* c, int until) {
   orc_source_b(o);                                              if (until == ORC_ST_SRC_B) return;    // cell 7b
   orc_source_c(o);                                              if (until == ORC_ST_SRC_C) return;    // cell 7c
   orc_source_d(o);                                              if (until == ORC_ST_SRC_D) return;    // cell 7d
-  // the source step leaves its result in (rho, ed, vxd, vyd, vzc); make it the state
-  o.e = o.ed; o.vx = o.vxd; o.vy = o.vyd; o.vz = o.vzc;
+  // the source step leaves its result in (rho, ed, vxd, vyd, vzd); make it the state
+  o.e = o.ed; o.vx = o.vxd; o.vy = o.vyd; o.vz = o.vzd;
   orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);                 if (until == ORC_ST_BC2) return;      // cell 9
   orc_momenta(o);                                               if (until == ORC_ST_MOM) return;      // cell 12a
   orc_sweep(o, 0);                                              if (until == ORC_ST_SWEEP_X) return;  // cells 12b-c
@@ -135,7 +135,7 @@ extern "C" int oracle_run_stage(oracle_ctx* c, int stage) {
     case ORC_ST_SRC_C: orc_source_c(o); break;
     case ORC_ST_SRC_D: orc_source_d(o); break;
     case ORC_ST_BC2:
-      o.e = o.ed; o.vx = o.vxd; o.vy = o.vyd; o.vz = o.vzc;
+      o.e = o.ed; o.vx = o.vxd; o.vy = o.vyd; o.vz = o.vzd;
       orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);
       break;
     case ORC_ST_MOM: orc_momenta(o); break;
@@ -156,7 +156,7 @@ static vec* find_array(oracle_ctx* c, const char* name) {
   const std::map<std::string, vec*> m = {
       {"rho", &c->rho}, {"e", &c->e}, {"vx", &c->vx}, {"vy", &c->vy}, {"vz", &c->vz}, {"phi", &c->phi},
       {"vxb", &c->vxb}, {"vyb", &c->vyb}, {"vzb", &c->vzb}, {"vxc", &c->vxc}, {"vyc", &c->vyc}, {"vzc", &c->vzc},
-      {"ec", &c->ec}, {"ed", &c->ed}, {"vxd", &c->vxd}, {"vyd", &c->vyd}, {"pxm", &c->pxm}, {"pxp", &c->pxp},
+      {"ec", &c->ec}, {"ed", &c->ed}, {"vxd", &c->vxd}, {"vyd", &c->vyd}, {"vzd", &c->vzd}, {"pxm", &c->pxm}, {"pxp", &c->pxp},
       {"pym", &c->pym}, {"pyp", &c->pyp}, {"pzm", &c->pzm}, {"pzp", &c->pzp}, {"v0", &c->v0},
       {"nshift", &c->nshift}, {"xi", &c->xi}};
   auto it = m.find(name ? name : "");

@@ -61,7 +61,7 @@ int oracle_step_until(oracle_ctx* c, int stage);
 int oracle_run_stage(oracle_ctx* c, int stage);
 int oracle_set_dt(oracle_ctx* c, double dt);
 /* Copy a named internal array INCLUDING ghosts (TX*TY*TZ doubles, or TY*TZ for "v0"/"nshift").
- * names: rho e vx vy vz phi vxb vyb vzb vxc vyc vzc ec ed vxd vyd pxm pxp pym pyp pzm pzp v0 nshift */
+ * names: rho e vx vy vz phi vxb vyb vzb vxc vyc vzc ec ed vxd vyd vzd pxm pxp pym pyp pzm pzp v0 nshift */
 int oracle_get_array(oracle_ctx* c, const char* name, double* out);
 int oracle_set_array(oracle_ctx* c, const char* name, const double* in);
 int oracle_dims(oracle_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz);

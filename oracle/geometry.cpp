@@ -78,10 +78,12 @@ void orc_build_tables(oracle_ctx& c, const oracle_mesh& m) {
   c.sxk.resize(TZ); c.syk.resize(TZ); c.inv_syk.resize(TZ); c.szk.resize(TZ + 1);
   c.Rxk.resize(TZ); c.invRxk.resize(TZ);
   c.sin_zc.resize(TZ); c.cos_zc.resize(TZ); c.sin_ze.resize(TZ + 1); c.cos_ze.resize(TZ + 1); c.cot_ze.resize(TZ + 1);
+  c.cot_zc.resize(TZ); c.inv_sin_ze.resize(TZ + 1);
   for (int k = 0; k <= TZ; ++k) {
     c.sin_ze[k] = std::sin(c.ze[k]);
     c.cos_ze[k] = std::cos(c.ze[k]);
     c.cot_ze[k] = c.cos_ze[k] / c.sin_ze[k];
+    c.inv_sin_ze[k] = 1.0 / c.sin_ze[k];
     c.szk[k] = (c.geometry == ORC_SPHERICAL) ? c.sin_ze[k] : 1.0;
   }
   for (int k = 0; k < TZ; ++k) {
@@ -91,6 +93,7 @@ void orc_build_tables(oracle_ctx& c, const oracle_mesh& m) {
     c.invdz[k] = 1.0 / c.dz[k];
     c.sin_zc[k] = std::sin(c.zc[k]);
     c.cos_zc[k] = std::cos(c.zc[k]);
+    c.cot_zc[k] = c.cos_zc[k] / c.sin_zc[k];
     c.sxk[k] = z1 - z0;
     switch (c.geometry) {
       case ORC_CARTESIAN: c.syk[k] = dx * (z1 - z0); c.Rxk[k] = 1.0; break;

@@ -34,6 +34,7 @@ struct oracle_ctx {
   vec LXj, invLXj;                     // LX(j,k) = LXj[j]*Rxk[k],  LXj = dx*Rxj
   vec Rzj, invRzj;                     // R_z(j) = 1 | 1 | r
   vec sin_zc, sin_ze, cos_zc, cos_ze, cot_ze;   // host libm tables (no transcendental elsewhere)
+  vec cot_zc, inv_sin_ze;                        // cos/sin at centres, 1/sin at edges (3-D viscous stress)
   vec cos_xc, sin_xc;                  // cos/sin of the azimuth of cell centres
 
   // ---- fields, ghost-inclusive, X fastest ----------------------------------------------------
@@ -42,7 +43,7 @@ struct oracle_ctx {
   vec vxb, vyb, vzb;                   // after 7a
   vec vxc, vyc, vzc, ec;               // after 7b
   vec ed;                              // after 7c
-  vec vxd, vyd;                        // after 7d (2-D cylindrical)
+  vec vxd, vyd, vzd;                   // after 7d (2-D cylindrical; 3-D in all three geometries)
   vec pxm, pxp, pym, pyp, pzm, pzp;    // left/right momenta (Eqs. 49-50)
   vec v0;                              // ring mean velocity, TY*TZ
   vec nshift;                          // integer shift per ring (stored as double), TY*TZ
@@ -85,6 +86,8 @@ void orc_source_a(oracle_ctx& c);
 void orc_source_b(oracle_ctx& c);
 void orc_source_c(oracle_ctx& c);
 void orc_source_d(oracle_ctx& c);
+bool orc_visc3d_on(const oracle_ctx& c);
+void orc_source_d3(oracle_ctx& c);   // viscosity3d.cpp
 void orc_momenta(oracle_ctx& c);
 void orc_sweep(oracle_ctx& c, int dir);
 void orc_orbital_frac(oracle_ctx& c);

@@ -5,7 +5,8 @@
 #include "oracle_impl.hpp"
 
 void orc_source_d(oracle_ctx& c) {
-  c.vxd = c.vxc; c.vyd = c.vyc;
+  if (orc_visc3d_on(c)) { orc_source_d3(c); return; }   // 3-D meshes, all geometries: viscosity3d.cpp
+  c.vxd = c.vxc; c.vyd = c.vyc; c.vzd = c.vzc;
   const bool on = c.p.nu > 0.0 && c.geometry == ORC_CYLINDRICAL && c.hasx && c.hasy && !c.hasz && c.xwrap;
   if (!on) return;   // other geometries: SURVEY.md 8(f) NEXT-1
   const double dt = c.dt, nu = c.p.nu, two3 = 2.0 / 3.0, invdx = 1.0 / c.dx;

@@ -42,7 +42,7 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 struct Layout {   // sizes shared by fargo_workspace_bytes and fargo_init
   int nx, ny, nz, ngx, ngy, ngz, TX, TY, TZ;
   long long pitch, plane, narr;
-  bool xwrap, hasx, hasy, hasz, has_pot, visc, fargo, adi;
+  bool xwrap, hasx, hasy, hasz, has_pot, visc, visc3d, fargo, adi;
   int n3d;             // number of 3-D arrays
   size_t table_elems;  // total 1-D table elements (each table padded to 32 elements)
   size_t bytes(size_t es) const {
@@ -78,13 +78,14 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.plane = L.pitch * L.TY;
   L.narr = L.plane * L.TZ;
   L.has_pot = geometry != FARGO_CARTESIAN && (p->gm_star != 0.0 || p->planet_mass != 0.0);
-  L.visc = p->nu > 0.0 && geometry == FARGO_CYLINDRICAL && L.hasx && L.hasy && !L.hasz && L.xwrap;
+  L.visc3d = p->nu > 0.0 && L.hasx && L.hasy && L.hasz;                                    // Eqs. B1-B6, any geometry
+  L.visc = L.visc3d || (p->nu > 0.0 && geometry == FARGO_CYLINDRICAL && L.hasx && L.hasy && !L.hasz && L.xwrap);
   L.fargo = p->fargo_on != 0;
   L.adi = eos == FARGO_ADIABATIC;
   L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4;   // state, Phi, two transport sets, the source step's output
   const size_t pad = 32;
   auto t1 = [&](int n) { return align_up((size_t)n, pad); };
-  L.table_elems = 7 * t1(L.TY + 1) + 10 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 4 * t1(L.TZ + 1) + 2 * t1(L.TX);
+  L.table_elems = 7 * t1(L.TY + 1) + 10 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 6 * t1(L.TZ + 1) + 2 * t1(L.TX);
   return true;
 }
 
@@ -223,6 +224,7 @@ struct Sim : CtxBase {
     d.Rxk = put(ht.Rxk); d.invRxk = put(ht.invRxk);
     d.sin_zc = put(ht.sin_zc); d.cos_zc = put(ht.cos_zc); d.sin_ze = put(ht.sin_ze); d.cot_ze = put(ht.cot_ze);
     d.cos_xc = put(ht.cos_xc); d.sin_xc = put(ht.sin_xc);
+    d.cot_zc = put(ht.cot_zc); d.inv_sin_ze = put(ht.inv_sin_ze);
     if (tpos > L.table_elems) { err = "internal: table area overflow"; return FARGO_EINVAL; }
     off += align_up(L.table_elems * sizeof(T), 256);
     const size_t ringb = align_up((size_t)L.TY * L.TZ * sizeof(T), 256);
@@ -402,6 +404,7 @@ struct Sim : CtxBase {
       if (until == FARGO_ST_SRC_A) return n;
       T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
       if (L.visc) { vxc = set_arr(1, 4); vyc = set_arr(1, 5); }
+      if (L.visc3d) vzc = set_arr(1, 6);
       // adiabatic: 7b and 7c run as ONE kernel (e_c is never stored); compared with the oracle at stage SRC_C
       if (L.adi) n += timed("source_bc", [&] { return launch_source_bc<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, st.e, stream); });
       else n += timed("source_b", [&] { return launch_source_b<T>(d, st, vxb, vyb, vzb, vxc, vyc, vzc, ec, stream); });   // cell 7b
@@ -409,9 +412,13 @@ struct Sim : CtxBase {
       dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
       dbg["ed"] = st.e;
       if (until == FARGO_ST_SRC_B || until == FARGO_ST_SRC_C) return n;
-      if (L.visc)                                                                      // cell 7d
+      if (L.visc3d) {                                                                  // cell 7d, 3-D (Eqs. B1-B6)
+        T* tens[6] = {set_arr(0, -1), set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), set_arr(0, 3), set_arr(0, 4)};
+        n += timed("source_d", [&] { return launch_source_d3<T>(d, st.rho, vxc, vyc, vzc, tens, st.vx, st.vy, st.vz, stream); });
+      } else if (L.visc) {                                                             // cell 7d, 2-D cylindrical
         n += timed("source_d", [&] { return launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream); });
-      dbg["vxd"] = st.vx; dbg["vyd"] = st.vy;
+      }
+      dbg["vxd"] = st.vx; dbg["vyd"] = st.vy; dbg["vzd"] = st.vz;
       dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
       if (until == FARGO_ST_SRC_D) return n;
       n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(false, L.adi), stream); });                      // cell 9

@@ -38,6 +38,10 @@ template <typename T> int launch_source_fused(const Dev<T>& d, const State<T>& s
 template <typename T> int launch_source_d(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, T* tpp, T* trr,
                                           T* tpr, T* vxd, T* vyd, cudaStream_t s);
 
+// cell 7d on a 3-D mesh, all three geometries (Eqs. B1-B6): (rho, vc) -> vd; t[0..5] = xx yy zz xy xz yz
+template <typename T> int launch_source_d3(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, const T* vzc,
+                                           T* const* t, T* vxd, T* vyd, T* vzd, cudaStream_t s);
+
 // cells 12a-12c: one directional sweep.  first != 0: the momenta are formed from the state (12a fused).
 template <typename T> struct SweepArgs {
   State<T> st;        // state: e and velocities for the momenta (first pass); the frozen face velocities

@@ -80,10 +80,12 @@ void build_tables(HostTables& t, int geometry, int TX, int TY, int TZ, int ngx, 
   // vertical / polar (k) tables
   std::vector<double> cos_ze(TZ + 1);
   t.sin_ze.resize(TZ + 1); t.cot_ze.resize(TZ + 1); t.szk.resize(TZ + 1);
+  t.inv_sin_ze.resize(TZ + 1); t.cot_zc.resize(TZ);
   for (int k = 0; k <= TZ; ++k) {
     t.sin_ze[k] = std::sin(ze[k]);
     cos_ze[k] = std::cos(ze[k]);
     t.cot_ze[k] = cos_ze[k] / t.sin_ze[k];
+    t.inv_sin_ze[k] = 1.0 / t.sin_ze[k];
     t.szk[k] = sph ? t.sin_ze[k] : 1.0;
   }
   t.zc.resize(TZ); t.dz.resize(TZ); t.sin_zc.resize(TZ); t.cos_zc.resize(TZ);
@@ -93,6 +95,7 @@ void build_tables(HostTables& t, int geometry, int TX, int TY, int TZ, int ngx, 
     t.dz[k] = ze[k + 1] - ze[k];
     t.sin_zc[k] = std::sin(t.zc[k]);
     t.cos_zc[k] = std::cos(t.zc[k]);
+    t.cot_zc[k] = t.cos_zc[k] / t.sin_zc[k];
     t.sxk[k] = ze[k + 1] - ze[k];
     t.syk[k] = cart ? dx * (ze[k + 1] - ze[k]) : cyl ? ze[k + 1] - ze[k] : cos_ze[k] - cos_ze[k + 1];
     t.Rxk[k] = sph ? t.sin_zc[k] : 1.0;

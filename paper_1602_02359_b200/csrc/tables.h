@@ -12,6 +12,7 @@ struct HostTables {
   std::vector<double> sxj, syj, szj, invVj, Rxj, invRxj, LXj, invLXj, Rzj, invRzj;
   std::vector<double> ze, zc, dz, invdz, invdzc, sxk, syk, inv_syk, szk, Rxk, invRxk;
   std::vector<double> sin_zc, cos_zc, sin_ze, cot_ze, cos_xc, sin_xc;
+  std::vector<double> cot_zc, inv_sin_ze;   // cos/sin at polar centres, 1/sin at polar edges (3-D viscous stress)
 };
 
 // edges: n+1 active edges or nullptr (uniform lo + j*(hi-lo)/n); ng ghost layers continue the mesh with

@@ -139,5 +139,26 @@ def nonuniform_cyl2d(nphi=50, nr=36, nsteps=6):
     return W.Workload("nonuniform_cyl2d", mesh, W.CYLINDRICAL, W.ISOTHERMAL, prm, rho, cs, vx, vy, None, nsteps)
 
 
-ALL = [cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
+def _with_nu(w, nu, name):
+    import dataclasses
+    return W.Workload(name, w.mesh, w.geometry, w.eos, dataclasses.replace(w.params, nu=nu), w.rho, w.e, w.vx, w.vy,
+                      w.vz, w.nsteps)
+
+
+def cart3d_visc_mixed_bc():
+    """3-D Cartesian viscous stress (B1, B4) with ghosted X, walls and outflow; nu large enough to matter in 5 steps."""
+    return _with_nu(cart_adi_mixed_bc(nx=34, ny=9, nz=20), 3e-3, "cart3d_visc_mixed_bc")
+
+
+def cyl3d_visc_fargo():
+    """3-D cylindrical viscous stress (B2, B5) with orbital advection and a planet."""
+    return _with_nu(cyl3d_adi_fargo(nphi=48, nr=22, nz=10), 2e-3, "cyl3d_visc_fargo")
+
+
+def sph3d_visc_fargo():
+    """3-D spherical viscous stress (B3, B6) on the config-4 recipe."""
+    return _with_nu(sph3d_iso_fargo(nphi=48, nr=24, nth=12), 1e-3, "sph3d_visc_fargo")
+
+
+ALL = [cart3d_visc_mixed_bc, cyl3d_visc_fargo, sph3d_visc_fargo, cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
        sph3d_adi_nofargo, x_only_1d, yz_only_2d, nonuniform_cyl2d]

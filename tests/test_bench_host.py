@@ -25,7 +25,16 @@ dist.destroy_process_group()
 """
 
 
-def _torchrun(args, port):
+def _free_port():
+    """A port nobody listens on now (a fixed one can still sit in TIME_WAIT from a run a minute ago)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def _torchrun(args, port=None):
+    port = port or _free_port()
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
            "127.0.0.1", "--master-port", str(port)] + args
     env = dict(os.environ, OMP_NUM_THREADS="1")
@@ -35,7 +44,7 @@ def _torchrun(args, port):
 def test_max_over_ranks_and_whole_job_rate_gloo_world2(tmp_path):
     script = tmp_path / "worker.py"
     script.write_text(_WORKER.format(root=ROOT))
-    r = _torchrun([str(script)], 29611)
+    r = _torchrun([str(script)])
     assert r.returncode == 0, r.stderr[-2000:]
     res = sorted(ln.split()[1:] for ln in r.stdout.splitlines() if ln.startswith("RESULT"))
     assert len(res) == 2
@@ -54,7 +63,7 @@ def test_single_rank_helpers_need_no_process_group():
 
 def test_reference_arm_two_ranks_prints_one_line():
     r = _torchrun(["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--workload",
-                   "sound"], 29612)
+                   "sound"])
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
     assert len(lines) == 1

@@ -54,7 +54,8 @@ def _stage_arrays(w, stage):
     mom = ([("pxm", "pxm"), ("pxp", "pxp")] if hx else []) + ([("pym", "pym"), ("pyp", "pyp")] if hy else []) + \
           ([("pzm", "pzm"), ("pzp", "pzp")] if hz else [])
     tr = [("trho", "rho")] + ([("te", "e")] if adi else []) + mom
-    visc = w.params.nu > 0 and w.geometry == W.CYLINDRICAL and hx and hy and not hz
+    visc3 = w.params.nu > 0 and hx and hy and hz
+    visc = visc3 or (w.params.nu > 0 and w.geometry == W.CYLINDRICAL and hx and hy and not hz)
     sfx = lambda s: ([("vx" + s, "vx" + s)] if hx else []) + ([("vy" + s, "vy" + s)] if hy else []) + \
         ([("vz" + s, "vz" + s)] if hz else [])
     return {
@@ -66,7 +67,7 @@ def _stage_arrays(w, stage):
         # adiabatic: 7b and 7c are one kernel (e_c is never stored): compared at the last stage it contains
         "SRC_B": [] if adi else sfx("c"),
         "SRC_C": (sfx("c") + [("ed", "ed")]) if adi else [],
-        "SRC_D": [("vxd", "vxd"), ("vyd", "vyd")] if visc else [],
+        "SRC_D": ([("vxd", "vxd"), ("vyd", "vyd")] + ([("vzd", "vzd")] if visc3 else [])) if visc else [],
         "BC2": [("rho", "rho"), ("e", "e")] + vel,
         "SWEEP_X": tr if hx else [],
         "SWEEP_Y": tr if hy else [],

@@ -51,6 +51,13 @@ def make_workload(name: str):
         return W.noise_box(n), sample, "same recipe on a %dx%dx%d slab" % (n, min(n, 64), min(n, 64))
     if name == "disk3d":
         return W.disk3d(), W.disk3d(1536, 32, 16), "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
+    if name == "disk3dvisc":   # config 4 with a kinematic viscosity: the 3-D viscous stress of NEXT-1 (Eqs. B3, B6)
+        import dataclasses
+        full, small = W.disk3d(), W.disk3d(1536, 32, 16)
+        for w in (full, small):
+            w.params = dataclasses.replace(w.params, nu=1e-5)
+            w.name += "_nu1e-5"
+        return full, small, "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
     if name == "disk2d":
         return W.disk2d(), W.disk2d(), "the whole 768x256 mesh"
     if name == "sound":
@@ -68,7 +75,7 @@ NCU_TRAFFIC_B_PER_CELL = {
                "orbital": 118.2, "newvel": 82.6},
 }
 
-CONFIG_OF = {"noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
+CONFIG_OF = {"disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
 def algorithmic_reals(w):
@@ -86,7 +93,8 @@ def algorithmic_reals(w):
         "source_a": (2 + nd + (1 if pot else 0)) + nd,
         "source_b": (1 + (1 if adi else 0) + nd) + (nd + (1 if adi else 0)),
         "source_bc": (2 + nd) + (nd + 1),
-        "source_d": (3 + 3) + (3 + 3 + 2),
+        # 7d: tensor kernel (rho, v -> components) + force kernel (rho, v, components -> v)
+        "source_d": ((1 + 3) + 6) + ((1 + 3 + 6) + 3) if nd == 3 else (3 + 3) + (3 + 3 + 2),
         "first_sweep": (1 + (1 if adi else 0) + nd) + (1 + nq),
         "sweep": (1 + nq + 1) + (1 + nq),
         "orbital": (1 + nq) + (1 + nq),

@@ -326,7 +326,7 @@ static int launch_sf(const Dev<T>& d, const State<T>& st, const T* phi, const St
   int nch = (148 * 12 + ntile * nrow - 1) / (ntile * nrow);
   if (nch < 1) nch = 1;
   int CH = (d.nz + nch - 1) / nch;
-  if (CH < 32) CH = 32;
+  if (CH < 16) CH = 16;   // shorter chunks on small meshes: the serial march, not the halo, is what costs there
   if (CH > d.nz) CH = d.nz;
   nch = (d.nz + CH - 1) / CH;
   dim3 b(32, SFW), g(ntile, nrow, nch);

@@ -486,7 +486,7 @@ static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cuda
   int nch = (int)((148LL * 3 * 6 + cols - 1) / cols);
   if (nch < 1) nch = 1;
   int CH = (TL + nch - 1) / nch;
-  if (CH < 32) CH = 32;
+  if (CH < 16) CH = 16;   // shorter chunks on small meshes: the serial march, not the halo, is what costs there
   if (CH > TL) CH = TL;
   nch = (TL + CH - 1) / CH;
   dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);

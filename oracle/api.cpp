@@ -7,10 +7,12 @@
 extern "C" int oracle_init(oracle_ctx** out, const oracle_mesh* m, int geometry, int eos, const oracle_params* p) {
   if (!out || !m || !p) return -1;
   if (m->nx < 1 || m->ny < 1 || m->nz < 1) return -1;
-  if (geometry < 0 || geometry > 2 || eos < 0 || eos > 1) return -1;
+  if (geometry < 0 || geometry > 3 || eos < 0 || eos > 1) return -1;
   oracle_ctx* c = new oracle_ctx();
   c->nx = m->nx; c->ny = m->ny; c->nz = m->nz;
   c->ng = m->nghost > 0 ? m->nghost : 3;
+  c->shear = geometry == ORC_SHEARING_SHEET;
+  if (c->shear) geometry = ORC_CARTESIAN;   // same metric; Tab. 2 and Eq. 29 are the differences (G32)
   c->geometry = geometry; c->eos = eos; c->p = *p;
   for (int d = 0; d < 3; ++d) for (int s = 0; s < 2; ++s) c->bc[d][s] = m->bc[d][s];
   c->hasx = m->nx > 1; c->hasy = m->ny > 1; c->hasz = m->nz > 1;
@@ -22,6 +24,7 @@ extern "C" int oracle_init(oracle_ctx** out, const oracle_mesh* m, int geometry,
   c->TX = c->nx + 2 * c->ngx; c->TY = c->ny + 2 * c->ngy; c->TZ = c->nz + 2 * c->ngz;
   c->xmin = m->xmin; c->dx = (m->xmax - m->xmin) / (double)m->nx;
   if (p->fargo_on && !c->xwrap) { delete c; return -1; }  // rings must be whole and periodic
+  if (c->shear && !(c->hasx && c->xwrap && c->hasy)) { delete c; return -1; }  // sheet: X along the flow, periodic; Y along the shear (Tab. 1)
   c->has_pot = (geometry != ORC_CARTESIAN) && (p->gm_star != 0.0 || p->planet_mass != 0.0);
   orc_build_tables(*c, *m);
   const size_t n = c->ncell();

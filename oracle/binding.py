@@ -37,7 +37,8 @@ class _Params(C.Structure):
                 ("omega_frame", C.c_double), ("gm_star", C.c_double), ("planet_mass", C.c_double),
                 ("planet_r", C.c_double), ("planet_phi0", C.c_double), ("planet_omega", C.c_double),
                 ("planet_eps", C.c_double),
-                ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double)]
+                ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double),
+                ("oort_a", C.c_double)]
 
 
 def build(force: bool = False) -> str:

@@ -6,6 +6,15 @@
  * /root/reference/PAPER.md ("P:n" = line n of that file) with the readings listed in DESIGN.md.
  * It shares no code with the CUDA path (paper_1602_02359_b200/csrc) and neither includes the other.
  *
+ * PARITY PINS: tests/test_oracle_*.py (closed forms, invariants, the paper's worked figures, brute force; the list is
+ * in DESIGN.md section 2).  PARITY UNPINNED -- conventions the paper leaves open and no closed form fixes, held only
+ * by oracle <-> CUDA agreement: the boundary formulas (reading G22), the form of the potential (G12), C_0 of Eq. 73
+ * (G10), C_q (G8; loosely pinned by the 2-3-zone Sod shock), when v0 is taken (G13), where the orbital step sits
+ * (G14), PPA on q rather than Q (G17), the disk initial states.
+ * Shearing sheet (geometry 3; Tab. 1/2 P:115; Eqs. 28-30; reading G32): pinned by the steady
+ * shear flow, the epicyclic frequency and amplitude ratio, conservation of Tab. 2's X momentum and the exact
+ * integer shift (tests/test_oracle_shearing_sheet.py).
+ *
  * Layout of every field passed through this interface: nz*ny*nx doubles, X (i) fastest, ACTIVE
  * cells only; velocities on the LOWER face of the cell in their own direction.
  */
@@ -16,7 +25,8 @@
 extern "C" {
 #endif
 
-enum { ORC_CARTESIAN = 0, ORC_CYLINDRICAL = 1, ORC_SPHERICAL = 2 };  /* Tab. 1 */
+enum { ORC_CARTESIAN = 0, ORC_CYLINDRICAL = 1, ORC_SPHERICAL = 2,
+       ORC_SHEARING_SHEET = 3 };  /* Tab. 1; shearing sheet: Cartesian metric */
 enum { ORC_ISOTHERMAL = 0, ORC_ADIABATIC = 1 };                      /* Eqs. 6, 7 */
 enum { ORC_PERIODIC = 0, ORC_OUTFLOW = 1, ORC_REFLECTING = 2 };
 
@@ -42,6 +52,7 @@ typedef struct oracle_params {
   int fargo_on;
   double omega_frame, gm_star, planet_mass, planet_r, planet_phi0, planet_omega, planet_eps;
   double shear_c0, t_stop, dt_fixed;
+  double oort_a;             /* Oort constant A of Eq. 29, shearing sheet only; Keplerian: -0.75 Omega_f */
 } oracle_params;
 
 typedef struct oracle_ctx oracle_ctx;

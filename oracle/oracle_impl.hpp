@@ -23,6 +23,8 @@ struct oracle_ctx {
   double dx, xmin;
   oracle_params p;
   bool has_pot;          // star or planet potential present (cyl / sph only)
+  bool shear;            // shearing sheet: `geometry` is then ORC_CARTESIAN (same metric, Tab. 5) and
+                         // only Tab. 2's X momentum and Eq. 29's source term differ (reading G32)
 
   // 1-D tables, ghost-inclusive.  j tables have TY (+1 for edges) entries, k tables TZ (+1).
   vec ye, yc, ze, zc;                  // edges and centres (centre = mean of edges, reading G26)

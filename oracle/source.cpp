@@ -45,6 +45,10 @@ void orc_source_a(oracle_ctx& c) {
             }
             vyb = vyb + dt * (G * c.inv_ye[j]);
           }
+          if (c.shear) {   // Eq. 29: + 2 Omega_f v_x - 4 A Omega_f y at the Y face; v_x averaged as in Eq. 38 (G32)
+            const double vxa = 0.25 * (((c.vx[l] + c.vx[c.id(ip, j, k)]) + c.vx[lm]) + c.vx[c.id(ip, j - 1, k)]);
+            vyb = vyb + dt * ((2.0 * om) * vxa - ((4.0 * c.p.oort_a) * om) * c.ye[j]);
+          }
         }
         if (c.hasz && k >= 1 && (!sph || ipok)) {
           const size_t lm = c.id(i, j, k - 1);

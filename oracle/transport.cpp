@@ -32,7 +32,8 @@ void orc_momenta(oracle_ctx& c) {
   const double om = (c.geometry == ORC_CARTESIAN) ? 0.0 : c.p.omega_frame;
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j) {
-      const double rx = c.Rx(j, k), rx2om = (rx * rx) * om, rz = c.Rzj[j];
+      // Tab. 2: the term added to R_x v_x; shearing sheet: 2 Omega_f y at the cell centre (G32)
+      const double rx = c.Rx(j, k), rx2om = c.shear ? (2.0 * c.p.omega_frame) * c.yc[j] : (rx * rx) * om, rz = c.Rzj[j];
       for (int i = 0; i < c.TX; ++i) {
         const size_t l = c.id(i, j, k);
         const double r = c.rho[l];
@@ -110,7 +111,8 @@ void orc_newvel(oracle_ctx& c) {
   const double om = (c.geometry == ORC_CARTESIAN) ? 0.0 : c.p.omega_frame;
   for (int k = c.k0(); k < c.k1(); ++k)
     for (int j = c.j0(); j < c.j1(); ++j) {
-      const double rx = c.Rx(j, k), rx2om = (rx * rx) * om, irx = c.invRx(j, k), irz = c.invRzj[j];
+      const double rx = c.Rx(j, k), rx2om = c.shear ? (2.0 * c.p.omega_frame) * c.yc[j] : (rx * rx) * om;
+      const double irx = c.invRx(j, k), irz = c.invRzj[j];
       for (int i = c.i0(); i < c.i1(); ++i) {
         const size_t l = c.id(i, j, k);
         if (c.hasx) {

@@ -18,7 +18,7 @@ from typing import Optional
 import numpy as np
 
 # geometry / eos / bc codes: must match include/fargo.h and oracle/fargo_oracle.h
-CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
+CARTESIAN, CYLINDRICAL, SPHERICAL, SHEARING_SHEET = 0, 1, 2, 3
 ISOTHERMAL, ADIABATIC = 0, 1
 PERIODIC, OUTFLOW, REFLECTING = 0, 1, 2
 
@@ -74,6 +74,7 @@ class Params:
     shear_c0: float = 0.5
     t_stop: float = 0.0         # <= 0: none
     dt_fixed: float = 0.0       # <= 0: CFL
+    oort_a: float = 0.0         # Oort constant A of Eq. 29 (shearing sheet only; Keplerian -0.75 Omega_f)
 
 
 @dataclasses.dataclass

@@ -58,6 +58,8 @@ def make_workload(name: str):
             w.params = dataclasses.replace(w.params, nu=1e-5)
             w.name += "_nu1e-5"
         return full, small, "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
+    if name == "sheet3d":   # NEXT-1: shearing sheet (Eqs. 28-30, Tab. 2), adiabatic, orbital advection on
+        return W.sheet3d(), W.sheet3d(1024, 32, 16), "same recipe on 1024x32x16 (full rows, fewer y and z cells)"
     if name == "disk2d":
         return W.disk2d(), W.disk2d(), "the whole 768x256 mesh"
     if name == "sound":
@@ -75,7 +77,7 @@ NCU_TRAFFIC_B_PER_CELL = {
                "orbital": 118.2, "newvel": 82.6},
 }
 
-CONFIG_OF = {"disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
+CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
 def algorithmic_reals(w):

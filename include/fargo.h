@@ -37,7 +37,10 @@
 extern "C" {
 #endif
 
-enum { FARGO_CARTESIAN = 0, FARGO_CYLINDRICAL = 1, FARGO_SPHERICAL = 2 }; /* Tab. 1 */
+enum { FARGO_CARTESIAN = 0, FARGO_CYLINDRICAL = 1, FARGO_SPHERICAL = 2,
+       FARGO_SHEARING_SHEET = 3 };   /* Tab. 1.  Shearing sheet (Tab. 2; Eqs. 28-30 P:249-255;
+                                        DESIGN.md reading G32): the Cartesian mesh with X along the flow (periodic)
+                                        and Y along the shear; needs nx > 1, ny > 1 and a periodic X axis */
 enum { FARGO_ISOTHERMAL = 0, FARGO_ADIABATIC = 1 };                       /* Eqs. 6-7 */
 enum { FARGO_PERIODIC = 0, FARGO_OUTFLOW = 1, FARGO_REFLECTING = 2 };
 
@@ -67,7 +70,7 @@ typedef struct fargo_params {
   double cvnr2;            /* C_q^2 of the artificial viscosity (reading G8; 2) */
   double nu;               /* constant kinematic viscosity, 0 = off (App. B) */
   int fargo_on;            /* orbital advection (section 3.5.1); needs periodic X */
-  double omega_frame;      /* Omega_f (ignored in Cartesian geometry) */
+  double omega_frame;      /* Omega_f (ignored in plain Cartesian geometry; constant in the sheet) */
   double gm_star;          /* G M of the central star (0 = none) */
   double planet_mass;      /* G m_p of the planet on a fixed circular orbit in the midplane (0 = none) */
   double planet_r, planet_phi0, planet_omega, planet_eps;   /* orbit radius, azimuth at t=0, angular
@@ -76,6 +79,7 @@ typedef struct fargo_params {
   double t_stop;           /* > 0: the step that would pass t_stop is clipped to land on it and later
                               steps are no-ops (reading G21); <= 0: none */
   double dt_fixed;         /* > 0: overrides the CFL time step */
+  double oort_a;           /* Oort constant A of Eq. 29; shearing sheet only (Keplerian: -0.75 Omega_f) */
   int precision;           /* 64 (double) or 32 (float) */
   int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (needs a non-default
                               cuda_stream; on the legacy default stream it falls back to plain launches);

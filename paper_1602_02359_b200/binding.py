@@ -37,7 +37,7 @@ class FargoParams(C.Structure):
                 ("omega_frame", C.c_double), ("gm_star", C.c_double), ("planet_mass", C.c_double),
                 ("planet_r", C.c_double), ("planet_phi0", C.c_double), ("planet_omega", C.c_double),
                 ("planet_eps", C.c_double),
-                ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double),
+                ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double), ("oort_a", C.c_double),
                 ("precision", C.c_int), ("use_graph", C.c_int),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p)]
 
@@ -119,7 +119,7 @@ class Fargo:
                 m.bc[d][s] = mesh.bc[d][s]
         p = FargoParams()
         for name in ("gamma", "cfl", "cvnr2", "nu", "fargo_on", "omega_frame", "gm_star", "planet_mass", "planet_r",
-                     "planet_phi0", "planet_omega", "planet_eps", "shear_c0", "t_stop", "dt_fixed"):
+                     "planet_phi0", "planet_omega", "planet_eps", "shear_c0", "t_stop", "dt_fixed", "oort_a"):
             setattr(p, name, getattr(params, name))
         p.precision = precision
         p.use_graph = 1 if use_graph else 0

@@ -57,7 +57,7 @@ struct Layout {   // sizes shared by fargo_workspace_bytes and fargo_init
 static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, const fargo_params* p, std::string& err) {
   if (!m || !p) { err = "null mesh or params"; return false; }
   if (m->nx < 1 || m->ny < 1 || m->nz < 1) { err = "mesh extents must be >= 1"; return false; }
-  if (geometry < 0 || geometry > 2) { err = "unknown geometry"; return false; }
+  if (geometry < 0 || geometry > 3) { err = "unknown geometry"; return false; }
   if (eos < 0 || eos > 1) { err = "unknown equation of state"; return false; }
   if (p->precision != 64 && p->precision != 32) { err = "precision must be 64 or 32"; return false; }
   for (int dd = 0; dd < 3; ++dd)
@@ -77,7 +77,11 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.pitch = (long long)align_up((size_t)L.TX, 16);
   L.plane = L.pitch * L.TY;
   L.narr = L.plane * L.TZ;
-  L.has_pot = geometry != FARGO_CARTESIAN && (p->gm_star != 0.0 || p->planet_mass != 0.0);
+  if (geometry == FARGO_SHEARING_SHEET && !(L.hasx && L.xwrap && L.hasy)) {
+    err = "the shearing sheet needs nx > 1 with a periodic X axis and ny > 1 (Tab. 1)"; return false;
+  }
+  const bool cartesian_metric = geometry == FARGO_CARTESIAN || geometry == FARGO_SHEARING_SHEET;
+  L.has_pot = !cartesian_metric && (p->gm_star != 0.0 || p->planet_mass != 0.0);
   L.visc3d = p->nu > 0.0 && L.hasx && L.hasy && L.hasz;                                    // Eqs. B1-B6, any geometry
   L.visc = L.visc3d || (p->nu > 0.0 && geometry == FARGO_CYLINDRICAL && L.hasx && L.hasy && !L.hasz && L.xwrap);
   L.fargo = p->fargo_on != 0;
@@ -173,8 +177,11 @@ struct Sim : CtxBase {
 
   T* set_arr(int s, int slot /* -1 = rho, 0 = e, 1..6 momenta */) { return pool[s * 8 + 1 + slot]; }
 
-  int init(const fargo_mesh* m, int geo, int eos_, const fargo_params* p) {
-    geometry = geo; eos = eos_; prm = *p;
+  int init(const fargo_mesh* m, int geo_in, int eos_, const fargo_params* p) {
+    // the sheet is the Cartesian mesh (Tab. 5 unchanged) with Tab. 2's X momentum and Eq. 29 switched on (G32)
+    const bool sheet = geo_in == FARGO_SHEARING_SHEET;
+    const int geo = sheet ? FARGO_CARTESIAN : geo_in;
+    geometry = geo_in; eos = eos_; prm = *p;
     stream = (cudaStream_t)p->cuda_stream;
     int ndev = 0;
     if (!ck(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev < 1) {
@@ -254,6 +261,9 @@ struct Sim : CtxBase {
     d.gamma = (T)p->gamma; d.gm1 = (T)(p->gamma - 1.0); d.gg1 = (T)(p->gamma * (p->gamma - 1.0));
     d.cfl = (T)p->cfl; d.cvnr2 = (T)p->cvnr2; d.nu = (T)p->nu;
     d.omega = (T)p->omega_frame; d.om_eff = geo == FARGO_CARTESIAN ? T(0) : (T)p->omega_frame;
+    d.shear = sheet ? 1 : 0;
+    d.two_om = sheet ? (T)(2.0 * p->omega_frame) : T(0);
+    d.four_a_om = sheet ? (T)((4.0 * p->oort_a) * p->omega_frame) : T(0);
     d.shear_c0 = (T)p->shear_c0;
     d.c3 = (T)(4.0 * p->cvnr2); d.c4 = (T)(4.0 * p->nu);
     d.t_stop = p->t_stop; d.dt_fixed = p->dt_fixed;

@@ -64,6 +64,11 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
         }
         v = v + dt * (G * d.inv_ye[j]);
       }
+      if (d.shear) {   // Eq. 29: + 2 Omega_f v_x - 4 A Omega_f y on the Y face, v_x averaged as in Eq. 38 (G32)
+        const long long lp = d.id(ip, j, k);
+        const T vxa = T(0.25) * (((vx[l] + vx[lp]) + vx[lm]) + vx[lp - d.pitch]);
+        v = v + dt * (d.two_om * vxa - d.four_a_om * d.ye[j]);
+      }
     }
     vyb[l] = v;
   }

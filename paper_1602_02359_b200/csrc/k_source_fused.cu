@@ -68,7 +68,9 @@ template <int N> __device__ __forceinline__ void sf_wait() { asm volatile("cp.as
 template <typename T, int GEO, bool ADI, bool POT, bool RING>
 __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, const State<T> st, const T* __restrict__ phi,
                                                            const State<T> out, const int CH) {
-  constexpr bool CURV = GEO != GEO_CART, SPH = GEO == GEO_SPH;
+  constexpr bool CURV = GEO == GEO_CYL || GEO == GEO_SPH, SPH = GEO == GEO_SPH;
+  constexpr bool SHEAR = GEO == GEO_SHEAR;   // shearing sheet: Cartesian metric + Eq. 29 on the Y faces (reading G32)
+  constexpr bool VXR = CURV || SHEAR;        // the Y faces need v_x of the neighbour rows
   constexpr int NV = ADI ? 4 : 3;   // Y faces whose v_b is needed: rows j-1 .. j-2+NV (7c needs v_c on the upper face too)
   if (d.ctl->done) return;
   const int lane = threadIdx.x;
@@ -93,7 +95,7 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
 #pragma unroll
   for (int t = 0; t < NV; ++t) {
     ilY[t] = d.invDY[j - 1 + t];
-    yeR[t] = CURV ? d.ye[j - 1 + t] : T(0);
+    yeR[t] = VXR ? d.ye[j - 1 + t] : T(0);
     iyeR[t] = CURV ? d.inv_ye[j - 1 + t] : T(0);
   }
   const T invLXj = d.invLXj[j], invRzj = d.invRzj[j], invLYj = d.invLY[j];
@@ -150,7 +152,7 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
         sf_prefetch_l1(en + lr);
         if (POT) sf_prefetch_l1(phi + lr);
         if (t >= 1) sf_prefetch_l1(vy + lr);
-        if (CURV) sf_prefetch_l1(vx + lr);
+        if (VXR) sf_prefetch_l1(vx + lr);
         if (SPH) { sf_prefetch_l1(vz + lr); sf_prefetch_l1(vz + lr + P); }
       }
     }
@@ -214,7 +216,7 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
           ff[t] = POT ? ldv(phi + lr) : zero;
         }
         vyr[t] = t == 2 ? own(m, 4) : (t >= 1 ? ldv(vy + lr) : zero);
-        vxr[t] = t == 2 ? own(m, 3) : (CURV ? ldv(vx + lr) : zero);
+        vxr[t] = t == 2 ? own(m, 3) : (VXR ? ldv(vx + lr) : zero);
         vz0[t] = SPH ? (t == 2 ? own(m, 2) : ldv(vz + lr)) : zero;
         vz1[t] = SPH ? (t == 2 ? own(m + 1, 2) : ldv(vz + lr + P)) : zero;
       }
@@ -243,7 +245,7 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
       {
         T vxn_t[NV + 1];   // vx of the right neighbour's first cell, per row (curvature terms)
 #pragma unroll
-        for (int t = 0; t <= NV; ++t) vxn_t[t] = CURV ? s_dn1(vxr[t].a) : T(0);
+        for (int t = 0; t <= NV; ++t) vxn_t[t] = VXR ? s_dn1(vxr[t].a) : T(0);
         const T Rxk = CURV ? d.Rxk[m] : T(0);
         const T Sy0 = syj0 * d.syk[m], Sy1 = syj1 * d.syk[m];
 #pragma unroll
@@ -268,6 +270,12 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
                 G = G + vth * vth;
               }
               v = v + dt * (G * iyeR[t - 1]);
+            }
+            if (SHEAR) {   // Eq. 29: + 2 Omega_f v_x - 4 A Omega_f y, v_x averaged as in Eq. 38
+              const T x00 = c ? vxr[t].b : vxr[t].a, x10 = c ? vxn_t[t] : vxr[t].b;
+              const T x01 = c ? vxr[t - 1].b : vxr[t - 1].a, x11 = c ? vxn_t[t - 1] : vxr[t - 1].b;
+              const T vxa = T(0.25) * (((x00 + x10) + x01) + x11);
+              v = v + dt * (d.two_om * vxa - d.four_a_om * yeR[t - 1]);
             }
             vby[t] = v;
           }
@@ -330,7 +338,7 @@ static int launch_sf(const Dev<T>& d, const State<T>& st, const T* phi, const St
   if (CH > d.nz) CH = d.nz;
   nch = (d.nz + CH - 1) / CH;
   dim3 b(32, SFW), g(ntile, nrow, nch);
-  constexpr bool RING = GEO == GEO_CART;
+  constexpr bool RING = GEO == GEO_CART || GEO == GEO_SHEAR;
   const size_t pair = 2 * sizeof(T);
   if (d.has_pot) {
     const int sm = RING ? (int)(SF_RS * 6 * 128 * pair) : 0;
@@ -348,6 +356,7 @@ static int launch_sf(const Dev<T>& d, const State<T>& st, const T* phi, const St
 template <typename T>
 int launch_source_fused(const Dev<T>& d, const State<T>& st, const T* phi, const State<T>& out, cudaStream_t s) {
   const bool adi = d.eos == EOS_ADI;
+  if (d.shear) return adi ? launch_sf<T, GEO_SHEAR, true>(d, st, phi, out, s) : launch_sf<T, GEO_SHEAR, false>(d, st, phi, out, s);
   switch (d.geometry) {
     case GEO_CART: return adi ? launch_sf<T, GEO_CART, true>(d, st, phi, out, s) : launch_sf<T, GEO_CART, false>(d, st, phi, out, s);
     case GEO_CYL: return adi ? launch_sf<T, GEO_CYL, true>(d, st, phi, out, s) : launch_sf<T, GEO_CYL, false>(d, st, phi, out, s);

@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
     if (valid) {
       if (lane == 31) wp = (d.xwrap || i + 1 < d.TX) ? A.st.vx[d.id(d.xw(i + 1), j, k)] : w;
       else if (!d.xwrap && i + 1 >= d.TX) wp = w;
-      const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, rz = d.Rzj[j];
+      const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), rz = d.Rzj[j];
       if (d.eos == EOS_ADI) mom[0] = A.st.e[l];
       mom[1] = r0 * (rx * w + rx2om);
       mom[2] = r0 * (rx * wp + rx2om);
@@ -230,7 +230,7 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
   // ---- 12a: the momenta of Tab. 2 ----
   T Q[NQ][2];
   {
-    const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, rz = d.Rzj[j];
+    const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), rz = d.Rzj[j];
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
       const T wp = c == 0 ? w[1] : wn;
@@ -534,7 +534,7 @@ __global__ void __launch_bounds__(128) k_newvel(const Dev<T> d, const T* __restr
   const long long l = d.id(i, j, k);
   const T r0 = rho[l];
   if (d.hasx) {
-    const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, irx = d.invRx(j, k);
+    const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), irx = d.invRx(j, k);
     const long long lm = d.id(d.xw(i - 1), j, k);
     st.vx[l] = (rdiv(S.q[2][lm] + S.q[1][l], rho[lm] + r0) - rx2om) * irx;
   }
@@ -574,7 +574,7 @@ __global__ void __launch_bounds__(128) k_newvel_dt(const Dev<T> d, const T* __re
   const int jp = j + 1 == d.ngy + d.ny ? d.ngy : j + 1, kp = k + 1 == d.ngz + d.nz ? d.ngz : k + 1;
   const long long lyp = d.id(i, jp, k), lzp = d.id(i, j, kp);
   const T r0 = rho[l];
-  const T rx = d.Rx(j, k), rx2om = (rx * rx) * d.om_eff, irx = d.invRx(j, k), irz = d.invRzj[j];
+  const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), irx = d.invRx(j, k), irz = d.invRzj[j];
   // Eq. 51 on the three lower faces (stored) ...
   const T ax = (rdiv(S.q[2][lxm] + S.q[1][l], rho[lxm] + r0) - rx2om) * irx;
   const T ay = rdiv(S.q[4][l - d.pitch] + S.q[3][l], rho[l - d.pitch] + r0);

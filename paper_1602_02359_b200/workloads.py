@@ -218,6 +218,25 @@ def disk3d(nphi: int = 1536, nr: int = 512, nth: int = 128, nsteps: int = 100) -
                     rho, cs, vx, vy, vz, nsteps)
 
 
+def sheet3d(nx: int = 1024, ny: int = 512, nz: int = 128, nsteps: int = 20) -> Workload:
+    """NEXT-1 workload (no BASELINE.json config): 3-D adiabatic Keplerian shearing sheet (Tab. 1, Eqs. 28-30),
+    X along the flow (periodic, 4 H long), Y along the shear (2 H, reflecting walls), Z periodic (H/2); Omega_f = 1,
+    A = -3/4, c_s = H Omega_f = 1 so that lengths are in scale heights; v_x = 2 A y plus noise of 1e-2 c_s on the three
+    components, rho = 1 + 0.01 U; orbital advection on."""
+    gamma, om, A = 5.0 / 3.0, 1.0, -0.75
+    bc = ((PERIODIC, PERIODIC), (REFLECTING, REFLECTING), (PERIODIC, PERIODIC))
+    mesh = Mesh(nx, ny, nz, -2.0, 2.0, uedges(-1.0, 1.0, ny), uedges(-0.25, 0.25, nz), bc)
+    prm = Params(gamma=gamma, fargo_on=1, omega_frame=om, oort_a=A)
+    n = mesh.ncells
+    shape = (nz, ny, nx)
+    rho = (1.0 + 0.01 * uniform_pm1(0, n)).reshape(shape)
+    e = rho / (gamma * (gamma - 1.0))                       # c_s^2 = gamma P / rho = 1
+    vx = 2.0 * A * mesh.yc()[None, :, None] * np.ones(shape) + 1e-2 * uniform_pm1(2, n).reshape(shape)
+    vy = 1e-2 * uniform_pm1(3, n).reshape(shape)
+    vz = 1e-2 * uniform_pm1(4, n).reshape(shape)
+    return Workload("sheet3d_%dx%dx%d" % (nx, ny, nz), mesh, SHEARING_SHEET, ADIABATIC, prm, rho, e, vx, vy, vz, nsteps)
+
+
 def noise_box(n: int = 64, nsteps: int = 50, shape3: Optional[tuple] = None) -> Workload:
     """Config 5: periodic Cartesian box with cell-scale white noise, gamma = 5/3."""
     gamma = 5.0 / 3.0

@@ -160,5 +160,41 @@ def sph3d_visc_fargo():
     return _with_nu(sph3d_iso_fargo(nphi=48, nr=24, nth=12), 1e-3, "sph3d_visc_fargo")
 
 
-ALL = [cart3d_visc_mixed_bc, cyl3d_visc_fargo, sph3d_visc_fargo, cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
+def _sheet(name, nx, ny, nz, eos, fargo, nsteps, nu=0.0):
+    """Shearing sheet (NEXT-1, reading G32): Keplerian shear v_x = 2 A y plus cell-scale noise, reflecting Y walls."""
+    om, A = 1.0, -0.75
+    bc = ((P, P), (R, R), (P, P))
+    mesh = W.Mesh(nx, ny, nz, 0.0, 2.0, W.uedges(-0.5, 0.5, ny), W.uedges(-0.25, 0.25, max(nz, 1)), bc)
+    prm = W.Params(gamma=1.4, fargo_on=fargo, omega_frame=om, oort_a=A, nu=nu)
+    shape = (nz, ny, nx)
+    y = mesh.yc()[None, :, None] * np.ones(shape)
+    rho = 1.0 + _noise(shape, 0, 0.2)
+    cs = 0.3
+    e = (cs * (1.0 + _noise(shape, 1, 0.1))) if eos == W.ISOTHERMAL else rho * cs * cs / 0.4 * (1.0 + _noise(shape, 1, 0.2))
+    vx = 2.0 * A * y + _noise(shape, 2, 0.3)
+    vy = _noise(shape, 3, 0.3)
+    vz = _noise(shape, 4, 0.3) if nz > 1 else None
+    return W.Workload(name, mesh, W.SHEARING_SHEET, eos, prm, rho, e, vx, vy, vz, nsteps)
+
+
+def sheet3d_adi_fargo():
+    """Even nx: fused source pass (GEO_SHEAR variant), two-cell X sweep and orbital kernel."""
+    return _sheet("sheet3d_adi_fargo", 66, 21, 10, W.ADIABATIC, 1, 5)
+
+
+def sheet3d_iso_nofargo_odd():
+    """Odd nx: unfused source kernels (k_source_a carries Eq. 29), one-cell X sweep, no orbital advection."""
+    return _sheet("sheet3d_iso_nofargo_odd", 45, 18, 9, W.ISOTHERMAL, 0, 5)
+
+
+def sheet2d_adi_fargo():
+    return _sheet("sheet2d_adi_fargo", 70, 33, 1, W.ADIABATIC, 1, 6)
+
+
+def sheet3d_visc():
+    """Sheet with the 3-D Cartesian viscous stress (B1, B4) on top."""
+    return _sheet("sheet3d_visc", 40, 16, 8, W.ADIABATIC, 1, 4, nu=2e-3)
+
+
+ALL = [sheet3d_adi_fargo, sheet3d_iso_nofargo_odd, sheet2d_adi_fargo, sheet3d_visc, cart3d_visc_mixed_bc, cyl3d_visc_fargo, sph3d_visc_fargo, cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
        sph3d_adi_nofargo, x_only_1d, yz_only_2d, nonuniform_cyl2d]

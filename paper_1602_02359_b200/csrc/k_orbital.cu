@@ -109,6 +109,10 @@ __global__ void __launch_bounds__(OBM) k_orbital(const Dev<T> d, const SweepArgs
 constexpr int O2W = 4;          // warps (rings) per block
 constexpr int O2IN = 56;        // cells stored per warp
 
+template <typename T> struct OPair;
+template <> struct OPair<double> { using type = double2; };
+template <> struct OPair<float> { using type = float2; };
+
 template <typename T> __device__ __forceinline__ T o_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 template <typename T> __device__ __forceinline__ T o_dn1(T v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 
@@ -118,7 +122,9 @@ __device__ __forceinline__ T ppa_mono(const T fm, const T f, const T fp, bool& f
   const T dd = T(0.5) * (fp - fm);
   flat = a * b <= T(0);
   const T mm = rmin(rmin(T(2) * rabs(a), T(2) * rabs(b)), rabs(dd));
-  const T dm = dd < T(0) ? -mm : mm;
+  // sign(dd) mm with one LOP3 on the high word (mm >= 0); where dd is a zero mm is a zero too and only the sign of
+  // that zero can differ from the select's, which no later value depends on
+  const T dm = copysign(mm, dd);
   return flat ? T(0) : dm;
 }
 
@@ -134,10 +140,12 @@ __device__ __forceinline__ void ppa_limit(const T f, const bool flat, T& fl, T& 
   fl = ol; fr = orr;
 }
 
-// star values on the upper faces of the lane's two cells (reading G15: x = |xi| in both branches)
-template <typename T>
-__device__ __forceinline__ void ppa_pair(const T fA, const T fB, const bool fwd, const T x, const T x1x, T& sA,
-                                         T& sB) {
+// star values on the upper faces of the lane's two cells (reading G15: x = |xi| in both branches).  FWD (xi >= 0:
+// the upwind cell of a face is the cell itself, otherwise the next one) is uniform over a ring, hence over the warp:
+// the kernel branches on it ONCE around its whole body, so each copy is a single basic block without the eight
+// selects (sixteen SEL instructions) per pair that a run-time choice costs, and the xi >= 0 copy drops two shuffles.
+template <typename T, bool FWD>
+__device__ __forceinline__ void ppa_pair(const T fA, const T fB, const T x, const T x1x, T& sA, T& sB) {
   const T fm = o_up1(fB);        // position t-1
   const T fn = o_dn1(fA);        // position t+2
   bool flatA, flatB;
@@ -148,19 +156,43 @@ __device__ __forceinline__ void ppa_pair(const T fA, const T fB, const bool fwd,
   T flA = o_up1(fuB), frA = fuA, flB = fuA, frB = fuB;
   ppa_limit(fA, flatA, flA, frA);
   ppa_limit(fB, flatB, flB, frB);
-  // the upwind cell of a face is the cell itself (xi >= 0) or the next one; selected without a branch so that the
-  // chains of the different quantities stay in one basic block and interleave
-  const T fln = o_dn1(flA), frn = o_dn1(frA);
-  const T uA = fwd ? fA : fB, ulA = fwd ? flA : flB, urA = fwd ? frA : frB;
-  const T uB = fwd ? fB : fn, ulB = fwd ? flB : fln, urB = fwd ? frB : frn;
-  const T eA = fwd ? urA : ulA, eB = fwd ? urB : ulB;
-  sA = (eA + x * (uA - eA)) + x1x * ((T(2) * uA - urA) - ulA);
-  sB = (eB + x * (uB - eB)) + x1x * ((T(2) * uB - urB) - ulB);
+  if (FWD) {
+    sA = (frA + x * (fA - frA)) + x1x * ((T(2) * fA - frA) - flA);
+    sB = (frB + x * (fB - frB)) + x1x * ((T(2) * fB - frB) - flB);
+  } else {
+    const T fln = o_dn1(flA), frn = o_dn1(frA);
+    sA = (flB + x * (fB - flB)) + x1x * ((T(2) * fB - frB) - flB);
+    sB = (fln + x * (fn - fln)) + x1x * ((T(2) * fn - frn) - fln);
+  }
 }
 
-template <typename T> struct OPair;
-template <> struct OPair<double> { using type = double2; };
-template <> struct OPair<float> { using type = float2; };
+template <typename T, int NQ, bool FWD>
+__device__ __forceinline__ void orbital2_body(const SweepArgs<T>& A, const typename OPair<T>::type r2,
+                                              const typename OPair<T>::type (&Q2)[NQ], const T xi, const T x, const T x1x,
+                                              const T g, const long long row, const int io, const int io1,
+                                              const bool stA, const bool stB, const bool vec) {
+  const T irA = rdiv(T(1), r2.x), irB = rdiv(T(1), r2.y);
+  T sA, sB;
+  ppa_pair<T, FWD>(r2.x, r2.y, x, x1x, sA, sB);
+  const T FrA = xi * sA, FrB = xi * sB;   // mass through the upper face per unit of (LX Sx)
+  {
+    const T Fm = o_up1(FrB);
+    const T oA = r2.x - g * (FrA - Fm), oB = r2.y - g * (FrB - FrA);
+    st2_if(A.drho + row + io, oA, oB, vec && stB);
+    st_if(A.drho + row + io, oA, stA && !(vec && stB));
+    st_if(A.drho + row + io1, oB, stB && !vec);
+  }
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) {
+    ppa_pair<T, FWD>(Q2[q].x * irA, Q2[q].y * irB, x, x1x, sA, sB);
+    const T FA = FrA * sA, FB = FrB * sB;
+    const T Fm = o_up1(FB);
+    const T oA = Q2[q].x - g * (FA - Fm), oB = Q2[q].y - g * (FB - FA);
+    st2_if(A.dq[q] + row + io, oA, oB, vec && stB);
+    st_if(A.dq[q] + row + io, oA, stA && !(vec && stB));
+    st_if(A.dq[q] + row + io1, oB, stB && !vec);
+  }
+}
 
 template <typename T, int NQ>
 __global__ void __launch_bounds__(32 * O2W) k_orbital2(const Dev<T> d, const SweepArgs<T> A, T* __restrict__ nshift_out) {
@@ -198,27 +230,9 @@ __global__ void __launch_bounds__(32 * O2W) k_orbital2(const Dev<T> d, const Swe
 #pragma unroll
   for (int q = 0; q < NQ; ++q) Q2[q] = *reinterpret_cast<const P2*>(A.sq[q] + l);
 
-  const T irA = rdiv(T(1), r2.x), irB = rdiv(T(1), r2.y);
-  T sA, sB;
-  ppa_pair<T>(r2.x, r2.y, fwd, x, x1x, sA, sB);
-  const T FrA = xi * sA, FrB = xi * sB;   // mass through the upper face per unit of (LX Sx)
-  {
-    const T Fm = o_up1(FrB);
-    const T oA = r2.x - g * (FrA - Fm), oB = r2.y - g * (FrB - FrA);
-    st2_if(A.drho + row + io, oA, oB, vec && stB);
-    st_if(A.drho + row + io, oA, stA && !(vec && stB));
-    st_if(A.drho + row + io1, oB, stB && !vec);
-  }
-#pragma unroll
-  for (int q = 0; q < NQ; ++q) {
-    ppa_pair<T>(Q2[q].x * irA, Q2[q].y * irB, fwd, x, x1x, sA, sB);
-    const T FA = FrA * sA, FB = FrB * sB;
-    const T Fm = o_up1(FB);
-    const T oA = Q2[q].x - g * (FA - Fm), oB = Q2[q].y - g * (FB - FA);
-    st2_if(A.dq[q] + row + io, oA, oB, vec && stB);
-    st_if(A.dq[q] + row + io, oA, stA && !(vec && stB));
-    st_if(A.dq[q] + row + io1, oB, stB && !vec);
-  }
+  // a vote result is uniform by construction: ptxas then emits no WARPSYNC region around the shuffles of either copy
+  if (__all_sync(0xffffffffu, fwd)) orbital2_body<T, NQ, true>(A, r2, Q2, xi, x, x1x, g, row, io, io1, stA, stB, vec);
+  else orbital2_body<T, NQ, false>(A, r2, Q2, xi, x, x1x, g, row, io, io1, stA, stB, vec);
 }
 
 template <typename T, int NQ>

@@ -69,6 +69,16 @@ def sph3d_iso_fargo(nphi=72, nr=33, nth=14, nsteps=6):
     return W.disk3d(nphi, nr, nth, nsteps)
 
 
+def sph3d_iso_fargo_quad():
+    """Longer rings: five 56-cell tiles of the orbital kernel with a ragged tail, shifts of several cells."""
+    return W.disk3d(248, 12, 8, 5)
+
+
+def cyl3d_adi_fargo_quad():
+    """The orbital kernel with the adiabatic quantity list (7 quantities) over three tiles."""
+    return cyl3d_adi_fargo(nphi=128, nr=14, nz=8, nsteps=4)
+
+
 def cyl3d_adi_fargo(nphi=64, nr=30, nz=12, nsteps=5):
     """3-D cylindrical (phi, r, z): in north_star's geometry list, in no config (SURVEY.md 8(a) note)."""
     h = 0.1
@@ -196,5 +206,5 @@ def sheet3d_visc():
     return _sheet("sheet3d_visc", 40, 16, 8, W.ADIABATIC, 1, 4, nu=2e-3)
 
 
-ALL = [sheet3d_adi_fargo, sheet3d_iso_nofargo_odd, sheet2d_adi_fargo, sheet3d_visc, cart3d_visc_mixed_bc, cyl3d_visc_fargo, sph3d_visc_fargo, cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
+ALL = [sph3d_iso_fargo_quad, cyl3d_adi_fargo_quad, sheet3d_adi_fargo, sheet3d_iso_nofargo_odd, sheet2d_adi_fargo, sheet3d_visc, cart3d_visc_mixed_bc, cyl3d_visc_fargo, sph3d_visc_fargo, cart_adi_periodic, cart_adi_periodic_even, cart_iso_periodic, sph3d_iso_fargo_odd, cart_adi_mixed_bc, sod_small, cyl2d_iso_fargo_visc, sph3d_iso_fargo, cyl3d_adi_fargo,
        sph3d_adi_nofargo, x_only_1d, yz_only_2d, nonuniform_cyl2d]

@@ -96,7 +96,9 @@ def algorithmic_reals(w):
         "source_b": (1 + (1 if adi else 0) + nd) + (nd + (1 if adi else 0)),
         "source_bc": (2 + nd) + (nd + 1),
         # 7d: tensor kernel (rho, v -> components) + force kernel (rho, v, components -> v)
-        "source_d": ((1 + 3) + 6) + ((1 + 3 + 6) + 3) if nd == 3 else (3 + 3) + (3 + 3 + 2),
+        # 3-D, wrapped X: one pass, the tensor is never stored (rho, v -> v); else tensor kernel + force kernel
+        "source_d": ((1 + 3) + 3 if w.mesh.bc[0][0] == W.PERIODIC else ((1 + 3) + 6) + ((1 + 3 + 6) + 3)) if nd == 3
+        else (3 + 3) + (3 + 3 + 2),
         "first_sweep": (1 + (1 if adi else 0) + nd) + (1 + nq),
         "sweep": (1 + nq + 1) + (1 + nq),
         "orbital": (1 + nq) + (1 + nq),

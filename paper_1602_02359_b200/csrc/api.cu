@@ -423,8 +423,13 @@ struct Sim : CtxBase {
       dbg["ed"] = st.e;
       if (until == FARGO_ST_SRC_B || until == FARGO_ST_SRC_C) return n;
       if (L.visc3d) {                                                                  // cell 7d, 3-D (Eqs. B1-B6)
-        T* tens[6] = {set_arr(0, -1), set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), set_arr(0, 3), set_arr(0, 4)};
-        n += timed("source_d", [&] { return launch_source_d3<T>(d, st.rho, vxc, vyc, vzc, tens, st.vx, st.vy, st.vz, stream); });
+        static const bool unfused_d = getenv("FARGO_UNFUSED_VISC") != nullptr;   // measurement switch
+        if (until < 0 && !unfused_d && source_d3_fused_ok<T>(d)) {   // one pass, the tensor is never stored
+          n += timed("source_d", [&] { return launch_source_d3_fused<T>(d, st.rho, vxc, vyc, vzc, st.vx, st.vy, st.vz, stream); });
+        } else {
+          T* tens[6] = {set_arr(0, -1), set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), set_arr(0, 3), set_arr(0, 4)};
+          n += timed("source_d", [&] { return launch_source_d3<T>(d, st.rho, vxc, vyc, vzc, tens, st.vx, st.vy, st.vz, stream); });
+        }
       } else if (L.visc) {                                                             // cell 7d, 2-D cylindrical
         n += timed("source_d", [&] { return launch_source_d<T>(d, st.rho, vxc, vyc, set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), st.vx, st.vy, stream); });
       }

@@ -156,6 +156,183 @@ __global__ void __launch_bounds__(128) k_visc3d_force(const Dev<T> d, const T* _
   vxd[l] = ox; vyd[l] = oy; vzd[l] = oz;
 }
 
+// ---- 7d as ONE pass (wrapped X): (rho, v_c) -> v_d on ACTIVE cells, the stress tensor never stored --------------
+// 56 B per cell instead of 184 B.  The ghost fill of cell 9 follows 7d and overwrites every ghost of v, so only active
+// cells are produced; their stencils reach one ghost layer, where v_c is what 7a-7c computed there (the unfused
+// kernels run over the whole allocated array for that reason).
+//   X : a warp owns 32 consecutive cells of a row; values at i-1 / i+1 cross lanes by shuffle; lanes 0 and 31 are
+//       recomputed halo (30 cells stored per warp).
+//   Z : the thread marches along Z with the rows j-1, j, j+1 of (rho, v) of the current and the leading plane in
+//       registers; t_xz, t_yz of the leading plane and the diagonal of the previous plane are carried.
+//   Y : the components at j-1 (diagonal) and j+1 (t_xy, t_yz) are recomputed from the neighbour rows (the warps of a
+//       block are consecutive rows, so L1/L2 serve them): 7 component evaluations per cell instead of 4.
+// Every component and force expression is the one of k_visc3d_tensor / k_visc3d_force (same operands, same order),
+// so the result is bit-identical to the two-kernel sequence on active cells.
+constexpr int V3W = 4;     // warps (consecutive rows) per block
+constexpr int V3IN = 30;   // cells stored per warp
+constexpr int V3_PF = 2;   // planes ahead that are prefetched into L1
+
+template <typename T> __device__ __forceinline__ T v_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <typename T> __device__ __forceinline__ T v_dn1(T v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+template <typename T> struct Rows3 { T m, c, p; };   // rows j-1, j, j+1 of one array at one plane
+
+template <typename T, int GEO>
+__global__ void __launch_bounds__(32 * V3W) k_visc3d_fused(const Dev<T> d, const T* __restrict__ rho, const T* __restrict__ vx,
+                                                           const T* __restrict__ vy, const T* __restrict__ vz,
+                                                           T* __restrict__ vxd, T* __restrict__ vyd, T* __restrict__ vzd,
+                                                           const int CH) {
+  constexpr bool CURV = GEO != GEO_CART, CYL = GEO == GEO_CYL, SPH = GEO == GEO_SPH;
+  if (d.ctl->done) return;
+  const int lane = threadIdx.x;
+  const int j = d.ngy + blockIdx.y * V3W + threadIdx.y;
+  if (j >= d.ngy + d.ny) return;   // whole warps leave together
+  const int m0 = d.ngz + blockIdx.z * CH;
+  const int m1 = (m0 + CH < d.ngz + d.nz) ? m0 + CH : d.ngz + d.nz;   // planes this thread writes: [m0, m1)
+  const int iu = blockIdx.x * V3IN - 1 + lane;   // un-wrapped cell index
+  int i = iu % d.nx; if (i < 0) i += d.nx;
+  const bool store = lane >= 1 && lane <= 30 && iu < d.nx;
+  const VMetric<T, GEO> M{d};
+  const T nu = d.nu, two3 = T(2) / T(3), dt = (T)d.ctl->dt;
+  const long long P = d.plane, R = d.pitch;
+  const long long base = d.id(i, j, 0);
+
+  auto pf = [](const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); };
+  auto load3 = [&](const T* __restrict__ a, const long long l) { Rows3<T> r; r.m = a[l - R]; r.c = a[l]; r.p = a[l + R]; return r; };
+  // diagonal components at the centre of (row jj, plane kk): u0, u1 = vx at i, i+1; w0, w1 = vy at jj, jj+1; z0, z1 = vz at kk, kk+1
+  auto diag = [&](const int jj, const int kk, const T rh, const T u0, const T u1, const T w0, const T w1, const T z0, const T z1,
+                  T& oxx, T& oyy, T& ozz) {
+    const T div = d.invV(jj, kk) * ((((u1 - u0) * d.Sx(jj, kk)) + (w1 * d.Sy(jj + 1, kk) - w0 * d.Sy(jj, kk))) +
+                                    (z1 * d.Sz(jj, kk + 1) - z0 * d.Sz(jj, kk)));
+    const T mrn = -(rh * nu);
+    const T vyc = T(0.5) * (w0 + w1), vzc = T(0.5) * (z0 + z1);
+    T ex = (u1 - u0) * M.ix_c(jj, kk);
+    if (CURV) ex = ex + vyc * d.inv_yc[jj];
+    if (SPH) ex = ex + (vzc * d.cot_zc[kk]) * d.inv_yc[jj];
+    const T ey = (w1 - w0) * d.invLY[jj];
+    T ez = (z1 - z0) * d.invLZ(jj, kk);
+    if (SPH) ez = ez + vyc * d.inv_yc[jj];
+    oxx = mrn * (T(2) * ex - two3 * div);
+    oyy = mrn * (T(2) * ey - two3 * div);
+    ozz = mrn * (T(2) * ez - two3 * div);
+  };
+  // t_xy at (i-1/2, jj-1/2, kk): r.. = rho at (i,jj) (i-1,jj) (i,jj-1) (i-1,jj-1); u = vx at jj, jj-1; w = vy(jj) at i, i-1
+  auto f_txy = [&](const int jj, const int kk, const T r00, const T r10, const T r01, const T r11, const T u, const T um,
+                   const T w, const T wm) {
+    const T rhob = T(0.25) * (((r00 + r10) + r01) + r11);
+    T a = (u - um) * d.invDY[jj];
+    if (CURV) a = a - (T(0.5) * (u + um)) * d.inv_ye[jj];
+    return -(rhob * nu) * (a + (w - wm) * M.ix_je(jj, kk));
+  };
+  // t_xz at (i-1/2, jj, kk-1/2): rho at (i,kk) (i-1,kk) (i,kk-1) (i-1,kk-1); u = vx at kk, kk-1; z = vz(kk) at i, i-1
+  auto f_txz = [&](const int jj, const int kk, const T r00, const T r10, const T r01, const T r11, const T u, const T um,
+                   const T z, const T zm) {
+    const T rhob = T(0.25) * (((r00 + r10) + r01) + r11);
+    T a;
+    if (SPH) a = ((u * d.invRxk[kk] - um * d.invRxk[kk - 1]) * d.sin_ze[kk]) * d.invDZ(jj, kk);
+    else a = (u - um) * d.invDZ(jj, kk);
+    return -(rhob * nu) * (a + (z - zm) * M.ix_ke(jj, kk));
+  };
+  // t_yz at (i, jj-1/2, kk-1/2): rho at (jj,kk) (jj-1,kk) (jj,kk-1) (jj-1,kk-1); z = vz(kk) at jj, jj-1; w = vy(jj) at kk, kk-1
+  auto f_tyz = [&](const int jj, const int kk, const T r00, const T r10, const T r01, const T r11, const T z, const T zm,
+                   const T w, const T wm) {
+    const T rhob = T(0.25) * (((r00 + r10) + r01) + r11);
+    T a = (z - zm) * d.invDY[jj];
+    if (SPH) a = a - (T(0.5) * (z + zm)) * d.inv_ye[jj];
+    return -(rhob * nu) * (a + (w - wm) * M.iz_je(jj, kk));
+  };
+
+  // current plane c = n - 1 (rows j-1, j, j+1) and what is carried from earlier planes
+  Rows3<T> rc = load3(rho, base + (long long)(m0 - 1) * P), uc = load3(vx, base + (long long)(m0 - 1) * P);
+  Rows3<T> wc = load3(vy, base + (long long)(m0 - 1) * P), zc = load3(vz, base + (long long)(m0 - 1) * P);
+  T txz_c = T(0), tyz_c = T(0), tyzp_c = T(0), tzz_b = T(0), txx_b = T(0), rho_b = T(1);   // rho_b: rho(i, j, c-1)
+  const T y0 = d.ye[j], y1 = d.ye[j + 1];
+
+#pragma unroll 1
+  for (int n = m0; n <= m1; ++n) {
+    const long long ln = base + (long long)n * P;
+    if (n + V3_PF <= m1) {   // rows of a later plane into L1 (the block's other warps prefetch the rows between)
+      const long long lq = ln + (long long)V3_PF * P;
+      pf(rho + lq); pf(vx + lq); pf(vy + lq); pf(vz + lq);
+      if (threadIdx.y == 0) { pf(rho + lq - R); pf(vx + lq - R); pf(vy + lq - R); pf(vz + lq - R); }
+      if (threadIdx.y == V3W - 1) { pf(rho + lq + R); pf(vx + lq + R); pf(vy + lq + R); pf(vz + lq + R); }
+    }
+    const Rows3<T> rn = load3(rho, ln), un = load3(vx, ln), wn = load3(vy, ln), zn = load3(vz, ln);
+    const int c = n - 1;
+    // ---- leading plane n: t_xz(j, n), t_yz(j, n), t_yz(j+1, n) ----
+    const T txz_n = f_txz(j, n, rn.c, v_up1(rn.c), rc.c, v_up1(rc.c), un.c, uc.c, zn.c, v_up1(zn.c));
+    const T tyz_n = f_tyz(j, n, rn.c, rn.m, rc.c, rc.m, zn.c, zn.m, wn.c, wc.c);
+    const T tyzp_n = f_tyz(j + 1, n, rn.p, rn.c, rc.p, rc.c, zn.p, zn.c, wn.p, wc.p);
+    // ---- current plane c: diagonal at j and j-1, t_xy at j and j+1 ----
+    T txx, tyy, tzz, txx_m, tyy_m, tzz_m;
+    diag(j, c, rc.c, uc.c, v_dn1(uc.c), wc.c, wc.p, zc.c, zn.c, txx, tyy, tzz);
+    diag(j - 1, c, rc.m, uc.m, v_dn1(uc.m), wc.m, wc.c, zc.m, zn.m, txx_m, tyy_m, tzz_m);
+    const T rcl = v_up1(rc.c);
+    const T txy = f_txy(j, c, rc.c, rcl, rc.m, v_up1(rc.m), uc.c, uc.m, wc.c, v_up1(wc.c));
+    const T txy_p = f_txy(j + 1, c, rc.p, v_up1(rc.p), rc.c, rcl, uc.p, uc.c, wc.p, v_up1(wc.p));
+    // ---- force on the three lower faces of cell (i, j, c): Eqs. B4 | B5 | B6 ----
+    T ox, oy, oz;
+    {   // X component, at (i-1/2, j, c)
+      T a;
+      if (CURV) a = (((y1 * y1) * txy_p - (y0 * y0) * txy) * (d.inv_yc[j] * d.inv_yc[j])) * d.invLY[j];
+      else a = (txy_p - txy) * d.invLY[j];
+      const T b = (txx - v_up1(txx)) * M.ix_c(j, c);
+      const T cc = (txz_n - txz_c) * d.invLZ(j, c);
+      T s = (a + b) + cc;
+      if (SPH) {
+        s = s + (T(0.5) * (txy + txy_p)) * d.inv_yc[j];
+        s = s + ((T(2) * (T(0.5) * (txz_c + txz_n))) * d.cot_zc[c]) * d.inv_yc[j];
+      }
+      ox = uc.c - dt * (rdiv(T(2), rc.c + rcl) * s);
+    }
+    {   // Y component, at (i, j-1/2, c)
+      T a, cc, s;
+      const T b = (v_dn1(txy) - txy) * M.ix_je(j, c);
+      if (!CURV) {
+        a = (tyy - tyy_m) * d.invDY[j];
+        cc = (tyz_n - tyz_c) * d.invdz[c];
+        s = (a + b) + cc;
+      } else if (CYL) {
+        a = ((d.yc[j] * tyy - d.yc[j - 1] * tyy_m) * d.inv_ye[j]) * d.invDY[j];
+        cc = (tyz_n - tyz_c) * d.invdz[c];
+        s = ((a + b) - (T(0.5) * (txx + txx_m)) * d.inv_ye[j]) + cc;
+      } else {
+        a = ((((d.yc[j] * d.yc[j]) * tyy - (d.yc[j - 1] * d.yc[j - 1]) * tyy_m)) * (d.inv_ye[j] * d.inv_ye[j])) * d.invDY[j];
+        cc = ((tyz_n * d.sin_ze[c + 1] - tyz_c * d.sin_ze[c]) * d.invdz[c]) * (d.inv_ye[j] * d.invRxk[c]);
+        s = ((a + cc) + b) - ((T(0.5) * (tzz + tzz_m)) + (T(0.5) * (txx + txx_m))) * d.inv_ye[j];
+      }
+      oy = wc.c - dt * (rdiv(T(2), rc.c + rc.m) * s);
+    }
+    {   // Z component, at (i, j, c-1/2)
+      T a, cc, s;
+      const T b = (v_dn1(txz_c) - txz_c) * M.ix_ke(j, c);
+      if (!CURV) {
+        a = (tyzp_c - tyz_c) * d.invLY[j];
+        cc = (tzz - tzz_b) * d.invdzc[c];
+        s = (a + b) + cc;
+      } else if (CYL) {
+        a = ((y1 * tyzp_c - y0 * tyz_c) * d.inv_yc[j]) * d.invLY[j];
+        cc = (tzz - tzz_b) * d.invdzc[c];
+        s = (a + b) + cc;
+      } else {
+        a = ((((y1 * y1) * y1) * tyzp_c - ((y0 * y0) * y0) * tyz_c) * ((d.inv_yc[j] * d.inv_yc[j]) * d.inv_yc[j])) * d.invLY[j];
+        cc = ((tzz * d.sin_zc[c] - tzz_b * d.sin_zc[c - 1]) * d.invdzc[c]) * (d.inv_yc[j] * d.inv_sin_ze[c]);
+        s = ((a + cc) + b) - ((T(0.5) * (txx + txx_b)) * d.cot_ze[c]) * d.inv_yc[j];
+      }
+      oz = zc.c - dt * (rdiv(T(2), rc.c + rho_b) * s);
+    }
+    const bool st = store && c >= m0;
+    const long long lc = base + (long long)c * P;
+    st_if(vxd + lc, ox, st);
+    st_if(vyd + lc, oy, st);
+    st_if(vzd + lc, oz, st);
+    // ---- shift the Z window ----
+    rho_b = rc.c;
+    rc = rn; uc = un; wc = wn; zc = zn;
+    txz_c = txz_n; tyz_c = tyz_n; tyzp_c = tyzp_n; tzz_b = tzz; txx_b = txx;
+  }
+}
+
 template <typename T, int GEO>
 static int launch_v3(const Dev<T>& d, const T* rho, const T* vx, const T* vy, const T* vz, T* const* t, T* vxd, T* vyd,
                      T* vzd, cudaStream_t s) {
@@ -175,6 +352,43 @@ int launch_source_d3(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, 
     default: return launch_v3<T, GEO_SPH>(d, rho, vxc, vyc, vzc, t, vxd, vyd, vzd, s);
   }
 }
+
+template <typename T, int GEO>
+static int launch_v3f(const Dev<T>& d, const T* rho, const T* vx, const T* vy, const T* vz, T* vxd, T* vyd, T* vzd,
+                      cudaStream_t s) {
+  // chunk the march so that the grid fills the machine a few times over; each chunk re-reads 2 planes
+  const int ntile = (d.nx + V3IN - 1) / V3IN, nrow = (d.ny + V3W - 1) / V3W;
+  int nch = (148 * 12 + ntile * nrow - 1) / (ntile * nrow);
+  if (nch < 1) nch = 1;
+  int CH = (d.nz + nch - 1) / nch;
+  if (CH < 16) CH = 16;
+  if (CH > d.nz) CH = d.nz;
+  nch = (d.nz + CH - 1) / CH;
+  dim3 b(32, V3W), g(ntile, nrow, nch);
+  k_visc3d_fused<T, GEO><<<g, b, 0, s>>>(d, rho, vx, vy, vz, vxd, vyd, vzd, CH);
+  return 1;
+}
+
+// cell 7d on a 3-D mesh with a wrapped X axis in one pass, active cells only (the stress tensor is never stored)
+template <typename T>
+bool source_d3_fused_ok(const Dev<T>& d) { return d.hasx && d.hasy && d.hasz && d.xwrap; }
+
+template <typename T>
+int launch_source_d3_fused(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, const T* vzc, T* vxd, T* vyd,
+                           T* vzd, cudaStream_t s) {
+  switch (d.geometry) {
+    case GEO_CART: return launch_v3f<T, GEO_CART>(d, rho, vxc, vyc, vzc, vxd, vyd, vzd, s);
+    case GEO_CYL: return launch_v3f<T, GEO_CYL>(d, rho, vxc, vyc, vzc, vxd, vyd, vzd, s);
+    default: return launch_v3f<T, GEO_SPH>(d, rho, vxc, vyc, vzc, vxd, vyd, vzd, s);
+  }
+}
+
+#define INSTF(T)                                                                                                  \
+  template bool source_d3_fused_ok<T>(const Dev<T>&);                                                             \
+  template int launch_source_d3_fused<T>(const Dev<T>&, const T*, const T*, const T*, const T*, T*, T*, T*, cudaStream_t);
+INSTF(double)
+INSTF(float)
+#undef INSTF
 
 template int launch_source_d3<double>(const Dev<double>&, const double*, const double*, const double*, const double*,
                                       double* const*, double*, double*, double*, cudaStream_t);

@@ -42,6 +42,11 @@ template <typename T> int launch_source_d(const Dev<T>& d, const T* rho, const T
 template <typename T> int launch_source_d3(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, const T* vzc,
                                            T* const* t, T* vxd, T* vyd, T* vzd, cudaStream_t s);
 
+// the same in ONE pass on a wrapped X axis, active cells only (the ghost fill of cell 9 follows): (rho, vc) -> vd
+template <typename T> bool source_d3_fused_ok(const Dev<T>& d);
+template <typename T> int launch_source_d3_fused(const Dev<T>& d, const T* rho, const T* vxc, const T* vyc, const T* vzc,
+                                                 T* vxd, T* vyd, T* vzd, cudaStream_t s);
+
 // cells 12a-12c: one directional sweep.  first != 0: the momenta are formed from the state (12a fused).
 template <typename T> struct SweepArgs {
   State<T> st;        // state: e and velocities for the momenta (first pass); the frozen face velocities

@@ -282,7 +282,9 @@ struct Sim : CtxBase {
     if (L.hasy) { slots[nq++] = 3; slots[nq++] = 4; }
     if (L.hasz) { slots[nq++] = 5; slots[nq++] = 6; }
     sweep_setup<T>();
-    fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE");
+    // with viscosity the fused pass must be followed by the fused 7d (it then also produces the ghost layer 7d reads)
+    fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE") &&
+                  (!L.visc || (L.visc3d && source_d3_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_VISC")));
     fuse_dt = newvel_dt_ok<T>(d) && !getenv("FARGO_UNFUSED_DT");
     return FARGO_OK;
   }
@@ -405,6 +407,10 @@ struct Sim : CtxBase {
       if (L.adi) s2.e = alt[0];
       s2.vx = alt[1]; s2.vy = alt[2]; s2.vz = alt[3];
       n += timed("source", [&] { return launch_source_fused<T>(d, st, phi, s2, stream); });
+      if (L.visc3d) {   // cell 7d in one pass: reads v_c from the fused pass's arrays, writes the (dead) state velocities
+        n += timed("source_d", [&] { return launch_source_d3_fused<T>(d, st.rho, s2.vx, s2.vy, s2.vz, st.vx, st.vy, st.vz, stream); });
+        s2.vx = st.vx; s2.vy = st.vy; s2.vz = st.vz;
+      }
       n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                    // cell 9
     } else {
     // source step: intermediates live in transport set B (idle until the second pass)

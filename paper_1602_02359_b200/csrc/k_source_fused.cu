@@ -67,17 +67,20 @@ template <int N> __device__ __forceinline__ void sf_wait() { asm volatile("cp.as
 
 template <typename T, int GEO, bool ADI, bool POT, bool RING>
 __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, const State<T> st, const T* __restrict__ phi,
-                                                           const State<T> out, const int CH) {
+                                                           const State<T> out, const int CH, const int ext) {
   constexpr bool CURV = GEO == GEO_CYL || GEO == GEO_SPH, SPH = GEO == GEO_SPH;
   constexpr bool SHEAR = GEO == GEO_SHEAR;   // shearing sheet: Cartesian metric + Eq. 29 on the Y faces (reading G32)
   constexpr bool VXR = CURV || SHEAR;        // the Y faces need v_x of the neighbour rows
   constexpr int NV = ADI ? 4 : 3;   // Y faces whose v_b is needed: rows j-1 .. j-2+NV (7c needs v_c on the upper face too)
   if (d.ctl->done) return;
   const int lane = threadIdx.x;
-  const int j = d.ngy + blockIdx.y * SFW + threadIdx.y;
-  if (j >= d.ngy + d.ny) return;   // whole warps leave together
-  const int m0 = d.ngz + blockIdx.z * CH;
-  const int m1 = (m0 + CH < d.ngz + d.nz) ? m0 + CH : d.ngz + d.nz;   // planes this thread writes: [m0, m1)
+  // ext = 1 (viscosity follows): one ghost layer more in Y and Z, where 7d reads v_c (its stencil still fits in
+  // the three ghost layers: rows j-2 .. j+2, planes m-2 .. m+1)
+  const int j = d.ngy - ext + blockIdx.y * SFW + threadIdx.y;
+  if (j >= d.ngy + d.ny + ext) return;   // whole warps leave together
+  const int m0 = d.ngz - ext + blockIdx.z * CH;
+  const int mend = d.ngz + d.nz + ext;
+  const int m1 = (m0 + CH < mend) ? m0 + CH : mend;   // planes this thread writes: [m0, m1)
   const int iu = blockIdx.x * SFIN - 2 + 2 * lane;   // un-wrapped index of the lane's first cell (even)
   int i = iu % d.nx; if (i < 0) i += d.nx;
   const bool store = lane >= 1 && lane <= 30 && iu < d.nx;
@@ -324,30 +327,32 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
 
 template <typename T>
 bool source_fused_ok(const Dev<T>& d) {
-  return d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0 && !d.visc;
+  return d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0;   // with viscosity: followed by k_visc3d_fused
 }
 
 template <typename T, int GEO, bool ADI>
 static int launch_sf(const Dev<T>& d, const State<T>& st, const T* phi, const State<T>& out, cudaStream_t s) {
   // chunk the march so that the grid fills the machine a few times over; each chunk re-reads 4 planes
-  const int ntile = (d.nx + SFIN - 1) / SFIN, nrow = (d.ny + SFW - 1) / SFW;
+  const int ext = d.visc ? 1 : 0;   // 7d reads v_c one ghost layer out in Y and Z
+  const int nyo = d.ny + 2 * ext, nzo = d.nz + 2 * ext;
+  const int ntile = (d.nx + SFIN - 1) / SFIN, nrow = (nyo + SFW - 1) / SFW;
   int nch = (148 * 12 + ntile * nrow - 1) / (ntile * nrow);
   if (nch < 1) nch = 1;
-  int CH = (d.nz + nch - 1) / nch;
+  int CH = (nzo + nch - 1) / nch;
   if (CH < 16) CH = 16;   // shorter chunks on small meshes: the serial march, not the halo, is what costs there
-  if (CH > d.nz) CH = d.nz;
-  nch = (d.nz + CH - 1) / CH;
+  if (CH > nzo) CH = nzo;
+  nch = (nzo + CH - 1) / CH;
   dim3 b(32, SFW), g(ntile, nrow, nch);
   constexpr bool RING = GEO == GEO_CART || GEO == GEO_SHEAR;
   const size_t pair = 2 * sizeof(T);
   if (d.has_pot) {
     const int sm = RING ? (int)(SF_RS * 6 * 128 * pair) : 0;
     if (RING) cudaFuncSetAttribute(k_source_fused<T, GEO, ADI, true, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-    k_source_fused<T, GEO, ADI, true, RING><<<g, b, sm, s>>>(d, st, phi, out, CH);
+    k_source_fused<T, GEO, ADI, true, RING><<<g, b, sm, s>>>(d, st, phi, out, CH, ext);
   } else {
     const int sm = RING ? (int)(SF_RS * 5 * 128 * pair) : 0;
     if (RING) cudaFuncSetAttribute(k_source_fused<T, GEO, ADI, false, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-    k_source_fused<T, GEO, ADI, false, RING><<<g, b, sm, s>>>(d, st, phi, out, CH);
+    k_source_fused<T, GEO, ADI, false, RING><<<g, b, sm, s>>>(d, st, phi, out, CH, ext);
   }
   return 1;
 }

@@ -90,6 +90,7 @@ static void full_update(oracle_ctx* c, int until) {
   orc_vmean(o);                                                 if (until == ORC_ST_VMEAN) return;    // cell 3
   orc_potential(o);                                             if (until == ORC_ST_POT) return;      // cells 4-5
   o.dt = orc_compute_dt(o, &clipped);                           if (until == ORC_ST_DT) return;       // cell 6
+  orc_planets_update(o);                                                                              // cell 5a (G33)
   orc_source_a(o);                                              if (until == ORC_ST_SRC_A) return;    // cell 7a
   orc_source_b(o);                                              if (until == ORC_ST_SRC_B) return;    // cell 7b
   orc_source_c(o);                                              if (until == ORC_ST_SRC_C) return;    // cell 7c

@@ -71,6 +71,10 @@ def lib():
             L.oracle_set_array.argtypes = [vp, C.c_char_p, _DP]
             L.oracle_dims.argtypes = [vp] + [C.POINTER(C.c_int)] * 6
             L.oracle_geometry.argtypes = [vp, C.c_int, C.c_int] + [_DP] * 7
+            L.oracle_set_planets.argtypes = [vp, C.c_int, _DP, _DP, _DP, _DP, C.c_int, C.c_double]
+            L.oracle_get_planets.argtypes = [vp, _DP, _DP, _DP]
+            L.oracle_planets_rk5.argtypes = [vp, C.c_double]
+            L.oracle_gas_force.argtypes = [vp, C.c_int, _DP]
             L.oracle_vanleer_slopes.argtypes = [C.c_int, _DP, _DP, _DP]
             L.oracle_vanleer_slopes.restype = None
             L.oracle_vanleer_star.argtypes = [C.c_int, _DP, _DP, _DP, _DP, C.c_double, _DP]
@@ -163,6 +167,31 @@ class Oracle:
         t, dt, n = C.c_double(), C.c_double(), C.c_longlong()
         lib().oracle_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n))
         return t.value, dt.value, n.value
+
+    # ---- live planets (NEXT-2) ----
+    def set_planets(self, gm, eps, pos, vel, force_mode: int = 1, gconst: float = 1.0):
+        gm, eps, pos, vel = (_f64(np.atleast_1d(a)).ravel() for a in (gm, eps, pos, vel))
+        n = len(gm)
+        assert len(eps) == n and len(pos) == 3 * n and len(vel) == 3 * n
+        if lib().oracle_set_planets(self._h, n, _p(gm), _p(eps), _p(pos), _p(vel), force_mode, float(gconst)) != 0:
+            raise ValueError("oracle_set_planets failed")
+        self._npl = n
+
+    def get_planets(self):
+        n = getattr(self, "_npl", 0)
+        pos, vel, acc = (np.zeros((n, 3)) for _ in range(3))
+        lib().oracle_get_planets(self._h, _p(pos), _p(vel), _p(acc))
+        return pos, vel, acc
+
+    def planets_rk5(self, h: float):
+        if lib().oracle_planets_rk5(self._h, float(h)) != 0:
+            raise RuntimeError("oracle_planets_rk5 failed")
+
+    def gas_force(self, p: int = 0):
+        F = np.zeros(3)
+        if lib().oracle_gas_force(self._h, p, _p(F)) != 0:
+            raise RuntimeError("oracle_gas_force failed")
+        return F
 
     def array(self, name: str) -> np.ndarray:
         """Ghost-inclusive copy of an internal array, shape (TZ, TY, TX) or (TZ, TY) for ring arrays."""

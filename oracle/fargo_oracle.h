@@ -65,6 +65,22 @@ int oracle_get_fields(oracle_ctx* c, double* rho, double* e, double* vx, double*
 int oracle_step(oracle_ctx* c, int n);
 int oracle_get_time(oracle_ctx* c, double* t, double* last_dt, long long* nsteps);
 
+/* NEXT-2, live planets (section 3.8; reading G33).  n <= ORC_MAX_PLANETS point masses: gm[p] = G m_p,
+ * eps[p] = softening length of planet p's potential and of the gas force on it, pos/vel = 3n Cartesian components
+ * in the frame rotating at omega_frame.  force_mode: 0 = the gas does not act on the planets, 1 = direct summation
+ * over all cells, 2 = axisymmetric part of the density removed first; gconst = G.  With n > 0 the
+ * fixed-orbit planet of oracle_params is ignored, the potential of cell 5 is that of the star and of these planets
+ * where they are at the beginning of the update, and cell 5a (gas kick + one Cash-Karp step over dt, Eq. 109 with
+ * Tab. 3) runs right after cell 6.  Cylindrical and spherical meshes only. */
+#define ORC_MAX_PLANETS 8
+int oracle_set_planets(oracle_ctx* c, int n, const double* gm, const double* eps, const double* pos,
+                       const double* vel, int force_mode, double gconst);
+/* returns n; gas_acc = the acceleration the gas gave each planet in the last update (3n) */
+int oracle_get_planets(oracle_ctx* c, double* pos, double* vel, double* gas_acc);
+/* test hooks: one Cash-Karp step of size h on the planets alone; sum_cells dm (x_c - x_p)/(d^2 + eps^2)^(3/2) for planet p */
+int oracle_planets_rk5(oracle_ctx* c, double h);
+int oracle_gas_force(oracle_ctx* c, int p, double* F);
+
 /* Run the NEXT update only up to and including `stage`, leaving intermediates in place.  The state
  * is then mid-step: inspect with oracle_get_array, do not call oracle_step afterwards. */
 int oracle_step_until(oracle_ctx* c, int stage);

@@ -26,7 +26,7 @@ void orc_build_tables(oracle_ctx& c, const oracle_mesh& m) {
   // ---- j tables ------------------------------------------------------------------------------
   c.yc.resize(TY); c.inv_yc.resize(TY); c.inv_ye.resize(TY + 1);
   c.LY.resize(TY); c.invLY.resize(TY); c.DY.resize(TY); c.invDY.resize(TY);
-  c.sxj.resize(TY); c.syj.resize(TY + 1); c.szj.resize(TY); c.invVj.resize(TY);
+  c.sxj.resize(TY); c.syj.resize(TY + 1); c.szj.resize(TY); c.invVj.resize(TY); c.Vj.resize(TY);
   c.Rxj.resize(TY); c.invRxj.resize(TY); c.LXj.resize(TY); c.invLXj.resize(TY);
   c.Rzj.resize(TY); c.invRzj.resize(TY);
   for (int j = 0; j <= TY; ++j) c.inv_ye[j] = 1.0 / c.ye[j];
@@ -63,6 +63,7 @@ void orc_build_tables(oracle_ctx& c, const oracle_mesh& m) {
         c.Rxj[j] = c.yc[j]; c.Rzj[j] = c.yc[j];
         break;
     }
+    c.Vj[j] = 1.0 / c.invVj[j];
     c.invRxj[j] = 1.0 / c.Rxj[j];
     c.invRzj[j] = 1.0 / c.Rzj[j];
     c.LXj[j] = dx * c.Rxj[j];

@@ -40,6 +40,13 @@ struct oracle_ctx {
   vec cos_xc, sin_xc;                  // cos/sin of the azimuth of cell centres
 
   // ---- fields, ghost-inclusive, X fastest ----------------------------------------------------
+  // ---- live planets (NEXT-2, planets.cpp) ------------------------------------------------------
+  int npl = 0, force_mode = 0;
+  double pl_gconst = 1.0;
+  double pl_gm[ORC_MAX_PLANETS], pl_eps[ORC_MAX_PLANETS];
+  double pl_x[ORC_MAX_PLANETS][3], pl_v[ORC_MAX_PLANETS][3], pl_f[ORC_MAX_PLANETS][3];
+  vec Vj;                              // 1 / invVj: V(j,k) = Vj[j] * syk[k] (Tab. 5)
+
   vec rho, e, vx, vy, vz;              // state
   vec phi;                             // potential at centres (cell 5)
   vec vxb, vyb, vzb;                   // after 7a
@@ -95,3 +102,4 @@ void orc_sweep(oracle_ctx& c, int dir);
 void orc_orbital_frac(oracle_ctx& c);
 void orc_orbital_shift(oracle_ctx& c);
 void orc_newvel(oracle_ctx& c);
+void orc_planets_update(oracle_ctx& c);   // planets.cpp, cell 5a

@@ -80,7 +80,13 @@ void orc_potential(oracle_ctx& c) {
       for (int i = 0; i < c.TX; ++i) {
         const double x = R * c.cos_xc[i], y = R * c.sin_xc[i];
         double phi = -(c.p.gm_star / r);
-        if (c.p.planet_mass != 0.0) {
+        if (c.npl > 0) {   // live planets (NEXT-2, reading G33): where they are at the beginning of the update
+          for (int p = 0; p < c.npl; ++p) {
+            const double ddx = x - c.pl_x[p][0], ddy = y - c.pl_x[p][1], ddz = z - c.pl_x[p][2];
+            const double d2 = ((ddx * ddx + ddy * ddy) + ddz * ddz) + c.pl_eps[p] * c.pl_eps[p];
+            phi = phi - c.pl_gm[p] / std::sqrt(d2);
+          }
+        } else if (c.p.planet_mass != 0.0) {
           const double ddx = x - xp, ddy = y - yp;
           const double d2 = ((ddx * ddx + ddy * ddy) + z * z) + eps2;
           phi = phi - c.p.planet_mass / std::sqrt(d2);

@@ -120,6 +120,23 @@ int fargo_get_time(fargo_ctx* c, double* t, double* last_dt, long long* nsteps);
 long long fargo_kernel_launches(const fargo_ctx* c);
 
 /* ---- inspection, for per-stage parity tests ---------------------------------------------------- */
+/* Live planets (section 3.8; reading G33).  n <= FARGO_MAX_PLANETS point
+ * masses around the star (gm_star of fargo_params, fixed at the origin).  All arrays are HOST, fp64, caller-owned:
+ * gm[n] = G m_p; eps[n] = softening length of planet p's potential and of the gas force on it; pos[3n], vel[3n] =
+ * Cartesian components in the frame rotating at omega_frame (constant).  force_mode: 0 = the gas does not act on the
+ * planets, 1 = direct summation over all active cells, 2 = the axisymmetric part of the density is removed first
+ * (P:717-720); gconst = G.  With n > 0 the fixed-orbit planet of fargo_params is ignored; every update then computes
+ * the potential of cell 5 from the planets' current positions and, right after cell 6, runs cell 5a on the device:
+ * v_p += dt a_gas(rho^n), then one fifth-order Cash-Karp step over dt (Eq. 109, Tab. 3).  The state
+ * lives on the device: fargo_step(n) needs no host synchronisation.  Cylindrical and spherical meshes whose context
+ * was created with a potential (gm_star != 0).  n = 0 switches back.  Errors: FARGO_EINVAL, FARGO_ESTATE, FARGO_ECUDA. */
+#define FARGO_MAX_PLANETS 8
+int fargo_set_planets(fargo_ctx* ctx, int n, const double* gm, const double* eps, const double* pos, const double* vel,
+                      int force_mode, double gconst);
+/* Synchronises the stream; copies positions, velocities and the acceleration the gas gave each planet in the last
+ * update (3n each, HOST, any may be NULL).  Returns n (>= 0) or a negative error code. */
+int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc);
+
 /* Run the NEXT update up to and including `stage`; the state is then mid-step (only
  * fargo_get_array / fargo_dims / fargo_destroy / fargo_set_fields are valid afterwards). */
 int fargo_step_until(fargo_ctx* c, int stage);

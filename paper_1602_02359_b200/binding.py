@@ -20,7 +20,8 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
           "SWEEP_X", "SWEEP_Y", "SWEEP_Z", "ORB_FRAC", "ORB_SHIFT", "NEWVEL"]
 EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
-           "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div"]
+           "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div",
+           "fargo_set_planets", "fargo_get_planets"]
 
 
 class FargoMesh(C.Structure):
@@ -73,6 +74,8 @@ def load():
     L.fargo_profile.argtypes = [vp, C.c_int]
     L.fargo_profile_report.argtypes = [vp, C.c_char_p, C.c_size_t]
     L.fargo_last_error.argtypes = [vp]
+    L.fargo_set_planets.argtypes = [vp, C.c_int, _DP, _DP, _DP, _DP, C.c_int, C.c_double]
+    L.fargo_get_planets.argtypes = [vp, _DP, _DP, _DP]
     L.fargo_selftest_div.argtypes = [vp, vp, vp, C.c_longlong, vp]
     L.fargo_selftest_div.restype = C.c_int
     L.fargo_last_error.restype = C.c_char_p
@@ -204,6 +207,26 @@ class Fargo:
         t, dt, n = C.c_double(), C.c_double(), C.c_longlong()
         self._check(load().fargo_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n)), "fargo_get_time")
         return t.value, dt.value, n.value
+
+    # -- live planets (NEXT-2) ------------------------------------------------------------------------
+    def set_planets(self, gm, eps, pos, vel, force_mode: int = 1, gconst: float = 1.0):
+        a = [np.ascontiguousarray(np.atleast_1d(x), dtype=np.float64).ravel() for x in (gm, eps, pos, vel)]
+        n = len(a[0])
+        if len(a[1]) != n or len(a[2]) != 3 * n or len(a[3]) != 3 * n:
+            raise ValueError("gm, eps need n entries, pos and vel 3 n")
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_set_planets(self._h, n, *[x.ctypes.data_as(_DP) for x in a], force_mode, float(gconst)),
+                        "fargo_set_planets")
+        self._npl = n
+
+    def get_planets(self):
+        n = getattr(self, "_npl", 0)
+        pos, vel, acc = (np.zeros((n, 3)) for _ in range(3))
+        with self._torch.cuda.device(self.device):
+            rc = load().fargo_get_planets(self._h, *[x.ctypes.data_as(_DP) for x in (pos, vel, acc)])
+        if rc < 0:
+            self._check(rc, "fargo_get_planets")
+        return pos, vel, acc
 
     def kernel_launches(self) -> int:
         return int(load().fargo_kernel_launches(self._h))

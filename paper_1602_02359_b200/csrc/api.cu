@@ -32,6 +32,8 @@ struct CtxBase {
   virtual int get_time(double*, double*, long long*) = 0;
   virtual int get_array(const char*, void*) = 0;
   virtual void dims(int*, int*, int*, int*, int*, int*) const = 0;
+  virtual int set_planets(int, const double*, const double*, const double*, const double*, int, double) = 0;
+  virtual int get_planets(double*, double*, double*) = 0;
   virtual int profile(int enable) = 0;
   virtual int profile_report(char* buf, size_t len) = 0;
   long long launches = 0;
@@ -47,6 +49,8 @@ struct Layout {   // sizes shared by fargo_workspace_bytes and fargo_init
   size_t table_elems;  // total 1-D table elements (each table padded to 32 elements)
   size_t bytes(size_t es) const {
     size_t b = 256;                                              // Ctl
+    b += align_up(sizeof(PlanetsDev), 256);                      // live planets (NEXT-2)
+    b += align_up((size_t)planets_blocks(ny, nz) * MAXPL * 3 * sizeof(double), 256);   // their force partials
     b += align_up(table_elems * es, 256);                        // tables
     b += 2 * align_up((size_t)TY * TZ * es, 256);                // v0, nshift
     b += (size_t)n3d * align_up((size_t)narr * es, 256);
@@ -89,7 +93,7 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4;   // state, Phi, two transport sets, the source step's output
   const size_t pad = 32;
   auto t1 = [&](int n) { return align_up((size_t)n, pad); };
-  L.table_elems = 7 * t1(L.TY + 1) + 10 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 6 * t1(L.TZ + 1) + 2 * t1(L.TX);
+  L.table_elems = 7 * t1(L.TY + 1) + 11 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 6 * t1(L.TZ + 1) + 2 * t1(L.TX);
   return true;
 }
 
@@ -99,6 +103,9 @@ struct Sim : CtxBase {
   Dev<T> d;
   State<T> st;
   T *phi = nullptr, *v0 = nullptr, *nshift = nullptr;
+  PlanetsDev* pl = nullptr;   // live planets (NEXT-2): device state, force partials, host copy of the constants
+  double* pl_part = nullptr;
+  int npl = 0, pl_mode = 0;
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
   bool fuse_source = false;
@@ -211,6 +218,8 @@ struct Sim : CtxBase {
     unsigned char* base = (unsigned char*)p->workspace;
     size_t off = 0;
     ctl = (Ctl*)base; off += 256;
+    pl = (PlanetsDev*)(base + off); off += align_up(sizeof(PlanetsDev), 256);
+    pl_part = (double*)(base + off); off += align_up((size_t)planets_blocks(L.ny, L.nz) * MAXPL * 3 * sizeof(double), 256);
     T* tab = (T*)(base + off);
     std::vector<T> htab(L.table_elems, T(0));
     size_t tpos = 0;
@@ -232,6 +241,11 @@ struct Sim : CtxBase {
     d.sin_zc = put(ht.sin_zc); d.cos_zc = put(ht.cos_zc); d.sin_ze = put(ht.sin_ze); d.cot_ze = put(ht.cot_ze);
     d.cos_xc = put(ht.cos_xc); d.sin_xc = put(ht.sin_xc);
     d.cot_zc = put(ht.cot_zc); d.inv_sin_ze = put(ht.inv_sin_ze);
+    {
+      std::vector<double> Vj(ht.invVj.size());
+      for (size_t n = 0; n < Vj.size(); ++n) Vj[n] = 1.0 / ht.invVj[n];
+      d.Vj = put(Vj);
+    }
     if (tpos > L.table_elems) { err = "internal: table area overflow"; return FARGO_EINVAL; }
     off += align_up(L.table_elems * sizeof(T), 256);
     const size_t ringb = align_up((size_t)L.TY * L.TZ * sizeof(T), 256);
@@ -360,6 +374,43 @@ struct Sim : CtxBase {
     return FARGO_OK;
   }
 
+  // ---- live planets (NEXT-2) ---------------------------------------------------------------------------
+  int set_planets(int n, const double* gm, const double* eps, const double* pos, const double* vel, int mode, double gconst) override {
+    if (n < 0 || n > MAXPL || mode < 0 || mode > 2) { err = "planet count or force mode out of range"; return FARGO_EINVAL; }
+    if (n > 0 && (!gm || !eps || !pos || !vel)) { err = "null planet array"; return FARGO_EINVAL; }
+    if (n > 0 && (d.geometry == GEO_CART || !L.hasx)) { err = "live planets need a cylindrical or spherical mesh"; return FARGO_EINVAL; }
+    if (n > 0 && !L.has_pot) { err = "the context was created without a potential (gm_star = 0 and planet_mass = 0)"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    PlanetsDev h;
+    memset(&h, 0, sizeof h);
+    h.n = n; h.mode = mode; h.gconst = gconst;
+    for (int p = 0; p < n; ++p) {
+      h.gm[p] = gm[p]; h.eps[p] = eps[p];
+      for (int c = 0; c < 3; ++c) { h.x[p][c] = pos[3 * p + c]; h.v[p][c] = vel[3 * p + c]; }
+    }
+    if (!ck(cudaMemcpyAsync(pl, &h, sizeof h, cudaMemcpyHostToDevice, stream), "upload planets")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "set_planets sync")) return FARGO_ECUDA;
+    if ((n > 0) != (npl > 0) || n != npl || mode != pl_mode) {   // the kernel sequence changes: capture it again
+      if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
+    }
+    npl = n; pl_mode = mode;
+    pot_valid = false;
+    return FARGO_OK;
+  }
+
+  int get_planets(double* pos, double* vel, double* gas_acc) override {
+    PlanetsDev h;
+    if (!ck(cudaMemcpyAsync(&h, pl, sizeof h, cudaMemcpyDeviceToHost, stream), "download planets")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "get_planets sync")) return FARGO_ECUDA;
+    for (int p = 0; p < npl; ++p)
+      for (int c = 0; c < 3; ++c) {
+        if (pos) pos[3 * p + c] = h.x[p][c];
+        if (vel) vel[3 * p + c] = h.v[p][c];
+        if (gas_acc) gas_acc[3 * p + c] = h.f[p][c];
+      }
+    return npl;
+  }
+
   // ---- one update --------------------------------------------------------------------------------------
   int field_mask(bool with_rho, bool with_e) const {
     int mk = F_VX;
@@ -387,7 +438,9 @@ struct Sim : CtxBase {
     if (until == FARGO_ST_BC1) return n;
     if (L.fargo) n += timed("vmean", [&] { return launch_vmean<T>(d, st.vx, v0, stream); });                         // cell 3
     if (until == FARGO_ST_VMEAN) return n;
-    if (L.has_pot && (!pot_valid || !pot_static)) {                                  // cell 5
+    if (npl > 0) {                                                                    // cell 5, live planets (on the device)
+      n += timed("potential", [&] { return launch_potential_live<T>(d, phi, (T)prm.gm_star, pl, npl, stream); });
+    } else if (L.has_pot && (!pot_valid || !pot_static)) {                           // cell 5
       double t = 0.0;
       if (!pot_static && !capturing) { get_time(&t, nullptr, nullptr); }
       n += timed("potential", [&] { return potential(t); });
@@ -401,6 +454,8 @@ struct Sim : CtxBase {
       dt_ready = false;   // k_dt_finish consumed and cleared the running max
     }
     if (until == FARGO_ST_DT) return n;
+    if (npl > 0)                                                                      // cell 5a (reading G33)
+      n += timed("planets", [&] { return launch_planets_update<T>(d, st.rho, pl, npl, pl_mode, pl_part, prm.gm_star, prm.omega_frame, stream); });
     State<T> s2 = st;   // the state the transport step reads: e and v after the source step
     if (fuse_source && until < 0) {
       // cells 7a-7c in one pass; it reads neighbours of the state, so its output goes to arrays of its own
@@ -507,7 +562,7 @@ struct Sim : CtxBase {
     if (nsteps < 0) { err = "negative step count"; return FARGO_EINVAL; }
     if (nsteps == 0) return FARGO_OK;
     // the legacy default stream cannot be captured: plain launches there
-    const bool graph_ok = prm.use_graph && pot_static && stream != nullptr && !prof;
+    const bool graph_ok = prm.use_graph && (pot_static || npl > 0) && stream != nullptr && !prof;
     int s = 0;
     if (graph_ok && fuse_dt && !dt_ready) {
       // the captured sequence relies on the previous update's k_newvel_dt for the per-cell CFL rate: the first
@@ -518,7 +573,7 @@ struct Sim : CtxBase {
     }
     if (graph_ok) {
       if (!gexec) {
-        if (L.has_pot && !pot_valid) { launches += potential(0.0); pot_valid = true; }   // keep it out of the graph
+        if (L.has_pot && !pot_valid && npl == 0) { launches += potential(0.0); pot_valid = true; }   // keep it out of the graph
         cudaGraph_t g = nullptr;
         if (!ck(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal), "begin capture")) return FARGO_ECUDA;
         launches_per_step = enqueue_update(-1, true);
@@ -628,6 +683,13 @@ int fargo_get_time(fargo_ctx* c, double* t, double* last_dt, long long* nsteps) 
   return c ? c->impl->get_time(t, last_dt, nsteps) : FARGO_EINVAL;
 }
 long long fargo_kernel_launches(const fargo_ctx* c) { return c ? c->impl->launches : 0; }
+int fargo_set_planets(fargo_ctx* c, int n, const double* gm, const double* eps, const double* pos, const double* vel,
+                      int force_mode, double gconst) {
+  return c ? c->impl->set_planets(n, gm, eps, pos, vel, force_mode, gconst) : FARGO_EINVAL;
+}
+int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
+  return c ? c->impl->get_planets(pos, vel, gas_acc) : FARGO_EINVAL;
+}
 int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }
 int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) {
   if (!c) return FARGO_EINVAL;

@@ -15,6 +15,12 @@ template <typename T> int launch_vmean(const Dev<T>& d, const T* vx, T* v0, cuda
 // cell 5: potential of the star and the planet at cell centres; cphi, sphi = cos, sin of the planet's azimuth
 template <typename T> int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2,
                                            cudaStream_t s);
+// live planets (NEXT-2, k_planets.cu): cell 5 with the planets where they are now (device state); cell 5a = gas force
+// (block partials in `part`, planets_blocks() x 3 MAXPL doubles), kick and one Cash-Karp step over ctl->dt
+int planets_blocks(int ny, int nz);
+template <typename T> int launch_potential_live(const Dev<T>& d, T* phi, T gm_star, const PlanetsDev* pl, int npl, cudaStream_t s);
+template <typename T> int launch_planets_update(const Dev<T>& d, const T* rho, PlanetsDev* pl, int npl, int mode, double* part,
+                                                double gm_star, double omega, cudaStream_t s);
 // cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
 enum { DT_BOTH = 0, DT_FINISH = 1, DT_CELLS = 2 };   // per-cell max + finish | finish only | per-cell max only
 template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode = DT_BOTH);

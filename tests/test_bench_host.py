@@ -3,6 +3,7 @@ gloo group: max-over-ranks timing, whole-job aggregation, and the reference arm 
 (rank 0 alone runs and prints; the other rank exits 0 without work)."""
 import json
 import os
+import re
 import subprocess
 import sys
 
@@ -20,7 +21,7 @@ rank, world = dist.get_rank(), dist.get_world_size()
 bench.rank_barrier(world)
 ms = bench.rank_max(10.0 + 5.0 * rank, world, "cpu")       # rank 1 is the slow replica
 rate = bench.whole_job_rate(1000, 4, world, ms)
-print("RESULT %d %.6f %.6f" % (rank, ms, rate), flush=True)
+sys.stdout.write("RESULT %d %.6f %.6f\n" % (rank, ms, rate)); sys.stdout.flush()   # one write: ranks share the pipe
 dist.destroy_process_group()
 """
 
@@ -46,7 +47,7 @@ def test_max_over_ranks_and_whole_job_rate_gloo_world2(tmp_path):
     script.write_text(_WORKER.format(root=ROOT))
     r = _torchrun([str(script)])
     assert r.returncode == 0, r.stderr[-2000:]
-    res = sorted(ln.split()[1:] for ln in r.stdout.splitlines() if ln.startswith("RESULT"))
+    res = sorted(re.findall(r"RESULT (\d+) ([0-9.]+?\d{6}) ([0-9.]+?\d{6})", r.stdout))
     assert len(res) == 2
     for rank, ms, rate in res:
         assert float(ms) == 15.0                       # every rank sees the slowest replica's time

@@ -1,0 +1,110 @@
+"""GPU parity for live planets (section 3.8; reading G33): the CUDA path through the
+C ABI (fargo_set_planets / fargo_step / fargo_get_planets) against the CPU oracle on the same seeded disks.
+
+Tolerances.  The Cash-Karp step is the same fp64 arithmetic in the same order on both sides: without a gas force the
+planets must agree BIT for bit.  The gas force is a floating-point sum over all cells: the oracle adds the cells one
+after the other, the kernel adds lanes, warps and blocks in a tree, so the two differ by rounding,
+|dF| <~ eps_64 sqrt(N) sum|f_i|; the test allows 1e-11 of sum|f_i| (estimated by |F| of the lopsided test disk) and
+the north_star's 1e-10 on the fields and on the planets' positions afterwards."""
+import numpy as np
+import pytest
+
+import gpu_cases as G
+from oracle.binding import Oracle
+from paper_1602_02359_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _pair(w, precision=64, use_graph=True):
+    from paper_1602_02359_b200 import Fargo
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=precision, use_graph=use_graph)
+    g.set_fields(*w.fields())
+    o = Oracle(w.mesh, w.geometry, w.eos, w.params)
+    o.set_fields(*w.fields())
+    return g, o
+
+
+def _rel(a, b):
+    s = float(np.max(np.abs(b)))
+    d = float(np.max(np.abs(np.asarray(a, dtype=np.float64) - b)))
+    return d / s if s > 0 else d
+
+
+def _lopsided(w):
+    """Give the disk an m = 1 asymmetry so that the gas force on the planets is well away from zero."""
+    phi = w.mesh.xc()[None, None, :]
+    w.rho = w.rho * (1.0 + 0.3 * np.cos(phi - 0.9))
+    return w
+
+
+PLANETS_1 = dict(gm=[1e-3], eps=[0.03], pos=[1.0, 0.0, 0.0], vel=[0.0, 0.0, 0.0])
+PLANETS_2 = dict(gm=[1e-3, 3e-4], eps=[0.03, 0.04], pos=[1.0, 0.0, 0.0, -0.2, 1.45, 0.01],
+                 vel=[0.0, 0.0, 0.0, 0.62, 0.09, 0.0])
+
+CASES = [("cyl2d", lambda: _lopsided(G.cyl2d_iso_fargo_visc(nsteps=8)), PLANETS_1, 1),
+         ("cyl2d_bm08", lambda: _lopsided(G.cyl2d_iso_fargo_visc(nsteps=6)), PLANETS_2, 2),
+         ("sph3d", lambda: _lopsided(G.sph3d_iso_fargo(nsteps=5)), PLANETS_2, 1),
+         ("cyl3d_adi", lambda: _lopsided(G.cyl3d_adi_fargo(nsteps=4)), PLANETS_1, 2)]
+
+
+@pytest.mark.parametrize("name,make,pl,mode", CASES, ids=[c[0] for c in CASES])
+def test_planets_and_fields_match_the_oracle(name, make, pl, mode):
+    w = make()
+    g, o = _pair(w)
+    for c in (g, o):
+        c.set_planets(pl["gm"], pl["eps"], pl["pos"], pl["vel"], force_mode=mode, gconst=1.0)
+    g.step(w.nsteps); o.step(w.nsteps)
+    gp, gv, ga = g.get_planets()
+    op, ov, oa = o.get_planets()
+    assert g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
+    assert np.max(np.abs(oa)) > 0
+    assert _rel(ga, oa) < 1e-11, (ga, oa)
+    assert _rel(gp, op) < 1e-12 and _rel(gv, ov) < 1e-10, (gp - op, gv - ov)
+    for a, b, nm in zip(g.get_fields(), o.get_fields(), ("rho", "e", "vx", "vy", "vz")):
+        if b is not None and a is not None and np.max(np.abs(b)) > 0:
+            assert _rel(a, b) <= 1e-10, nm
+
+
+def test_without_gas_force_the_planets_are_bit_identical():
+    w = G.sph3d_iso_fargo(nsteps=6)
+    g, o = _pair(w)
+    for c in (g, o):
+        c.set_planets(PLANETS_2["gm"], PLANETS_2["eps"], PLANETS_2["pos"], PLANETS_2["vel"], force_mode=0)
+    g.step(w.nsteps); o.step(w.nsteps)
+    gp, gv, ga = g.get_planets()
+    op, ov, oa = o.get_planets()
+    assert np.array_equal(gp, op) and np.array_equal(gv, ov) and not ga.any()
+    assert not np.array_equal(gp.ravel(), np.asarray(PLANETS_2["pos"]))     # they did move
+    for a, b in zip(g.get_fields(), o.get_fields()):
+        assert _rel(a, b) <= 1e-10
+
+
+def test_graph_replay_equals_plain_launches_and_fp32_is_close():
+    w = _lopsided(G.cyl2d_iso_fargo_visc(nsteps=6))
+    out = []
+    for precision, graph in ((64, True), (64, False), (32, True)):
+        g, _ = _pair(w, precision=precision, use_graph=graph)
+        g.set_planets(**PLANETS_1, force_mode=1)
+        g.step(3); g.step(w.nsteps - 3)
+        out.append((g.get_planets(), g.get_fields()))
+    for a, b in zip(out[0][0], out[1][0]):
+        assert np.array_equal(a, b)
+    for a, b in zip(out[0][1], out[1][1]):
+        assert a is None or np.array_equal(a, b)
+    assert _rel(out[2][0][0], out[0][0][0]) < 1e-4 and _rel(out[2][0][2], out[0][0][2]) < 1e-3
+    for a, b in zip(out[2][1], out[0][1]):
+        assert a is None or _rel(a, b) < 1e-4
+
+
+def test_set_planets_argument_errors():
+    from paper_1602_02359_b200 import Fargo
+    w = G.cart_adi_periodic(nx=16, ny=8, nz=8)
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params)
+    g.set_fields(*w.fields())
+    with pytest.raises(RuntimeError):
+        g.set_planets(**PLANETS_1)                     # Cartesian mesh
+    w = G.cyl2d_iso_fargo_visc()
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params)
+    with pytest.raises(RuntimeError):
+        g.set_planets([1e-3] * 9, [0.1] * 9, np.zeros(27) + 1.0, np.zeros(27))     # more than FARGO_MAX_PLANETS

@@ -60,6 +60,8 @@ def make_workload(name: str):
         return full, small, "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
     if name == "sheet3d":   # NEXT-1: shearing sheet (Eqs. 28-30, Tab. 2), adiabatic, orbital advection on
         return W.sheet3d(), W.sheet3d(1024, 32, 16), "same recipe on 1024x32x16 (full rows, fewer y and z cells)"
+    if name == "disk3dlive":   # NEXT-2: config 4 with its planet live (RK5 + gas force by direct summation)
+        return W.disk3d_live(), W.disk3d_live(1536, 32, 16), "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
     if name == "disk2d":
         return W.disk2d(), W.disk2d(), "the whole 768x256 mesh"
     if name == "sound":
@@ -77,7 +79,7 @@ NCU_TRAFFIC_B_PER_CELL = {
                "orbital": 118.2, "newvel": 82.6},
 }
 
-CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
+CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dlive": "4 with a live planet (NEXT-2 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
 def algorithmic_reals(w):
@@ -103,6 +105,8 @@ def algorithmic_reals(w):
         "sweep": (1 + nq + 1) + (1 + nq),
         "orbital": (1 + nq) + (1 + nq),
         "newvel": (1 + 2 * nd) + nd,
+        "potential": 1,     # live planets: Phi rewritten every update
+        "planets": 1,       # gas force: rho read once per planet (ring served by L1 for the further ones)
         "newvel_dt": (1 + 2 * nd + (1 if adi else 0)) + nd,
     }
     if not adi:
@@ -210,6 +214,8 @@ def oracle_rate(sample, steps, warmup):
     from oracle.binding import Oracle
     o = Oracle(sample.mesh, sample.geometry, sample.eos, sample.params)
     o.set_fields(*sample.fields())
+    if sample.planets:
+        o.set_planets(**sample.planets)
     o.step(warmup)
     t0 = time.perf_counter()
     o.step(steps)
@@ -269,6 +275,8 @@ def run_ours(args):
     tdt = torch.float64 if prec == 64 else torch.float32
     host_in = [None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(tdt).pin_memory() for a in w.fields()]
     g.set_fields(*host_in)
+    if w.planets:
+        g.set_planets(**w.planets)
     K, Wm = args.steps, max(args.warmup, 3)
 
     # ---- region 1: device-resident throughput (graph replay) ----

@@ -15,28 +15,42 @@ constexpr int PFW = 8;   // warps (rings) per block of the force kernel
 
 int planets_blocks(int ny, int nz) { return (ny * nz + PFW - 1) / PFW; }
 
+// One block per row (j, k): what depends on the row only (R, z, the star's term with its division) is formed once per
+// thread, the planets' constants once per planet, and the thread walks the row.
 template <typename T>
-__global__ void k_potential_live(const Dev<T> d, T* __restrict__ phi, const T gm_star, const PlanetsDev* __restrict__ pl,
-                                 const int npl) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-  if (i >= d.TX) return;
+__global__ void __launch_bounds__(128) k_potential_live(const Dev<T> d, T* __restrict__ phi, const T gm_star,
+                                                        const PlanetsDev* __restrict__ pl, const int npl) {
+  const int j = blockIdx.x, k = blockIdx.y;
   T R, z, r;
   if (d.geometry == GEO_SPH) { R = d.yc[j] * d.sin_zc[k]; z = d.yc[j] * d.cos_zc[k]; r = d.yc[j]; }
   else { R = d.yc[j]; z = d.zc[k]; r = rsqrt_ieee(R * R + z * z); }
-  const T x = R * d.cos_xc[i], y = R * d.sin_xc[i];
-  T p = -(gm_star / r);
-  for (int q = 0; q < npl; ++q) {
-    const T ddx = x - (T)pl->x[q][0], ddy = y - (T)pl->x[q][1], ddz = z - (T)pl->x[q][2];
-    const T d2 = ((ddx * ddx + ddy * ddy) + ddz * ddz) + (T)(pl->eps[q] * pl->eps[q]);
-    p = p - (T)pl->gm[q] / rsqrt_ieee(d2);
+  const T star = -(gm_star / r);
+  T* __restrict__ row = phi + d.id(0, j, k);
+  if (npl == 1) {   // the common case: the planet's constants in registers
+    const T xp = (T)pl->x[0][0], yp = (T)pl->x[0][1], ddz = z - (T)pl->x[0][2];
+    const T eps2 = (T)(pl->eps[0] * pl->eps[0]), gm = (T)pl->gm[0];
+    for (int i = threadIdx.x; i < d.TX; i += 128) {
+      const T ddx = R * d.cos_xc[i] - xp, ddy = R * d.sin_xc[i] - yp;
+      const T d2 = ((ddx * ddx + ddy * ddy) + ddz * ddz) + eps2;
+      row[i] = star - rdiv(gm, rsqrt_ieee(d2));
+    }
+    return;
   }
-  phi[d.id(i, j, k)] = p;
+  for (int i = threadIdx.x; i < d.TX; i += 128) {
+    const T x = R * d.cos_xc[i], y = R * d.sin_xc[i];
+    T p = star;
+    for (int q = 0; q < npl; ++q) {
+      const T ddx = x - (T)pl->x[q][0], ddy = y - (T)pl->x[q][1], ddz = z - (T)pl->x[q][2];
+      const T d2 = ((ddx * ddx + ddy * ddy) + ddz * ddz) + (T)(pl->eps[q] * pl->eps[q]);
+      p = p - rdiv((T)pl->gm[q], rsqrt_ieee(d2));
+    }
+    row[i] = p;
+  }
 }
 
 template <typename T>
 int launch_potential_live(const Dev<T>& d, T* phi, T gm_star, const PlanetsDev* pl, int npl, cudaStream_t s) {
-  dim3 b(128), g((d.TX + 127) / 128, d.TY, d.TZ);
-  k_potential_live<T><<<g, b, 0, s>>>(d, phi, gm_star, pl, npl);
+  k_potential_live<T><<<dim3(d.TY, d.TZ), 128, 0, s>>>(d, phi, gm_star, pl, npl);
   return 1;
 }
 
@@ -73,7 +87,8 @@ __global__ void __launch_bounds__(32 * PFW) k_planet_force(const Dev<T> d, const
     const T ddz = z - zp;
     T Fx = T(0), Fy = T(0), Fz = T(0);
     if (live)
-      for (int i = lane; i < d.nx; i += 32) {
+#pragma unroll 4
+      for (int i = lane; i < d.nx; i += 32) {   // unrolled: the square-root and division chains of four cells overlap
         const T x = R * d.cos_xc[d.ngx + i], y = R * d.sin_xc[d.ngx + i];
         const T ddx = x - xp, ddy = y - yp;
         const T d2 = ((ddx * ddx + ddy * ddy) + ddz * ddz) + eps2;

@@ -90,6 +90,7 @@ class Workload:
     vy: Optional[np.ndarray]
     vz: Optional[np.ndarray]
     nsteps: int
+    planets: Optional[dict] = None   # live planets (NEXT-2): keyword arguments of set_planets, or None
 
     def fields(self):
         return self.rho, self.e, self.vx, self.vy, self.vz
@@ -235,6 +236,16 @@ def sheet3d(nx: int = 1024, ny: int = 512, nz: int = 128, nsteps: int = 20) -> W
     vy = 1e-2 * uniform_pm1(3, n).reshape(shape)
     vz = 1e-2 * uniform_pm1(4, n).reshape(shape)
     return Workload("sheet3d_%dx%dx%d" % (nx, ny, nz), mesh, SHEARING_SHEET, ADIABATIC, prm, rho, e, vx, vy, vz, nsteps)
+
+
+def disk3d_live(nphi: int = 1536, nr: int = 512, nth: int = 128, nsteps: int = 100) -> Workload:
+    """NEXT-2 workload (no BASELINE.json config): config 4 with its planet LIVE (section 3.8): same mass, softening and
+    starting point (r, phi) = (1, 0), at rest in the corotating frame, feeling the gas by direct summation."""
+    w = disk3d(nphi, nr, nth, nsteps)
+    w.name = w.name.replace("disk3d", "disk3d_live")
+    w.planets = dict(gm=[w.params.planet_mass], eps=[w.params.planet_eps], pos=[w.params.planet_r, 0.0, 0.0],
+                     vel=[0.0, 0.0, 0.0], force_mode=1, gconst=1.0)
+    return w
 
 
 def noise_box(n: int = 64, nsteps: int = 50, shape3: Optional[tuple] = None) -> Workload:

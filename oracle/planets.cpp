@@ -154,3 +154,29 @@ extern "C" int oracle_gas_force(oracle_ctx* c, int p, double* F) {
   orc_gas_force(*c, p, F);
   return 0;
 }
+
+// ---- cell 5b: change of the frame's rotation rate, Eq. 44 --------------------------------------------
+// v_phi^c = v_phi^b - (Omega_f' - Omega_f) r sin(theta), the geometric factor taken at the centre of the face that
+// carries v_phi, i.e. R_x(j, k) of Tab. 5.  Live planets are carried into the new frame the same way
+// (v' = v - dOmega z^ x x), the fixed-orbit planet keeps its azimuth (its phase is re-based).  The paper does not say
+// how Omega_f' is chosen (reading G33): the caller supplies it between updates.
+extern "C" int oracle_set_omega_frame(oracle_ctx* c, double omega_new) {
+  if (!c || c->midstep) return -1;
+  if (c->geometry == ORC_CARTESIAN) return -1;   // no rotation; constant in the shearing sheet
+  const double dom = omega_new - c->p.omega_frame;
+  for (int k = 0; k < c->TZ; ++k)
+    for (int j = 0; j < c->TY; ++j) {
+      const double corr = dom * c->Rx(j, k);
+      for (int i = 0; i < c->TX; ++i) c->vx[c->id(i, j, k)] = c->vx[c->id(i, j, k)] - corr;
+    }
+  for (int p = 0; p < c->npl; ++p) {
+    const double x = c->pl_x[p][0], y = c->pl_x[p][1];
+    c->pl_v[p][0] = c->pl_v[p][0] + dom * y;
+    c->pl_v[p][1] = c->pl_v[p][1] - dom * x;
+  }
+  // fixed-orbit planet: same azimuth now, new drift rate afterwards
+  const double phip = c->p.planet_phi0 + (c->p.planet_omega - c->p.omega_frame) * c->t;
+  c->p.planet_phi0 = phip - (c->p.planet_omega - omega_new) * c->t;
+  c->p.omega_frame = omega_new;
+  return 0;
+}

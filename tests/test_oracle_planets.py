@@ -200,3 +200,82 @@ def test_one_update_kicks_the_planet_by_dt_times_the_gas_acceleration():
     dv = out[1][1][0] - out[0][1][0]
     assert np.allclose(dv[:2], 1e-3 * F[:2], rtol=2e-3, atol=1e-12) and np.allclose(out[1][2][0], F)
     assert np.max(np.abs(out[0][2])) == 0.0
+
+
+# ---- cell 5b: change of the frame's rotation rate, Eq. 44 ---------------------------------------------
+def test_eq44_leaves_the_inertial_azimuthal_velocity_and_angular_momentum_alone():
+    nphi, nr, nth = 16, 10, 6
+    m = W.Mesh(nphi, nr, nth, -math.pi, math.pi, W.uedges(0.6, 1.8, nr), W.uedges(1.3, 1.8, nth), (PER, REF, REF))
+    om0, om1 = 0.35, 1.15
+    o = Oracle(m, W.SPHERICAL, W.ISOTHERMAL, W.Params(gm_star=1.0, omega_frame=om0))
+    shape = (nth, nr, nphi)
+    rng = np.random.default_rng(4)
+    rho = 1.0 + 0.3 * rng.uniform(-1, 1, shape)
+    vx, vy, vz = (0.2 * rng.uniform(-1, 1, shape) for _ in range(3))
+    o.set_fields(rho, np.full(shape, 0.05), vx, vy, vz)
+    R = (m.yc()[None, :, None] * np.sin(m.zc())[:, None, None]) * np.ones(shape)      # r sin(theta) at the phi face
+    before = vx + om0 * R
+    o.set_omega_frame(om1)
+    r1, _, vx1, vy1, vz1 = o.get_fields()
+    assert np.max(np.abs((vx1 + om1 * R) - before)) < 1e-15 * np.max(np.abs(before))
+    assert np.array_equal(vy1, vy) and np.array_equal(vz1, vz) and np.array_equal(r1, rho)
+    # "trivially conserves angular momentum to machine accuracy": Tab. 2's momentum, face-mean density
+    rf = 0.5 * (rho + np.roll(rho, 1, axis=2))
+    L0, L1 = np.sum(rf * R * before), np.sum(rf * R * (vx1 + om1 * R))
+    assert abs(L1 - L0) < 1e-15 * abs(L0) * 10
+
+
+def test_a_disk_in_balance_stays_in_balance_across_a_change_of_frame():
+    """Keplerian, cold, axisymmetric disk: three updates in the frame om1 reached through Eq. 44 from om0 give the
+    fields of the same disk set up in the frame om1 directly (to rounding: the correction is one subtraction)."""
+    m = _disk_mesh(nphi=24, nr=20)
+    shape = (1, m.ny, m.nx)
+    r = m.yc()[None, :, None] * np.ones(shape)
+    om0, om1 = 0.2, 0.8
+    out = []
+    for start in (om0, om1):
+        o = Oracle(m, W.CYLINDRICAL, W.ISOTHERMAL, W.Params(gm_star=1.0, omega_frame=start, fargo_on=1))
+        o.set_fields(r ** -0.5, 1e-3 * r ** -0.5, r ** -0.5 - start * r, np.zeros(shape), None)
+        if start != om1:
+            o.set_omega_frame(om1)
+        o.step(3)
+        out.append(o.get_fields())
+    for a, b in zip(out[0][:4], out[1][:4]):
+        assert np.max(np.abs(a - b)) < 1e-13 * max(1.0, np.max(np.abs(b)))
+    assert np.max(np.abs(out[0][3][:, 3:-3])) < 2e-3          # and it is a balance up to the O(dr^2) of the 20-cell mesh
+
+
+def test_live_planet_is_carried_into_the_new_frame():
+    rp = 1.25
+    omk = rp ** -1.5
+    _, o = _ctx(om=omk)
+    o.set_planets([1e-30], [0.0], [rp, 0, 0], [0, 0, 0], force_mode=0)       # at rest in its corotating frame
+    for _ in range(50):
+        o.planets_rk5(0.04)
+    om1 = 0.3 * omk
+    o.set_omega_frame(om1)
+    n, h = 200, 0.03
+    for _ in range(n):
+        o.planets_rk5(h)
+    pos, vel, _ = o.get_planets()
+    ang = (omk - om1) * n * h
+    assert abs(pos[0, 0] - rp * math.cos(ang)) < 1e-9 and abs(pos[0, 1] - rp * math.sin(ang)) < 1e-9
+
+
+def test_fixed_orbit_planet_keeps_its_azimuth_when_the_frame_changes():
+    m = _disk_mesh(nphi=32, nr=12)
+    shape = (1, m.ny, m.nx)
+    prm = W.Params(gm_star=1.0, planet_mass=1e-3, planet_r=1.1, planet_phi0=0.3, planet_omega=0.9, planet_eps=0.05,
+                   omega_frame=0.5, dt_fixed=0.01)
+    f = (np.ones(shape), np.full(shape, 0.05), np.zeros(shape), np.zeros(shape), None)
+    a = Oracle(m, W.CYLINDRICAL, W.ISOTHERMAL, prm); a.set_fields(*f); a.step(4)
+    a.run_stage("POT"); phi_before = a.array("phi").copy()
+    b = Oracle(m, W.CYLINDRICAL, W.ISOTHERMAL, prm); b.set_fields(*f); b.step(4)
+    b.set_omega_frame(0.1); b.run_stage("POT")
+    assert np.max(np.abs(b.array("phi") - phi_before)) < 1e-14
+    with pytest.raises(ValueError):
+        Oracle(mesh_cart(), W.CARTESIAN, W.ADIABATIC, W.Params()).set_omega_frame(0.5)
+
+
+def mesh_cart():
+    return W.Mesh(8, 8, 1, 0.0, 1.0, W.uedges(0.0, 1.0, 8), np.array([0.0, 1.0]))

@@ -137,6 +137,13 @@ int fargo_set_planets(fargo_ctx* ctx, int n, const double* gm, const double* eps
  * update (3n each, HOST, any may be NULL).  Returns n (>= 0) or a negative error code. */
 int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc);
 
+/* Cell 5b, Eq. 44: from the next update on the frame rotates at omega_new.  v_phi is corrected by
+ * -(omega_new - omega_frame) R_x(j,k) on every cell (R_x = r or r sin(theta) at the centre of the phi face), which
+ * conserves angular momentum to rounding; live planets are carried into the new frame; the fixed-orbit planet keeps
+ * its azimuth.  Host-initiated, between two fargo_step calls (it synchronises the stream; the paper does not say how
+ * the new rate is chosen: DESIGN.md reading G33).  Cylindrical and spherical meshes only: FARGO_EINVAL otherwise. */
+int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
+
 /* Run the NEXT update up to and including `stage`; the state is then mid-step (only
  * fargo_get_array / fargo_dims / fargo_destroy / fargo_set_fields are valid afterwards). */
 int fargo_step_until(fargo_ctx* c, int stage);

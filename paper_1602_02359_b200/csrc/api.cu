@@ -34,6 +34,7 @@ struct CtxBase {
   virtual void dims(int*, int*, int*, int*, int*, int*) const = 0;
   virtual int set_planets(int, const double*, const double*, const double*, const double*, int, double) = 0;
   virtual int get_planets(double*, double*, double*) = 0;
+  virtual int set_omega_frame(double) = 0;
   virtual int profile(int enable) = 0;
   virtual int profile_report(char* buf, size_t len) = 0;
   long long launches = 0;
@@ -398,6 +399,27 @@ struct Sim : CtxBase {
     return FARGO_OK;
   }
 
+  // cell 5b, Eq. 44: the frame rotates at omega_new from the next update on
+  int set_omega_frame(double omega_new) override {
+    if (d.geometry == GEO_CART) { err = "the frame rate is fixed on Cartesian meshes (P:214) and in the shearing sheet (P:101)"; return FARGO_EINVAL; }
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    double t = 0.0;
+    const int rc = get_time(&t, nullptr, nullptr);   // synchronises the stream
+    if (rc != FARGO_OK) return rc;
+    launches += launch_frame_change<T>(d, st.vx, omega_new - prm.omega_frame, pl, npl, stream);
+    // fixed-orbit planet: same azimuth now, new drift rate afterwards
+    const double phip = prm.planet_phi0 + (prm.planet_omega - prm.omega_frame) * t;
+    prm.planet_phi0 = phip - (prm.planet_omega - omega_new) * t;
+    prm.omega_frame = omega_new;
+    d.omega = (T)omega_new; d.om_eff = (T)omega_new;
+    pot_static = !(L.has_pot && prm.planet_mass != 0.0 && prm.planet_omega != prm.omega_frame);
+    pot_valid = false;
+    if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }   // Omega_f is a kernel argument: capture again
+    if (!ck(cudaGetLastError(), "frame change launch")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
   int get_planets(double* pos, double* vel, double* gas_acc) override {
     PlanetsDev h;
     if (!ck(cudaMemcpyAsync(&h, pl, sizeof h, cudaMemcpyDeviceToHost, stream), "download planets")) return FARGO_ECUDA;
@@ -690,6 +712,7 @@ int fargo_set_planets(fargo_ctx* c, int n, const double* gm, const double* eps, 
 int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
   return c ? c->impl->get_planets(pos, vel, gas_acc) : FARGO_EINVAL;
 }
+int fargo_set_omega_frame(fargo_ctx* c, double omega_new) { return c ? c->impl->set_omega_frame(omega_new) : FARGO_EINVAL; }
 int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }
 int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) {
   if (!c) return FARGO_EINVAL;

@@ -206,8 +206,33 @@ int launch_planets_update(const Dev<T>& d, const T* rho, PlanetsDev* pl, int npl
   return n + 1;
 }
 
+// ---- cell 5b: the frame's rotation rate changes by dom between two updates, Eq. 44 --------------------
+// v_phi -= dom R_x(j, k) on every cell of the allocated array (R_x = r | r sin(theta) at the centre of the phi face,
+// P:312); block (0, 0) also carries the live planets into the new frame: v' = v - dom z^ x x.
+template <typename T>
+__global__ void __launch_bounds__(128) k_frame_change(const Dev<T> d, T* __restrict__ vx, const T dom, PlanetsDev* __restrict__ pl,
+                                                      const int npl, const double dom64) {
+  const int j = blockIdx.x, k = blockIdx.y;
+  const T corr = dom * d.Rx(j, k);
+  T* __restrict__ row = vx + d.id(0, j, k);
+  for (int i = threadIdx.x; i < d.TX; i += 128) row[i] = row[i] - corr;
+  if (j == 0 && k == 0 && (int)threadIdx.x < npl) {
+    const int p = threadIdx.x;
+    const double x = pl->x[p][0], y = pl->x[p][1];
+    pl->v[p][0] = pl->v[p][0] + dom64 * y;
+    pl->v[p][1] = pl->v[p][1] - dom64 * x;
+  }
+}
+
+template <typename T>
+int launch_frame_change(const Dev<T>& d, T* vx, double dom, PlanetsDev* pl, int npl, cudaStream_t s) {
+  k_frame_change<T><<<dim3(d.TY, d.TZ), 128, 0, s>>>(d, vx, (T)dom, pl, npl, dom);
+  return 1;
+}
+
 #define INST(T)                                                                                               \
   template int launch_potential_live<T>(const Dev<T>&, T*, T, const PlanetsDev*, int, cudaStream_t);          \
+  template int launch_frame_change<T>(const Dev<T>&, T*, double, PlanetsDev*, int, cudaStream_t);             \
   template int launch_planets_update<T>(const Dev<T>&, const T*, PlanetsDev*, int, int, double*, double, double, cudaStream_t);
 INST(double)
 INST(float)

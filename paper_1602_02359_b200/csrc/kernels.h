@@ -21,6 +21,8 @@ int planets_blocks(int ny, int nz);
 template <typename T> int launch_potential_live(const Dev<T>& d, T* phi, T gm_star, const PlanetsDev* pl, int npl, cudaStream_t s);
 template <typename T> int launch_planets_update(const Dev<T>& d, const T* rho, PlanetsDev* pl, int npl, int mode, double* part,
                                                 double gm_star, double omega, cudaStream_t s);
+// cell 5b, Eq. 44: vx -= dom R_x(j,k) on the whole array; the live planets follow into the new frame
+template <typename T> int launch_frame_change(const Dev<T>& d, T* vx, double dom, PlanetsDev* pl, int npl, cudaStream_t s);
 // cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
 enum { DT_BOTH = 0, DT_FINISH = 1, DT_CELLS = 2 };   // per-cell max + finish | finish only | per-cell max only
 template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode = DT_BOTH);

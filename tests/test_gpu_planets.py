@@ -108,3 +108,29 @@ def test_set_planets_argument_errors():
     g = Fargo(w.mesh, w.geometry, w.eos, w.params)
     with pytest.raises(RuntimeError):
         g.set_planets([1e-3] * 9, [0.1] * 9, np.zeros(27) + 1.0, np.zeros(27))     # more than FARGO_MAX_PLANETS
+
+
+@pytest.mark.parametrize("live", [False, True], ids=["fixed_orbit_planet", "live_planets"])
+def test_change_of_frame_rate_eq44(live):
+    """Cell 5b: three updates, fargo_set_omega_frame, three more -- fields, clock and planets against the oracle."""
+    w = _lopsided(G.sph3d_iso_fargo(nsteps=3))
+    g, o = _pair(w)
+    for c in (g, o):
+        if live:
+            c.set_planets(PLANETS_2["gm"], PLANETS_2["eps"], PLANETS_2["pos"], PLANETS_2["vel"], force_mode=1)
+        c.step(3)
+        c.set_omega_frame(0.6)
+        c.step(3)
+    assert g.time() == pytest.approx(o.time(), rel=1e-12)
+    for a, b, nm in zip(g.get_fields(), o.get_fields(), ("rho", "e", "vx", "vy", "vz")):
+        assert _rel(a, b) <= 1e-10, nm
+    if live:
+        gp, gv, _ = g.get_planets()
+        op, ov, _ = o.get_planets()
+        assert _rel(gp, op) < 1e-12 and _rel(gv, ov) < 1e-10
+    w2 = G.cart_adi_periodic(nx=16, ny=8, nz=8)
+    from paper_1602_02359_b200 import Fargo
+    gc = Fargo(w2.mesh, w2.geometry, w2.eos, w2.params)
+    gc.set_fields(*w2.fields())
+    with pytest.raises(RuntimeError):
+        gc.set_omega_frame(0.5)

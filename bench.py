@@ -77,6 +77,10 @@ NCU_TRAFFIC_B_PER_CELL = {
     "noise512": {"dt": 41.4, "source": 90.2, "sweep_x": 106.1, "sweep_y": 139.5, "sweep_z": 139.5, "newvel": 79.9},
     "disk3d": {"vmean": 8.5, "dt": 33.0, "source": 77.2, "sweep_x": 95.1, "sweep_y": 127.2, "sweep_z": 127.2,
                "orbital": 118.2, "newvel": 82.6},
+    # profiles/r01h_sheet_visc.md, profiles/r01i_planets.md
+    "disk3dvisc": {"source": 78.9, "source_d": 59.5, "orbital": 118.2},
+    "sheet3d": {"source": 82.3, "orbital": 134.9},
+    "disk3dlive": {"orbital": 118.2, "planets": 8.0, "potential": 7.9},
 }
 
 CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dlive": "4 with a live planet (NEXT-2 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
@@ -324,7 +328,7 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kernels[dom]["frac"],
                 "traffic": (NCU_TRAFFIC_B_PER_CELL.get(args.workload, {}).get(dom) or 0) * ncell * (es / 8) or None,
-                "traffic_source": "ncu --set full, profiles/r01f_fused_source.md (bytes per cell x cells)",
+                "traffic_source": "ncu --set full at this size, profiles/r01f_fused_source.md, r01h_sheet_visc.md, r01i_planets.md (bytes per cell x cells)",
                 "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_cell"] * ncell,
                 "ms_per_launch": kernels[dom]["ms_per_launch"], "share_of_step": kernels[dom]["share"]}

@@ -76,6 +76,7 @@ def lib():
             L.oracle_planets_rk5.argtypes = [vp, C.c_double]
             L.oracle_gas_force.argtypes = [vp, C.c_int, _DP]
             L.oracle_set_omega_frame.argtypes = [vp, C.c_double]
+            L.oracle_diagnostics.argtypes = [vp, _DP]
             L.oracle_vanleer_slopes.argtypes = [C.c_int, _DP, _DP, _DP]
             L.oracle_vanleer_slopes.restype = None
             L.oracle_vanleer_star.argtypes = [C.c_int, _DP, _DP, _DP, _DP, C.c_double, _DP]
@@ -187,6 +188,13 @@ class Oracle:
     def set_omega_frame(self, omega_new: float):
         if lib().oracle_set_omega_frame(self._h, float(omega_new)) != 0:
             raise ValueError("oracle_set_omega_frame failed")
+
+    def diagnostics(self):
+        """(mass, X, Y, Z momentum of Tab. 2, internal energy): sums over the active cells."""
+        out = np.zeros(5)
+        if lib().oracle_diagnostics(self._h, _p(out)) != 0:
+            raise RuntimeError("oracle_diagnostics failed")
+        return out
 
     def planets_rk5(self, h: float):
         if lib().oracle_planets_rk5(self._h, float(h)) != 0:

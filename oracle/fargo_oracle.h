@@ -82,6 +82,9 @@ int oracle_get_planets(oracle_ctx* c, double* pos, double* vel, double* gas_acc)
  * -(omega_new - omega_old) R_x(j,k) on every cell, live planets are carried into the new frame, the fixed-orbit
  * planet keeps its azimuth.  Cylindrical and spherical meshes (not the shearing sheet). */
 int oracle_set_omega_frame(oracle_ctx* c, double omega_new);
+/* Diagnostics (sum reductions): out[5] = mass, X / Y / Z momentum of Tab. 2 (mean of the left and right momenta
+ * per cell; X = angular momentum on curvilinear meshes), internal energy (adiabatic).  Applies the ghost fill of cell 2. */
+int oracle_diagnostics(oracle_ctx* c, double* out);
 int oracle_planets_rk5(oracle_ctx* c, double h);
 int oracle_gas_force(oracle_ctx* c, int p, double* F);
 

@@ -180,3 +180,30 @@ extern "C" int oracle_set_omega_frame(oracle_ctx* c, double omega_new) {
   c->p.omega_frame = omega_new;
   return 0;
 }
+
+// ---- diagnostics: sum reductions over the whole mesh ("mass or angular momentum ... sum") -------------------
+// out[0] = mass sum rho V; out[1..3] = the X, Y, Z momenta of Tab. 2 (X = angular momentum on curvilinear
+// meshes), each cell carrying the mean of its left and right momenta (Eqs. 49-50); out[4] = internal energy sum e V
+// (adiabatic; 0 otherwise).  Active cells, i fastest; the ghost fill of cell 2 is applied first (the upper-face
+// velocities of the last active row and plane live in the ghosts; the next update starts with the same fill).
+extern "C" int oracle_diagnostics(oracle_ctx* c, double* out) {
+  if (!c || !out || c->midstep) return -1;
+  oracle_ctx& o = *c;
+  orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);
+  orc_momenta(o);
+  double m = 0.0, px = 0.0, py = 0.0, pz = 0.0, en = 0.0;
+  for (int k = o.k0(); k < o.k1(); ++k)
+    for (int j = o.j0(); j < o.j1(); ++j) {
+      const double vol = o.Vj[j] * o.syk[k];
+      for (int i = o.i0(); i < o.i1(); ++i) {
+        const size_t l = o.id(i, j, k);
+        m = m + o.rho[l] * vol;
+        if (o.hasx) px = px + (0.5 * (o.pxm[l] + o.pxp[l])) * vol;
+        if (o.hasy) py = py + (0.5 * (o.pym[l] + o.pyp[l])) * vol;
+        if (o.hasz) pz = pz + (0.5 * (o.pzm[l] + o.pzp[l])) * vol;
+        if (o.eos == ORC_ADIABATIC) en = en + o.e[l] * vol;
+      }
+    }
+  out[0] = m; out[1] = px; out[2] = py; out[3] = pz; out[4] = en;
+  return 0;
+}

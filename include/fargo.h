@@ -144,6 +144,13 @@ int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc)
  * the new rate is chosen: DESIGN.md reading G33).  Cylindrical and spherical meshes only: FARGO_EINVAL otherwise. */
 int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
 
+/* Diagnostics, the sum reductions of P:787 ("the mass or angular momentum"): out[5] (HOST) = total mass, the X, Y and Z
+ * momenta of Tab. 2 (per cell the mean of its left and right momenta, Eqs. 49-50; X is the angular
+ * momentum on cylindrical and spherical meshes) and the internal energy (adiabatic; 0 otherwise), summed over the
+ * active cells with the volumes of Tab. 5.  Applies the ghost fill of cell 2 first (the next update starts with the
+ * same fill); synchronises the stream.  Reduced on the device in a fixed-shape tree: reproducible. */
+int fargo_diagnostics(fargo_ctx* ctx, double* out);
+
 /* Run the NEXT update up to and including `stage`; the state is then mid-step (only
  * fargo_get_array / fargo_dims / fargo_destroy / fargo_set_fields are valid afterwards). */
 int fargo_step_until(fargo_ctx* c, int stage);

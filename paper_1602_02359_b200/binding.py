@@ -21,7 +21,7 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
 EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
            "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div",
-           "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame"]
+           "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics"]
 
 
 class FargoMesh(C.Structure):
@@ -77,6 +77,7 @@ def load():
     L.fargo_set_planets.argtypes = [vp, C.c_int, _DP, _DP, _DP, _DP, C.c_int, C.c_double]
     L.fargo_get_planets.argtypes = [vp, _DP, _DP, _DP]
     L.fargo_set_omega_frame.argtypes = [vp, C.c_double]
+    L.fargo_diagnostics.argtypes = [vp, _DP]
     L.fargo_selftest_div.argtypes = [vp, vp, vp, C.c_longlong, vp]
     L.fargo_selftest_div.restype = C.c_int
     L.fargo_last_error.restype = C.c_char_p
@@ -219,6 +220,13 @@ class Fargo:
             self._check(load().fargo_set_planets(self._h, n, *[x.ctypes.data_as(_DP) for x in a], force_mode, float(gconst)),
                         "fargo_set_planets")
         self._npl = n
+
+    def diagnostics(self):
+        """(mass, X, Y, Z momentum of Tab. 2, internal energy): sums over the active cells, reduced on the device."""
+        out = np.zeros(5)
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_diagnostics(self._h, out.ctypes.data_as(_DP)), "fargo_diagnostics")
+        return out
 
     def set_omega_frame(self, omega_new: float):
         with self._torch.cuda.device(self.device):

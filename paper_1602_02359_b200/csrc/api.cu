@@ -35,6 +35,7 @@ struct CtxBase {
   virtual int set_planets(int, const double*, const double*, const double*, const double*, int, double) = 0;
   virtual int get_planets(double*, double*, double*) = 0;
   virtual int set_omega_frame(double) = 0;
+  virtual int diagnostics(double*) = 0;
   virtual int profile(int enable) = 0;
   virtual int profile_report(char* buf, size_t len) = 0;
   long long launches = 0;
@@ -420,6 +421,25 @@ struct Sim : CtxBase {
     return FARGO_OK;
   }
 
+  // sum reductions over the mesh: mass, Tab. 2 momenta, internal energy; applies the ghost fill of cell 2
+  int diagnostics(double* out) override {
+    if (!out) { err = "null argument"; return FARGO_EINVAL; }
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    launches += launch_bc<T>(d, st, field_mask(true, true), stream);
+    launches += launch_diagnostics<T>(d, st, pl_part, stream);
+    const int nblk = planets_blocks(L.ny, L.nz);
+    std::vector<double> h((size_t)nblk * 5);
+    if (!ck(cudaMemcpyAsync(h.data(), pl_part, h.size() * sizeof(double), cudaMemcpyDeviceToHost, stream), "D2H partial sums")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "diagnostics sync")) return FARGO_ECUDA;
+    for (int c = 0; c < 5; ++c) {
+      double s = 0.0;
+      for (int b = 0; b < nblk; ++b) s = s + h[(size_t)b * 5 + c];
+      out[c] = s;
+    }
+    return FARGO_OK;
+  }
+
   int get_planets(double* pos, double* vel, double* gas_acc) override {
     PlanetsDev h;
     if (!ck(cudaMemcpyAsync(&h, pl, sizeof h, cudaMemcpyDeviceToHost, stream), "download planets")) return FARGO_ECUDA;
@@ -713,6 +733,7 @@ int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
   return c ? c->impl->get_planets(pos, vel, gas_acc) : FARGO_EINVAL;
 }
 int fargo_set_omega_frame(fargo_ctx* c, double omega_new) { return c ? c->impl->set_omega_frame(omega_new) : FARGO_EINVAL; }
+int fargo_diagnostics(fargo_ctx* c, double* out) { return c ? c->impl->diagnostics(out) : FARGO_EINVAL; }
 int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }
 int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) {
   if (!c) return FARGO_EINVAL;

@@ -230,9 +230,64 @@ int launch_frame_change(const Dev<T>& d, T* vx, double dom, PlanetsDev* pl, int 
   return 1;
 }
 
+// ---- diagnostics: sum reductions over the active cells ("the mass or angular momentum") -------------------
+// part[block][5] = mass, X / Y / Z momentum of Tab. 2 (mean of the cell's left and right momenta, formed as cell 12a
+// forms them), internal energy (adiabatic).  One warp per ring, warp-shuffle sums, one partial per block of 8 rings;
+// the host adds the partials in block order (fixed shape: reproducible).
+template <typename T>
+__global__ void __launch_bounds__(32 * PFW) k_diagnostics(const Dev<T> d, const State<T> st, double* __restrict__ part) {
+  __shared__ double sh[PFW][5];
+  const int lane = threadIdx.x, w = threadIdx.y;
+  const int row = blockIdx.x * PFW + w;
+  const bool live = row < d.ny * d.nz;
+  const int j = d.ngy + (live ? row % d.ny : 0), k = d.ngz + (live ? row / d.ny : 0);
+  const T vol = d.Vj[j] * d.syk[k];
+  const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), rz = d.Rzj[j];
+  T m = T(0), px = T(0), py = T(0), pz = T(0), en = T(0);
+  if (live)
+    for (int ia = lane; ia < d.nx; ia += 32) {
+      const int i = d.ngx + ia;
+      const long long l = d.id(i, j, k);
+      const T r0 = st.rho[l];
+      m = m + r0 * vol;
+      if (d.hasx) {
+        const T v = st.vx[l];
+        const T vp = (d.xwrap || i + 1 < d.TX) ? st.vx[d.id(d.xw(i + 1), j, k)] : v;
+        px = px + (T(0.5) * (r0 * (rx * v + rx2om) + r0 * (rx * vp + rx2om))) * vol;
+      }
+      if (d.hasy) {
+        const T v = st.vy[l];
+        const T vp = j + 1 < d.TY ? st.vy[l + d.pitch] : v;
+        py = py + (T(0.5) * (r0 * v + r0 * vp)) * vol;
+      }
+      if (d.hasz) {
+        const T v = st.vz[l];
+        const T vp = k + 1 < d.TZ ? st.vz[l + d.plane] : v;
+        pz = pz + (T(0.5) * (r0 * (rz * v) + r0 * (rz * vp))) * vol;
+      }
+      if (d.eos == EOS_ADI) en = en + st.e[l] * vol;
+    }
+  m = warp_sum(m); px = warp_sum(px); py = warp_sum(py); pz = warp_sum(pz); en = warp_sum(en);
+  if (lane == 0) { sh[w][0] = (double)m; sh[w][1] = (double)px; sh[w][2] = (double)py; sh[w][3] = (double)pz; sh[w][4] = (double)en; }
+  __syncthreads();
+  const int t = w * 32 + lane;
+  if (t < 5) {
+    double s = 0.0;
+    for (int q = 0; q < PFW; ++q) s = s + sh[q][t];
+    part[(size_t)blockIdx.x * 5 + t] = s;
+  }
+}
+
+template <typename T>
+int launch_diagnostics(const Dev<T>& d, const State<T>& st, double* part, cudaStream_t s) {
+  k_diagnostics<T><<<planets_blocks(d.ny, d.nz), dim3(32, PFW), 0, s>>>(d, st, part);
+  return 1;
+}
+
 #define INST(T)                                                                                               \
   template int launch_potential_live<T>(const Dev<T>&, T*, T, const PlanetsDev*, int, cudaStream_t);          \
   template int launch_frame_change<T>(const Dev<T>&, T*, double, PlanetsDev*, int, cudaStream_t);             \
+  template int launch_diagnostics<T>(const Dev<T>&, const State<T>&, double*, cudaStream_t);                  \
   template int launch_planets_update<T>(const Dev<T>&, const T*, PlanetsDev*, int, int, double*, double, double, cudaStream_t);
 INST(double)
 INST(float)

@@ -23,6 +23,8 @@ template <typename T> int launch_planets_update(const Dev<T>& d, const T* rho, P
                                                 double gm_star, double omega, cudaStream_t s);
 // cell 5b, Eq. 44: vx -= dom R_x(j,k) on the whole array; the live planets follow into the new frame
 template <typename T> int launch_frame_change(const Dev<T>& d, T* vx, double dom, PlanetsDev* pl, int npl, cudaStream_t s);
+// diagnostics: per-block partial sums of mass, Tab. 2 momenta and internal energy: part[planets_blocks()][5]
+template <typename T> int launch_diagnostics(const Dev<T>& d, const State<T>& st, double* part, cudaStream_t s);
 // cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
 enum { DT_BOTH = 0, DT_FINISH = 1, DT_CELLS = 2 };   // per-cell max + finish | finish only | per-cell max only
 template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode = DT_BOTH);

@@ -111,6 +111,7 @@ struct Sim : CtxBase {
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
   bool fuse_source = false;
+  bool fuse_visc = false;   // 7d in one pass (k_visc3d_fused)
   bool fuse_dt = false;   // Eq. 51 and the next update's per-cell CFL rate in one kernel (k_newvel_dt)
   bool dt_ready = false;  // ctl->m2bits holds the running max for the coming update
   Ctl* ctl = nullptr;
@@ -299,8 +300,8 @@ struct Sim : CtxBase {
     if (L.hasz) { slots[nq++] = 5; slots[nq++] = 6; }
     sweep_setup<T>();
     // with viscosity the fused pass must be followed by the fused 7d (it then also produces the ghost layer 7d reads)
-    fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE") &&
-                  (!L.visc || (L.visc3d && source_d3_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_VISC")));
+    fuse_visc = L.visc3d && source_d3_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_VISC");   // measurement switch
+    fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE") && (!L.visc || fuse_visc);
     fuse_dt = newvel_dt_ok<T>(d) && !getenv("FARGO_UNFUSED_DT");
     return FARGO_OK;
   }
@@ -526,8 +527,7 @@ struct Sim : CtxBase {
       dbg["ed"] = st.e;
       if (until == FARGO_ST_SRC_B || until == FARGO_ST_SRC_C) return n;
       if (L.visc3d) {                                                                  // cell 7d, 3-D (Eqs. B1-B6)
-        static const bool unfused_d = getenv("FARGO_UNFUSED_VISC") != nullptr;   // measurement switch
-        if (until < 0 && !unfused_d && source_d3_fused_ok<T>(d)) {   // one pass, the tensor is never stored
+        if (until < 0 && fuse_visc) {   // one pass, the tensor is never stored
           n += timed("source_d", [&] { return launch_source_d3_fused<T>(d, st.rho, vxc, vyc, vzc, st.vx, st.vy, st.vz, stream); });
         } else {
           T* tens[6] = {set_arr(0, -1), set_arr(0, 0), set_arr(0, 1), set_arr(0, 2), set_arr(0, 3), set_arr(0, 4)};

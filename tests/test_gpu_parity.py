@@ -127,7 +127,8 @@ def test_multi_step(make, use_graph):
     assert g.kernel_launches() > 0
 
 
-FUSED = [G.cart_adi_periodic_even, G.cart_iso_periodic, G.sph3d_iso_fargo, G.cyl3d_adi_fargo, G.sph3d_adi_nofargo]
+FUSED = [G.cart_adi_periodic_even, G.cart_iso_periodic, G.sph3d_iso_fargo, G.cyl3d_adi_fargo, G.sph3d_adi_nofargo,
+         G.sheet3d_adi_fargo]
 
 
 @pytest.mark.parametrize("make", FUSED, ids=[m.__name__ for m in FUSED])
@@ -145,6 +146,34 @@ def test_fused_source_equals_the_kernel_sequence(make, monkeypatch):
     assert g1.kernel_launches() < g2.kernel_launches()      # the fused path really is the one that ran
     for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), g1.get_fields(), g2.get_fields()):
         assert np.array_equal(a, b), _diff_report(name, a, b)
+
+
+VISC_FUSED = [G.cyl3d_visc_fargo, G.sph3d_visc_fargo, G.sheet3d_visc]
+
+
+@pytest.mark.parametrize("make", VISC_FUSED, ids=[m.__name__ for m in VISC_FUSED])
+def test_fused_viscous_step_equals_the_kernel_sequence(make, monkeypatch):
+    """7a-7c in one pass (with the extra ghost layer) followed by 7d in one pass (k_visc3d_fused) against
+    k_source_a -> k_source_b(c) -> k_visc3d_tensor -> k_visc3d_force (FARGO_UNFUSED_VISC, read at fargo_init and at
+    the first update): bit-identical fields."""
+    w = make()
+    g1 = _gpu(w)
+    g1.step(w.nsteps)
+    monkeypatch.setenv("FARGO_UNFUSED_VISC", "1")
+    g2 = _gpu(w)
+    g2.step(w.nsteps)
+    monkeypatch.delenv("FARGO_UNFUSED_VISC")
+    assert g1.time() == g2.time()
+    assert g1.kernel_launches() < g2.kernel_launches()
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), g1.get_fields(), g2.get_fields()):
+        assert np.array_equal(a, b), _diff_report(name, a, b)
+
+
+@pytest.mark.parametrize("make", [G.sheet3d_adi_fargo, G.sph3d_visc_fargo], ids=["sheet3d_adi_fargo", "sph3d_visc_fargo"])
+def test_next1_cases_fp32(make):
+    """fp32 build of the NEXT-1 paths (shearing sheet; fused 7d) against the fp64 oracle: <= 1e-4."""
+    w = make()
+    _run_config(w, w.nsteps, precision=32, tol=TOL32)
 
 
 # ---------------------------------------------------------------- the five configs ---------------------

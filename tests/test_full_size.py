@@ -125,7 +125,7 @@ def sub_workload(w, lo, size):
     return sw, idx, flags
 
 
-def compare_boxes(w, gpu_fields, boxes, nsteps, dt_fixed):
+def compare_boxes(w, gpu_fields, boxes, nsteps, dt_fixed, margin=MARGIN):
     """Advance each sub-box with the oracle (dt_fixed) and compare its interior with the GPU's full-size result."""
     worst = {}
     for lo, size in boxes:
@@ -136,7 +136,7 @@ def compare_boxes(w, gpu_fields, boxes, nsteps, dt_fixed):
         o.step(nsteps)
         fo = o.get_fields()
         o.close()
-        mg = MARGIN * nsteps
+        mg = margin * nsteps
         sl, gi = [], []
         for ax in (2, 1, 0):   # array axes are (z, y, x)
             whole, tl, th = flags[ax]
@@ -162,7 +162,7 @@ def _mass(w, rho):
     """Sum of rho * V over active cells with the closed-form cell volumes (Tab. 5)."""
     m = w.mesh
     ye, ze = np.asarray(m.yedges), np.asarray(m.zedges)
-    if w.geometry == W.CARTESIAN:
+    if w.geometry in (W.CARTESIAN, W.SHEARING_SHEET):
         vj, vk = np.diff(ye), np.diff(ze)
     elif w.geometry == W.CYLINDRICAL:
         vj, vk = 0.5 * np.diff(ye ** 2), np.diff(ze)
@@ -247,3 +247,54 @@ def test_disk3d_three_updates_fixed_dt(disk3d):
     boxes = [((0, 0, 0), (nx, 56, 56)), ((0, 118, 36), (nx, 56, 56))]
     worst = compare_boxes(w, fg, boxes, 3, dt)
     print("disk3d three updates, worst rel per field:", {k: "%.2e" % v for k, v in worst.items()})
+
+
+# ---------------------------------------------------------------- NEXT-1 workloads at the sizes bench.py times -----
+@pytest.fixture(scope="module")
+def sheet3d():
+    return W.sheet3d()
+
+
+def test_sheet3d_one_update_cfl_dt_and_three_with_fixed_dt(sheet3d):
+    """Shearing sheet 1024x512x128 (bench workload sheet3d): dt bit-equal by slabs; fields on whole-row sub-boxes at
+    both walls and in the middle (rows are never cut: orbital advection); mass conserved between the walls."""
+    w = sheet3d
+    dt_o = oracle_dt_by_slabs(w, 8)
+    g = _gpu(w)
+    g.step(1)
+    t, dt_g, ns = g.time()
+    assert ns == 1 and dt_g == dt_o, "dt: gpu %.17g oracle %.17g" % (dt_g, dt_o)
+    fg = g.get_fields()
+    g.close()
+    nx = w.mesh.nx
+    boxes = [((0, 0, 0), (nx, 40, 40)), ((0, 236, 100), (nx, 40, 40)), ((0, 472, 50), (nx, 40, 40))]
+    worst = compare_boxes(w, fg, boxes, 1, dt_o)
+    print("sheet3d one update, worst rel per field:", {k: "%.2e" % v for k, v in worst.items()})
+    dt = 2e-3
+    g = _gpu(w, _copy_params(w.params, dt_fixed=dt))
+    g.step(3)
+    fg = g.get_fields()
+    g.close()
+    m0, m1 = _mass(w, w.rho), _mass(w, fg[0])
+    assert abs(m1 - m0) <= 1e-12 * abs(m0), (m0, m1)
+    worst = compare_boxes(w, fg, [((0, 0, 90), (nx, 56, 56)), ((0, 300, 10), (nx, 56, 56))], 3, dt)
+    print("sheet3d three updates, worst rel per field:", {k: "%.2e" % v for k, v in worst.items()})
+
+
+def test_disk3d_viscous_one_update_cfl_dt(disk3d):
+    """Config 4 with nu = 1e-5 (bench workload disk3dvisc: fused source pass with the extra ghost layer, then 7d in
+    one pass): dt bit-equal (the viscous limit of Eq. 59 is per cell), fields on whole-ring sub-boxes; the viscous
+    stencil adds two cells to the domain of dependence, hence the wider margin."""
+    import dataclasses
+    w = dataclasses.replace(disk3d, params=_copy_params(disk3d.params, nu=1e-5))
+    dt_o = oracle_dt_by_slabs(w, 8)
+    g = _gpu(w)
+    g.step(1)
+    t, dt_g, ns = g.time()
+    assert ns == 1 and dt_g == dt_o, "dt: gpu %.17g oracle %.17g" % (dt_g, dt_o)
+    fg = g.get_fields()
+    g.close()
+    nx = w.mesh.nx
+    boxes = [((0, 0, 0), (nx, 44, 44)), ((0, 126, 42), (nx, 44, 44)), ((0, 468, 84), (nx, 44, 44))]
+    worst = compare_boxes(w, fg, boxes, 1, dt_o, margin=10)
+    print("disk3dvisc one update, worst rel per field:", {k: "%.2e" % v for k, v in worst.items()})

@@ -83,6 +83,18 @@ NCU_TRAFFIC_B_PER_CELL = {
     "disk3dlive": {"orbital": 118.2, "planets": 8.0, "potential": 7.9},
 }
 
+# fp64 pipe utilisation (sm__inst_executed_pipe_fp64, % of peak while active) of the same ncu captures: the second
+# bound of DESIGN.md section 5 -- with contraction off a kernel cannot run the pipe above 2F / (2F + N) (F fp64, N other
+# instructions per cell).  Context for the roofline object, fp64 build only.  None = not captured.
+NCU_FP64_PIPE_PCT = {
+    "noise512": {"dt": 30.8, "source": 46.3, "sweep_x": 61.6, "sweep_y": 42.6, "sweep_z": 42.6, "newvel": 16.4},
+    "disk3d": {"vmean": 11.1, "dt": 33.7, "source": 40.9, "sweep_x": 58.6, "sweep_y": 42.3, "sweep_z": 42.3,
+               "orbital": 68.2, "newvel": 16.0},
+    "disk3dvisc": {"source": 44.7, "source_d": 60.4, "orbital": 68.2},
+    "sheet3d": {"source": 51.1, "orbital": 70.6},
+    "disk3dlive": {"orbital": 68.2, "planets": 49.3, "potential": 68.4},
+}
+
 CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dlive": "4 with a live planet (NEXT-2 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
@@ -330,6 +342,7 @@ def run_ours(args):
                 "traffic": (NCU_TRAFFIC_B_PER_CELL.get(args.workload, {}).get(dom) or 0) * ncell * (es / 8) or None,
                 "traffic_source": "ncu --set full at this size, profiles/r01f_fused_source.md, r01h_sheet_visc.md, r01i_planets.md (bytes per cell x cells)",
                 "peak_source": peak_src,
+                "fp64_pipe_pct_ncu": NCU_FP64_PIPE_PCT.get(args.workload, {}).get(dom) if prec == 64 else None,
                 "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_cell"] * ncell,
                 "ms_per_launch": kernels[dom]["ms_per_launch"], "share_of_step": kernels[dom]["share"]}
     step_gbs = fused_reals * es * ncell / (ms / K * 1e-3) / 1e9

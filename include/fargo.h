@@ -42,7 +42,8 @@ enum { FARGO_CARTESIAN = 0, FARGO_CYLINDRICAL = 1, FARGO_SPHERICAL = 2,
                                         DESIGN.md reading G32): the Cartesian mesh with X along the flow (periodic)
                                         and Y along the shear; needs nx > 1, ny > 1 and a periodic X axis */
 enum { FARGO_ISOTHERMAL = 0, FARGO_ADIABATIC = 1 };                       /* Eqs. 6-7 */
-enum { FARGO_PERIODIC = 0, FARGO_OUTFLOW = 1, FARGO_REFLECTING = 2 };
+enum { FARGO_PERIODIC = 0, FARGO_OUTFLOW = 1, FARGO_REFLECTING = 2,
+       FARGO_EXTERNAL = 3 };   /* Y faces only: the ghosts beyond this face come from a neighbouring slab (below) */
 
 enum { FARGO_OK = 0, FARGO_EINVAL = -1, FARGO_ENOMEM = -2, FARGO_ECUDA = -3, FARGO_ESTATE = -4 };
 
@@ -57,7 +58,9 @@ enum {
 typedef struct fargo_mesh {
   int nx, ny, nz;          /* active cells per direction; 1 = direction absent */
   double xmin, xmax;       /* X is uniform */
-  const double* yedges;    /* HOST, ny+1 active cell edges, or NULL: uniform ymin + j*(ymax-ymin)/ny */
+  const double* yedges;    /* HOST, ny+1 active cell edges, or NULL: uniform ymin + j*(ymax-ymin)/ny.  A slab (a Y face of
+                              kind FARGO_EXTERNAL) must give them, preceded by the 3 edges beyond a cut lower face and
+                              followed by the 3 edges beyond a cut upper face (the neighbouring slab's) */
   const double* zedges;    /* HOST, nz+1 active cell edges, or NULL */
   double ymin, ymax, zmin, zmax;
   int bc[3][2];            /* [direction][lower, upper]; X periodic => ghost-free wrapped X,
@@ -143,6 +146,26 @@ int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc)
  * its azimuth.  Host-initiated, between two fargo_step calls (it synchronises the stream; the paper does not say how
  * the new rate is chosen: DESIGN.md reading G33).  Cylindrical and spherical meshes only: FARGO_EINVAL otherwise. */
 int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
+
+/* Slab decomposition in Y (section 4.1: the mesh is split in Y (and Z), never in X;
+ * 3 ghost layers are exchanged at cells 2 and 9 of Fig. 2; the time step is the minimum over the sub-domains).
+ * A slab is an ordinary context whose mesh holds a range of rows and whose cut Y faces have the kind FARGO_EXTERNAL.
+ * fargo_step is refused on it; one update is, for every slab,
+ *     exchange the state's halos -> fargo_update_phase(0)   cells 2-6: ghost fill of the other faces, v0, Phi, local dt
+ *     all-reduce (min) of *fargo_dt_device_ptr  -> fargo_update_phase(1)   t_stop flag retaken, source step (cell 7)
+ *     exchange the halos of (e, v)          -> fargo_update_phase(2)   cell 9, transport, Eq. 51, clock
+ * fargo_halo(which, side, pack, buf): which = 0 the state (rho, e, vx, vy, vz), 1 = (e, vx, vy, vz) after the source
+ * step; side = 0 lower / 1 upper Y face; pack != 0 copies the 3 ACTIVE rows next to the face into buf, pack == 0 copies
+ * buf into the 3 GHOST rows beyond it.  buf is DEVICE memory of fargo_halo_bytes(which) bytes, caller-owned; what was
+ * packed on the lower side of a slab is unpacked on the upper side of the slab below it, and vice versa (over NCCL,
+ * peer copies, or directly when both slabs live on one device).  Everything is enqueued on the context's stream; no
+ * host synchronisation.  The result is bit-identical to the undivided mesh (tests/test_gpu_slabs.py).  Not with live
+ * planets.  Errors: FARGO_EINVAL, FARGO_ESTATE (phases out of order), FARGO_ECUDA. */
+int fargo_update_phase(fargo_ctx* ctx, int phase);
+size_t fargo_halo_bytes(const fargo_ctx* ctx, int which);
+int fargo_halo(fargo_ctx* ctx, int which, int side, int pack, void* device_buffer);
+/* DEVICE address of the current time step (one double): all-reduce it in place (min) between phases 0 and 1. */
+void* fargo_dt_device_ptr(fargo_ctx* ctx);
 
 /* Diagnostics, the sum reductions of P:787 ("the mass or angular momentum"): out[5] (HOST) = total mass, the X, Y and Z
  * momenta of Tab. 2 (per cell the mean of its left and right momenta, Eqs. 49-50; X is the angular

@@ -21,7 +21,8 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
 EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
            "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div",
-           "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics"]
+           "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics",
+           "fargo_update_phase", "fargo_halo_bytes", "fargo_halo", "fargo_dt_device_ptr"]
 
 
 class FargoMesh(C.Structure):
@@ -78,6 +79,12 @@ def load():
     L.fargo_get_planets.argtypes = [vp, _DP, _DP, _DP]
     L.fargo_set_omega_frame.argtypes = [vp, C.c_double]
     L.fargo_diagnostics.argtypes = [vp, _DP]
+    L.fargo_update_phase.argtypes = [vp, C.c_int]
+    L.fargo_halo_bytes.argtypes = [vp, C.c_int]
+    L.fargo_halo_bytes.restype = C.c_size_t
+    L.fargo_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+    L.fargo_dt_device_ptr.argtypes = [vp]
+    L.fargo_dt_device_ptr.restype = vp
     L.fargo_selftest_div.argtypes = [vp, vp, vp, C.c_longlong, vp]
     L.fargo_selftest_div.restype = C.c_int
     L.fargo_last_error.restype = C.c_char_p
@@ -111,13 +118,17 @@ class Fargo:
         self.dtype = np.float64 if precision == 64 else np.float32
         self.tdtype = torch.float64 if precision == 64 else torch.float32
         self._ye = np.ascontiguousarray(mesh.yedges, dtype=np.float64)
+        ext = getattr(mesh, "yedges_ext", None)
+        if ext is not None:   # a slab: the neighbours' edges beyond the cut faces travel with the active ones
+            self._ye = np.ascontiguousarray(np.concatenate([np.asarray(a, dtype=np.float64) for a in (ext[0], mesh.yedges, ext[1])
+                                                            if a is not None]))
         self._ze = np.ascontiguousarray(mesh.zedges, dtype=np.float64)
         m = FargoMesh()
         m.nx, m.ny, m.nz = mesh.nx, mesh.ny, mesh.nz
         m.xmin, m.xmax = mesh.xmin, mesh.xmax
         m.yedges = self._ye.ctypes.data_as(_DP)
         m.zedges = self._ze.ctypes.data_as(_DP)
-        m.ymin, m.ymax = float(self._ye[0]), float(self._ye[-1])
+        m.ymin, m.ymax = float(mesh.yedges[0]), float(mesh.yedges[-1])
         m.zmin, m.zmax = float(self._ze[0]), float(self._ze[-1])
         for d in range(3):
             for s in range(2):
@@ -209,6 +220,28 @@ class Fargo:
         t, dt, n = C.c_double(), C.c_double(), C.c_longlong()
         self._check(load().fargo_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n)), "fargo_get_time")
         return t.value, dt.value, n.value
+
+    # -- slab decomposition in Y (NEXT-3; driven by slabs.SlabRun) -------------------------------------
+    def update_phase(self, phase: int):
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_update_phase(self._h, phase), "fargo_update_phase")
+
+    def halo_bytes(self, which: int) -> int:
+        return int(load().fargo_halo_bytes(self._h, which))
+
+    def halo(self, which: int, side: int, pack: bool, buf):
+        """buf: a contiguous CUDA uint8 tensor of halo_bytes(which) bytes on this context's device."""
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.halo_bytes(which)
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_halo(self._h, which, side, 1 if pack else 0, buf.data_ptr()), "fargo_halo")
+
+    def dt_tensor(self):
+        """The device-resident time step as a 1-element float64 tensor VIEW (for an in-place all-reduce)."""
+        ptr = load().fargo_dt_device_ptr(self._h)
+
+        class _View:
+            __cuda_array_interface__ = {"shape": (1,), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+        return self._torch.as_tensor(_View(), device=self.device)
 
     # -- live planets (NEXT-2) ------------------------------------------------------------------------
     def set_planets(self, gm, eps, pos, vel, force_mode: int = 1, gconst: float = 1.0):

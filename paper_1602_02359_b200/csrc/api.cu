@@ -32,6 +32,10 @@ struct CtxBase {
   virtual int get_time(double*, double*, long long*) = 0;
   virtual int get_array(const char*, void*) = 0;
   virtual void dims(int*, int*, int*, int*, int*, int*) const = 0;
+  virtual int update_phase(int) = 0;
+  virtual int halo(int, int, int, void*) = 0;
+  virtual size_t halo_bytes(int) const = 0;
+  virtual void* dt_ptr() = 0;
   virtual int set_planets(int, const double*, const double*, const double*, const double*, int, double) = 0;
   virtual int get_planets(double*, double*, double*) = 0;
   virtual int set_omega_frame(double) = 0;
@@ -68,7 +72,11 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   if (p->precision != 64 && p->precision != 32) { err = "precision must be 64 or 32"; return false; }
   for (int dd = 0; dd < 3; ++dd)
     for (int s = 0; s < 2; ++s)
-      if (m->bc[dd][s] < 0 || m->bc[dd][s] > 2) { err = "unknown boundary kind"; return false; }
+      if (m->bc[dd][s] < 0 || m->bc[dd][s] > 3) { err = "unknown boundary kind"; return false; }
+  for (int s = 0; s < 2; ++s)
+    if (m->bc[0][s] == FARGO_EXTERNAL || m->bc[2][s] == FARGO_EXTERNAL || (m->bc[1][s] == FARGO_EXTERNAL && m->ny < 3)) {
+      err = "FARGO_EXTERNAL is for the Y faces of a slab of at least 3 rows (X is never cut, P:728)"; return false;
+    }
   if (!(m->xmax > m->xmin)) { err = "xmax must exceed xmin"; return false; }
   L.nx = m->nx; L.ny = m->ny; L.nz = m->nz;
   L.hasx = m->nx > 1; L.hasy = m->ny > 1; L.hasz = m->nz > 1;
@@ -110,6 +118,8 @@ struct Sim : CtxBase {
   int npl = 0, pl_mode = 0;
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
+  int next_phase = 0;   // slab mode: the phase fargo_update_phase expects next
+  State<T> s2m;         // slab mode: where e and v are after the source step (phase 1 -> phase 2)
   bool fuse_source = false;
   bool fuse_visc = false;   // 7d in one pass (k_visc3d_fused)
   bool fuse_dt = false;   // Eq. 51 and the next update's per-cell CFL rate in one kernel (k_newvel_dt)
@@ -210,7 +220,14 @@ struct Sim : CtxBase {
 
     // ---- host tables (fp64, libm) ----
     const double dx = (m->xmax - m->xmin) / (double)m->nx;
-    std::vector<double> ye = ghosted_edges(m->yedges, L.ny, L.ngy, m->ymin, m->ymax);
+    // a slab's cut faces (FARGO_EXTERNAL) come with the neighbour's true edges: 3 before the active ones when the lower
+    // face is cut, 3 after them when the upper one is (a continuation by the last cell's width would differ from the
+    // undivided mesh, in rounding on a uniform mesh and altogether on a non-uniform one)
+    const int elo = m->bc[1][0] == FARGO_EXTERNAL ? 3 : 0, ehi = m->bc[1][1] == FARGO_EXTERNAL ? 3 : 0;
+    if ((elo || ehi) && !m->yedges) { err = "a slab needs its yedges, with the neighbours' edges beyond the cut faces"; return FARGO_EINVAL; }
+    std::vector<double> ye = ghosted_edges(m->yedges ? m->yedges + elo : nullptr, L.ny, L.ngy, m->ymin, m->ymax);
+    for (int g = 0; g < elo; ++g) ye[g] = m->yedges[g];
+    for (int g = 0; g < ehi; ++g) ye[L.ngy + L.ny + 1 + g] = m->yedges[elo + L.ny + 1 + g];
     std::vector<double> ze = ghosted_edges(m->zedges, L.nz, L.ngz, m->zmin, m->zmax);
     for (size_t n = 1; n < ye.size(); ++n) if (!(ye[n] > ye[n - 1])) { err = "yedges must increase"; return FARGO_EINVAL; }
     for (size_t n = 1; n < ze.size(); ++n) if (!(ze[n] > ze[n - 1])) { err = "zedges must increase"; return FARGO_EINVAL; }
@@ -340,7 +357,7 @@ struct Sim : CtxBase {
     dt_ready = false;
     if (!ck(cudaGetLastError(), "set_fields launch")) return FARGO_ECUDA;
     if (!ck(cudaStreamSynchronize(stream), "set_fields sync")) return FARGO_ECUDA;
-    have_fields = true; midstep = false;
+    have_fields = true; midstep = false; next_phase = 0;
     return FARGO_OK;
   }
 
@@ -376,6 +393,50 @@ struct Sim : CtxBase {
     if (ns) *ns = h.nsteps;
     return FARGO_OK;
   }
+
+  // ---- slab decomposition in Y (NEXT-3; section 4.1) ------------------------------------------------------
+  bool is_slab() const { return d.bc[1][0] == BC_EXTERNAL || d.bc[1][1] == BC_EXTERNAL; }
+
+  int update_phase(int phase) override {
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step (fargo_step_until)"; return FARGO_ESTATE; }
+    if (phase < 0 || phase > 2) { err = "phase must be 0, 1 or 2"; return FARGO_EINVAL; }
+    if (phase != next_phase) { err = "phases run in the order 0, 1, 2"; return FARGO_ESTATE; }
+    if (npl > 0) { err = "live planets are not supported on slabs (the gas force is a sum over the whole mesh)"; return FARGO_EINVAL; }
+    launches += enqueue_update(-1, false, phase);
+    next_phase = (phase + 1) % 3;
+    if (!ck(cudaGetLastError(), "phase launch")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
+  // bytes of one halo message: 3 layers x the full allocated X extent x every plane, per field
+  size_t halo_bytes(int which) const override { return (size_t)(which == 0 ? 5 : 4) * 3 * (size_t)L.pitch * L.TZ * sizeof(T); }
+
+  // which: 0 = the state (rho, e, vx, vy, vz; before phase 0), 1 = (e, vx, vy, vz) after the source step (between
+  // phases 1 and 2).  side: 0 = lower Y face, 1 = upper.  pack: the 3 active rows next to that face -> buf;
+  // unpack: buf -> the 3 ghost rows beyond it.  Strided device-to-device copies on the context's stream.
+  int halo(int which, int side, int pack, void* buf) override {
+    if (!buf || which < 0 || which > 1 || side < 0 || side > 1) { err = "bad halo argument"; return FARGO_EINVAL; }
+    if (!L.hasy) { err = "no Y direction"; return FARGO_EINVAL; }
+    if (which == 1 && next_phase != 2) { err = "the source-step halo exists between phases 1 and 2"; return FARGO_ESTATE; }
+    const State<T>& a = which == 0 ? st : s2m;
+    T* f[5] = {a.rho, a.e, a.vx, a.vy, a.vz};
+    const int first = which == 0 ? 0 : 1;
+    const int j = pack ? (side == 0 ? L.ngy : L.ngy + L.ny - 3) : (side == 0 ? 0 : L.ngy + L.ny);
+    const size_t row3 = 3 * (size_t)L.pitch * sizeof(T), per_field = row3 * L.TZ;
+    unsigned char* b = (unsigned char*)buf;
+    for (int q = first; q < 5; ++q) {
+      if (!f[q]) continue;
+      unsigned char* field = (unsigned char*)(f[q] + (size_t)j * L.pitch);
+      unsigned char* msg = b + (size_t)(q - first) * per_field;
+      const cudaError_t e = pack ? cudaMemcpy2DAsync(msg, row3, field, (size_t)L.plane * sizeof(T), row3, L.TZ, cudaMemcpyDeviceToDevice, stream)
+                                 : cudaMemcpy2DAsync(field, (size_t)L.plane * sizeof(T), msg, row3, row3, L.TZ, cudaMemcpyDeviceToDevice, stream);
+      if (!ck(e, "halo copy")) return FARGO_ECUDA;
+    }
+    return FARGO_OK;
+  }
+
+  void* dt_ptr() override { return &ctl->dt; }
 
   // ---- live planets (NEXT-2) ---------------------------------------------------------------------------
   int set_planets(int n, const double* gm, const double* eps, const double* pos, const double* vel, int mode, double gconst) override {
@@ -472,8 +533,15 @@ struct Sim : CtxBase {
   }
 
   // Enqueue the kernels of one update up to and including `until` (-1 = all).  Returns the launch count.
-  int enqueue_update(int until, bool capturing) {
+  // `phase` (slab decomposition, NEXT-3): -1 = the whole update; 0 = cells 2-6 (ghost fill of the non-external faces,
+  // v0, potential, local dt); 1 = the dt fix-up after the all-reduce and the source step; 2 = cell 9 and the transport
+  // step.  The caller exchanges the Y halos of the state before phase 0 and those of (e, v) between phases 1 and 2.
+  int enqueue_update(int until, bool capturing, int phase = -1) {
     int n = 0;
+    const T* v0p = L.fargo ? v0 : nullptr;
+    State<T> s2 = st;   // the state the transport step reads: e and v after the source step
+    if (phase == 2) { s2 = s2m; goto cell9; }
+    if (phase == 1) { n += launch_dt_sync(ctl, prm.t_stop, sizeof(T) == 4, stream); goto cell7; }
     dbg.clear();
     dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
     dbg["phi"] = phi; dbg["v0"] = v0;
@@ -490,7 +558,6 @@ struct Sim : CtxBase {
       pot_valid = true;
     }
     if (until == FARGO_ST_POT) return n;
-    const T* v0p = L.fargo ? v0 : nullptr;
     {                                                                                // cell 6
       const int mode = (fuse_dt && dt_ready) ? DT_FINISH : DT_BOTH;
       n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream, mode); });
@@ -499,7 +566,8 @@ struct Sim : CtxBase {
     if (until == FARGO_ST_DT) return n;
     if (npl > 0)                                                                      // cell 5a (reading G33)
       n += timed("planets", [&] { return launch_planets_update<T>(d, st.rho, pl, npl, pl_mode, pl_part, prm.gm_star, prm.omega_frame, stream); });
-    State<T> s2 = st;   // the state the transport step reads: e and v after the source step
+    if (phase == 0) return n;
+  cell7:
     if (fuse_source && until < 0) {
       // cells 7a-7c in one pass; it reads neighbours of the state, so its output goes to arrays of its own
       if (L.adi) s2.e = alt[0];
@@ -509,7 +577,6 @@ struct Sim : CtxBase {
         n += timed("source_d", [&] { return launch_source_d3_fused<T>(d, st.rho, s2.vx, s2.vy, s2.vz, st.vx, st.vy, st.vz, stream); });
         s2.vx = st.vx; s2.vy = st.vy; s2.vz = st.vz;
       }
-      n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                    // cell 9
     } else {
     // source step: intermediates live in transport set B (idle until the second pass)
       T *vxb = set_arr(1, 0), *vyb = set_arr(1, 1), *vzb = set_arr(1, 2), *ec = set_arr(1, 3);
@@ -539,9 +606,11 @@ struct Sim : CtxBase {
       dbg["vxd"] = st.vx; dbg["vyd"] = st.vy; dbg["vzd"] = st.vz;
       dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
       if (until == FARGO_ST_SRC_D) return n;
-      n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(false, L.adi), stream); });                      // cell 9
-      if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
     }
+    if (phase == 1) { s2m = s2; return n; }
+  cell9:
+    n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                      // cell 9
+    if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
     // transport: pass p reads set (p-1)%2 (the state on the first pass) and writes set p%2; the last pass
     // writes rho and e straight back into the state arrays, so one update leaves every array where it
     // started and the same captured graph serves every update.
@@ -602,6 +671,8 @@ struct Sim : CtxBase {
     if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
     if (midstep) { err = "context is mid-step (fargo_step_until)"; return FARGO_ESTATE; }
     if (nsteps < 0) { err = "negative step count"; return FARGO_EINVAL; }
+    if (is_slab() && nsteps > 0) { err = "a slab advances through fargo_update_phase (its Y halos come from its neighbours)"; return FARGO_ESTATE; }
+    if (next_phase != 0) { err = "an update is in progress (fargo_update_phase)"; return FARGO_ESTATE; }
     if (nsteps == 0) return FARGO_OK;
     // the legacy default stream cannot be captured: plain launches there
     const bool graph_ok = prm.use_graph && (pot_static || npl > 0) && stream != nullptr && !prof;
@@ -734,6 +805,12 @@ int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
 }
 int fargo_set_omega_frame(fargo_ctx* c, double omega_new) { return c ? c->impl->set_omega_frame(omega_new) : FARGO_EINVAL; }
 int fargo_diagnostics(fargo_ctx* c, double* out) { return c ? c->impl->diagnostics(out) : FARGO_EINVAL; }
+int fargo_update_phase(fargo_ctx* c, int phase) { return c ? c->impl->update_phase(phase) : FARGO_EINVAL; }
+size_t fargo_halo_bytes(const fargo_ctx* c, int which) { return c ? c->impl->halo_bytes(which) : 0; }
+int fargo_halo(fargo_ctx* c, int which, int side, int pack, void* device_buffer) {
+  return c ? c->impl->halo(which, side, pack, device_buffer) : FARGO_EINVAL;
+}
+void* fargo_dt_device_ptr(fargo_ctx* c) { return c ? c->impl->dt_ptr() : nullptr; }
 int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }
 int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) {
   if (!c) return FARGO_EINVAL;

@@ -31,10 +31,10 @@ __global__ void k_bc(const Dev<T> d, const State<T> st, const int mask) {
     for (int g = 0; g < ng; ++g) {
       if (lo == BC_PERIODIC) a[(m0 - 1 - g) * str] = a[(m1 - 1 - g) * str];
       else if (lo == BC_OUTFLOW) a[(m0 - 1 - g) * str] = a[m0 * str];
-      else if (!normal) a[(m0 - 1 - g) * str] = a[(m0 + g) * str];
+      else if (lo == BC_REFLECTING && !normal) a[(m0 - 1 - g) * str] = a[(m0 + g) * str];   // BC_EXTERNAL: left alone
       if (hi == BC_PERIODIC) a[(m1 + g) * str] = a[(m0 + g) * str];
       else if (hi == BC_OUTFLOW) a[(m1 + g) * str] = a[(m1 - 1) * str];
-      else if (!normal) a[(m1 + g) * str] = a[(m1 - 1 - g) * str];
+      else if (hi == BC_REFLECTING && !normal) a[(m1 + g) * str] = a[(m1 - 1 - g) * str];
     }
     if (normal && lo == BC_REFLECTING) {  // wall face at rest, velocity antisymmetric about it
       a[m0 * str] = T(0);

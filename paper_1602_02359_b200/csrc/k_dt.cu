@@ -206,7 +206,8 @@ __global__ void __launch_bounds__(1024) k_dt_finish(const Dev<T> d, const T* __r
   if (c->done) return;
   T s = T(0);
   if (d.fargo) {
-    const int nyp = d.ny - 1;
+    // pairs of radially neighbouring rings, both active; a slab also owns the pair across its upper (external) face
+    const int nyp = d.ny - 1 + (d.bc[1][1] == BC_EXTERNAL ? 1 : 0);
     const int n = nyp > 0 ? nyp * d.nz : 0;
     for (int r = threadIdx.x; r < n; r += blockDim.x) {
       const int j = d.ngy + r % nyp, k = d.ngz + r / nyp;
@@ -260,6 +261,18 @@ __global__ void k_advance(Ctl* c, const double t_stop) {
   c->t = c->clipped ? t_stop : c->t + c->dt;
   c->nsteps += 1;
   if (t_stop > 0.0 && c->t >= t_stop) c->done = 1;
+}
+// Slab decomposition (NEXT-3): ctl->dt now holds the minimum over the slabs of their local time steps (all-reduced in
+// place by the caller).  Each slab clipped its own dt to t_stop; the minimum is the right step (a clipped value is
+// never below an unclipped one that ends before t_stop), only the `clipped` flag has to be taken again.
+__global__ void k_dt_sync(Ctl* c, const double t_stop, const int single) {
+  if (c->done) return;
+  const double rest = single ? (double)(float)(t_stop - c->t) : t_stop - c->t;
+  c->clipped = (t_stop > 0.0 && (c->t + c->dt >= t_stop || c->dt == rest)) ? 1 : 0;
+}
+int launch_dt_sync(Ctl* ctl, double t_stop, bool single, cudaStream_t s) {
+  k_dt_sync<<<1, 1, 0, s>>>(ctl, t_stop, single ? 1 : 0);
+  return 1;
 }
 int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s) {
   k_advance<<<1, 1, 0, s>>>(ctl, t_stop);

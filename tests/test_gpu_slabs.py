@@ -1,0 +1,75 @@
+"""Slab decomposition in Y (section 4.1) on ONE GPU: N contexts, each a slab of rows
+with FARGO_EXTERNAL cut faces, advanced through fargo_update_phase with their halos passed buffer to buffer, against
+the undivided mesh.  The paper's "indiscernibility" criterion (3 ghost layers make the cut invisible) is here
+exact: every field and the clock must agree BIT for bit with the single-context run (which the other tests hold to
+the oracle).  The NCCL transport of slabs.py shares everything but the message routing, which tests/test_slabs_host.py
+covers with gloo on CPU."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import gpu_cases as G
+from paper_1602_02359_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+CASES = [(G.cart_adi_periodic_even, 2), (G.cart_adi_periodic_even, 3), (G.sph3d_iso_fargo, 2), (G.sph3d_iso_fargo, 3),
+         (G.cyl3d_visc_fargo, 2), (G.cart_adi_mixed_bc, 3), (G.cyl2d_iso_fargo_visc, 4), (G.sheet3d_adi_fargo, 3),
+         (G.nonuniform_cyl2d, 2)]
+
+
+def _single(w, params=None):
+    from paper_1602_02359_b200 import Fargo
+    g = Fargo(w.mesh, w.geometry, w.eos, params or w.params)
+    g.set_fields(*w.fields())
+    return g
+
+
+@pytest.mark.parametrize("make,nslabs", CASES, ids=["%s-%d" % (m.__name__, n) for m, n in CASES])
+def test_slabs_equal_the_undivided_mesh(make, nslabs):
+    from paper_1602_02359_b200.slabs import SlabRun
+    w = make()
+    g = _single(w)
+    g.step(w.nsteps)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, nslabs=nslabs)
+    s.set_fields(*w.fields())
+    s.step(w.nsteps)
+    s.synchronize()
+    assert s.time() == g.time()
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), s.get_fields(), g.get_fields()):
+        assert (a is None) == (b is None)
+        if a is not None:
+            assert np.array_equal(a, b), "%s: %d cells differ, max %.3e" % (name, int((a != b).sum()), float(np.max(np.abs(a - b))))
+    s.close()
+
+
+def test_t_stop_is_reached_together():
+    """Each slab clips its own dt; the minimum decides and the flag is retaken after the all-reduce."""
+    from paper_1602_02359_b200.slabs import SlabRun
+    w = G.cart_adi_periodic_even(nx=66, ny=12, nz=10)
+    g0 = _single(w)
+    g0.step(3)
+    prm = dataclasses.replace(w.params, t_stop=0.93 * g0.time()[0])          # lands inside the third update
+    g = _single(w, prm)
+    g.step(6)
+    s = SlabRun(w.mesh, w.geometry, w.eos, prm, nslabs=3)
+    s.set_fields(*w.fields())
+    s.step(6)
+    s.synchronize()
+    assert s.time() == g.time() and g.time()[0] == prm.t_stop and g.time()[2] == 3
+    for a, b in zip(s.get_fields(), g.get_fields()):
+        assert np.array_equal(a, b)
+
+
+def test_a_slab_refuses_fargo_step_and_out_of_order_phases():
+    from paper_1602_02359_b200.slabs import SlabRun
+    w = G.cart_adi_periodic_even(nx=66, ny=12, nz=10)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, nslabs=2)
+    s.set_fields(*w.fields())
+    with pytest.raises(RuntimeError):
+        s.ctx[0].step(1)
+    with pytest.raises(RuntimeError):
+        s.ctx[0].update_phase(1)
+    s.step(1)
+    s.synchronize()

@@ -404,6 +404,73 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_local_slabs(args):
+    """Cost of the Y-slab decomposition on ONE device: the same workload as N slabs, halos
+    passed buffer to buffer, dt reduced over the slabs, plain launches (no graph), against nothing but itself --
+    compare with the default line of the same workload.  Device-resident, CUDA events on the slabs' stream."""
+    import torch
+    from paper_1602_02359_b200.slabs import SlabRun
+    torch.cuda.set_device(0)
+    w, _, _ = make_workload(args.workload)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, nslabs=args.local_slabs, precision=32 if args.fp32 else 64)
+    s.set_fields(*w.fields())
+    K, Wm = args.steps, max(args.warmup, 3)
+    s.step(Wm)
+    s.synchronize()
+    l0 = sum(c.kernel_launches() for c in s.ctx.values())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    s.step(K)
+    e1.record(s.stream)
+    s.synchronize()
+    ms = e0.elapsed_time(e1)
+    halo = sum(2 * (c.halo_bytes(0) + c.halo_bytes(1)) * len([p for p in (c.mesh_bc_y) if p == 3]) for c in s.ctx.values())
+    print(json.dumps({
+        "metric": METRIC, "value": w.mesh.ncells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": Wm,
+        "ms_per_step": ms / K, "higher_is_better": True, "dtype": "f32" if args.fp32 else "f64", "data": "synthetic",
+        "config": {"workload": w.name, "local_slabs": args.local_slabs, "rows": [list(r) for r in s.rows.values()],
+                   "launch": "plain launches, three phases per update and slab, halos device to device on one stream",
+                   "halo_bytes_copied_per_update": halo},
+        "gpu_launches": sum(c.kernel_launches() for c in s.ctx.values()) - l0}))
+
+
+def run_dist_slabs(args):
+    """NEXT-3 over torch.distributed (NCCL): ONE mesh split into one Y-slab per rank, halos by batch_isend_irecv, dt by
+    all_reduce(MIN) on the device.  Strong scaling (the total work is fixed).  Opt-in (--slabs): the contract line stays
+    the replica run, because this box has one GPU and the NCCL transport has only been run at world size 1 on it
+    (the routing itself is covered by the gloo tests at world size 2 and 3)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1602_02359_b200.slabs import SlabRun
+    rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29517")
+    os.environ.setdefault("RANK", "0"); os.environ.setdefault("WORLD_SIZE", "1")
+    torch.cuda.set_device(local)
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    w, _, _ = make_workload(args.workload)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, group=dist.group.WORLD, precision=32 if args.fp32 else 64)
+    s.set_fields(*w.fields())
+    K, Wm = args.steps, max(args.warmup, 3)
+    s.step(Wm)
+    s.synchronize()
+    rank_barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    s.step(K)
+    e1.record(s.stream)
+    s.synchronize()
+    rank_barrier(world)
+    ms = rank_max(e0.elapsed_time(e1), world, "cuda")
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": w.mesh.ncells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong",
+            "dtype": "f32" if args.fp32 else "f64", "data": "synthetic",
+            "config": {"workload": w.name, "parallelism": "%d Y-slabs, one per GPU, NCCL halos + all_reduce(MIN) of dt" % world,
+                       "rows_of_rank0": list(s.rows[0])}}))
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -415,9 +482,19 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer region (short runs under ncu)")
+    ap.add_argument("--slabs", action="store_true",
+                    help="NEXT-3, under torchrun: one mesh split into one Y-slab per rank over NCCL (strong scaling) "
+                         "instead of independent replicas")
+    ap.add_argument("--local-slabs", type=int, default=0,
+                    help="NEXT-3: advance the workload as N Y-slabs on THIS GPU (slabs.SlabRun, local transport) and "
+                         "print what the decomposition costs on one device; not the contract line")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.local_slabs > 0:
+        run_local_slabs(args)
+    elif args.slabs:
+        run_dist_slabs(args)
     else:
         run_ours(args)
 

@@ -158,6 +158,7 @@ class Fargo:
             rc = L.fargo_init(C.byref(self._h), C.byref(m), geometry, eos, C.byref(p))
         if rc != 0:
             raise RuntimeError("fargo_init failed (%d): %s" % (rc, L.fargo_last_error(None).decode()))
+        self.mesh_bc_y = tuple(mesh.bc[1])
         self.shape = (mesh.nz, mesh.ny, mesh.nx)
         self.ncells = mesh.nx * mesh.ny * mesh.nz
         self.hasy, self.hasz = mesh.ny > 1, mesh.nz > 1

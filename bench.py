@@ -424,7 +424,7 @@ def run_local_slabs(args):
     e1.record(s.stream)
     s.synchronize()
     ms = e0.elapsed_time(e1)
-    halo = sum(2 * (c.halo_bytes(0) + c.halo_bytes(1)) * len([p for p in (c.mesh_bc_y) if p == 3]) for c in s.ctx.values())
+    halo = sum(2 * (c.halo_bytes(0, 1) + c.halo_bytes(1, 1)) * len([p for p in (c.mesh_bc_y) if p == 3]) for c in s.ctx.values())
     print(json.dumps({
         "metric": METRIC, "value": w.mesh.ncells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": Wm,
         "ms_per_step": ms / K, "higher_is_better": True, "dtype": "f32" if args.fp32 else "f64", "data": "synthetic",

@@ -43,7 +43,7 @@ enum { FARGO_CARTESIAN = 0, FARGO_CYLINDRICAL = 1, FARGO_SPHERICAL = 2,
                                         and Y along the shear; needs nx > 1, ny > 1 and a periodic X axis */
 enum { FARGO_ISOTHERMAL = 0, FARGO_ADIABATIC = 1 };                       /* Eqs. 6-7 */
 enum { FARGO_PERIODIC = 0, FARGO_OUTFLOW = 1, FARGO_REFLECTING = 2,
-       FARGO_EXTERNAL = 3 };   /* Y faces only: the ghosts beyond this face come from a neighbouring slab (below) */
+       FARGO_EXTERNAL = 3 };   /* Y and Z faces: the ghosts beyond this face come from a neighbouring sub-domain (below) */
 
 enum { FARGO_OK = 0, FARGO_EINVAL = -1, FARGO_ENOMEM = -2, FARGO_ECUDA = -3, FARGO_ESTATE = -4 };
 
@@ -61,7 +61,7 @@ typedef struct fargo_mesh {
   const double* yedges;    /* HOST, ny+1 active cell edges, or NULL: uniform ymin + j*(ymax-ymin)/ny.  A slab (a Y face of
                               kind FARGO_EXTERNAL) must give them, preceded by the 3 edges beyond a cut lower face and
                               followed by the 3 edges beyond a cut upper face (the neighbouring slab's) */
-  const double* zedges;    /* HOST, nz+1 active cell edges, or NULL */
+  const double* zedges;    /* HOST, nz+1 active cell edges, or NULL (cut Z faces: as for yedges) */
   double ymin, ymax, zmin, zmax;
   int bc[3][2];            /* [direction][lower, upper]; X periodic => ghost-free wrapped X,
                               X non-periodic => 3 ghost layers in X too (reading G20) */
@@ -147,23 +147,28 @@ int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc)
  * the new rate is chosen: DESIGN.md reading G33).  Cylindrical and spherical meshes only: FARGO_EINVAL otherwise. */
 int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
 
-/* Slab decomposition in Y (section 4.1: the mesh is split in Y (and Z), never in X;
- * 3 ghost layers are exchanged at cells 2 and 9 of Fig. 2; the time step is the minimum over the sub-domains).
- * A slab is an ordinary context whose mesh holds a range of rows and whose cut Y faces have the kind FARGO_EXTERNAL.
- * fargo_step is refused on it; one update is, for every slab,
- *     exchange the state's halos -> fargo_update_phase(0)   cells 2-6: ghost fill of the other faces, v0, Phi, local dt
- *     all-reduce (min) of *fargo_dt_device_ptr  -> fargo_update_phase(1)   t_stop flag retaken, source step (cell 7)
- *     exchange the halos of (e, v)          -> fargo_update_phase(2)   cell 9, transport, Eq. 51, clock
- * fargo_halo(which, side, pack, buf): which = 0 the state (rho, e, vx, vy, vz), 1 = (e, vx, vy, vz) after the source
- * step; side = 0 lower / 1 upper Y face; pack != 0 copies the 3 ACTIVE rows next to the face into buf, pack == 0 copies
- * buf into the 3 GHOST rows beyond it.  buf is DEVICE memory of fargo_halo_bytes(which) bytes, caller-owned; what was
- * packed on the lower side of a slab is unpacked on the upper side of the slab below it, and vice versa (over NCCL,
- * peer copies, or directly when both slabs live on one device).  Everything is enqueued on the context's stream; no
- * host synchronisation.  The result is bit-identical to the undivided mesh (tests/test_gpu_slabs.py).  Not with live
- * planets.  Errors: FARGO_EINVAL, FARGO_ESTATE (phases out of order), FARGO_ECUDA. */
+/* Domain decomposition in Y and Z (section 4.1: the mesh is split in Y and Z, never
+ * in X; 3 ghost layers are exchanged at cells 2 and 9 of Fig. 2; the time step is the minimum over the sub-domains,
+ * P:407).  A sub-domain is an ordinary context whose mesh holds a range of rows / planes and whose cut faces have the
+ * kind FARGO_EXTERNAL (with the neighbours' edges in yedges / zedges, see fargo_mesh).  fargo_step is refused on it;
+ * one update is, on every sub-domain,
+ *     exchange Y halos of the state -> fargo_update_phase(0)  cell 2: ghost fill of the faces that are not cut
+ *     exchange Z halos of the state -> fargo_update_phase(1)  cells 3-6: v0, Phi, local dt
+ *     all-reduce (min) of *fargo_dt_device_ptr -> fargo_update_phase(2)  t_stop flag retaken, source step (cell 7)
+ *     exchange Y halos of (e, v)    -> fargo_update_phase(3)  cell 9
+ *     exchange Z halos of (e, v)    -> fargo_update_phase(4)  transport, Eq. 51, clock
+ * (Y before the fill and Z after it: the Z planes sent carry the Y ghosts, which is how the edges and corners travel.)
+ * fargo_halo(which, dir, side, pack, buf): which = 0 the state (rho, e, vx, vy, vz), 1 = (e, vx, vy, vz) after the
+ * source step; dir = 1 (Y, rows) or 2 (Z, planes); side = 0 lower / 1 upper face; pack != 0 copies the 3 ACTIVE layers
+ * next to the face into buf, pack == 0 copies buf into the 3 GHOST layers beyond it.  buf is DEVICE memory of
+ * fargo_halo_bytes(which, dir) bytes, caller-owned; what was packed on the lower side of a sub-domain is unpacked on the
+ * upper side of the one below it, and vice versa (over NCCL, peer copies, or directly when both live on one device).
+ * Everything is enqueued on the context's stream; no host synchronisation.  The result is bit-identical to the
+ * undivided mesh (tests/test_gpu_slabs.py).  Not with live planets.  Errors: FARGO_EINVAL, FARGO_ESTATE (phases out of
+ * order), FARGO_ECUDA. */
 int fargo_update_phase(fargo_ctx* ctx, int phase);
-size_t fargo_halo_bytes(const fargo_ctx* ctx, int which);
-int fargo_halo(fargo_ctx* ctx, int which, int side, int pack, void* device_buffer);
+size_t fargo_halo_bytes(const fargo_ctx* ctx, int which, int dir);
+int fargo_halo(fargo_ctx* ctx, int which, int dir, int side, int pack, void* device_buffer);
 /* DEVICE address of the current time step (one double): all-reduce it in place (min) between phases 0 and 1. */
 void* fargo_dt_device_ptr(fargo_ctx* ctx);
 

@@ -80,9 +80,9 @@ def load():
     L.fargo_set_omega_frame.argtypes = [vp, C.c_double]
     L.fargo_diagnostics.argtypes = [vp, _DP]
     L.fargo_update_phase.argtypes = [vp, C.c_int]
-    L.fargo_halo_bytes.argtypes = [vp, C.c_int]
+    L.fargo_halo_bytes.argtypes = [vp, C.c_int, C.c_int]
     L.fargo_halo_bytes.restype = C.c_size_t
-    L.fargo_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+    L.fargo_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]
     L.fargo_dt_device_ptr.argtypes = [vp]
     L.fargo_dt_device_ptr.restype = vp
     L.fargo_selftest_div.argtypes = [vp, vp, vp, C.c_longlong, vp]
@@ -123,13 +123,17 @@ class Fargo:
             self._ye = np.ascontiguousarray(np.concatenate([np.asarray(a, dtype=np.float64) for a in (ext[0], mesh.yedges, ext[1])
                                                             if a is not None]))
         self._ze = np.ascontiguousarray(mesh.zedges, dtype=np.float64)
+        zext = getattr(mesh, "zedges_ext", None)
+        if zext is not None:
+            self._ze = np.ascontiguousarray(np.concatenate([np.asarray(a, dtype=np.float64) for a in (zext[0], mesh.zedges, zext[1])
+                                                            if a is not None]))
         m = FargoMesh()
         m.nx, m.ny, m.nz = mesh.nx, mesh.ny, mesh.nz
         m.xmin, m.xmax = mesh.xmin, mesh.xmax
         m.yedges = self._ye.ctypes.data_as(_DP)
         m.zedges = self._ze.ctypes.data_as(_DP)
         m.ymin, m.ymax = float(mesh.yedges[0]), float(mesh.yedges[-1])
-        m.zmin, m.zmax = float(self._ze[0]), float(self._ze[-1])
+        m.zmin, m.zmax = float(mesh.zedges[0]), float(mesh.zedges[-1])
         for d in range(3):
             for s in range(2):
                 m.bc[d][s] = mesh.bc[d][s]
@@ -158,7 +162,7 @@ class Fargo:
             rc = L.fargo_init(C.byref(self._h), C.byref(m), geometry, eos, C.byref(p))
         if rc != 0:
             raise RuntimeError("fargo_init failed (%d): %s" % (rc, L.fargo_last_error(None).decode()))
-        self.mesh_bc_y = tuple(mesh.bc[1])
+        self.mesh_bc_y, self.mesh_bc_z = tuple(mesh.bc[1]), tuple(mesh.bc[2])
         self.shape = (mesh.nz, mesh.ny, mesh.nx)
         self.ncells = mesh.nx * mesh.ny * mesh.nz
         self.hasy, self.hasz = mesh.ny > 1, mesh.nz > 1
@@ -227,14 +231,14 @@ class Fargo:
         with self._torch.cuda.device(self.device):
             self._check(load().fargo_update_phase(self._h, phase), "fargo_update_phase")
 
-    def halo_bytes(self, which: int) -> int:
-        return int(load().fargo_halo_bytes(self._h, which))
+    def halo_bytes(self, which: int, direction: int = 1) -> int:
+        return int(load().fargo_halo_bytes(self._h, which, direction))
 
-    def halo(self, which: int, side: int, pack: bool, buf):
-        """buf: a contiguous CUDA uint8 tensor of halo_bytes(which) bytes on this context's device."""
-        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.halo_bytes(which)
+    def halo(self, which: int, direction: int, side: int, pack: bool, buf):
+        """buf: a contiguous CUDA uint8 tensor of halo_bytes(which, direction) bytes on this context's device."""
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.halo_bytes(which, direction)
         with self._torch.cuda.device(self.device):
-            self._check(load().fargo_halo(self._h, which, side, 1 if pack else 0, buf.data_ptr()), "fargo_halo")
+            self._check(load().fargo_halo(self._h, which, direction, side, 1 if pack else 0, buf.data_ptr()), "fargo_halo")
 
     def dt_tensor(self):
         """The device-resident time step as a 1-element float64 tensor VIEW (for an in-place all-reduce)."""

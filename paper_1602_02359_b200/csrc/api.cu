@@ -33,8 +33,8 @@ struct CtxBase {
   virtual int get_array(const char*, void*) = 0;
   virtual void dims(int*, int*, int*, int*, int*, int*) const = 0;
   virtual int update_phase(int) = 0;
-  virtual int halo(int, int, int, void*) = 0;
-  virtual size_t halo_bytes(int) const = 0;
+  virtual int halo(int, int, int, int, void*) = 0;
+  virtual size_t halo_bytes(int, int) const = 0;
   virtual void* dt_ptr() = 0;
   virtual int set_planets(int, const double*, const double*, const double*, const double*, int, double) = 0;
   virtual int get_planets(double*, double*, double*) = 0;
@@ -74,8 +74,8 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
     for (int s = 0; s < 2; ++s)
       if (m->bc[dd][s] < 0 || m->bc[dd][s] > 3) { err = "unknown boundary kind"; return false; }
   for (int s = 0; s < 2; ++s)
-    if (m->bc[0][s] == FARGO_EXTERNAL || m->bc[2][s] == FARGO_EXTERNAL || (m->bc[1][s] == FARGO_EXTERNAL && m->ny < 3)) {
-      err = "FARGO_EXTERNAL is for the Y faces of a slab of at least 3 rows (X is never cut, P:728)"; return false;
+    if (m->bc[0][s] == FARGO_EXTERNAL || (m->bc[1][s] == FARGO_EXTERNAL && m->ny < 3) || (m->bc[2][s] == FARGO_EXTERNAL && m->nz < 3)) {
+      err = "FARGO_EXTERNAL is for the Y and Z faces of a sub-domain of at least 3 layers (X is never cut, P:728)"; return false;
     }
   if (!(m->xmax > m->xmin)) { err = "xmax must exceed xmin"; return false; }
   L.nx = m->nx; L.ny = m->ny; L.nz = m->nz;
@@ -119,7 +119,7 @@ struct Sim : CtxBase {
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
   int next_phase = 0;   // slab mode: the phase fargo_update_phase expects next
-  State<T> s2m;         // slab mode: where e and v are after the source step (phase 1 -> phase 2)
+  State<T> s2m;         // slab mode: where e and v are after the source step (phase 2 -> phases 3, 4)
   bool fuse_source = false;
   bool fuse_visc = false;   // 7d in one pass (k_visc3d_fused)
   bool fuse_dt = false;   // Eq. 51 and the next update's per-cell CFL rate in one kernel (k_newvel_dt)
@@ -228,7 +228,11 @@ struct Sim : CtxBase {
     std::vector<double> ye = ghosted_edges(m->yedges ? m->yedges + elo : nullptr, L.ny, L.ngy, m->ymin, m->ymax);
     for (int g = 0; g < elo; ++g) ye[g] = m->yedges[g];
     for (int g = 0; g < ehi; ++g) ye[L.ngy + L.ny + 1 + g] = m->yedges[elo + L.ny + 1 + g];
-    std::vector<double> ze = ghosted_edges(m->zedges, L.nz, L.ngz, m->zmin, m->zmax);
+    const int zlo = m->bc[2][0] == FARGO_EXTERNAL ? 3 : 0, zhi = m->bc[2][1] == FARGO_EXTERNAL ? 3 : 0;
+    if ((zlo || zhi) && !m->zedges) { err = "a sub-domain cut in Z needs its zedges, with the neighbours' edges beyond the cut faces"; return FARGO_EINVAL; }
+    std::vector<double> ze = ghosted_edges(m->zedges ? m->zedges + zlo : nullptr, L.nz, L.ngz, m->zmin, m->zmax);
+    for (int g = 0; g < zlo; ++g) ze[g] = m->zedges[g];
+    for (int g = 0; g < zhi; ++g) ze[L.ngz + L.nz + 1 + g] = m->zedges[zlo + L.nz + 1 + g];
     for (size_t n = 1; n < ye.size(); ++n) if (!(ye[n] > ye[n - 1])) { err = "yedges must increase"; return FARGO_EINVAL; }
     for (size_t n = 1; n < ze.size(); ++n) if (!(ze[n] > ze[n - 1])) { err = "zedges must increase"; return FARGO_EINVAL; }
     HostTables ht;
@@ -395,42 +399,56 @@ struct Sim : CtxBase {
   }
 
   // ---- slab decomposition in Y (NEXT-3; section 4.1) ------------------------------------------------------
-  bool is_slab() const { return d.bc[1][0] == BC_EXTERNAL || d.bc[1][1] == BC_EXTERNAL; }
+  bool is_slab() const {
+    return d.bc[1][0] == BC_EXTERNAL || d.bc[1][1] == BC_EXTERNAL || d.bc[2][0] == BC_EXTERNAL || d.bc[2][1] == BC_EXTERNAL;
+  }
 
   int update_phase(int phase) override {
     if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
     if (midstep) { err = "context is mid-step (fargo_step_until)"; return FARGO_ESTATE; }
-    if (phase < 0 || phase > 2) { err = "phase must be 0, 1 or 2"; return FARGO_EINVAL; }
-    if (phase != next_phase) { err = "phases run in the order 0, 1, 2"; return FARGO_ESTATE; }
+    if (phase < 0 || phase > 4) { err = "phase must be 0 .. 4"; return FARGO_EINVAL; }
+    if (phase != next_phase) { err = "phases run in the order 0, 1, 2, 3, 4"; return FARGO_ESTATE; }
     if (npl > 0) { err = "live planets are not supported on slabs (the gas force is a sum over the whole mesh)"; return FARGO_EINVAL; }
     launches += enqueue_update(-1, false, phase);
-    next_phase = (phase + 1) % 3;
+    next_phase = (phase + 1) % 5;
     if (!ck(cudaGetLastError(), "phase launch")) return FARGO_ECUDA;
     return FARGO_OK;
   }
 
-  // bytes of one halo message: 3 layers x the full allocated X extent x every plane, per field
-  size_t halo_bytes(int which) const override { return (size_t)(which == 0 ? 5 : 4) * 3 * (size_t)L.pitch * L.TZ * sizeof(T); }
+  // bytes of one halo message: 3 layers (rows for dir = 1, planes for dir = 2) over the full allocated extent, per field
+  size_t halo_bytes(int which, int dir) const override {
+    const size_t layer = dir == 1 ? (size_t)L.pitch * L.TZ : (size_t)L.plane;
+    return (size_t)(which == 0 ? 5 : 4) * 3 * layer * sizeof(T);
+  }
 
-  // which: 0 = the state (rho, e, vx, vy, vz; before phase 0), 1 = (e, vx, vy, vz) after the source step (between
-  // phases 1 and 2).  side: 0 = lower Y face, 1 = upper.  pack: the 3 active rows next to that face -> buf;
-  // unpack: buf -> the 3 ghost rows beyond it.  Strided device-to-device copies on the context's stream.
-  int halo(int which, int side, int pack, void* buf) override {
-    if (!buf || which < 0 || which > 1 || side < 0 || side > 1) { err = "bad halo argument"; return FARGO_EINVAL; }
-    if (!L.hasy) { err = "no Y direction"; return FARGO_EINVAL; }
-    if (which == 1 && next_phase != 2) { err = "the source-step halo exists between phases 1 and 2"; return FARGO_ESTATE; }
+  // which: 0 = the state (rho, e, vx, vy, vz), 1 = (e, vx, vy, vz) after the source step.  dir: 1 = Y, 2 = Z.
+  // side: 0 = lower face, 1 = upper.  pack: the 3 active layers next to that face -> buf; unpack: buf -> the 3 ghost
+  // layers beyond it.  Device-to-device copies on the context's stream (3 rows of a plane, and 3 planes, are contiguous).
+  int halo(int which, int dir, int side, int pack, void* buf) override {
+    if (!buf || which < 0 || which > 1 || side < 0 || side > 1 || dir < 1 || dir > 2) { err = "bad halo argument"; return FARGO_EINVAL; }
+    if ((dir == 1 && !L.hasy) || (dir == 2 && !L.hasz)) { err = "no such direction"; return FARGO_EINVAL; }
+    if (which == 1 && next_phase != 3 && next_phase != 4) { err = "the source-step halos exist between phases 2 and 4"; return FARGO_ESTATE; }
     const State<T>& a = which == 0 ? st : s2m;
     T* f[5] = {a.rho, a.e, a.vx, a.vy, a.vz};
     const int first = which == 0 ? 0 : 1;
-    const int j = pack ? (side == 0 ? L.ngy : L.ngy + L.ny - 3) : (side == 0 ? 0 : L.ngy + L.ny);
-    const size_t row3 = 3 * (size_t)L.pitch * sizeof(T), per_field = row3 * L.TZ;
+    const int ng = dir == 1 ? L.ngy : L.ngz, na = dir == 1 ? L.ny : L.nz;
+    const int m = pack ? (side == 0 ? ng : ng + na - 3) : (side == 0 ? 0 : ng + na);
     unsigned char* b = (unsigned char*)buf;
+    const size_t per_field = halo_bytes(0, dir) / 5;
     for (int q = first; q < 5; ++q) {
       if (!f[q]) continue;
-      unsigned char* field = (unsigned char*)(f[q] + (size_t)j * L.pitch);
       unsigned char* msg = b + (size_t)(q - first) * per_field;
-      const cudaError_t e = pack ? cudaMemcpy2DAsync(msg, row3, field, (size_t)L.plane * sizeof(T), row3, L.TZ, cudaMemcpyDeviceToDevice, stream)
-                                 : cudaMemcpy2DAsync(field, (size_t)L.plane * sizeof(T), msg, row3, row3, L.TZ, cudaMemcpyDeviceToDevice, stream);
+      cudaError_t e;
+      if (dir == 1) {
+        const size_t row3 = 3 * (size_t)L.pitch * sizeof(T);
+        unsigned char* field = (unsigned char*)(f[q] + (size_t)m * L.pitch);
+        e = pack ? cudaMemcpy2DAsync(msg, row3, field, (size_t)L.plane * sizeof(T), row3, L.TZ, cudaMemcpyDeviceToDevice, stream)
+                 : cudaMemcpy2DAsync(field, (size_t)L.plane * sizeof(T), msg, row3, row3, L.TZ, cudaMemcpyDeviceToDevice, stream);
+      } else {
+        unsigned char* field = (unsigned char*)(f[q] + (size_t)m * L.plane);
+        e = pack ? cudaMemcpyAsync(msg, field, per_field, cudaMemcpyDeviceToDevice, stream)
+                 : cudaMemcpyAsync(field, msg, per_field, cudaMemcpyDeviceToDevice, stream);
+      }
       if (!ck(e, "halo copy")) return FARGO_ECUDA;
     }
     return FARGO_OK;
@@ -533,20 +551,23 @@ struct Sim : CtxBase {
   }
 
   // Enqueue the kernels of one update up to and including `until` (-1 = all).  Returns the launch count.
-  // `phase` (slab decomposition, NEXT-3): -1 = the whole update; 0 = cells 2-6 (ghost fill of the non-external faces,
-  // v0, potential, local dt); 1 = the dt fix-up after the all-reduce and the source step; 2 = cell 9 and the transport
-  // step.  The caller exchanges the Y halos of the state before phase 0 and those of (e, v) between phases 1 and 2.
+  // `phase` (domain decomposition, NEXT-3): -1 = the whole update; 0 = cell 2 (ghost fill of the faces that are not cut);
+  // 1 = cells 3-6 (v0, potential, local dt); 2 = the dt fix-up after the all-reduce and the source step; 3 = cell 9;
+  // 4 = the transport step.  The caller exchanges the Y halos before the fill (phases 0, 3) and the Z halos after it.
   int enqueue_update(int until, bool capturing, int phase = -1) {
     int n = 0;
     const T* v0p = L.fargo ? v0 : nullptr;
     State<T> s2 = st;   // the state the transport step reads: e and v after the source step
-    if (phase == 2) { s2 = s2m; goto cell9; }
-    if (phase == 1) { n += launch_dt_sync(ctl, prm.t_stop, sizeof(T) == 4, stream); goto cell7; }
+    if (phase == 4) { s2 = s2m; goto cell12; }
+    if (phase == 3) { s2 = s2m; goto cell9; }
+    if (phase == 2) { n += launch_dt_sync(ctl, prm.t_stop, sizeof(T) == 4, stream); goto cell7; }
+    if (phase == 1) goto cell3;
     dbg.clear();
     dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
     dbg["phi"] = phi; dbg["v0"] = v0;
     n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(true, true), stream); });                        // cell 2
-    if (until == FARGO_ST_BC1) return n;
+    if (until == FARGO_ST_BC1 || phase == 0) return n;
+  cell3:
     if (L.fargo) n += timed("vmean", [&] { return launch_vmean<T>(d, st.vx, v0, stream); });                         // cell 3
     if (until == FARGO_ST_VMEAN) return n;
     if (npl > 0) {                                                                    // cell 5, live planets (on the device)
@@ -566,7 +587,7 @@ struct Sim : CtxBase {
     if (until == FARGO_ST_DT) return n;
     if (npl > 0)                                                                      // cell 5a (reading G33)
       n += timed("planets", [&] { return launch_planets_update<T>(d, st.rho, pl, npl, pl_mode, pl_part, prm.gm_star, prm.omega_frame, stream); });
-    if (phase == 0) return n;
+    if (phase == 1) return n;
   cell7:
     if (fuse_source && until < 0) {
       // cells 7a-7c in one pass; it reads neighbours of the state, so its output goes to arrays of its own
@@ -607,10 +628,11 @@ struct Sim : CtxBase {
       dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
       if (until == FARGO_ST_SRC_D) return n;
     }
-    if (phase == 1) { s2m = s2; return n; }
+    if (phase == 2) { s2m = s2; return n; }
   cell9:
     n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                      // cell 9
-    if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM) return n;
+    if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM || phase == 3) return n;
+  cell12:
     // transport: pass p reads set (p-1)%2 (the state on the first pass) and writes set p%2; the last pass
     // writes rho and e straight back into the state arrays, so one update leaves every array where it
     // started and the same captured graph serves every update.
@@ -806,9 +828,9 @@ int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
 int fargo_set_omega_frame(fargo_ctx* c, double omega_new) { return c ? c->impl->set_omega_frame(omega_new) : FARGO_EINVAL; }
 int fargo_diagnostics(fargo_ctx* c, double* out) { return c ? c->impl->diagnostics(out) : FARGO_EINVAL; }
 int fargo_update_phase(fargo_ctx* c, int phase) { return c ? c->impl->update_phase(phase) : FARGO_EINVAL; }
-size_t fargo_halo_bytes(const fargo_ctx* c, int which) { return c ? c->impl->halo_bytes(which) : 0; }
-int fargo_halo(fargo_ctx* c, int which, int side, int pack, void* device_buffer) {
-  return c ? c->impl->halo(which, side, pack, device_buffer) : FARGO_EINVAL;
+size_t fargo_halo_bytes(const fargo_ctx* c, int which, int dir) { return c ? c->impl->halo_bytes(which, dir) : 0; }
+int fargo_halo(fargo_ctx* c, int which, int dir, int side, int pack, void* device_buffer) {
+  return c ? c->impl->halo(which, dir, side, pack, device_buffer) : FARGO_EINVAL;
 }
 void* fargo_dt_device_ptr(fargo_ctx* c) { return c ? c->impl->dt_ptr() : nullptr; }
 int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }

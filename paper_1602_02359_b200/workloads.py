@@ -35,6 +35,7 @@ class Mesh:
     yedges: np.ndarray  # ny+1 active edges
     zedges: np.ndarray  # nz+1 active edges
     bc: tuple = ((PERIODIC, PERIODIC), (PERIODIC, PERIODIC), (PERIODIC, PERIODIC))
+    zedges_ext: Optional[tuple] = None   # sub-domains only: the same for cut Z faces
     yedges_ext: Optional[tuple] = None   # slabs only: (3 edges beyond a cut lower Y face or None, 3 beyond a cut upper face or None)
 
     @property

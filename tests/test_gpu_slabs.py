@@ -16,7 +16,10 @@ pytestmark = pytest.mark.gpu
 
 CASES = [(G.cart_adi_periodic_even, 2), (G.cart_adi_periodic_even, 3), (G.sph3d_iso_fargo, 2), (G.sph3d_iso_fargo, 3),
          (G.cyl3d_visc_fargo, 2), (G.cart_adi_mixed_bc, 3), (G.cyl2d_iso_fargo_visc, 4), (G.sheet3d_adi_fargo, 3),
-         (G.nonuniform_cyl2d, 2)]
+         (G.nonuniform_cyl2d, 2),
+         # cuts in Y and Z (py, pz): edges and corners travel with the Z planes
+         (G.cart_adi_periodic_even, (2, 2)), (G.sph3d_iso_fargo, (2, 2)), (G.cart_adi_mixed_bc, (1, 3)), (G.cyl3d_visc_fargo, (2, 2)),
+         (G.sph3d_adi_nofargo, (2, 3))]
 
 
 def _single(w, params=None):
@@ -26,7 +29,7 @@ def _single(w, params=None):
     return g
 
 
-@pytest.mark.parametrize("make,nslabs", CASES, ids=["%s-%d" % (m.__name__, n) for m, n in CASES])
+@pytest.mark.parametrize("make,nslabs", CASES, ids=["%s-%s" % (m.__name__, n) for m, n in CASES])
 def test_slabs_equal_the_undivided_mesh(make, nslabs):
     from paper_1602_02359_b200.slabs import SlabRun
     w = make()

@@ -33,6 +33,17 @@ def test_neighbours_and_faces():
     subs = [slab_mesh(m, r, 3) for r in range(3)]
     assert [s.bc[1] for s, _ in subs] == [(W.REFLECTING, 3), (3, 3), (3, W.OUTFLOW)]
     assert np.array_equal(np.concatenate([s.yedges[:-1] for s, _ in subs] + [m.yedges[-1:]]), m.yedges)
+    # the edges beyond a cut are the neighbour's; at a real wall there are none
+    assert subs[0][0].yedges_ext[0] is None and np.array_equal(subs[0][0].yedges_ext[1], m.yedges[5:8])
+    assert np.array_equal(subs[1][0].yedges_ext[0], m.yedges[1:4]) and subs[2][0].yedges_ext[1] is None
+    # a 2 x 2 grid: Y fastest; Z periodic, so every Z face is cut and the seam's edges continue the mesh
+    m2 = W.Mesh(8, 12, 8, 0.0, 1.0, W.uedges(0.5, 2.0, 12), W.uedges(0.0, 1.0, 8),
+                ((W.PERIODIC,) * 2, (W.REFLECTING, W.OUTFLOW), (W.PERIODIC,) * 2))
+    g = [slab_mesh(m2, r, (2, 2)) for r in range(4)]
+    assert [x[1] for x in g] == [((0, 6), (0, 4)), ((6, 12), (0, 4)), ((0, 6), (4, 8)), ((6, 12), (4, 8))]
+    assert all(x[0].bc[2] == (3, 3) for x in g)
+    assert np.allclose(g[0][0].zedges_ext[0], [-0.375, -0.25, -0.125]) and np.array_equal(g[0][0].zedges_ext[1], m2.zedges[5:8])
+    assert np.array_equal(g[2][0].zedges_ext[0], m2.zedges[1:4]) and np.allclose(g[2][0].zedges_ext[1], [1.125, 1.25, 1.375])
 
 
 def test_every_send_has_its_receive():

@@ -429,7 +429,7 @@ def run_local_slabs(args):
         "metric": METRIC, "value": w.mesh.ncells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": Wm,
         "ms_per_step": ms / K, "higher_is_better": True, "dtype": "f32" if args.fp32 else "f64", "data": "synthetic",
         "config": {"workload": w.name, "local_slabs": args.local_slabs, "rows": [list(r) for r in s.rows.values()],
-                   "launch": "plain launches, three phases per update and slab, halos device to device on one stream",
+                   "launch": "plain launches, five phases per update and slab, halos device to device on one stream",
                    "halo_bytes_copied_per_update": halo},
         "gpu_launches": sum(c.kernel_launches() for c in s.ctx.values()) - l0}))
 

@@ -1,8 +1,8 @@
-"""Slab decomposition in Y over several contexts (section 4.1).
+"""Domain decomposition in Y and Z over several contexts (section 4.1).
 
 The paper splits the mesh in Y (and Z), never in X, exchanges 3 ghost layers at cells 2 and 9 of Fig. 2 and takes the
-minimum of the time step over the sub-domains.  Here a slab is an ordinary context (C ABI, include/fargo.h)
-whose cut Y faces have the kind FARGO_EXTERNAL; this module only does the plumbing the ABI leaves to the caller:
+minimum of the time step over the sub-domains.  Here a sub-domain is an ordinary context (C ABI,
+include/fargo.h) whose cut Y / Z faces have the kind FARGO_EXTERNAL; this module only does the plumbing the ABI leaves to the caller:
 who is whose neighbour, the halo messages, the all-reduce of dt.  No arithmetic of the method lives here.
 
 Two transports:

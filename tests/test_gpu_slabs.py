@@ -76,3 +76,19 @@ def test_a_slab_refuses_fargo_step_and_out_of_order_phases():
         s.ctx[0].update_phase(1)
     s.step(1)
     s.synchronize()
+
+
+def test_fp32_sub_domains_equal_the_undivided_fp32_mesh():
+    from paper_1602_02359_b200 import Fargo
+    from paper_1602_02359_b200.slabs import SlabRun
+    w = G.sph3d_iso_fargo()
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=32)
+    g.set_fields(*w.fields())
+    g.step(w.nsteps)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, nslabs=(3, 2), precision=32)
+    s.set_fields(*w.fields())
+    s.step(w.nsteps)
+    s.synchronize()
+    assert s.time() == g.time()
+    for a, b in zip(s.get_fields(), g.get_fields()):
+        assert a.dtype == np.float32 and np.array_equal(a, b)

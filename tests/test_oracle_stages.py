@@ -272,3 +272,79 @@ def test_src_c_divergence_uses_exact_surfaces_in_spherical_geometry():
     a = 0.5 * dt * (g - 1.0) * 3 * A
     ed = o2.active(o2.array("ed"))[:, 1:-1, :]
     assert np.allclose(ed, 2.0 * (1 - a) / (1 + a), rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------- Eq. 36: the v_theta^2 / r term
+def _sph_src_a(nphi, nr, nth, vphi, vth, om=0.0):
+    """One 7a sub-step (dt = 1, uniform pressure, no potential) on a spherical mesh with v_phi(phi, r, theta) and
+    v_theta(phi, r, theta) sampled at their own faces; returns the mesh and the radial / polar accelerations."""
+    m = mesh(nphi, nr, nth, x=(-math.pi, math.pi), y=(1.0, 2.0), z=(0.5 * math.pi - 0.6, 0.5 * math.pi + 0.4),
+             bc=(PER, OUT, OUT))
+    s = (nth, nr, nphi)
+    one = np.ones(s)
+    pf, pc = m.xf()[None, None, :] * one, m.xc()[None, None, :] * one
+    rc = m.yc()[None, :, None] * one
+    tc, tf = m.zc()[:, None, None] * one, m.zedges[:-1][:, None, None] * one
+    o = Oracle(m, W.SPHERICAL, W.ISOTHERMAL, W.Params(dt_fixed=1.0, omega_frame=om))
+    vz_in = vth(pc, rc, tf)
+    o.set_fields(one, np.full(s, 1e-9), vphi(pf, rc, tc), np.zeros(s), vz_in)
+    o.step_until("SRC_A")
+    return m, o.active(o.array("vyb")), o.active(o.array("vzb")) - vz_in   # dt = 1, v_r = 0: the accelerations
+
+
+def _eq36_error(n, vphi, vth, om=0.0):
+    """max |a_r - (v_phi^t^2 + v_theta^2)/r| over the interior radial faces, relative to max |a_r| (Eq. 36),
+    and the same for Eq. 37's (v_phi^t)^2 cot(theta) / r on the polar faces; v^t = v + Omega_f r sin(theta)."""
+    m, ar, at = _sph_src_a(2 * n, n, n, vphi, vth, om)
+    P = m.xc()[None, None, :]
+    rf, rc = m.yedges[:-1][None, :, None], m.yc()[None, :, None]
+    tc, tf = m.zc()[:, None, None], m.zedges[:-1][:, None, None]
+    ex_r = ((vphi(P, rf, tc) + om * rf * np.sin(tc)) ** 2 + vth(P, rf, tc) ** 2) / rf
+    ex_t = (vphi(P, rc, tf) + om * rc * np.sin(tf)) ** 2 / (np.tan(tf) * rc)
+    I = (slice(1, -1), slice(1, -1), slice(None))
+    return (np.max(np.abs(ar[I] - ex_r[I])) / np.max(np.abs(ex_r[I])),
+            np.max(np.abs(at[I] - ex_t[I])) / max(np.max(np.abs(ex_t[I])), 1e-300))
+
+
+def test_src_a_eq36_rigid_rotation_about_a_perpendicular_axis():
+    """Rigid rotation Omega about the x axis (perpendicular to the polar axis): v_r = 0, v_theta = -Omega r sin(phi),
+    v_phi = -Omega r cos(theta) cos(phi).  The radial equation (Eq. 36) must then supply the centripetal term
+    |v|^2 / r = Omega^2 r (1 - sin^2(theta) cos^2(phi)) = Omega^2 times the distance to the axis, projected on r;
+    Eq. 37 supplies v_phi^2 cot(theta) / r.  Second-order in the mesh spacing: the 4-point averages of Eq. 38 are
+    centred on the face.  A dropped v_theta^2, a radius taken at the cell centre or a one-sided average leaves an
+    O(1) or first-order error and fails the bounds and the convergence order below."""
+    Om = 0.7
+    vphi = lambda p, r, t: -Om * r * np.cos(t) * np.cos(p)
+    vth = lambda p, r, t: -Om * r * np.sin(p) + 0.0 * t
+    e1, e2 = _eq36_error(16, vphi, vth), _eq36_error(32, vphi, vth)
+    assert e2[0] < 1.5e-3 and e2[1] < 3e-3, (e1, e2)          # second-order truncation only
+    assert 3.0 < e1[0] / e2[0] < 5.0 and 3.0 < e1[1] / e2[1] < 5.0, (e1, e2)   # first-order mistakes give 2
+    # physical reading at one face: centripetal acceleration of the rotation about x
+    m, ar, _ = _sph_src_a(64, 32, 32, vphi, vth)
+    k, j, i = 9, 11, 20
+    r, t, p = m.yedges[j], m.zc()[k], m.xc()[i]
+    x = np.array([r * math.sin(t) * math.cos(p), r * math.sin(t) * math.sin(p), r * math.cos(t)])
+    perp = x - np.array([x[0], 0.0, 0.0])                      # from the x axis to the point
+    assert ar[k, j, i] == pytest.approx(Om ** 2 * float(perp @ x) / r, rel=2e-3)
+
+
+def test_src_a_eq36_v_theta_alone_on_a_meridian_flow():
+    """v_phi = 0 everywhere, frame at rest: the only term left in Eq. 36 is v_theta^2 / r.  v_theta varies with r,
+    theta AND phi, so each leg of the 4-point average (j, j-1) x (k, k+1) and the position of 1/r (the radial FACE)
+    matters: a_r -> v_theta(phi_c, r_face, theta_c)^2 / r_face at second order; Eq. 37 gives exactly zero."""
+    vphi = lambda p, r, t: 0.0 * (p + r + t)
+    vth = lambda p, r, t: 0.3 * r ** 1.5 * (1.0 + 0.5 * np.sin(3.0 * t)) * (1.0 + 0.4 * np.cos(p))
+    e1, e2 = _eq36_error(16, vphi, vth)[0], _eq36_error(32, vphi, vth)[0]
+    assert e2 < 2e-3, (e1, e2)
+    assert 3.0 < e1 / e2 < 5.0, (e1, e2)
+    _, _, at = _sph_src_a(16, 8, 8, vphi, vth)
+    assert not np.any(at[1:-1, 1:-1])   # v_theta untouched bit for bit: no v_phi, uniform P
+
+
+def test_src_a_eq36_with_both_terms_and_a_rotating_frame():
+    """Both terms together with Omega_f != 0: (v_phi + Omega_f r sin(theta))^2 + v_theta^2 over r (Eqs. 36, 38)."""
+    vphi = lambda p, r, t: 0.2 * r ** -0.5 * np.sin(t) * (1.0 + 0.3 * np.sin(p))
+    vth = lambda p, r, t: 0.25 * r * np.cos(2.0 * t) * (1.0 + 0.3 * np.cos(2.0 * p))
+    e1, e2 = _eq36_error(16, vphi, vth, om=0.35), _eq36_error(32, vphi, vth, om=0.35)
+    assert e2[0] < 2e-3 and e2[1] < 4e-3, (e1, e2)
+    assert 3.0 < e1[0] / e2[0] < 5.0 and 3.0 < e1[1] / e2[1] < 5.0, (e1, e2)

@@ -15,8 +15,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle.so")
+_OMP_PATH = os.path.join(_HERE, "liboracle_omp.so")   # same sources + OpenMP on the outer loops; bit-identical (tests)
 _lock = threading.Lock()
-_lib = None
+_libs = {}
 
 STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2", "MOM",
           "SWEEP_X", "SWEEP_Y", "SWEEP_Z", "ORB_FRAC", "ORB_SHIFT", "NEWVEL"]
@@ -42,21 +43,24 @@ class _Params(C.Structure):
 
 
 def build(force: bool = False) -> str:
-    """Compile liboracle.so with g++ (make) if it is missing or older than its sources."""
-    srcs = [os.path.join(_HERE, f) for f in os.listdir(_HERE) if f.endswith((".cpp", ".hpp", ".h"))]
-    stale = force or not os.path.exists(_LIB_PATH) or any(
-        os.path.getmtime(s) > os.path.getmtime(_LIB_PATH) for s in srcs)
-    if stale:
-        subprocess.run(["make", "-C", _HERE, "-B", "liboracle.so"], check=True, capture_output=True)
+    """Compile liboracle.so and liboracle_omp.so with g++ (make) if missing or older than their sources."""
+    srcs = [os.path.join(_HERE, f) for f in os.listdir(_HERE) if f.endswith((".cpp", ".hpp", ".h")) or f == "Makefile"]
+    for path in (_LIB_PATH, _OMP_PATH):
+        stale = force or not os.path.exists(path) or any(os.path.getmtime(s) > os.path.getmtime(path) for s in srcs)
+        if stale:
+            r = subprocess.run(["make", "-C", _HERE, "-B", os.path.basename(path)], capture_output=True, text=True)
+            if r.returncode != 0:
+                raise RuntimeError("building %s failed:\n%s%s" % (os.path.basename(path), r.stdout, r.stderr))
     return _LIB_PATH
 
 
-def lib():
-    global _lib
+def lib(omp: bool = False):
+    """The one-thread library (the reference of every parity test) or, with omp=True, the OpenMP build of the same
+    sources (full-length references at 512^3 and config 4 only)."""
     with _lock:
-        if _lib is None:
+        if omp not in _libs:
             build()
-            L = C.CDLL(_LIB_PATH)
+            L = C.CDLL(_OMP_PATH if omp else _LIB_PATH)
             vp = C.c_void_p
             L.oracle_init.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(_Params)]
             L.oracle_destroy.argtypes = [vp]
@@ -85,8 +89,8 @@ def lib():
             L.oracle_ppa_star.restype = None
             L.oracle_ppa_interfaces.argtypes = [C.c_int, _DP, _DP, _DP]
             L.oracle_ppa_interfaces.restype = None
-            _lib = L
-    return _lib
+            _libs[omp] = L
+    return _libs[omp]
 
 
 def _p(a):
@@ -101,8 +105,8 @@ class Oracle:
     """One oracle context.  `mesh` and `params` are the plain dataclasses of workloads.py
     (any objects with the same attribute names work)."""
 
-    def __init__(self, mesh, geometry: int, eos: int, params, nghost: int = 3):
-        L = lib()
+    def __init__(self, mesh, geometry: int, eos: int, params, nghost: int = 3, omp: bool = False):
+        L = self._L = lib(omp)
         self._ye = _f64(mesh.yedges)
         self._ze = _f64(mesh.zedges)
         m = _Mesh()
@@ -129,7 +133,7 @@ class Oracle:
 
     def close(self):
         if self._h:
-            lib().oracle_destroy(self._h)
+            self._L.oracle_destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -142,32 +146,32 @@ class Oracle:
         a = [_f64(x) for x in (rho, e, vx, vy, vz)]
         for x in a:
             assert x is None or x.size == int(np.prod(self.shape))
-        if lib().oracle_set_fields(self._h, *[_p(x) for x in a]) != 0:
+        if self._L.oracle_set_fields(self._h, *[_p(x) for x in a]) != 0:
             raise ValueError("oracle_set_fields failed")
 
     def get_fields(self):
         out = [np.empty(self.shape, dtype=np.float64) for _ in range(5)]
-        lib().oracle_get_fields(self._h, *[_p(x) for x in out])
+        self._L.oracle_get_fields(self._h, *[_p(x) for x in out])
         return tuple(out)
 
     def step(self, n: int = 1):
-        if lib().oracle_step(self._h, n) != 0:
+        if self._L.oracle_step(self._h, n) != 0:
             raise RuntimeError("oracle_step failed")
 
     def step_until(self, stage: str):
-        if lib().oracle_step_until(self._h, STAGES.index(stage)) != 0:
+        if self._L.oracle_step_until(self._h, STAGES.index(stage)) != 0:
             raise RuntimeError("oracle_step_until failed")
 
     def run_stage(self, stage: str):
-        if lib().oracle_run_stage(self._h, STAGES.index(stage)) != 0:
+        if self._L.oracle_run_stage(self._h, STAGES.index(stage)) != 0:
             raise RuntimeError("oracle_run_stage failed")
 
     def set_dt(self, dt: float):
-        lib().oracle_set_dt(self._h, float(dt))
+        self._L.oracle_set_dt(self._h, float(dt))
 
     def time(self):
         t, dt, n = C.c_double(), C.c_double(), C.c_longlong()
-        lib().oracle_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n))
+        self._L.oracle_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n))
         return t.value, dt.value, n.value
 
     # ---- live planets (NEXT-2) ----
@@ -175,34 +179,34 @@ class Oracle:
         gm, eps, pos, vel = (_f64(np.atleast_1d(a)).ravel() for a in (gm, eps, pos, vel))
         n = len(gm)
         assert len(eps) == n and len(pos) == 3 * n and len(vel) == 3 * n
-        if lib().oracle_set_planets(self._h, n, _p(gm), _p(eps), _p(pos), _p(vel), force_mode, float(gconst)) != 0:
+        if self._L.oracle_set_planets(self._h, n, _p(gm), _p(eps), _p(pos), _p(vel), force_mode, float(gconst)) != 0:
             raise ValueError("oracle_set_planets failed")
         self._npl = n
 
     def get_planets(self):
         n = getattr(self, "_npl", 0)
         pos, vel, acc = (np.zeros((n, 3)) for _ in range(3))
-        lib().oracle_get_planets(self._h, _p(pos), _p(vel), _p(acc))
+        self._L.oracle_get_planets(self._h, _p(pos), _p(vel), _p(acc))
         return pos, vel, acc
 
     def set_omega_frame(self, omega_new: float):
-        if lib().oracle_set_omega_frame(self._h, float(omega_new)) != 0:
+        if self._L.oracle_set_omega_frame(self._h, float(omega_new)) != 0:
             raise ValueError("oracle_set_omega_frame failed")
 
     def diagnostics(self):
         """(mass, X, Y, Z momentum of Tab. 2, internal energy): sums over the active cells."""
         out = np.zeros(5)
-        if lib().oracle_diagnostics(self._h, _p(out)) != 0:
+        if self._L.oracle_diagnostics(self._h, _p(out)) != 0:
             raise RuntimeError("oracle_diagnostics failed")
         return out
 
     def planets_rk5(self, h: float):
-        if lib().oracle_planets_rk5(self._h, float(h)) != 0:
+        if self._L.oracle_planets_rk5(self._h, float(h)) != 0:
             raise RuntimeError("oracle_planets_rk5 failed")
 
     def gas_force(self, p: int = 0):
         F = np.zeros(3)
-        if lib().oracle_gas_force(self._h, p, _p(F)) != 0:
+        if self._L.oracle_gas_force(self._h, p, _p(F)) != 0:
             raise RuntimeError("oracle_gas_force failed")
         return F
 
@@ -211,13 +215,13 @@ class Oracle:
         ring = name in ("v0", "nshift", "xi")
         shape = (self.TZ, self.TY) if ring else (self.TZ, self.TY, self.TX)
         out = np.empty(shape, dtype=np.float64)
-        if lib().oracle_get_array(self._h, name.encode(), _p(out)) != 0:
+        if self._L.oracle_get_array(self._h, name.encode(), _p(out)) != 0:
             raise KeyError(name)
         return out
 
     def set_array(self, name: str, a):
         a = _f64(a)
-        if lib().oracle_set_array(self._h, name.encode(), _p(a)) != 0:
+        if self._L.oracle_set_array(self._h, name.encode(), _p(a)) != 0:
             raise KeyError(name)
 
     def active(self, a: np.ndarray) -> np.ndarray:
@@ -226,7 +230,7 @@ class Oracle:
 
     def geometry(self, j: int, k: int):
         v = [C.c_double() for _ in range(7)]
-        if lib().oracle_geometry(self._h, j, k, *[C.byref(x) for x in v]) != 0:
+        if self._L.oracle_geometry(self._h, j, k, *[C.byref(x) for x in v]) != 0:
             raise IndexError((j, k))
         return dict(zip(("sx", "sy", "sz", "invv", "lx", "ly", "lz"), [x.value for x in v]))
 

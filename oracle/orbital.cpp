@@ -69,7 +69,10 @@ void orc_orbital_frac(oracle_ctx& c) {
   const int n = c.TX;   // FARGO requires wrapped X: TX = nx
   std::vector<vec*> Qs = {&c.pxm, &c.pxp, &c.pym, &c.pyp, &c.pzm, &c.pzp};
   if (c.eos == ORC_ADIABATIC) Qs.push_back(&c.e);
-  vec r(n), ir(n), f(n), rs(n), fs(n), Fr(n), FQ(n);
+#pragma omp parallel   // OpenMP build only: rings are independent
+  {
+  vec r(n), ir(n), f(n), rs(n), fs(n), Fr(n), FQ(n);   // ring buffers
+#pragma omp for collapse(2) schedule(static)
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j) {
       const double s = (c.v0[c.rid(j, k)] * c.dt) * c.invLX(j, k);
@@ -91,6 +94,7 @@ void orc_orbital_frac(oracle_ctx& c) {
       }
       for (int i = 0; i < n; ++i) c.rho[base + i] = r[i] - g * (Fr[i] - Fr[wrapi(i - 1, n)]);
     }
+  }
 }
 
 // ---- O10b: integer shift, Q_i <- Q_{i-N} (Eq. 69) ---------------------------------------
@@ -99,7 +103,10 @@ void orc_orbital_shift(oracle_ctx& c) {
   const int n = c.TX;
   std::vector<vec*> Qs = {&c.rho, &c.pxm, &c.pxp, &c.pym, &c.pyp, &c.pzm, &c.pzp};
   if (c.eos == ORC_ADIABATIC) Qs.push_back(&c.e);
+#pragma omp parallel   // OpenMP build only: rings are independent
+  {
   vec tmp(n);
+#pragma omp for collapse(2) schedule(static)
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j) {
       const long long N = (long long)c.nshift[c.rid(j, k)];
@@ -112,4 +119,5 @@ void orc_orbital_shift(oracle_ctx& c) {
         for (int i = 0; i < n; ++i) Qa[base + i] = tmp[i];
       }
     }
+  }
 }

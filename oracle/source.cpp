@@ -13,6 +13,7 @@ static inline double pressure(const oracle_ctx& c, size_t l) {   // cell 4: Eq. 
 void orc_source_a(oracle_ctx& c) {
   const double dt = c.dt, om = c.p.omega_frame;
   const bool curv = c.geometry != ORC_CARTESIAN, sph = c.geometry == ORC_SPHERICAL;
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j)
       for (int i = 0; i < c.TX; ++i) {
@@ -72,6 +73,7 @@ void orc_source_b(oracle_ctx& c) {
   const double dt = c.dt, cq2 = c.p.cvnr2;
   const size_t n = c.ncell();
   vec qx(n, 0.0), qy(n, 0.0), qz(n, 0.0), dvx(n, 0.0), dvy(n, 0.0), dvz(n, 0.0);
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j)
       for (int i = 0; i < c.TX; ++i) {
@@ -89,6 +91,7 @@ void orc_source_b(oracle_ctx& c) {
           dvz[l] = d; qz[l] = d < 0.0 ? (cq2 * c.rho[l]) * (d * d) : 0.0;
         }
       }
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j)
       for (int i = 0; i < c.TX; ++i) {
@@ -121,6 +124,7 @@ void orc_source_b(oracle_ctx& c) {
 // ---- 7c: compression work, time-centred form valid for gamma-law gases (G19) --------
 void orc_source_c(oracle_ctx& c) {
   const double hd = (0.5 * c.dt) * (c.p.gamma - 1.0);
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j)
       for (int i = 0; i < c.TX; ++i) {

@@ -13,6 +13,7 @@ static void fill_dir(oracle_ctx& c, vec& a, int dir, bool normal) {
   const int m0 = ng, m1 = ng + N;
   const int P = dir == 0 ? c.TY : c.TX;                  // extents of the two other directions
   const int Q = dir == 2 ? c.TY : c.TZ;
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): lines are independent
   for (int q = 0; q < Q; ++q)
     for (int p = 0; p < P; ++p) {
       auto A = [&](int m) -> double& {
@@ -50,6 +51,7 @@ void orc_bc_fill(oracle_ctx& c, vec& rho, vec& e, vec& vx, vec& vy, vec& vz) {
 
 // ---- O2: v0_jk = (max_i v + min_i v)/2 per ring, ghost rings included (Eq. 72) ----------
 void orc_vmean(oracle_ctx& c) {
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only: rings are independent
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j) {
       double v0 = 0.0;
@@ -72,6 +74,7 @@ void orc_potential(oracle_ctx& c) {
   const double phip = c.p.planet_phi0 + (c.p.planet_omega - c.p.omega_frame) * c.t;
   const double xp = c.p.planet_r * std::cos(phip), yp = c.p.planet_r * std::sin(phip);
   const double eps2 = c.p.planet_eps * c.p.planet_eps;
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only: cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j) {
       double R, z, r;
@@ -105,6 +108,7 @@ double orc_compute_dt(oracle_ctx& c, bool* clipped) {
   const double c3 = 4.0 * c.p.cvnr2;   // dt_3 = Delta/(4 C_q^2 |dv|)  (reading G8)
   const double c4 = 4.0 * c.p.nu;      // dt_4 = Delta^2/(4 nu)
   double M2 = 0.0;
+#pragma omp parallel for collapse(2) schedule(static) reduction(max : M2)   // OpenMP build only: max is exact in any order
   for (int k = c.k0(); k < c.k1(); ++k)
     for (int j = c.j0(); j < c.j1(); ++j) {
       const double ilx = c.invLX(j, k), ily = c.invLY[j], ilz = c.invLZ(j, k);
@@ -142,8 +146,9 @@ double orc_compute_dt(oracle_ctx& c, bool* clipped) {
   double dt = 1.0 / std::sqrt(M2);
   if (c.p.fargo_on) {   // Eq. 73 with V_X = v0_jk, C_0 = shear_c0 (reading G10)
     double s = 0.0;
+#pragma omp parallel for collapse(2) schedule(static) reduction(max : s)
     for (int k = c.k0(); k < c.k1(); ++k)
-      for (int j = c.j0(); j + 1 < c.j1(); ++j)
+      for (int j = c.j0(); j < c.j1() - 1; ++j)
         s = std::max(s, std::fabs(c.v0[c.rid(j, k)] * c.invLX(j, k) - c.v0[c.rid(j + 1, k)] * c.invLX(j + 1, k)));
     if (s > 0.0) dt = std::min(dt, c.p.shear_c0 / s);
   }

@@ -30,6 +30,7 @@ extern "C" void oracle_vanleer_star(int n, const double* f, const double* a, con
 // ---- 12a: left / right momenta with the quantities of Tab. 2 -----------------------
 void orc_momenta(oracle_ctx& c) {
   const double om = (c.geometry == ORC_CARTESIAN) ? 0.0 : c.p.omega_frame;
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j) {
       // Tab. 2: the term added to R_x v_x; shearing sheet: 2 Omega_f y at the cell centre (G32)
@@ -64,7 +65,10 @@ void orc_sweep(oracle_ctx& c, int dir) {
   const int P = dir == 0 ? c.TY : c.TX, Q = dir == 2 ? c.TY : c.TZ;
   std::vector<vec*> Qs = {&c.pxm, &c.pxp, &c.pym, &c.pyp, &c.pzm, &c.pzp};
   if (c.eos == ORC_ADIABATIC) Qs.push_back(&c.e);
-  vec r(n), ir(n), f(n), a(n), fs(n), rs(n), Fr(n), FQ(n), w(n), len(n), invd(n), S(n + 1), dtiv(n);
+#pragma omp parallel   // OpenMP build only: lines are independent (a line reads and writes only its own cells)
+  {
+  vec r(n), ir(n), f(n), a(n), fs(n), rs(n), Fr(n), FQ(n), w(n), len(n), invd(n), S(n + 1), dtiv(n);   // line buffers
+#pragma omp for collapse(2) schedule(static)
   for (int q = 0; q < Q; ++q)
     for (int p = 0; p < P; ++p) {
       auto L = [&](int m) -> size_t {   // line position (halo-inclusive) -> linear index
@@ -104,11 +108,13 @@ void orc_sweep(oracle_ctx& c, int dir) {
       }
       for (int m = 2; m + 2 < n; ++m) c.rho[L(m)] = r[m] - dtiv[m] * (Fr[m + 1] - Fr[m]);
     }
+  }
 }
 
 // ---- 12d: new velocities, Eq. 51 with Tab. 2 inverted (reading G28) ----------------------
 void orc_newvel(oracle_ctx& c) {
   const double om = (c.geometry == ORC_CARTESIAN) ? 0.0 : c.p.omega_frame;
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only: writes v of its own cell, reads momenta and rho
   for (int k = c.k0(); k < c.k1(); ++k)
     for (int j = c.j0(); j < c.j1(); ++j) {
       const double rx = c.Rx(j, k), rx2om = c.shear ? (2.0 * c.p.omega_frame) * c.yc[j] : (rx * rx) * om;

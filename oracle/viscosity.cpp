@@ -14,6 +14,7 @@ void orc_source_d(oracle_ctx& c) {
   vec tpp(n, 0.0), trr(n, 0.0), tpr(n, 0.0);
   const int k = 0;
   const vec &vx = c.vxc, &vy = c.vyc, &rho = c.rho;
+#pragma omp parallel for schedule(static)   // OpenMP build only: cell-independent body
   for (int j = 0; j < c.TY; ++j)
     for (int i = 0; i < c.TX; ++i) {
       const size_t l = c.id(i, j, k), lip = c.id(c.xw(i + 1), j, k), lim = c.id(c.xw(i - 1), j, k);
@@ -33,7 +34,8 @@ void orc_source_d(oracle_ctx& c) {
                                  + (vy[l] - vy[lim]) * ilf);
       }
     }
-  for (int j = 1; j + 1 < c.TY; ++j)
+#pragma omp parallel for schedule(static)   // OpenMP build only: cell-independent body
+  for (int j = 1; j < c.TY - 1; ++j)
     for (int i = 0; i < c.TX; ++i) {
       const size_t l = c.id(i, j, k), lip = c.id(c.xw(i + 1), j, k), lim = c.id(c.xw(i - 1), j, k);
       const size_t ljp = c.id(i, j + 1, k), ljm = c.id(i, j - 1, k);

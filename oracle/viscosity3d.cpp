@@ -50,6 +50,7 @@ void orc_source_d3(oracle_ctx& c) {
   const vec &vx = c.vxc, &vy = c.vyc, &vz = c.vzc, &rho = c.rho;
 
   // ---- stress tensor (B1 | B2 | B3) ----------------------------------------------------------------------
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
   for (int k = 0; k < c.TZ; ++k)
     for (int j = 0; j < c.TY; ++j)
       for (int i = 0; i < c.TX; ++i) {
@@ -99,8 +100,9 @@ void orc_source_d3(oracle_ctx& c) {
 
   // ---- force (B4 | B5 | B6), each divided by the face-mean density (G24) -----------------------------------
   c.vxd = c.vxc; c.vyd = c.vyc; c.vzd = c.vzc;   // pass-through where the stencil does not fit
-  for (int k = 1; k + 1 < c.TZ; ++k)
-    for (int j = 1; j + 1 < c.TY; ++j)
+#pragma omp parallel for collapse(2) schedule(static)   // OpenMP build only (liboracle_omp.so): cell-independent body
+  for (int k = 1; k < c.TZ - 1; ++k)
+    for (int j = 1; j < c.TY - 1; ++j)
       for (int i = 0; i < c.TX; ++i) {
         if (!c.xwrap && (i < 1 || i + 1 >= c.TX)) continue;
         const size_t l = c.id(i, j, k), lip = c.id(c.xw(i + 1), j, k), lim = c.id(c.xw(i - 1), j, k);

@@ -67,6 +67,13 @@ typedef struct fargo_mesh {
                               X non-periodic => 3 ghost layers in X too (reading G20) */
 } fargo_mesh;
 
+/* fargo_params.kernel_plan flags */
+enum {
+  FARGO_PLAN_UNFUSED_SOURCE = 1,   /* cells 7a-7c as k_source_a + k_source_b(c) instead of one pass */
+  FARGO_PLAN_UNFUSED_VISC = 2,     /* cell 7d (3-D) as tensor + force kernels instead of one pass */
+  FARGO_PLAN_UNFUSED_DT = 4        /* cell 6 as its own pass instead of being folded into the previous update's last kernel */
+};
+
 typedef struct fargo_params {
   double gamma;            /* adiabatic index (Eq. 7) */
   double cfl;              /* Courant number C of Eq. 59 (0.44) */
@@ -87,6 +94,9 @@ typedef struct fargo_params {
   int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (needs a non-default
                               cuda_stream; on the legacy default stream it falls back to plain launches);
                               0: plain stream launches */
+  int kernel_plan;         /* 0 = the fused kernels wherever they apply (default).  Bit flags select the unfused
+                              sequences instead, for measurements and for tests that compare the two (results are
+                              bit-identical): FARGO_PLAN_UNFUSED_SOURCE, FARGO_PLAN_UNFUSED_VISC, FARGO_PLAN_UNFUSED_DT */
   void* workspace;         /* DEVICE memory, >= fargo_workspace_bytes(), 256-byte aligned; caller-owned */
   size_t workspace_bytes;
   void* cuda_stream;       /* cudaStream_t on which every kernel and copy of this context is enqueued */

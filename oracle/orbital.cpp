@@ -29,7 +29,7 @@ extern "C" void oracle_ppa_interfaces(int n, const double* f, double* fl, double
   }
   for (int i = 0; i < n; ++i) {
     const int ip = wrapi(i + 1, n);
-    const double v = (f[i] + 0.5 * (f[ip] - f[i])) - (dm[ip] - dm[i]) / 6.0;
+    const double v = std::fma(0.5, f[ip] - f[i], f[i]) - (dm[ip] - dm[i]) / 6.0;
     fr[i] = v;
     fl[ip] = v;
   }
@@ -38,10 +38,10 @@ extern "C" void oracle_ppa_interfaces(int n, const double* f, double* fl, double
     const double a = f0 - fm, b = fp - f0;
     if (a * b <= 0.0) { fl[i] = f0; fr[i] = f0; continue; }
     const double D = fr[i] - fl[i];
-    const double C = f0 - 0.5 * (fl[i] + fr[i]);
+    const double C = std::fma(-0.5, fl[i] + fr[i], f0);
     const double DC = D * C, D26 = (D * D) / 6.0;
-    if (DC > D26) fl[i] = 3.0 * f0 - 2.0 * fr[i];
-    else if (-D26 > DC) fr[i] = 3.0 * f0 - 2.0 * fl[i];
+    if (DC > D26) fl[i] = std::fma(3.0, f0, -(2.0 * fr[i]));
+    else if (-D26 > DC) fr[i] = std::fma(3.0, f0, -(2.0 * fl[i]));
   }
 }
 
@@ -56,7 +56,7 @@ extern "C" void oracle_ppa_star(int n, const double* f, double xi, double* fstar
   for (int i = 0; i < n; ++i) {
     const int u = (xi >= 0.0) ? i : wrapi(i + 1, n);   // upwind cell of face i+1/2
     const double edge = (xi >= 0.0) ? fr[u] : fl[u];   // its interface value on that face
-    fstar[i] = (edge + x * (f[u] - edge)) + x1x * ((2.0 * f[u] - fr[u]) - fl[u]);
+    fstar[i] = std::fma(x1x, std::fma(2.0, f[u], -fr[u]) - fl[u], std::fma(x, f[u] - edge, edge));
   }
 }
 
@@ -90,9 +90,9 @@ void orc_orbital_frac(oracle_ctx& c) {
         for (int i = 0; i < n; ++i) f[i] = Qa[base + i] * ir[i];
         oracle_ppa_star(n, f.data(), xi, fs.data());
         for (int i = 0; i < n; ++i) FQ[i] = Fr[i] * fs[i];
-        for (int i = 0; i < n; ++i) Qa[base + i] = Qa[base + i] - g * (FQ[i] - FQ[wrapi(i - 1, n)]);
+        for (int i = 0; i < n; ++i) Qa[base + i] = std::fma(-g, FQ[i] - FQ[wrapi(i - 1, n)], Qa[base + i]);
       }
-      for (int i = 0; i < n; ++i) c.rho[base + i] = r[i] - g * (Fr[i] - Fr[wrapi(i - 1, n)]);
+      for (int i = 0; i < n; ++i) c.rho[base + i] = std::fma(-g, Fr[i] - Fr[wrapi(i - 1, n)], r[i]);
     }
   }
 }

@@ -26,29 +26,29 @@ void orc_source_a(oracle_ctx& c) {
           const double il = c.invLX(j, k);
           const double wf = (2.0 * il) / (c.rho[l] + c.rho[lm]);
           double acc = wf * (pressure(c, l) - pressure(c, lm));
-          if (c.has_pot) acc = acc + (c.phi[l] - c.phi[lm]) * il;
-          vxb = c.vx[l] - dt * acc;
+          if (c.has_pot) acc = std::fma(c.phi[l] - c.phi[lm], il, acc);
+          vxb = std::fma(-dt, acc, c.vx[l]);
         }
         if (c.hasy && j >= 1 && (!curv || ipok) && (!(sph && c.hasz) || k + 1 < c.TZ)) {
           const size_t lm = c.id(i, j - 1, k);
           const double il = c.invDY[j];
           const double wf = (2.0 * il) / (c.rho[l] + c.rho[lm]);
           double acc = wf * (pressure(c, l) - pressure(c, lm));
-          if (c.has_pot) acc = acc + (c.phi[l] - c.phi[lm]) * il;
-          vyb = c.vy[l] - dt * acc;
+          if (c.has_pot) acc = std::fma(c.phi[l] - c.phi[lm], il, acc);
+          vyb = std::fma(-dt, acc, c.vy[l]);
           if (curv) {   // Eq. 38: average the velocities, add the frame term, then square (G27)
-            const double vphi = 0.25 * (((c.vx[l] + c.vx[c.id(ip, j, k)]) + c.vx[lm]) + c.vx[c.id(ip, j - 1, k)])
-                                + om * (c.ye[j] * c.Rxk[k]);
+            const double vphi = std::fma(0.25, ((c.vx[l] + c.vx[c.id(ip, j, k)]) + c.vx[lm]) + c.vx[c.id(ip, j - 1, k)],
+                                         om * (c.ye[j] * c.Rxk[k]));
             double G = vphi * vphi;
             if (sph && c.hasz) {   // Eq. 36: + v_theta^2
               const double vth = 0.25 * (((c.vz[l] + c.vz[c.id(i, j, k + 1)]) + c.vz[lm]) + c.vz[c.id(i, j - 1, k + 1)]);
-              G = G + vth * vth;
+              G = std::fma(vth, vth, G);
             }
-            vyb = vyb + dt * (G * c.inv_ye[j]);
+            vyb = std::fma(dt, G * c.inv_ye[j], vyb);
           }
           if (c.shear) {   // Eq. 29: + 2 Omega_f v_x - 4 A Omega_f y at the Y face; v_x averaged as in Eq. 38 (G32)
             const double vxa = 0.25 * (((c.vx[l] + c.vx[c.id(ip, j, k)]) + c.vx[lm]) + c.vx[c.id(ip, j - 1, k)]);
-            vyb = vyb + dt * ((2.0 * om) * vxa - ((4.0 * c.p.oort_a) * om) * c.ye[j]);
+            vyb = std::fma(dt, std::fma(2.0 * om, vxa, -(((4.0 * c.p.oort_a) * om) * c.ye[j])), vyb);
           }
         }
         if (c.hasz && k >= 1 && (!sph || ipok)) {
@@ -56,12 +56,12 @@ void orc_source_a(oracle_ctx& c) {
           const double il = c.invDZ(j, k);
           const double wf = (2.0 * il) / (c.rho[l] + c.rho[lm]);
           double acc = wf * (pressure(c, l) - pressure(c, lm));
-          if (c.has_pot) acc = acc + (c.phi[l] - c.phi[lm]) * il;
-          vzb = c.vz[l] - dt * acc;
+          if (c.has_pot) acc = std::fma(c.phi[l] - c.phi[lm], il, acc);
+          vzb = std::fma(-dt, acc, c.vz[l]);
           if (sph) {   // Eq. 37: (v_phi^t)^2 cot(theta) / r at the theta face
-            const double vphi = 0.25 * (((c.vx[l] + c.vx[c.id(ip, j, k)]) + c.vx[lm]) + c.vx[c.id(ip, j, k - 1)])
-                                + om * (c.yc[j] * c.sin_ze[k]);
-            vzb = vzb + dt * (((vphi * vphi) * c.cot_ze[k]) * c.inv_yc[j]);
+            const double vphi = std::fma(0.25, ((c.vx[l] + c.vx[c.id(ip, j, k)]) + c.vx[lm]) + c.vx[c.id(ip, j, k - 1)],
+                                         om * (c.yc[j] * c.sin_ze[k]));
+            vzb = std::fma(dt, ((vphi * vphi) * c.cot_ze[k]) * c.inv_yc[j], vzb);
           }
         }
         c.vxb[l] = vxb; c.vyb[l] = vyb; c.vzb[l] = vzb;
@@ -100,23 +100,26 @@ void orc_source_b(oracle_ctx& c) {
         if (c.hasx && (c.xwrap || i >= 1)) {
           const size_t lm = c.id(c.xw(i - 1), j, k);
           const double wf = (2.0 * c.invLX(j, k)) / (c.rho[l] + c.rho[lm]);
-          vxc = c.vxb[l] - dt * (wf * (qx[l] - qx[lm]));
+          vxc = std::fma(-dt, wf * (qx[l] - qx[lm]), c.vxb[l]);
         }
         if (c.hasy && j >= 1) {
           const size_t lm = c.id(i, j - 1, k);
           const double wf = (2.0 * c.invDY[j]) / (c.rho[l] + c.rho[lm]);
-          vyc = c.vyb[l] - dt * (wf * (qy[l] - qy[lm]));
+          vyc = std::fma(-dt, wf * (qy[l] - qy[lm]), c.vyb[l]);
         }
         if (c.hasz && k >= 1) {
           const size_t lm = c.id(i, j, k - 1);
           const double wf = (2.0 * c.invDZ(j, k)) / (c.rho[l] + c.rho[lm]);
-          vzc = c.vzb[l] - dt * (wf * (qz[l] - qz[lm]));
+          vzc = std::fma(-dt, wf * (qz[l] - qz[lm]), c.vzb[l]);
         }
         c.vxc[l] = vxc; c.vyc[l] = vyc; c.vzc[l] = vzc;
         double ec = c.e[l];
-        if (c.eos == ORC_ADIABATIC)   // heating -q_d dv_d / Delta_d, same dv as in q (G19)
-          ec = c.e[l] - dt * (((qx[l] * dvx[l]) * c.invLX(j, k) + (qy[l] * dvy[l]) * c.invLY[j])
-                              + (qz[l] * dvz[l]) * c.invLZ(j, k));
+        if (c.eos == ORC_ADIABATIC) {   // heating -q_d dv_d / Delta_d, same dv as in q (G19)
+          double h = (qx[l] * dvx[l]) * c.invLX(j, k);
+          h = std::fma(qy[l] * dvy[l], c.invLY[j], h);
+          h = std::fma(qz[l] * dvz[l], c.invLZ(j, k), h);
+          ec = std::fma(-dt, h, c.e[l]);
+        }
         c.ec[l] = ec;
       }
 }
@@ -134,8 +137,8 @@ void orc_source_c(oracle_ctx& c) {
         if (c.eos == ORC_ADIABATIC && ok) {
           double tx = 0.0, ty = 0.0, tz = 0.0;
           if (c.hasx) tx = (c.vxc[c.id(c.xw(i + 1), j, k)] - c.vxc[l]) * c.Sx(j, k);
-          if (c.hasy) ty = c.vyc[c.id(i, j + 1, k)] * c.Sy(j + 1, k) - c.vyc[l] * c.Sy(j, k);
-          if (c.hasz) tz = c.vzc[c.id(i, j, k + 1)] * c.Sz(j, k + 1) - c.vzc[l] * c.Sz(j, k);
+          if (c.hasy) ty = std::fma(c.vyc[c.id(i, j + 1, k)], c.Sy(j + 1, k), -(c.vyc[l] * c.Sy(j, k)));
+          if (c.hasz) tz = std::fma(c.vzc[c.id(i, j, k + 1)], c.Sz(j, k + 1), -(c.vzc[l] * c.Sz(j, k)));
           const double D = c.invV(j, k) * ((tx + ty) + tz);
           const double a = hd * D;
           ed = (c.ec[l] * (1.0 - a)) / (1.0 + a);

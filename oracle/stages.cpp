@@ -124,7 +124,7 @@ double orc_compute_dt(oracle_ctx& c, bool* clipped) {
         double I2 = 0.0, I3 = 0.0;
         if (c.hasx) {
           const double a = c.vx[l], b = c.vx[c.id(c.xw(i + 1), j, k)];
-          I2 = std::max(I2, std::fabs(0.5 * (a + b) - v0) * ilx);
+          I2 = std::max(I2, std::fabs(std::fma(0.5, a + b, -v0)) * ilx);
           I3 = std::max(I3, std::fabs(b - a) * ilx);
         }
         if (c.hasy) {
@@ -139,7 +139,7 @@ double orc_compute_dt(oracle_ctx& c, bool* clipped) {
         }
         I3 = c3 * I3;
         const double I4 = c4 * (ilmax * ilmax);
-        const double Isq = ((I1sq + I2 * I2) + I3 * I3) + I4 * I4;
+        const double Isq = std::fma(I4, I4, std::fma(I3, I3, std::fma(I2, I2, I1sq)));
         M2 = std::max(M2, Isq);
       }
     }

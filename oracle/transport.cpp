@@ -23,8 +23,8 @@ extern "C" void oracle_vanleer_star(int n, const double* f, const double* a, con
                                     double dt, double* fstar) {
   fstar[0] = f[0];
   for (int m = 1; m < n; ++m)
-    fstar[m] = (w[m] >= 0.0) ? f[m - 1] + a[m - 1] * ((len[m - 1] - w[m] * dt) * 0.5)
-                             : f[m] - a[m] * ((len[m] + w[m] * dt) * 0.5);
+    fstar[m] = (w[m] >= 0.0) ? std::fma(a[m - 1], std::fma(-w[m], dt, len[m - 1]) * 0.5, f[m - 1])
+                             : std::fma(-a[m], std::fma(w[m], dt, len[m]) * 0.5, f[m]);
 }
 
 // ---- 12a: left / right momenta with the quantities of Tab. 2 -----------------------
@@ -42,8 +42,8 @@ void orc_momenta(oracle_ctx& c) {
         const double vxp = (c.hasx && ipok) ? c.vx[c.id(c.xw(i + 1), j, k)] : c.vx[l];
         const double vyp = (c.hasy && j + 1 < c.TY) ? c.vy[c.id(i, j + 1, k)] : c.vy[l];
         const double vzp = (c.hasz && k + 1 < c.TZ) ? c.vz[c.id(i, j, k + 1)] : c.vz[l];
-        c.pxm[l] = r * (rx * c.vx[l] + rx2om);
-        c.pxp[l] = r * (rx * vxp + rx2om);
+        c.pxm[l] = r * std::fma(rx, c.vx[l], rx2om);
+        c.pxp[l] = r * std::fma(rx, vxp, rx2om);
         c.pym[l] = r * c.vy[l];
         c.pyp[l] = r * vyp;
         c.pzm[l] = r * (rz * c.vz[l]);
@@ -104,9 +104,9 @@ void orc_sweep(oracle_ctx& c, int dir) {
         oracle_vanleer_slopes(n, f.data(), invd.data(), a.data());
         oracle_vanleer_star(n, f.data(), a.data(), len.data(), w.data(), dt, fs.data());
         for (int m = 0; m < n; ++m) FQ[m] = Fr[m] * fs[m];
-        for (int m = 2; m + 2 < n; ++m) Qa[L(m)] = Qa[L(m)] - dtiv[m] * (FQ[m + 1] - FQ[m]);
+        for (int m = 2; m + 2 < n; ++m) Qa[L(m)] = std::fma(-dtiv[m], FQ[m + 1] - FQ[m], Qa[L(m)]);
       }
-      for (int m = 2; m + 2 < n; ++m) c.rho[L(m)] = r[m] - dtiv[m] * (Fr[m + 1] - Fr[m]);
+      for (int m = 2; m + 2 < n; ++m) c.rho[L(m)] = std::fma(-dtiv[m], Fr[m + 1] - Fr[m], r[m]);
     }
   }
 }

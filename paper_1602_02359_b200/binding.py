@@ -40,9 +40,11 @@ class FargoParams(C.Structure):
                 ("planet_r", C.c_double), ("planet_phi0", C.c_double), ("planet_omega", C.c_double),
                 ("planet_eps", C.c_double),
                 ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double), ("oort_a", C.c_double),
-                ("precision", C.c_int), ("use_graph", C.c_int),
+                ("precision", C.c_int), ("use_graph", C.c_int), ("kernel_plan", C.c_int),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p)]
 
+
+PLAN_UNFUSED_SOURCE, PLAN_UNFUSED_VISC, PLAN_UNFUSED_DT = 1, 2, 4   # fargo_params.kernel_plan flags (include/fargo.h)
 
 _lib = None
 
@@ -108,7 +110,7 @@ class Fargo:
     """
 
     def __init__(self, mesh, geometry: int, eos: int, params, precision: int = 64, use_graph: bool = True,
-                 device: Optional[str] = None):
+                 device: Optional[str] = None, kernel_plan: int = 0):
         import torch
         L = load()
         if not torch.cuda.is_available():
@@ -143,18 +145,20 @@ class Fargo:
             setattr(p, name, getattr(params, name))
         p.precision = precision
         p.use_graph = 1 if use_graph else 0
+        p.kernel_plan = int(kernel_plan)   # PLAN_* flags: the unfused kernel sequences (measurements, tests)
         nbytes = L.fargo_workspace_bytes(C.byref(m), geometry, eos, C.byref(p))
         if nbytes == 0:
             raise ValueError("fargo_workspace_bytes rejected the mesh / parameters")
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            base = self.workspace.data_ptr()
-            off = (-base) % 256
             self.stream = torch.cuda.current_stream(self.device)
             if self.stream.cuda_stream == 0:
                 # the legacy default stream cannot be captured into a CUDA graph: give the context its own
                 self.stream = torch.cuda.Stream(self.device)
                 torch.cuda.current_stream(self.device).synchronize()
+            with torch.cuda.stream(self.stream):   # the caching allocator ties the block to the stream that uses it
+                self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            off = (-base) % 256
             p.workspace = base + off
             p.workspace_bytes = nbytes
             p.cuda_stream = self.stream.cuda_stream
@@ -173,6 +177,7 @@ class Fargo:
     # -- lifetime ------------------------------------------------------------------------------
     def close(self):
         if getattr(self, "_h", None):
+            self.stream.synchronize()   # queued kernels still use the workspace
             load().fargo_destroy(self._h)
             self._h = None
             self.workspace = None

@@ -141,6 +141,7 @@ struct Sim : CtxBase {
   int nq = 0, slots[8];
 
   ~Sim() override {
+    cudaStreamSynchronize(stream);   // nothing of this context may still be running when the caller frees the workspace
     if (gexec) cudaGraphExecDestroy(gexec);
     for (auto& sp : spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   }
@@ -321,9 +322,9 @@ struct Sim : CtxBase {
     if (L.hasz) { slots[nq++] = 5; slots[nq++] = 6; }
     sweep_setup<T>();
     // with viscosity the fused pass must be followed by the fused 7d (it then also produces the ghost layer 7d reads)
-    fuse_visc = L.visc3d && source_d3_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_VISC");   // measurement switch
-    fuse_source = source_fused_ok<T>(d) && !getenv("FARGO_UNFUSED_SOURCE") && (!L.visc || fuse_visc);
-    fuse_dt = newvel_dt_ok<T>(d) && !getenv("FARGO_UNFUSED_DT");
+    fuse_visc = L.visc3d && source_d3_fused_ok<T>(d) && !(p->kernel_plan & FARGO_PLAN_UNFUSED_VISC);
+    fuse_source = source_fused_ok<T>(d) && !(p->kernel_plan & FARGO_PLAN_UNFUSED_SOURCE) && (!L.visc || fuse_visc);
+    fuse_dt = newvel_dt_ok<T>(d) && !(p->kernel_plan & FARGO_PLAN_UNFUSED_DT);
     return FARGO_OK;
   }
 
@@ -707,8 +708,10 @@ struct Sim : CtxBase {
       dt_ready = true;
     }
     if (graph_ok) {
+      // the static potential stays out of the graph: written once after every fargo_set_fields (which clears it),
+      // also when the graph already exists
+      if (L.has_pot && !pot_valid && npl == 0) { launches += potential(0.0); pot_valid = true; }
       if (!gexec) {
-        if (L.has_pot && !pot_valid && npl == 0) { launches += potential(0.0); pot_valid = true; }   // keep it out of the graph
         cudaGraph_t g = nullptr;
         if (!ck(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal), "begin capture")) return FARGO_ECUDA;
         launches_per_step = enqueue_update(-1, true);

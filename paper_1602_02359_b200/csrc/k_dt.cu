@@ -80,7 +80,6 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
     if (d.hasz) ilmax = rmax(ilmax, ilz);
     const T il2 = ilmax * ilmax;
     const T I4 = d.c4 * il2;
-    const T I4sq = I4 * I4;
     const T vm = v0 ? v0[d.rid(j, k)] : T(0);
     for (int ia = threadIdx.x; ia < d.nx; ia += blockDim.x) {
       const int i = d.ngx + ia;
@@ -90,7 +89,7 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
       T I2 = T(0), I3 = T(0);
       if (d.hasx) {
         const T a = st.vx[l], b = st.vx[d.id(d.xw(i + 1), j, k)];
-        I2 = rmax(I2, rabs(T(0.5) * (a + b) - vm) * ilx);
+        I2 = rmax(I2, rabs(rfma(T(0.5), a + b, -vm)) * ilx);
         I3 = rmax(I3, rabs(b - a) * ilx);
       }
       if (d.hasy) {
@@ -104,7 +103,7 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
         I3 = rmax(I3, rabs(b - a) * ilz);
       }
       I3 = d.c3 * I3;
-      const T Isq = ((I1sq + I2 * I2) + I3 * I3) + I4sq;
+      const T Isq = rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq)));
       m2 = rmax(m2, Isq);
     }
   }
@@ -143,7 +142,6 @@ __global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T
     const T ilmax = rmax(rmax(rmax(T(0), ilx), ily), ilz);
     const T il2 = ilmax * ilmax;
     const T I4 = d.c4 * il2;
-    const T I4sq = I4 * I4;
     const T vm = v0 ? v0[d.rid(j, k)] : T(0);
     const long long base = d.id(0, j, k);
     for (int i0 = 0; i0 < nx; i0 += 64) {
@@ -167,7 +165,7 @@ __global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T
         T I2 = T(0), I3 = T(0);
         {
           const T a = c ? ax.y : ax.x, b = c ? nxt : ax.y;
-          I2 = rmax(I2, rabs(T(0.5) * (a + b) - vm) * ilx);
+          I2 = rmax(I2, rabs(rfma(T(0.5), a + b, -vm)) * ilx);
           I3 = rmax(I3, rabs(b - a) * ilx);
         }
         {
@@ -181,7 +179,7 @@ __global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T
           I3 = rmax(I3, rabs(b - a) * ilz);
         }
         I3 = d.c3 * I3;
-        const T Isq = ((I1sq + I2 * I2) + I3 * I3) + I4sq;
+        const T Isq = rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq)));
         if (live) m2 = rmax(m2, Isq);
       }
     }

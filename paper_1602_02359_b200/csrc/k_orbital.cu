@@ -33,17 +33,17 @@ __device__ __forceinline__ T ppa_star_upper(const T f, const int tm, const bool 
   s_dm[tm] = dm;
   __syncthreads();
   T fr = f;
-  if (tm < OBM - 1) fr = (f + T(0.5) * (s_f[tm + 1] - f)) - rdiv(s_dm[tm + 1] - dm, T(6));   // Eq. 71
+  if (tm < OBM - 1) fr = rfma(T(0.5), s_f[tm + 1] - f, f) - rdiv(s_dm[tm + 1] - dm, T(6));   // Eq. 71
   s_fu[tm] = fr;
   __syncthreads();
   T fl = tm >= 1 ? s_fu[tm - 1] : f;
   if (a * b <= T(0)) { fl = f; fr = f; }   // the three mutually exclusive tests of P:484
   else {
     const T D = fr - fl;
-    const T C = f - T(0.5) * (fl + fr);
+    const T C = rfma(T(-0.5), fl + fr, f);
     const T DC = D * C, D26 = rdiv(D * D, T(6));
-    if (DC > D26) fl = T(3) * f - T(2) * fr;
-    else if (-D26 > DC) fr = T(3) * f - T(2) * fl;
+    if (DC > D26) fl = rfma(T(3), f, -(T(2) * fr));
+    else if (-D26 > DC) fr = rfma(T(3), f, -(T(2) * fl));
   }
   s_fl[tm] = fl; s_fr[tm] = fr;
   __syncthreads();
@@ -51,7 +51,7 @@ __device__ __forceinline__ T ppa_star_upper(const T f, const int tm, const bool 
   const int u = fwd ? tm : (tm + 1 < OBM ? tm + 1 : tm);
   const T fu = s_f[u], flu = s_fl[u], fru = s_fr[u];
   const T edge = fwd ? fru : flu;
-  return (edge + x * (fu - edge)) + x1x * ((T(2) * fu - fru) - flu);
+  return rfma(x1x, rfma(T(2), fu, -fru) - flu, rfma(x, fu - edge, edge));
 }
 
 template <typename T>
@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(OBM) k_orbital(const Dev<T> d, const SweepArgs
   const T Fr = xi * rs;   // mass through face i+1/2 per unit of (LX Sx)
   s_F[tm] = Fr;
   __syncthreads();
-  if (inner) A.drho[lo] = r0 - g * (Fr - s_F[tm - 1]);
+  if (inner) A.drho[lo] = rfma(-g, Fr - s_F[tm - 1], r0);
 
 #pragma unroll
   for (int q = 0; q < 7; ++q) {
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(OBM) k_orbital(const Dev<T> d, const SweepArgs
     const T FQ = Fr * fs;
     s_F[tm] = FQ;
     __syncthreads();
-    if (inner) A.dq[q][lo] = Q - g * (FQ - s_F[tm - 1]);
+    if (inner) A.dq[q][lo] = rfma(-g, FQ - s_F[tm - 1], Q);
   }
 }
 
@@ -131,9 +131,9 @@ __device__ __forceinline__ T ppa_mono(const T fm, const T f, const T fp, bool& f
 template <typename T>
 __device__ __forceinline__ void ppa_limit(const T f, const bool flat, T& fl, T& fr) {   // the three tests of P:484
   const T D = fr - fl;
-  const T C = f - T(0.5) * (fl + fr);
+  const T C = rfma(T(-0.5), fl + fr, f);
   const T DC = D * C, D26 = rdiv6(D * D);
-  const T fl2 = T(3) * f - T(2) * fr, fr2 = T(3) * f - T(2) * fl;
+  const T fl2 = rfma(T(3), f, -(T(2) * fr)), fr2 = rfma(T(3), f, -(T(2) * fl));
   const bool c1 = DC > D26, c2 = -D26 > DC;
   const T ol = flat ? f : (c1 ? fl2 : fl);
   const T orr = flat ? f : (c1 ? fr : (c2 ? fr2 : fr));
@@ -151,18 +151,18 @@ __device__ __forceinline__ void ppa_pair(const T fA, const T fB, const T x, cons
   bool flatA, flatB;
   const T dmA = ppa_mono(fm, fA, fB, flatA), dmB = ppa_mono(fA, fB, fn, flatB);
   const T dmn = o_dn1(dmA);
-  const T fuA = (fA + T(0.5) * (fB - fA)) - rdiv6(dmB - dmA);   // Eq. 71, un-limited
-  const T fuB = (fB + T(0.5) * (fn - fB)) - rdiv6(dmn - dmB);
+  const T fuA = rfma(T(0.5), fB - fA, fA) - rdiv6(dmB - dmA);   // Eq. 71, un-limited
+  const T fuB = rfma(T(0.5), fn - fB, fB) - rdiv6(dmn - dmB);
   T flA = o_up1(fuB), frA = fuA, flB = fuA, frB = fuB;
   ppa_limit(fA, flatA, flA, frA);
   ppa_limit(fB, flatB, flB, frB);
   if (FWD) {
-    sA = (frA + x * (fA - frA)) + x1x * ((T(2) * fA - frA) - flA);
-    sB = (frB + x * (fB - frB)) + x1x * ((T(2) * fB - frB) - flB);
+    sA = rfma(x1x, rfma(T(2), fA, -frA) - flA, rfma(x, fA - frA, frA));
+    sB = rfma(x1x, rfma(T(2), fB, -frB) - flB, rfma(x, fB - frB, frB));
   } else {
     const T fln = o_dn1(flA), frn = o_dn1(frA);
-    sA = (flB + x * (fB - flB)) + x1x * ((T(2) * fB - frB) - flB);
-    sB = (fln + x * (fn - fln)) + x1x * ((T(2) * fn - frn) - fln);
+    sA = rfma(x1x, rfma(T(2), fB, -frB) - flB, rfma(x, fB - flB, flB));
+    sB = rfma(x1x, rfma(T(2), fn, -frn) - fln, rfma(x, fn - fln, fln));
   }
 }
 
@@ -177,7 +177,7 @@ __device__ __forceinline__ void orbital2_body(const SweepArgs<T>& A, const typen
   const T FrA = xi * sA, FrB = xi * sB;   // mass through the upper face per unit of (LX Sx)
   {
     const T Fm = o_up1(FrB);
-    const T oA = r2.x - g * (FrA - Fm), oB = r2.y - g * (FrB - FrA);
+    const T oA = rfma(-g, FrA - Fm, r2.x), oB = rfma(-g, FrB - FrA, r2.y);
     st2_if(A.drho + row + io, oA, oB, vec && stB);
     st_if(A.drho + row + io, oA, stA && !(vec && stB));
     st_if(A.drho + row + io1, oB, stB && !vec);
@@ -187,7 +187,7 @@ __device__ __forceinline__ void orbital2_body(const SweepArgs<T>& A, const typen
     ppa_pair<T, FWD>(Q2[q].x * irA, Q2[q].y * irB, x, x1x, sA, sB);
     const T FA = FrA * sA, FB = FrB * sB;
     const T Fm = o_up1(FB);
-    const T oA = Q2[q].x - g * (FA - Fm), oB = Q2[q].y - g * (FB - FA);
+    const T oA = rfma(-g, FA - Fm, Q2[q].x), oB = rfma(-g, FB - FA, Q2[q].y);
     st2_if(A.dq[q] + row + io, oA, oB, vec && stB);
     st_if(A.dq[q] + row + io, oA, stA && !(vec && stB));
     st_if(A.dq[q] + row + io1, oB, stB && !vec);

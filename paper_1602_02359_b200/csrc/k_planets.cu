@@ -253,7 +253,7 @@ __global__ void __launch_bounds__(32 * PFW) k_diagnostics(const Dev<T> d, const 
       if (d.hasx) {
         const T v = st.vx[l];
         const T vp = (d.xwrap || i + 1 < d.TX) ? st.vx[d.id(d.xw(i + 1), j, k)] : v;
-        px = px + (T(0.5) * (r0 * (rx * v + rx2om) + r0 * (rx * vp + rx2om))) * vol;
+        px = px + (T(0.5) * (r0 * rfma(rx, v, rx2om) + r0 * rfma(rx, vp, rx2om))) * vol;
       }
       if (d.hasy) {
         const T v = st.vy[l];

@@ -40,8 +40,8 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
       const T il = d.invLX(j, k);
       const T wf = rdiv(T(2) * il, r0 + rho[lm]);
       T acc = wf * (p0 - pressure(d, rho, e, lm));
-      if (d.has_pot) acc = acc + (f0 - phi[lm]) * il;
-      v = vx[l] - dt * acc;
+      if (d.has_pot) acc = rfma(f0 - phi[lm], il, acc);
+      v = rfma(-dt, acc, vx[l]);
     }
     vxb[l] = v;
   }
@@ -52,22 +52,22 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
       const T il = d.invDY[j];
       const T wf = rdiv(T(2) * il, r0 + rho[lm]);
       T acc = wf * (p0 - pressure(d, rho, e, lm));
-      if (d.has_pot) acc = acc + (f0 - phi[lm]) * il;
-      v = vy[l] - dt * acc;
+      if (d.has_pot) acc = rfma(f0 - phi[lm], il, acc);
+      v = rfma(-dt, acc, vy[l]);
       if (curv) {   // Eq. 38: average the velocities, add the frame term, square (reading G27)
         const long long lp = d.id(ip, j, k);
-        const T vphi = T(0.25) * (((vx[l] + vx[lp]) + vx[lm]) + vx[lp - d.pitch]) + om * (d.ye[j] * d.Rxk[k]);
+        const T vphi = rfma(T(0.25), ((vx[l] + vx[lp]) + vx[lm]) + vx[lp - d.pitch], om * (d.ye[j] * d.Rxk[k]));
         T G = vphi * vphi;
         if (sph && d.hasz) {   // Eq. 36: + v_theta^2
           const T vth = T(0.25) * (((vz[l] + vz[l + d.plane]) + vz[lm]) + vz[lm + d.plane]);
-          G = G + vth * vth;
+          G = rfma(vth, vth, G);
         }
-        v = v + dt * (G * d.inv_ye[j]);
+        v = rfma(dt, G * d.inv_ye[j], v);
       }
       if (d.shear) {   // Eq. 29: + 2 Omega_f v_x - 4 A Omega_f y on the Y face, v_x averaged as in Eq. 38 (G32)
         const long long lp = d.id(ip, j, k);
         const T vxa = T(0.25) * (((vx[l] + vx[lp]) + vx[lm]) + vx[lp - d.pitch]);
-        v = v + dt * (d.two_om * vxa - d.four_a_om * d.ye[j]);
+        v = rfma(dt, rfma(d.two_om, vxa, -(d.four_a_om * d.ye[j])), v);
       }
     }
     vyb[l] = v;
@@ -79,12 +79,12 @@ __global__ void __launch_bounds__(128) k_source_a(const Dev<T> d, const State<T>
       const T il = d.invDZ(j, k);
       const T wf = rdiv(T(2) * il, r0 + rho[lm]);
       T acc = wf * (p0 - pressure(d, rho, e, lm));
-      if (d.has_pot) acc = acc + (f0 - phi[lm]) * il;
-      v = vz[l] - dt * acc;
+      if (d.has_pot) acc = rfma(f0 - phi[lm], il, acc);
+      v = rfma(-dt, acc, vz[l]);
       if (sph) {   // Eq. 37: (v_phi^t)^2 cot(theta) / r on the theta face
         const long long lp = d.id(ip, j, k);
-        const T vphi = T(0.25) * (((vx[l] + vx[lp]) + vx[lm]) + vx[lp - d.plane]) + om * (d.yc[j] * d.sin_ze[k]);
-        v = v + dt * (((vphi * vphi) * d.cot_ze[k]) * d.inv_yc[j]);
+        const T vphi = rfma(T(0.25), ((vx[l] + vx[lp]) + vx[lm]) + vx[lp - d.plane], om * (d.yc[j] * d.sin_ze[k]));
+        v = rfma(dt, ((vphi * vphi) * d.cot_ze[k]) * d.inv_yc[j], v);
       }
     }
     vzb[l] = v;
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(128) k_source_b(const Dev<T> d, const State<T>
       const T rm = rho[lm];
       const T qm = qvisc(cq2, rm, v0 - vxb[lm]);   // q of the lower neighbour: its dv = v0 - vb[lm]
       const T wf = rdiv(T(2) * d.invLX(j, k), r0 + rm);
-      v = v0 - dt * (wf * (q - qm));
+      v = rfma(-dt, wf * (q - qm), v0);
     }
     vxc[l] = v;
     heat = (q * dv) * d.invLX(j, k);
@@ -144,12 +144,10 @@ __global__ void __launch_bounds__(128) k_source_b(const Dev<T> d, const State<T>
       const T rm = rho[lm];
       const T qm = qvisc(cq2, rm, v0 - vyb[lm]);
       const T wf = rdiv(T(2) * d.invDY[j], r0 + rm);
-      v = v0 - dt * (wf * (q - qm));
+      v = rfma(-dt, wf * (q - qm), v0);
     }
     vyc[l] = v;
-    heat = heat + (q * dv) * d.invLY[j];
-  } else {
-    heat = heat + T(0);
+    heat = rfma(q * dv, d.invLY[j], heat);
   }
   if (d.hasz) {
     const T v0 = vzb[l];
@@ -161,12 +159,12 @@ __global__ void __launch_bounds__(128) k_source_b(const Dev<T> d, const State<T>
       const T rm = rho[lm];
       const T qm = qvisc(cq2, rm, v0 - vzb[lm]);
       const T wf = rdiv(T(2) * d.invDZ(j, k), r0 + rm);
-      v = v0 - dt * (wf * (q - qm));
+      v = rfma(-dt, wf * (q - qm), v0);
     }
     vzc[l] = v;
-    heat = heat + (q * dv) * d.invLZ(j, k);
+    heat = rfma(q * dv, d.invLZ(j, k), heat);
   }
-  if (d.eos == EOS_ADI) ec[l] = st.e[l] - dt * heat;   // heating -q_d dv_d / Delta_d (G19)
+  if (d.eos == EOS_ADI) ec[l] = rfma(-dt, heat, st.e[l]);   // heating -q_d dv_d / Delta_d (G19)
 }
 
 template <typename T>
@@ -192,8 +190,8 @@ __global__ void __launch_bounds__(128) k_source_c(const Dev<T> d, const T* __res
   if (ok) {
     T tx = T(0), ty = T(0), tz = T(0);
     if (d.hasx) tx = (vxc[d.id(d.xw(i + 1), j, k)] - vxc[l]) * d.Sx(j, k);
-    if (d.hasy) ty = vyc[l + d.pitch] * d.Sy(j + 1, k) - vyc[l] * d.Sy(j, k);
-    if (d.hasz) tz = vzc[l + d.plane] * d.Sz(j, k + 1) - vzc[l] * d.Sz(j, k);
+    if (d.hasy) ty = rfma(vyc[l + d.pitch], d.Sy(j + 1, k), -(vyc[l] * d.Sy(j, k)));
+    if (d.hasz) tz = rfma(vzc[l + d.plane], d.Sz(j, k + 1), -(vzc[l] * d.Sz(j, k)));
     const T D = d.invV(j, k) * ((tx + ty) + tz);
     const T a = hd * D;
     v = rdiv(ec[l] * (T(1) - a), T(1) + a);
@@ -215,15 +213,14 @@ int launch_source_c(const Dev<T>& d, const T* vxc, const T* vyc, const T* vzc, c
 // re-reading v_c (9 reals per cell instead of 14).  Every expression is the one k_source_b / k_source_c
 // evaluate for the same face, so the results are bit-identical to the two-kernel sequence.
 template <typename T>
-struct FaceBC { T vc0, vc1, heat; };   // v_c on the lower and upper face of the cell, q dv / L of the cell
+struct FaceBC { T vc0, vc1, qdv; };   // v_c on the lower and upper face of the cell, q dv of the cell
 
 // one direction: vb[] = v_b at m-1, m, m+1, m+2; rr[] = rho at m-1, m, m+1; have* say which exist;
-// il0 / il1 = inverse centre distance across the lower / upper face; ilc = inverse cell width
+// il0 / il1 = inverse centre distance across the lower / upper face
 template <typename T>
 __device__ __forceinline__ FaceBC<T> face_bc(const T cq2, const T dt, const T vbm, const T vb0, const T vb1,
                                              const T vb2, const T rm, const T r0, const T r1, const bool has_m,
-                                             const bool has_1, const bool has_2, const T il0, const T il1,
-                                             const T ilc) {
+                                             const bool has_1, const bool has_2, const T il0, const T il1) {
   FaceBC<T> o;
   T dv = T(0), q = T(0);
   if (has_1) { dv = vb1 - vb0; q = qvisc(cq2, r0, dv); }
@@ -231,16 +228,16 @@ __device__ __forceinline__ FaceBC<T> face_bc(const T cq2, const T dt, const T vb
   if (has_m) {
     const T qm = qvisc(cq2, rm, vb0 - vbm);
     const T wf = rdiv(T(2) * il0, r0 + rm);
-    o.vc0 = vb0 - dt * (wf * (q - qm));
+    o.vc0 = rfma(-dt, wf * (q - qm), vb0);
   }
   o.vc1 = vb1;
   if (has_1) {   // the upper face: what k_source_b computes at the upper neighbour
     T q1 = T(0);
     if (has_2) q1 = qvisc(cq2, r1, vb2 - vb1);
     const T wf = rdiv(T(2) * il1, r1 + r0);
-    o.vc1 = vb1 - dt * (wf * (q1 - q));
+    o.vc1 = rfma(-dt, wf * (q1 - q), vb1);
   }
-  o.heat = (q * dv) * ilc;
+  o.qdv = q * dv;
   return o;
 }
 
@@ -265,9 +262,9 @@ __global__ void __launch_bounds__(128) k_source_bc(const Dev<T> d, const State<T
     const long long lm = row + d.xw(i - 1), l1 = row + d.xw(i + 1), l2 = row + d.xw(i + 2);
     const T il = d.invLX(j, k);
     const FaceBC<T> f = face_bc<T>(cq2, dt, hm ? vxb[lm] : T(0), vxb[l], h1 ? vxb[l1] : T(0), h2 ? vxb[l2] : T(0),
-                                   hm ? rho[lm] : T(0), r0, h1 ? rho[l1] : T(0), hm, h1, h2, il, il, il);
+                                   hm ? rho[lm] : T(0), r0, h1 ? rho[l1] : T(0), hm, h1, h2, il, il);
     vxc[l] = f.vc0;
-    heat = f.heat;
+    heat = f.qdv * il;
     ok = ok && h1;
     tx = (f.vc1 - f.vc0) * d.Sx(j, k);
   }
@@ -276,26 +273,24 @@ __global__ void __launch_bounds__(128) k_source_bc(const Dev<T> d, const State<T
     const long long p = d.pitch;
     const FaceBC<T> f = face_bc<T>(cq2, dt, hm ? vyb[l - p] : T(0), vyb[l], h1 ? vyb[l + p] : T(0),
                                    h2 ? vyb[l + 2 * p] : T(0), hm ? rho[l - p] : T(0), r0, h1 ? rho[l + p] : T(0), hm,
-                                   h1, h2, d.invDY[j], h1 ? d.invDY[j + 1] : T(0), d.invLY[j]);
+                                   h1, h2, d.invDY[j], h1 ? d.invDY[j + 1] : T(0));
     vyc[l] = f.vc0;
-    heat = heat + f.heat;
+    heat = rfma(f.qdv, d.invLY[j], heat);
     ok = ok && h1;
-    if (h1) ty = f.vc1 * d.Sy(j + 1, k) - f.vc0 * d.Sy(j, k);
-  } else {
-    heat = heat + T(0);
+    if (h1) ty = rfma(f.vc1, d.Sy(j + 1, k), -(f.vc0 * d.Sy(j, k)));
   }
   if (d.hasz) {
     const bool hm = k >= 1, h1 = k + 1 < d.TZ, h2 = k + 2 < d.TZ;
     const long long p = d.plane;
     const FaceBC<T> f = face_bc<T>(cq2, dt, hm ? vzb[l - p] : T(0), vzb[l], h1 ? vzb[l + p] : T(0),
                                    h2 ? vzb[l + 2 * p] : T(0), hm ? rho[l - p] : T(0), r0, h1 ? rho[l + p] : T(0), hm,
-                                   h1, h2, d.invDZ(j, k), h1 ? d.invDZ(j, k + 1) : T(0), d.invLZ(j, k));
+                                   h1, h2, d.invDZ(j, k), h1 ? d.invDZ(j, k + 1) : T(0));
     vzc[l] = f.vc0;
-    heat = heat + f.heat;
+    heat = rfma(f.qdv, d.invLZ(j, k), heat);
     ok = ok && h1;
-    if (h1) tz = f.vc1 * d.Sz(j, k + 1) - f.vc0 * d.Sz(j, k);
+    if (h1) tz = rfma(f.vc1, d.Sz(j, k + 1), -(f.vc0 * d.Sz(j, k)));
   }
-  const T ec = st.e[l] - dt * heat;   // heating -q_d dv_d / Delta_d (G19)
+  const T ec = rfma(-dt, heat, st.e[l]);   // heating -q_d dv_d / Delta_d (G19)
   T v = ec;
   if (ok) {
     const T hd = (T(0.5) * dt) * d.gm1;

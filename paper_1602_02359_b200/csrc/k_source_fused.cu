@@ -183,17 +183,17 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
       const T rN = c ? rn.b : rn.a, rL = c ? r1.b : r1.a, pN = c ? pn.b : pn.a, pL = c ? p1.b : p1.a;
       const T w = rdiv(T(2) * ilz, rN + rL);
       T acc = w * (pN - pL);
-      if (POT) acc = acc + ((c ? fn.b : fn.a) - (c ? f1.b : f1.a)) * ilz;
-      T v = (c ? vzn.b : vzn.a) - dt * acc;
+      if (POT) acc = rfma((c ? fn.b : fn.a) - (c ? f1.b : f1.a), ilz, acc);
+      T v = rfma(-dt, acc, c ? vzn.b : vzn.a);
       if (SPH) {   // Eq. 37: (v_phi^t)^2 cot(theta) / r on the theta face (reading G27)
         const T x00 = c ? vxn.b : vxn.a, x10 = c ? vxn_r : vxn.b, x01 = c ? vx1.b : vx1.a, x11 = c ? vx1_r : vx1.b;
-        const T vphi = T(0.25) * (((x00 + x10) + x01) + x11) + frame_z;
-        v = v + dt * (((vphi * vphi) * geo_z) * iycj);
+        const T vphi = rfma(T(0.25), ((x00 + x10) + x01) + x11, frame_z);
+        v = rfma(dt, ((vphi * vphi) * geo_z) * iycj, v);
       }
       const T vprev = c ? vbz1.b : vbz1.a;
       const T dv = v - vprev;
       const T q = qv(cq2, rL, dv);                                      // q of plane n-1
-      const T vc = vprev - dt * ((c ? wfz1.b : wfz1.a) * (q - (c ? qz2.b : qz2.a)));   // v_c, lower Z face of plane n-1
+      const T vc = rfma(-dt, (c ? wfz1.b : wfz1.a) * (q - (c ? qz2.b : qz2.a)), vprev);   // v_c, lower Z face of plane n-1
       if (c) { vbz.b = v; wfz.b = w; qz1.b = q; hz1.b = q * dv; vcz1.b = vc; }
       else { vbz.a = v; wfz.a = w; qz1.a = q; hz1.a = q * dv; vcz1.a = vc; }
     }
@@ -230,14 +230,14 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
         const T rL = s_up1(r2.b), pL = s_up1(p2.b), fL = POT ? s_up1(f2.b) : T(0);
         const T wA = rdiv(T(2) * il, r2.a + rL), wB = rdiv(T(2) * il, r2.b + r2.a);
         T accA = wA * (p2.a - pL), accB = wB * (p2.b - p2.a);
-        if (POT) { accA = accA + (f2.a - fL) * il; accB = accB + (f2.b - f2.a) * il; }
-        const T vbA = vxr[2].a - dt * accA, vbB = vxr[2].b - dt * accB;
+        if (POT) { accA = rfma(f2.a - fL, il, accA); accB = rfma(f2.b - f2.a, il, accB); }
+        const T vbA = rfma(-dt, accA, vxr[2].a), vbB = rfma(-dt, accB, vxr[2].b);
         const T vbR = s_dn1(vbA);
         const T dvA = vbB - vbA, dvB = vbR - vbB;
         const T qA = qv(cq2, r2.a, dvA), qB = qv(cq2, r2.b, dvB);
         const T qL = s_up1(qB);
-        vcx.a = vbA - dt * (wA * (qA - qL));
-        vcx.b = vbB - dt * (wB * (qB - qA));
+        vcx.a = rfma(-dt, wA * (qA - qL), vbA);
+        vcx.b = rfma(-dt, wB * (qB - qA), vbB);
         const T vcR = s_dn1(vcx.a);
         hx.a = (qA * dvA) * il; hx.b = (qB * dvB) * il;
         const T Sx = sxj * d.sxk[m];
@@ -260,37 +260,37 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
             const T ily = ilY[t - 1];
             wfy[t] = rdiv(T(2) * ily, rT + rB);
             T acc = wfy[t] * ((c ? pp[t].b : pp[t].a) - (c ? pp[t - 1].b : pp[t - 1].a));
-            if (POT) acc = acc + ((c ? ff[t].b : ff[t].a) - (c ? ff[t - 1].b : ff[t - 1].a)) * ily;
-            T v = (c ? vyr[t].b : vyr[t].a) - dt * acc;
+            if (POT) acc = rfma((c ? ff[t].b : ff[t].a) - (c ? ff[t - 1].b : ff[t - 1].a), ily, acc);
+            T v = rfma(-dt, acc, c ? vyr[t].b : vyr[t].a);
             if (CURV) {   // Eq. 38: average the velocities, add the frame term, square (reading G27)
               const T x00 = c ? vxr[t].b : vxr[t].a, x10 = c ? vxn_t[t] : vxr[t].b;
               const T x01 = c ? vxr[t - 1].b : vxr[t - 1].a, x11 = c ? vxn_t[t - 1] : vxr[t - 1].b;
-              const T vphi = T(0.25) * (((x00 + x10) + x01) + x11) + om * (yeR[t - 1] * Rxk);
+              const T vphi = rfma(T(0.25), ((x00 + x10) + x01) + x11, om * (yeR[t - 1] * Rxk));
               T G = vphi * vphi;
               if (SPH) {   // Eq. 36: + v_theta^2
                 const T vth = T(0.25) * ((((c ? vz0[t].b : vz0[t].a) + (c ? vz1[t].b : vz1[t].a)) +
                                           (c ? vz0[t - 1].b : vz0[t - 1].a)) + (c ? vz1[t - 1].b : vz1[t - 1].a));
-                G = G + vth * vth;
+                G = rfma(vth, vth, G);
               }
-              v = v + dt * (G * iyeR[t - 1]);
+              v = rfma(dt, G * iyeR[t - 1], v);
             }
             if (SHEAR) {   // Eq. 29: + 2 Omega_f v_x - 4 A Omega_f y, v_x averaged as in Eq. 38
               const T x00 = c ? vxr[t].b : vxr[t].a, x10 = c ? vxn_t[t] : vxr[t].b;
               const T x01 = c ? vxr[t - 1].b : vxr[t - 1].a, x11 = c ? vxn_t[t - 1] : vxr[t - 1].b;
               const T vxa = T(0.25) * (((x00 + x10) + x01) + x11);
-              v = v + dt * (d.two_om * vxa - d.four_a_om * yeR[t - 1]);
+              v = rfma(dt, rfma(d.two_om, vxa, -(d.four_a_om * yeR[t - 1])), v);
             }
             vby[t] = v;
           }
           T qy[NV];
 #pragma unroll
           for (int t = 1; t < NV; ++t) qy[t] = qv(cq2, c ? rr[t].b : rr[t].a, vby[t + 1] - vby[t]);
-          const T vc0 = vby[2] - dt * (wfy[2] * (qy[2] - qy[1]));
+          const T vc0 = rfma(-dt, wfy[2] * (qy[2] - qy[1]), vby[2]);
           if (c) vcy.b = vc0; else vcy.a = vc0;
           if (ADI) {
-            const T vc1 = vby[3] - dt * (wfy[3] * (qy[NV - 1] - qy[2]));
-            const T h = (qy[2] * (vby[3] - vby[2])) * invLYj;
-            const T tt = vc1 * Sy1 - vc0 * Sy0;
+            const T vc1 = rfma(-dt, wfy[3] * (qy[NV - 1] - qy[2]), vby[3]);
+            const T h = qy[2] * (vby[3] - vby[2]);   // q dv of the cell; scaled by 1/LY in the heating chain below
+            const T tt = rfma(vc1, Sy1, -(vc0 * Sy0));
             if (c) { hy.b = h; ty.b = tt; } else { hy.a = h; ty.a = tt; }
           }
         }
@@ -308,10 +308,10 @@ __global__ void __launch_bounds__(32 * SFW, 3) k_source_fused(const Dev<T> d, co
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           T heat = c ? hx.b : hx.a;
-          heat = heat + (c ? hy.b : hy.a);
-          heat = heat + (c ? hz2.b : hz2.a) * ilZ;
-          const T ec = (c ? e2.b : e2.a) - dt * heat;
-          const T tz = (c ? vcz1.b : vcz1.a) * Sz1 - (c ? vcz2.b : vcz2.a) * Sz0;
+          heat = rfma(c ? hy.b : hy.a, invLYj, heat);
+          heat = rfma(c ? hz2.b : hz2.a, ilZ, heat);
+          const T ec = rfma(-dt, heat, c ? e2.b : e2.a);
+          const T tz = rfma(c ? vcz1.b : vcz1.a, Sz1, -((c ? vcz2.b : vcz2.a) * Sz0));
           const T D = iV * (((c ? tx.b : tx.a) + (c ? ty.b : ty.a)) + tz);
           const T a = hd * D;
           ed[c] = rdiv(ec * (T(1) - a), T(1) + a);

@@ -98,8 +98,8 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
       else if (!d.xwrap && i + 1 >= d.TX) wp = w;
       const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), rz = d.Rzj[j];
       if (d.eos == EOS_ADI) mom[0] = A.st.e[l];
-      mom[1] = r0 * (rx * w + rx2om);
-      mom[2] = r0 * (rx * wp + rx2om);
+      mom[1] = r0 * rfma(rx, w, rx2om);
+      mom[2] = r0 * rfma(rx, wp, rx2om);
       if (d.hasy) {
         const T v = A.st.vy[l];
         const T vp = j + 1 < d.TY ? A.st.vy[l + d.pitch] : v;
@@ -127,8 +127,7 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
   }
   if (A.v0) w = w - A.v0[d.rid(j, k)];   // residual velocity under orbital advection
   const bool up = w >= T(0);              // reading G3: ties go to the first branch
-  const T wdt = w * dt;
-  const T hup = (len - wdt) * T(0.5), hdn = (len + wdt) * T(0.5);   // Eq. 48
+  const T hup = rfma(-w, dt, len) * T(0.5), hdn = rfma(w, dt, len) * T(0.5);   // Eq. 48
   const T ir = rdiv(T(1), r0);
 
   // density: its mass flux F = w rho* S multiplies every other star value
@@ -137,10 +136,10 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
     const T fm = shfl_up1(r0), fp = shfl_dn1(r0);
     const T a = vl_slope(fm, r0, fp, invd, invd);
     const T am = shfl_up1(a);
-    const T rs = up ? fm + am * hup : r0 - a * hdn;
+    const T rs = up ? rfma(am, hup, fm) : rfma(-a, hdn, r0);
     Fr = (w * rs) * Sm;
     const T Fp = shfl_dn1(Fr);
-    if (inner) A.drho[l] = upd ? r0 - dtiv * (Fp - Fr) : r0;
+    if (inner) A.drho[l] = upd ? rfma(-dtiv, Fp - Fr, r0) : r0;
   }
 #pragma unroll
   for (int q = 0; q < NQ; ++q) {
@@ -148,10 +147,10 @@ __global__ void __launch_bounds__(32 * XW) k_sweep_x(const Dev<T> d, const Sweep
     const T fm = shfl_up1(f), fp = shfl_dn1(f);
     const T a = vl_slope(fm, f, fp, invd, invd);
     const T am = shfl_up1(a);
-    const T fs = up ? fm + am * hup : f - a * hdn;
+    const T fs = up ? rfma(am, hup, fm) : rfma(-a, hdn, f);
     const T F = Fr * fs;
     const T Fp = shfl_dn1(F);
-    if (inner) A.dq[q][l] = upd ? Q[q] - dtiv * (Fp - F) : Q[q];
+    if (inner) A.dq[q][l] = upd ? rfma(-dtiv, Fp - F, Q[q]) : Q[q];
   }
 }
 
@@ -236,8 +235,8 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
       const T wp = c == 0 ? w[1] : wn;
       int q = 0;
       if (ADI) Q[q++][c] = en[c];
-      Q[q++][c] = r[c] * (rx * w[c] + rx2om);
-      Q[q++][c] = r[c] * (rx * wp + rx2om);
+      Q[q++][c] = r[c] * rfma(rx, w[c], rx2om);
+      Q[q++][c] = r[c] * rfma(rx, wp, rx2om);
       if (HASY) { Q[q++][c] = r[c] * vy0[c]; Q[q++][c] = r[c] * vy1[c]; }
       if (HASZ) { Q[q++][c] = r[c] * (rz * vz0[c]); Q[q++][c] = r[c] * (rz * vz1[c]); }
     }
@@ -248,8 +247,7 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
 #pragma unroll
   for (int c = 0; c < 2; ++c) {
     up[c] = w[c] >= T(0);                 // reading G3
-    const T wdt = w[c] * dt;
-    hup[c] = (len - wdt) * T(0.5); hdn[c] = (len + wdt) * T(0.5);   // Eq. 48
+    hup[c] = rfma(-w[c], dt, len) * T(0.5); hdn[c] = rfma(w[c], dt, len) * T(0.5);   // Eq. 48
     ir[c] = rdiv(T(1), r[c]);
   }
   const bool store = lane >= 1 && lane <= 30 && (WRAP ? iu < d.nx : have);
@@ -261,13 +259,13 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
     const T a0 = vl_slope(fl, r[0], r[1], invd, invd);
     const T a1 = vl_slope(r[0], r[1], fr, invd, invd);
     const T al = shfl_up1(a1);
-    const T s0 = up[0] ? fl + al * hup[0] : r[0] - a0 * hdn[0];
-    const T s1 = up[1] ? r[0] + a0 * hup[1] : r[1] - a1 * hdn[1];
+    const T s0 = up[0] ? rfma(al, hup[0], fl) : rfma(-a0, hdn[0], r[0]);
+    const T s1 = up[1] ? rfma(a0, hup[1], r[0]) : rfma(-a1, hdn[1], r[1]);
     Fr[0] = (w[0] * s0) * Sm;
     Fr[1] = (w[1] * s1) * Sm;
     const T Fn = shfl_dn1(Fr[0]);
     {
-      const T o0 = r[0] - dtiv * (Fr[1] - Fr[0]), o1 = r[1] - dtiv * (Fn - Fr[1]);
+      const T o0 = rfma(-dtiv, Fr[1] - Fr[0], r[0]), o1 = rfma(-dtiv, Fn - Fr[1], r[1]);
       if (WRAP) st2_if(A.drho + l, o0, o1, store);
       else {
         st_if(A.drho + l, (i >= 2 && i < d.TX - 2) ? o0 : r[0], store);
@@ -282,12 +280,12 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
     const T a0 = vl_slope(fl, f0, f1, invd, invd);
     const T a1 = vl_slope(f0, f1, fr, invd, invd);
     const T al = shfl_up1(a1);
-    const T s0 = up[0] ? fl + al * hup[0] : f0 - a0 * hdn[0];
-    const T s1 = up[1] ? f0 + a0 * hup[1] : f1 - a1 * hdn[1];
+    const T s0 = up[0] ? rfma(al, hup[0], fl) : rfma(-a0, hdn[0], f0);
+    const T s1 = up[1] ? rfma(a0, hup[1], f0) : rfma(-a1, hdn[1], f1);
     const T F0 = Fr[0] * s0, F1 = Fr[1] * s1;
     const T Fn = shfl_dn1(F0);
     {
-      const T o0 = Q[q][0] - dtiv * (F1 - F0), o1 = Q[q][1] - dtiv * (Fn - F1);
+      const T o0 = rfma(-dtiv, F1 - F0, Q[q][0]), o1 = rfma(-dtiv, Fn - F1, Q[q][1]);
       if (WRAP) st2_if(A.dq[q] + l, o0, o1, store);
       else {
         st_if(A.dq[q] + l, (i >= 2 && i < d.TX - 2) ? o0 : Q[q][0], store);
@@ -416,8 +414,7 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
     const T ir = rdiv(T(1), rho0);
     // face between cells r-2 and r-1 (Eq. 48, Eqs. 45-47)
     const bool up = w1 >= T(0);
-    const T wdt = w1 * dt;
-    const T hup = (len2 - wdt) * T(0.5), hdn = (len1 + wdt) * T(0.5);
+    const T hup = rfma(-w1, dt, len2) * T(0.5), hdn = rfma(w1, dt, len1) * T(0.5);
     const int m = r - 2;
     const bool wr = n >= 4 && live;
     const bool upd = m >= 2 && m < TL - 2;
@@ -426,18 +423,18 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
     {
       const T f0 = rho0;
       const T a1 = vl_slope(f2[0], f1[0], f0, invd1, invd0);
-      const T rs = up ? f2[0] + a2[0] * hup : f1[0] - a1 * hdn;
+      const T rs = up ? rfma(a2[0], hup, f2[0]) : rfma(-a1, hdn, f1[0]);
       Fr = (w1 * rs) * S1;
-      { const T Qo = old[0]; st_if(A.drho + lo, upd ? Qo - dtiv2 * (Fr - F2[0]) : Qo, wr); }
+      { const T Qo = old[0]; st_if(A.drho + lo, upd ? rfma(-dtiv2, Fr - F2[0], Qo) : Qo, wr); }
       f2[0] = f0; a2[0] = a1; F2[0] = Fr;
     }
 #pragma unroll
     for (int q = 1; q <= NQ; ++q) {
       const T f0 = cur[q * MTHREADS] * ir;
       const T a1 = vl_slope(f2[q], f1[q], f0, invd1, invd0);
-      const T fs = up ? f2[q] + a2[q] * hup : f1[q] - a1 * hdn;
+      const T fs = up ? rfma(a2[q], hup, f2[q]) : rfma(-a1, hdn, f1[q]);
       const T F1 = Fr * fs;
-      { const T Qo = old[q * MTHREADS]; st_if(A.dq[q - 1] + lo, upd ? Qo - dtiv2 * (F1 - F2[q]) : Qo, wr); }
+      { const T Qo = old[q * MTHREADS]; st_if(A.dq[q - 1] + lo, upd ? rfma(-dtiv2, F1 - F2[q], Qo) : Qo, wr); }
       f2[q] = f0; a2[q] = a1; F2[q] = F1;
     }
     len2 = len1; len1 = len0; invd1 = invd0; w1 = w0; S1 = S0; dtiv2 = dtiv1; dtiv1 = dtiv0;
@@ -604,7 +601,7 @@ __global__ void __launch_bounds__(128) k_newvel_dt(const Dev<T> d, const T* __re
   I2 = rmax(I2, rabs(T(0.5) * (az + bz)) * ilz);
   I3 = rmax(I3, rabs(bz - az) * ilz);
   I3 = d.c3 * I3;
-  T m2 = live ? ((I1sq + I2 * I2) + I3 * I3) + I4 * I4 : T(0);
+  T m2 = live ? rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq))) : T(0);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
   __shared__ T sm[4];

@@ -19,9 +19,9 @@ TOL64 = 1e-10
 TOL32 = 1e-4
 
 
-def _gpu(w, precision=64, use_graph=True):
+def _gpu(w, precision=64, use_graph=True, kernel_plan=0):
     from paper_1602_02359_b200 import Fargo
-    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=precision, use_graph=use_graph)
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=precision, use_graph=use_graph, kernel_plan=kernel_plan)
     g.set_fields(*w.fields())
     return g
 
@@ -132,15 +132,14 @@ FUSED = [G.cart_adi_periodic_even, G.cart_iso_periodic, G.sph3d_iso_fargo, G.cyl
 
 
 @pytest.mark.parametrize("make", FUSED, ids=[m.__name__ for m in FUSED])
-def test_fused_source_equals_the_kernel_sequence(make, monkeypatch):
+def test_fused_source_equals_the_kernel_sequence(make):
     """The one-pass source step (k_source_fused) against the 7a -> 7b -> 7c kernels it replaces (selected with
-    FARGO_UNFUSED_SOURCE, read at fargo_init): bit-identical fields after several updates, and both within the bar
-    of the oracle (test_multi_step)."""
+    fargo_params.kernel_plan = FARGO_PLAN_UNFUSED_SOURCE): bit-identical fields after several updates, and both within
+    the bar of the oracle (test_multi_step)."""
+    from paper_1602_02359_b200 import binding as B
     w = make()
     g1 = _gpu(w)
-    monkeypatch.setenv("FARGO_UNFUSED_SOURCE", "1")
-    g2 = _gpu(w)
-    monkeypatch.delenv("FARGO_UNFUSED_SOURCE")
+    g2 = _gpu(w, kernel_plan=B.PLAN_UNFUSED_SOURCE)
     g1.step(w.nsteps); g2.step(w.nsteps)
     assert g1.time() == g2.time()
     assert g1.kernel_launches() < g2.kernel_launches()      # the fused path really is the one that ran
@@ -152,17 +151,16 @@ VISC_FUSED = [G.cyl3d_visc_fargo, G.sph3d_visc_fargo, G.sheet3d_visc]
 
 
 @pytest.mark.parametrize("make", VISC_FUSED, ids=[m.__name__ for m in VISC_FUSED])
-def test_fused_viscous_step_equals_the_kernel_sequence(make, monkeypatch):
+def test_fused_viscous_step_equals_the_kernel_sequence(make):
     """7a-7c in one pass (with the extra ghost layer) followed by 7d in one pass (k_visc3d_fused) against
-    k_source_a -> k_source_b(c) -> k_visc3d_tensor -> k_visc3d_force (FARGO_UNFUSED_VISC, read at fargo_init and at
-    the first update): bit-identical fields."""
+    k_source_a -> k_source_b(c) -> k_visc3d_tensor -> k_visc3d_force (kernel_plan = FARGO_PLAN_UNFUSED_VISC):
+    bit-identical fields."""
+    from paper_1602_02359_b200 import binding as B
     w = make()
     g1 = _gpu(w)
     g1.step(w.nsteps)
-    monkeypatch.setenv("FARGO_UNFUSED_VISC", "1")
-    g2 = _gpu(w)
+    g2 = _gpu(w, kernel_plan=B.PLAN_UNFUSED_VISC)
     g2.step(w.nsteps)
-    monkeypatch.delenv("FARGO_UNFUSED_VISC")
     assert g1.time() == g2.time()
     assert g1.kernel_launches() < g2.kernel_launches()
     for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), g1.get_fields(), g2.get_fields()):
@@ -245,6 +243,24 @@ def test_uniform_state_is_preserved():
     g.step(5)
     rho, e, vx, vy, vz = g.get_fields()
     assert np.all(rho == 1.0) and np.all(e == w.e) and np.all(vx == 0.25) and np.all(vy == -0.5) and np.all(vz == 0.125)
+
+
+@pytest.mark.parametrize("make", [G.cyl2d_iso_fargo_visc, G.sph3d_iso_fargo, G.cyl3d_adi_fargo],
+                         ids=["cyl2d_iso_fargo_visc", "sph3d_iso_fargo", "cyl3d_adi_fargo"])
+def test_second_set_fields_keeps_the_static_potential(make):
+    """Restart path: fargo_set_fields clears the arrays (the stored potential among them); on a context whose graph
+    already exists the potential must be written again before the next replay.  set, step, set, step == a fresh
+    context == the oracle."""
+    w = make()
+    g = _gpu(w)
+    g.step(2)
+    g.set_fields(*w.fields())
+    g.step(w.nsteps)
+    o = _oracle(w)
+    o.step(w.nsteps)
+    assert g.time() == o.time()
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), g.get_fields(), o.get_fields()):
+        assert _rel(a, b) <= TOL64, _diff_report(name, a, b)
 
 
 def test_set_get_roundtrip_and_device_pointers():

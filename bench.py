@@ -71,30 +71,9 @@ def make_workload(name: str):
     raise SystemExit("unknown workload " + name)
 
 
-# DRAM bytes per ACTIVE cell per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one
-# `--set full` capture at the bench's own size; profiles/r01f_fused_source.md names the command).  None = not captured.
-NCU_TRAFFIC_B_PER_CELL = {
-    "noise512": {"dt": 41.4, "source": 90.2, "sweep_x": 106.1, "sweep_y": 139.5, "sweep_z": 139.5, "newvel": 79.9},
-    "disk3d": {"vmean": 8.5, "dt": 33.0, "source": 77.2, "sweep_x": 95.1, "sweep_y": 127.2, "sweep_z": 127.2,
-               "orbital": 118.2, "newvel": 82.6},
-    # profiles/r01h_sheet_visc.md, profiles/r01i_planets.md
-    "disk3dvisc": {"source": 78.9, "source_d": 59.5, "orbital": 118.2},
-    "sheet3d": {"source": 82.3, "orbital": 134.9},
-    "disk3dlive": {"orbital": 118.2, "planets": 8.0, "potential": 7.9},
-}
-
-# fp64 pipe utilisation (sm__inst_executed_pipe_fp64, % of peak while active) of the same ncu captures: the second
-# bound of DESIGN.md section 5 -- with contraction off a kernel cannot run the pipe above 2F / (2F + N) (F fp64, N other
-# instructions per cell).  Context for the roofline object, fp64 build only.  None = not captured.
-NCU_FP64_PIPE_PCT = {
-    "noise512": {"dt": 30.8, "source": 46.3, "sweep_x": 61.6, "sweep_y": 42.6, "sweep_z": 42.6, "newvel": 16.4},
-    "disk3d": {"vmean": 11.1, "dt": 33.7, "source": 40.9, "sweep_x": 58.6, "sweep_y": 42.3, "sweep_z": 42.3,
-               "orbital": 68.2, "newvel": 16.0},
-    "disk3dvisc": {"source": 44.7, "source_d": 60.4, "orbital": 68.2},
-    "sheet3d": {"source": 51.1, "orbital": 70.6},
-    "disk3dlive": {"orbital": 68.2, "planets": 49.3, "potential": 68.4},
-}
-
+# roofline.traffic and the fp64-pipe figure are READ from the tracked raw ncu export of this workload
+# (profiles/ncu_raw_<workload>_<kernel source hash>.csv, see paper_1602_02359_b200/profiling.py); when the export was
+# captured on other kernel sources than the ones built here, traffic is null and the line says "stale".
 CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dlive": "4 with a live planet (NEXT-2 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
@@ -302,11 +281,14 @@ def run_ours(args):
     sampler.start()
     l0 = g.kernel_launches()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = g.time()[2]
     e0.record(g.stream)
     g.step(K)
     e1.record(g.stream)
     barrier()
     clocks = sampler.stop()
+    if g.time()[2] - n0 != K:   # t_stop reached: later updates are no-ops and must not be counted as cell updates
+        raise SystemExit("only %d of %d updates ran inside the timed region (t_stop reached): use fewer steps" % (g.time()[2] - n0, K))
     ms = max_over_ranks(e0.elapsed_time(e1))
     launches = g.kernel_launches() - l0
     value = whole_job_rate(ncell, K, world, ms)
@@ -337,12 +319,25 @@ def run_ours(args):
                          "algorithmic_bytes_per_cell": r * es, "achieved_gbs": gbs,
                          "frac": (gbs / peak) if gbs else None}
     dom = max((n for n in kernels if kernels[n]["achieved_gbs"]), key=lambda n: kernels[n]["share"])
+    from paper_1602_02359_b200 import profiling as P
+    ncu, ncu_file, ncu_stale = P.ncu_table(args.workload + ("_fp32" if prec == 32 else ""))
+    for name, e in ncu.items():   # per launch, beside the live timing of the same launcher
+        if name in kernels and e["launches"]:
+            per = max(1, kernels[name]["kernels"]) * (2 if name == "bc" else 1)   # kernels of this launcher per update
+            upd = e["launches"] / per
+            kernels[name]["ncu_dram_bytes_per_cell"] = None if ncu_stale else e["dram_bytes"] / upd / ncell
+            kernels[name]["ncu_fp64_pipe_pct"] = None if (ncu_stale or not e["fp64"]) else sum(e["fp64"]) / len(e["fp64"])
+    dom_ncu = kernels[dom].get("ncu_dram_bytes_per_cell")
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kernels[dom]["frac"],
-                "traffic": (NCU_TRAFFIC_B_PER_CELL.get(args.workload, {}).get(dom) or 0) * ncell * (es / 8) or None,
-                "traffic_source": "ncu --set full at this size, profiles/r01f_fused_source.md, r01h_sheet_visc.md, r01i_planets.md (bytes per cell x cells)",
+                "traffic": dom_ncu * ncell if dom_ncu else None,
+                "traffic_source": ("%s (ncu --set full --clock-control none of this command; dram__bytes_read.sum + "
+                                   "dram__bytes_write.sum per launch)" % ncu_file) if ncu_file else "no tracked ncu export for this workload",
+                "traffic_note": ("stale: %s was captured on other kernel sources than %s" % (ncu_file, P.kernel_source_hash()))
+                if ncu_stale else None,
+                "kernel_source_hash": P.kernel_source_hash(),
                 "peak_source": peak_src,
-                "fp64_pipe_pct_ncu": NCU_FP64_PIPE_PCT.get(args.workload, {}).get(dom) if prec == 64 else None,
+                "fp64_pipe_pct_ncu": kernels[dom].get("ncu_fp64_pipe_pct"),
                 "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_cell"] * ncell,
                 "ms_per_launch": kernels[dom]["ms_per_launch"], "share_of_step": kernels[dom]["share"]}
     step_gbs = fused_reals * es * ncell / (ms / K * 1e-3) / 1e9
@@ -471,6 +466,20 @@ def run_dist_slabs(args):
     dist.destroy_process_group()
 
 
+def self_launch(n: int, argv, backend_env=None) -> int:
+    """`python bench.py --gpus N` started without torchrun: start N ranks of this same command line under
+    torch.distributed.run on this node (one process per GPU) and pass their exit code on."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ)
+    env.update(backend_env or {})
+    return subprocess.call(cmd, env=env)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -489,6 +498,8 @@ def main():
                     help="NEXT-3: advance the workload as N Y-slabs on THIS GPU (slabs.SlabRun, local transport) and "
                          "print what the decomposition costs on one device; not the contract line")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.local_slabs == 0:
+        sys.exit(self_launch(args.gpus, sys.argv[1:]))
     if args.impl == "reference":
         run_reference(args)
     elif args.local_slabs > 0:

@@ -71,7 +71,9 @@ typedef struct fargo_mesh {
 enum {
   FARGO_PLAN_UNFUSED_SOURCE = 1,   /* cells 7a-7c as k_source_a + k_source_b(c) instead of one pass */
   FARGO_PLAN_UNFUSED_VISC = 2,     /* cell 7d (3-D) as tensor + force kernels instead of one pass */
-  FARGO_PLAN_UNFUSED_DT = 4        /* cell 6 as its own pass instead of being folded into the previous update's last kernel */
+  FARGO_PLAN_UNFUSED_DT = 4,       /* cell 6 as its own pass instead of being folded into the previous update's last kernel */
+  FARGO_PLAN_SEAM_ABOVE = 8        /* sub-domains: the upper FARGO_EXTERNAL Y face of this one is the periodic seam of the
+                                      undivided mesh, whose first and last rings form no pair of Eq. 73 */
 };
 
 typedef struct fargo_params {
@@ -122,8 +124,9 @@ int fargo_set_fields(fargo_ctx* c, const void* rho, const void* e, const void* v
  * boundary fill is applied first. */
 int fargo_get_fields(fargo_ctx* c, void* rho, void* e, void* vx, void* vy, void* vz);
 
-/* Enqueue n full updates on the stream.  No host synchronisation inside (except when the planet
- * moves in the frame, planet_omega != omega_frame, where the host needs t once per update). */
+/* Enqueue n full updates on the stream.  No host synchronisation inside.  (When the fixed-orbit planet moves in the
+ * frame, planet_omega != omega_frame, every update carries one enqueued host node that forms the planet's position
+ * from the device clock with the host's libm; the caller still does not wait and the update stays one graph.) */
 int fargo_step(fargo_ctx* c, int n);
 
 /* Synchronise and read the clock: simulated time, last time step, number of updates done. */

@@ -44,7 +44,7 @@ class FargoParams(C.Structure):
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p)]
 
 
-PLAN_UNFUSED_SOURCE, PLAN_UNFUSED_VISC, PLAN_UNFUSED_DT = 1, 2, 4   # fargo_params.kernel_plan flags (include/fargo.h)
+PLAN_UNFUSED_SOURCE, PLAN_UNFUSED_VISC, PLAN_UNFUSED_DT, PLAN_SEAM_ABOVE = 1, 2, 4, 8   # fargo_params.kernel_plan flags (include/fargo.h)
 
 _lib = None
 

@@ -56,6 +56,7 @@ struct Layout {   // sizes shared by fargo_workspace_bytes and fargo_init
   size_t bytes(size_t es) const {
     size_t b = 256;                                              // Ctl
     b += align_up(sizeof(PlanetsDev), 256);                      // live planets (NEXT-2)
+    b += 256;                                                    // position of the fixed-orbit planet when it moves in the frame
     b += align_up((size_t)planets_blocks(ny, nz) * MAXPL * 3 * sizeof(double), 256);   // their force partials
     b += align_up(table_elems * es, 256);                        // tables
     b += 2 * align_up((size_t)TY * TZ * es, 256);                // v0, nshift
@@ -113,6 +114,9 @@ struct Sim : CtxBase {
   Dev<T> d;
   State<T> st;
   T *phi = nullptr, *v0 = nullptr, *nshift = nullptr;
+  T* ppos = nullptr;          // device: (x_p, y_p) of the fixed-orbit planet when it moves in the frame
+  double* hclock = nullptr;   // pinned host: the clock read back for the planet's azimuth
+  T* hppos = nullptr;         // pinned host: (x_p, y_p) formed by the host node with libm
   PlanetsDev* pl = nullptr;   // live planets (NEXT-2): device state, force partials, host copy of the constants
   double* pl_part = nullptr;
   int npl = 0, pl_mode = 0;
@@ -143,6 +147,7 @@ struct Sim : CtxBase {
   ~Sim() override {
     cudaStreamSynchronize(stream);   // nothing of this context may still be running when the caller frees the workspace
     if (gexec) cudaGraphExecDestroy(gexec);
+    if (hclock) cudaFreeHost(hclock);
     for (auto& sp : spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   }
 
@@ -244,6 +249,7 @@ struct Sim : CtxBase {
     size_t off = 0;
     ctl = (Ctl*)base; off += 256;
     pl = (PlanetsDev*)(base + off); off += align_up(sizeof(PlanetsDev), 256);
+    ppos = (T*)(base + off); off += 256;
     pl_part = (double*)(base + off); off += align_up((size_t)planets_blocks(L.ny, L.nz) * MAXPL * 3 * sizeof(double), 256);
     T* tab = (T*)(base + off);
     std::vector<T> htab(L.table_elems, T(0));
@@ -308,6 +314,11 @@ struct Sim : CtxBase {
     d.t_stop = p->t_stop; d.dt_fixed = p->dt_fixed;
     d.ctl = ctl;
     pot_static = !(L.has_pot && p->planet_mass != 0.0 && p->planet_omega != p->omega_frame);
+    d.seam_above = (p->kernel_plan & FARGO_PLAN_SEAM_ABOVE) ? 1 : 0;
+    if (L.has_pot && p->planet_mass != 0.0) {   // the planet may move in the frame (now, or after fargo_set_omega_frame)
+      if (!ck(cudaHostAlloc((void**)&hclock, 64, cudaHostAllocDefault), "cudaHostAlloc(planet clock)")) return FARGO_ENOMEM;
+      hppos = (T*)(hclock + 2);
+    }
 
     // ---- transport plan: X, Y, Z sweeps (reading G14), then orbital advection ----
     npass = 0;
@@ -548,7 +559,25 @@ struct Sim : CtxBase {
     const double phip = prm.planet_phi0 + (prm.planet_omega - prm.omega_frame) * t;
     const double xp = prm.planet_r * std::cos(phip), yp = prm.planet_r * std::sin(phip);
     const double eps2 = prm.planet_eps * prm.planet_eps;
-    return launch_potential<T>(d, phi, (T)prm.gm_star, (T)prm.planet_mass, (T)xp, (T)yp, (T)eps2, stream);
+    return launch_potential<T>(d, phi, (T)prm.gm_star, (T)prm.planet_mass, (T)xp, (T)yp, (T)eps2, nullptr, stream);
+  }
+
+  // The fixed-orbit planet moves in the frame (planet_omega != omega_frame): its azimuth needs the clock, which lives
+  // on the device, and its cosine and sine come from the host's libm (no device transcendental).
+  // Everything is enqueued -- clock to pinned memory, a host node that forms (x_p, y_p), back to the device, the
+  // kernel -- so fargo_step neither waits for the stream nor leaves its captured graph.
+  static void CUDART_CB planet_host_node(void* self) {
+    Sim* s = (Sim*)self;
+    const double phip = s->prm.planet_phi0 + (s->prm.planet_omega - s->prm.omega_frame) * s->hclock[0];
+    s->hppos[0] = (T)(s->prm.planet_r * std::cos(phip));
+    s->hppos[1] = (T)(s->prm.planet_r * std::sin(phip));
+  }
+  int potential_moving() {
+    const double eps2 = prm.planet_eps * prm.planet_eps;
+    if (!ck(cudaMemcpyAsync(hclock, &ctl->t, sizeof(double), cudaMemcpyDeviceToHost, stream), "clock to host node")) return 0;
+    if (!ck(cudaLaunchHostFunc(stream, planet_host_node, this), "planet host node")) return 0;
+    if (!ck(cudaMemcpyAsync(ppos, hppos, 2 * sizeof(T), cudaMemcpyHostToDevice, stream), "planet position to device")) return 0;
+    return launch_potential<T>(d, phi, (T)prm.gm_star, (T)prm.planet_mass, T(0), T(0), (T)eps2, ppos, stream);
   }
 
   // Enqueue the kernels of one update up to and including `until` (-1 = all).  Returns the launch count.
@@ -573,10 +602,10 @@ struct Sim : CtxBase {
     if (until == FARGO_ST_VMEAN) return n;
     if (npl > 0) {                                                                    // cell 5, live planets (on the device)
       n += timed("potential", [&] { return launch_potential_live<T>(d, phi, (T)prm.gm_star, pl, npl, stream); });
-    } else if (L.has_pot && (!pot_valid || !pot_static)) {                           // cell 5
-      double t = 0.0;
-      if (!pot_static && !capturing) { get_time(&t, nullptr, nullptr); }
-      n += timed("potential", [&] { return potential(t); });
+    } else if (L.has_pot && !pot_static) {                                           // cell 5, planet moving in the frame
+      n += timed("potential", [&] { return potential_moving(); });
+    } else if (L.has_pot && !pot_valid) {                                            // cell 5, static in the frame
+      n += timed("potential", [&] { return potential(0.0); });
       pot_valid = true;
     }
     if (until == FARGO_ST_POT) return n;
@@ -590,14 +619,20 @@ struct Sim : CtxBase {
       n += timed("planets", [&] { return launch_planets_update<T>(d, st.rho, pl, npl, pl_mode, pl_part, prm.gm_star, prm.omega_frame, stream); });
     if (phase == 1) return n;
   cell7:
-    if (fuse_source && until < 0) {
+    if (fuse_source && (until < 0 || until == FARGO_ST_SRC_C || until == FARGO_ST_SRC_D)) {
       // cells 7a-7c in one pass; it reads neighbours of the state, so its output goes to arrays of its own
       if (L.adi) s2.e = alt[0];
       s2.vx = alt[1]; s2.vy = alt[2]; s2.vz = alt[3];
       n += timed("source", [&] { return launch_source_fused<T>(d, st, phi, s2, stream); });
+      // fargo_step_until: the pass is observable at the last stage it contains (active cells; with viscosity one layer more)
+      dbg["vxc"] = s2.vx; dbg["vyc"] = s2.vy; dbg["vzc"] = s2.vz; dbg["ed"] = L.adi ? alt[0] : nullptr;
+      dbg["vx"] = dbg["vy"] = dbg["vz"] = nullptr;
+      if (until == FARGO_ST_SRC_C || (until == FARGO_ST_SRC_D && !L.visc3d)) return n;
       if (L.visc3d) {   // cell 7d in one pass: reads v_c from the fused pass's arrays, writes the (dead) state velocities
         n += timed("source_d", [&] { return launch_source_d3_fused<T>(d, st.rho, s2.vx, s2.vy, s2.vz, st.vx, st.vy, st.vz, stream); });
         s2.vx = st.vx; s2.vy = st.vy; s2.vz = st.vz;
+        dbg["vxd"] = st.vx; dbg["vyd"] = st.vy; dbg["vzd"] = st.vz;
+        if (until == FARGO_ST_SRC_D) return n;
       }
     } else {
     // source step: intermediates live in transport set B (idle until the second pass)
@@ -698,7 +733,7 @@ struct Sim : CtxBase {
     if (next_phase != 0) { err = "an update is in progress (fargo_update_phase)"; return FARGO_ESTATE; }
     if (nsteps == 0) return FARGO_OK;
     // the legacy default stream cannot be captured: plain launches there
-    const bool graph_ok = prm.use_graph && (pot_static || npl > 0) && stream != nullptr && !prof;
+    const bool graph_ok = prm.use_graph && stream != nullptr && !prof;
     int s = 0;
     if (graph_ok && fuse_dt && !dt_ready) {
       // the captured sequence relies on the previous update's k_newvel_dt for the per-cell CFL rate: the first
@@ -710,7 +745,7 @@ struct Sim : CtxBase {
     if (graph_ok) {
       // the static potential stays out of the graph: written once after every fargo_set_fields (which clears it),
       // also when the graph already exists
-      if (L.has_pot && !pot_valid && npl == 0) { launches += potential(0.0); pot_valid = true; }
+      if (L.has_pot && !pot_valid && npl == 0 && pot_static) { launches += potential(0.0); pot_valid = true; }
       if (!gexec) {
         cudaGraph_t g = nullptr;
         if (!ck(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal), "begin capture")) return FARGO_ECUDA;

@@ -38,10 +38,11 @@ int launch_vmean(const Dev<T>& d, const T* vx, T* v0, cudaStream_t s) {
 // ---- cell 5: Phi = -GM/|x| - G m_p / sqrt(|x - x_p|^2 + eps^2) at cell centres ----------------------
 // Trigonometry comes from host tables only (no device transcendental).
 template <typename T>
-__global__ void k_potential(const Dev<T> d, T* __restrict__ phi, const T gm_star, const T gm_planet, const T xp,
-                            const T yp, const T eps2) {
+__global__ void k_potential(const Dev<T> d, T* __restrict__ phi, const T gm_star, const T gm_planet, T xp,
+                            T yp, const T eps2, const T* __restrict__ ppos) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
   if (i >= d.TX) return;
+  if (ppos) { xp = ppos[0]; yp = ppos[1]; }   // the planet moves in the frame: (x_p, y_p) of this update, device resident
   T R, z, r;
   if (d.geometry == GEO_SPH) { R = d.yc[j] * d.sin_zc[k]; z = d.yc[j] * d.cos_zc[k]; r = d.yc[j]; }
   else { R = d.yc[j]; z = d.zc[k]; r = rsqrt_ieee(R * R + z * z); }
@@ -56,9 +57,9 @@ __global__ void k_potential(const Dev<T> d, T* __restrict__ phi, const T gm_star
 }
 
 template <typename T>
-int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2, cudaStream_t s) {
+int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2, const T* ppos, cudaStream_t s) {
   dim3 b(128), g((d.TX + 127) / 128, d.TY, d.TZ);
-  k_potential<T><<<g, b, 0, s>>>(d, phi, gm_star, gm_planet, xp, yp, eps2);
+  k_potential<T><<<g, b, 0, s>>>(d, phi, gm_star, gm_planet, xp, yp, eps2, ppos);
   return 1;
 }
 
@@ -204,8 +205,9 @@ __global__ void __launch_bounds__(1024) k_dt_finish(const Dev<T> d, const T* __r
   if (c->done) return;
   T s = T(0);
   if (d.fargo) {
-    // pairs of radially neighbouring rings, both active; a slab also owns the pair across its upper (external) face
-    const int nyp = d.ny - 1 + (d.bc[1][1] == BC_EXTERNAL ? 1 : 0);
+    // pairs of radially neighbouring rings, both active; a slab also owns the pair across its upper (external) face,
+    // unless that face is the periodic seam of the undivided mesh (rings ny-1 and 0 are no pair there either)
+    const int nyp = d.ny - 1 + ((d.bc[1][1] == BC_EXTERNAL && !d.seam_above) ? 1 : 0);
     const int n = nyp > 0 ? nyp * d.nz : 0;
     for (int r = threadIdx.x; r < n; r += blockDim.x) {
       const int j = d.ngy + r % nyp, k = d.ngz + r / nyp;
@@ -289,7 +291,7 @@ int launch_selftest_div(const double* a, const double* b, double* out, long long
 
 #define INST(T)                                                                              \
   template int launch_vmean<T>(const Dev<T>&, const T*, T*, cudaStream_t);                   \
-  template int launch_potential<T>(const Dev<T>&, T*, T, T, T, T, T, cudaStream_t);          \
+  template int launch_potential<T>(const Dev<T>&, T*, T, T, T, T, T, const T*, cudaStream_t);          \
   template int launch_dt<T>(const Dev<T>&, const State<T>&, const T*, cudaStream_t, int);
 INST(double)
 INST(float)

@@ -13,8 +13,9 @@ template <typename T> int launch_bc(const Dev<T>& d, const State<T>& st, int mas
 // cell 3: v0_jk = (max_i vx + min_i vx)/2 (Eq. 72)
 template <typename T> int launch_vmean(const Dev<T>& d, const T* vx, T* v0, cudaStream_t s);
 // cell 5: potential of the star and the planet at cell centres; cphi, sphi = cos, sin of the planet's azimuth
+// (ppos != nullptr: the planet's (x_p, y_p) are read from that device address instead)
 template <typename T> int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp, T eps2,
-                                           cudaStream_t s);
+                                           const T* ppos, cudaStream_t s);
 // live planets (NEXT-2, k_planets.cu): cell 5 with the planets where they are now (device state); cell 5a = gas force
 // (block partials in `part`, planets_blocks() x 3 MAXPL doubles), kick and one Cash-Karp step over ctl->dt
 int planets_blocks(int ny, int nz);

@@ -20,6 +20,7 @@ from typing import List, Optional, Tuple
 import numpy as np
 
 from . import workloads as W
+from .binding import PLAN_SEAM_ABOVE
 
 EXTERNAL = 3   # FARGO_EXTERNAL of include/fargo.h
 
@@ -133,7 +134,10 @@ class SlabRun:
         with torch.cuda.stream(self.stream):          # every context picks up this (non-default) stream
             for r in self.ranks:
                 sub, (rows, planes) = slab_mesh(mesh, r, self.grid)
-                self.ctx[r] = Fargo(sub, geometry, eos, prm, precision=precision, use_graph=False)
+                # the last sub-domain of a periodic Y axis: its upper cut is the seam, no ring pair of Eq. 73 across it
+                seam = self.periodic[1] and self.grid[0] > 1 and grid_coords(r, self.grid)[0] == self.grid[0] - 1
+                self.ctx[r] = Fargo(sub, geometry, eos, prm, precision=precision, use_graph=False,
+                                    kernel_plan=PLAN_SEAM_ABOVE if seam else 0)
                 self.rows[r], self.planes[r] = rows, planes
         self._buf = {}
 

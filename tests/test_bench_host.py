@@ -81,3 +81,38 @@ def test_algorithmic_bytes_match_design_table():
     reals, fused = bench.algorithmic_reals(W.noise_box(shape3=(8, 8, 8)))
     assert 8 * reals["first_sweep"] == 104 and 8 * reals["sweep"] == 136 and 8 * reals["newvel"] == 80
     assert 8 * fused == 464                                   # SURVEY.md 8(d.3), 3-D adiabatic, no FARGO
+
+
+def test_gpus_2_without_torchrun_launches_two_ranks():
+    """`python bench.py --gpus 2` started directly (WORLD_SIZE unset) re-launches itself under torch.distributed.run
+    with one process per GPU; the reference arm reaches the same code on CPU: rank 0 prints the one line, n_gpus = 2."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env["OMP_NUM_THREADS"] = "1"
+    r = subprocess.run([sys.executable, "bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0",
+                        "--workload", "sound"], cwd=ROOT, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True,
+                       timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1 and json.loads(lines[0])["n_gpus"] == 2
+
+
+def test_ncu_exports_are_keyed_by_the_kernel_source_hash(tmp_path, monkeypatch):
+    """profiling.ncu_table: an export named after the current kernel sources is read as is; one with another hash is
+    reported stale; launches of one launcher add up."""
+    sys.path.insert(0, ROOT)
+    from paper_1602_02359_b200 import profiling as P
+    h = P.kernel_source_hash()
+    assert len(h) == 10 and h == P.kernel_source_hash()
+    head = '"ID","Kernel Name","gpu__time_duration.sum","dram__bytes_read.sum","dram__bytes_write.sum"\n' \
+           '"","","ms","Gbyte","Mbyte"\n'
+    rows = '"0","void fg::k_sweep_ring<double, (int)1, (int)7>(fg::Dev<double>)","3.5","10","8000"\n' \
+           '"1","void fg::k_sweep_ring<double, (int)2, (int)7>(fg::Dev<double>)","3.6","10","8000"\n' \
+           '"2","void fg::k_sweep_ring<double, (int)1, (int)7>(fg::Dev<double>)","3.5","10","8000"\n'
+    monkeypatch.setattr(P, "PROFILES", str(tmp_path))
+    (tmp_path / ("ncu_raw_wl_%s.csv" % h)).write_text(head + rows)
+    t, f, stale = P.ncu_table("wl")
+    assert stale is False and t["sweep_y"]["launches"] == 2 and t["sweep_z"]["launches"] == 1
+    assert t["sweep_y"]["dram_bytes"] == pytest.approx(2 * 18e9) and t["sweep_y"]["ms"] == pytest.approx(7.0)
+    (tmp_path / ("ncu_raw_other_0123456789.csv")).write_text(head + rows)
+    assert P.ncu_table("other")[2] is True
+    assert P.ncu_table("absent") == ({}, None, None)

@@ -84,13 +84,15 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
 def test_stage_by_stage(make):
     """Every kernel alone: run both sides up to each stage of Fig. 2 and compare the arrays it wrote,
     ghost zones included (both sides compute wherever the stencil fits and pass the input through elsewhere)."""
+    from paper_1602_02359_b200 import binding as B
     w = make()
     bad = []
     for stage in STAGES:
         pairs = _stage_arrays(w, stage)
         if not pairs and stage != "DT":
             continue
-        o, g = _oracle(w), _gpu(w, use_graph=False)
+        # the kernel-per-cell sequence: it computes in the ghost zones too (the fused passes: test_fused_stages)
+        o, g = _oracle(w), _gpu(w, use_graph=False, kernel_plan=B.PLAN_UNFUSED_SOURCE | B.PLAN_UNFUSED_VISC)
         o.step_until(stage)
         g.step_until(stage)
         if stage == "DT":
@@ -125,6 +127,42 @@ def test_multi_step(make, use_graph):
             bad.append(_diff_report(name, a, b))
     assert not bad, "\n".join(bad)
     assert g.kernel_launches() > 0
+
+
+FUSED_STAGES = [G.cart_adi_periodic_even, G.cart_iso_periodic, G.sph3d_iso_fargo, G.cyl3d_adi_fargo, G.sph3d_adi_nofargo,
+                G.sheet3d_adi_fargo, G.cyl3d_visc_fargo, G.sph3d_visc_fargo, G.sheet3d_visc]
+
+
+@pytest.mark.parametrize("make", FUSED_STAGES, ids=[m.__name__ for m in FUSED_STAGES])
+def test_fused_stages(make):
+    """The one-pass source step (k_source_fused) and the one-pass 7d (k_visc3d_fused) ALONE against the oracle:
+    fargo_step_until takes them when fargo_step would, and they are observable at the last stage they contain
+    (SRC_C: v_c and, adiabatic, e after 7c; SRC_D: v after 7d).  They produce active cells only (the ghost fill of cell
+    9 follows), so the comparison is over the active cells."""
+    w = make()
+    visc = w.params.nu > 0
+    adi = w.eos == W.ADIABATIC
+    bad = []
+    for stage, names in (("SRC_C", ["vxc", "vyc", "vzc"] + (["ed"] if adi else [])), ("SRC_D", ["vxd", "vyd", "vzd"] if visc else [])):
+        if not names:
+            continue
+        o, g = _oracle(w), _gpu(w, use_graph=False)
+        l0 = g.kernel_launches()
+        o.step_until(stage)
+        g.step_until(stage)
+        # bc, [vmean], [potential], dt (2 kernels) + ONE source kernel (+ ONE 7d kernel): the unfused sequence has more
+        unf = _gpu(w, use_graph=False, kernel_plan=3)
+        u0 = unf.kernel_launches()
+        unf.step_until(stage)
+        assert g.kernel_launches() - l0 < unf.kernel_launches() - u0, "the fused pass did not run"
+        unf.close()
+        sl = tuple(slice(ng, ng + n) for ng, n in ((g.ngz, w.mesh.nz), (g.ngy, w.mesh.ny), (g.ngx, w.mesh.nx)))
+        for nm in names:
+            a, b = g.array(nm)[sl], o.array(nm)[sl]
+            if _rel(a, b) > TOL64 or not np.isfinite(a).all():
+                bad.append(stage + " " + _diff_report(nm, a, b))
+        g.close(); o.close()
+    assert not bad, "\n".join(bad)
 
 
 FUSED = [G.cart_adi_periodic_even, G.cart_iso_periodic, G.sph3d_iso_fargo, G.cyl3d_adi_fargo, G.sph3d_adi_nofargo,

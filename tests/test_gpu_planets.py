@@ -134,3 +134,33 @@ def test_change_of_frame_rate_eq44(live):
     gc.set_fields(*w2.fields())
     with pytest.raises(RuntimeError):
         gc.set_omega_frame(0.5)
+
+
+@pytest.mark.parametrize("use_graph", [True, False], ids=["graph", "stream"])
+def test_fixed_orbit_planet_moving_in_the_frame(use_graph):
+    """planet_omega != omega_frame: the planet's azimuth needs the device clock every update.  It is formed by an
+    enqueued host node (host libm, as the oracle), so fargo_step keeps its captured graph and never waits: potential,
+    fields and the clock against the oracle, graph replay and plain launches alike."""
+    import dataclasses
+    import gpu_cases as G
+    from oracle.binding import Oracle
+    from paper_1602_02359_b200 import Fargo
+    w = G.cyl3d_adi_fargo()
+    prm = dataclasses.replace(w.params, planet_omega=1.3, planet_phi0=0.4)     # frame at 0.7: the planet drifts
+    g = Fargo(w.mesh, w.geometry, w.eos, prm, use_graph=use_graph)
+    g.set_fields(*w.fields())
+    o = Oracle(w.mesh, w.geometry, w.eos, prm)
+    o.set_fields(*w.fields())
+    l0 = g.kernel_launches()
+    g.step(2); g.step(4)
+    o.step(6)
+    assert g.time() == o.time()
+    assert g.kernel_launches() - l0 > 0
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), g.get_fields(), o.get_fields()):
+        rel = float(np.max(np.abs(a - b))) / float(np.max(np.abs(b)))
+        assert rel <= 1e-10, (name, rel)
+    # the potential of the NEXT update (t = t6) as both sides form it
+    g.step_until("POT"); o.step_until("POT")
+    a, b = g.array("phi"), o.array("phi")
+    assert float(np.max(np.abs(a - b))) <= 1e-13 * float(np.max(np.abs(b)))
+    g.close(); o.close()

@@ -47,6 +47,58 @@ def test_slabs_equal_the_undivided_mesh(make, nslabs):
     s.close()
 
 
+def _sheet_periodic_y():
+    """Orbital advection with a PERIODIC Y axis: v0 jumps across the seam, so the ring pair (ny-1, 0) would bind the
+    shear limit of Eq. 73 if a sub-domain took it; the undivided mesh does not (rings ny-1 and 0 are no pair there)."""
+    w = G.sheet3d_adi_fargo()
+    P = W.PERIODIC
+    m = w.mesh
+    mesh = W.Mesh(m.nx, m.ny, m.nz, m.xmin, m.xmax, m.yedges, m.zedges, ((P, P), (P, P), (P, P)))
+    return W.Workload("sheet3d_periodic_y", mesh, w.geometry, w.eos, w.params, w.rho, w.e, w.vx, w.vy, w.vz, w.nsteps)
+
+
+@pytest.mark.parametrize("nslabs", [2, 3, (2, 2)])
+def test_orbital_advection_with_a_periodic_y_axis(nslabs):
+    from paper_1602_02359_b200.slabs import SlabRun
+    w = _sheet_periodic_y()
+    g = _single(w)
+    g.step(w.nsteps)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, nslabs=nslabs)
+    s.set_fields(*w.fields())
+    s.step(w.nsteps)
+    s.synchronize()
+    assert s.time() == g.time()
+    for a, b in zip(s.get_fields(), g.get_fields()):
+        assert np.array_equal(a, b)
+    s.close()
+
+
+ORACLE_CASES = [(G.sph3d_iso_fargo, (2, 2)), (G.cart_adi_mixed_bc, 3), (G.cyl3d_visc_fargo, 2), (_sheet_periodic_y, 3)]
+
+
+@pytest.mark.parametrize("make,nslabs", ORACLE_CASES, ids=["%s-%s" % (m.__name__, n) for m, n in ORACLE_CASES])
+def test_slabs_against_the_oracle(make, nslabs):
+    """The decomposed run DIRECTLY against the CPU oracle of the undivided mesh (not through the single-context CUDA
+    run): fields within 1e-10, the clock bit-equal."""
+    from oracle.binding import Oracle
+    from paper_1602_02359_b200.slabs import SlabRun
+    w = make()
+    o = Oracle(w.mesh, w.geometry, w.eos, w.params)
+    o.set_fields(*w.fields())
+    o.step(w.nsteps)
+    s = SlabRun(w.mesh, w.geometry, w.eos, w.params, nslabs=nslabs)
+    s.set_fields(*w.fields())
+    s.step(w.nsteps)
+    s.synchronize()
+    assert s.time() == o.time(), (s.time(), o.time())
+    for name, a, b in zip(("rho", "e", "vx", "vy", "vz"), s.get_fields(), o.get_fields()):
+        if a is None:
+            continue
+        rel = float(np.max(np.abs(a - b))) / float(np.max(np.abs(b)))
+        assert rel <= 1e-10, "%s: rel %.3e" % (name, rel)
+    s.close(); o.close()
+
+
 def test_t_stop_is_reached_together():
     """Each slab clips its own dt; the minimum decides and the flag is retaken after the all-reduce."""
     from paper_1602_02359_b200.slabs import SlabRun

@@ -67,6 +67,36 @@ extern "C" int oracle_set_fields(oracle_ctx* c, const double* rho, const double*
   return 0;
 }
 
+// NEXT-4: switch the MHD substeps on and load the face-centred field (active cells, like the velocities; a component of
+// an absent direction is uniform along it).  Cartesian meshes without orbital advection only.
+extern "C" int oracle_set_bfield(oracle_ctx* c, const double* bx, const double* by, const double* bz, double mu0,
+                                 double eta, int passive) {
+  if (!c || !bx || !by || !bz || !(mu0 > 0.0) || eta < 0.0) return -1;
+  if (c->geometry != ORC_CARTESIAN || c->shear || c->p.fargo_on) return -1;
+  for (vec* f : {&c->bx, &c->by, &c->bz, &c->emfx, &c->emfy, &c->emfz, &c->bstar[0][0], &c->bstar[0][1], &c->bstar[1][0],
+                 &c->bstar[1][1], &c->bstar[2][0], &c->bstar[2][1]})
+    f->assign(c->ncell(), 0.0);
+  scatter(c, c->bx, bx); scatter(c, c->by, by); scatter(c, c->bz, bz);
+  c->mhd = true; c->mhd_passive = passive != 0; c->mu0 = mu0; c->eta = eta;
+  orc_mhd_bc_fill(*c);
+  return 0;
+}
+extern "C" int oracle_get_bfield(oracle_ctx* c, double* bx, double* by, double* bz) {
+  if (!c || !c->mhd) return -1;
+  gather(c, c->bx, bx); gather(c, c->by, by); gather(c, c->bz, bz);
+  return 0;
+}
+// max over the active cells of |div B| (the ghost fill of cell 2 is applied first: the upper boundary faces)
+extern "C" double oracle_max_divb(oracle_ctx* c) {
+  if (!c || !c->mhd) return -1.0;
+  orc_mhd_bc_fill(*c);
+  double m = 0.0;
+  for (int k = c->k0(); k < c->k1(); ++k)
+    for (int j = c->j0(); j < c->j1(); ++j)
+      for (int i = c->i0(); i < c->i1(); ++i) m = std::max(m, std::fabs(orc_mhd_divb(*c, i, j, k)));
+  return m;
+}
+
 extern "C" int oracle_get_fields(oracle_ctx* c, double* rho, double* e, double* vx, double* vy, double* vz) {
   if (!c) return -1;
   gather(c, c->rho, rho); gather(c, c->e, e); gather(c, c->vx, vx); gather(c, c->vy, vy); gather(c, c->vz, vz);
@@ -86,17 +116,28 @@ static void full_update(oracle_ctx* c, int until) {
   oracle_ctx& o = *c;
   if (o.p.t_stop > 0.0 && o.t >= o.p.t_stop) return;  // reading G21: nothing happens after t_stop
   bool clipped = false;
-  orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);                 if (until == ORC_ST_BC1) return;      // cell 2
+  orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);                                                       // cell 2
+  if (o.mhd) orc_mhd_bc_fill(o);
+  if (until == ORC_ST_BC1) return;
   orc_vmean(o);                                                 if (until == ORC_ST_VMEAN) return;    // cell 3
   orc_potential(o);                                             if (until == ORC_ST_POT) return;      // cells 4-5
   o.dt = orc_compute_dt(o, &clipped);                           if (until == ORC_ST_DT) return;       // cell 6
   orc_planets_update(o);                                                                              // cell 5a (G33)
-  orc_source_a(o);                                              if (until == ORC_ST_SRC_A) return;    // cell 7a
+  orc_source_a(o);                                                                                    // cell 7a
+  if (o.mhd) orc_mhd_source_a(o);
+  if (until == ORC_ST_SRC_A) return;
   orc_source_b(o);                                              if (until == ORC_ST_SRC_B) return;    // cell 7b
   orc_source_c(o);                                              if (until == ORC_ST_SRC_C) return;    // cell 7c
   orc_source_d(o);                                              if (until == ORC_ST_SRC_D) return;    // cell 7d
   // the source step leaves its result in (rho, ed, vxd, vyd, vzd); make it the state
   o.e = o.ed; o.vx = o.vxd; o.vy = o.vyd; o.vz = o.vzd;
+  if (o.mhd) {   // cells 8 and 10 (reading G34): the star values reach two zones out, so the ghosts of the velocities
+                 // are filled before cell 8 as well as after it (8d changes the velocities); B is transported here
+    orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);
+    orc_mhd_emf(o);                                                                                   // cells 8a-8c
+    orc_mhd_lorentz(o);                                                                               // cell 8d
+    orc_mhd_ct(o);                                                                                    // cell 10
+  }
   orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);                 if (until == ORC_ST_BC2) return;      // cell 9
   orc_momenta(o);                                               if (until == ORC_ST_MOM) return;      // cell 12a
   orc_sweep(o, 0);                                              if (until == ORC_ST_SWEEP_X) return;  // cells 12b-c
@@ -162,7 +203,8 @@ static vec* find_array(oracle_ctx* c, const char* name) {
       {"vxb", &c->vxb}, {"vyb", &c->vyb}, {"vzb", &c->vzb}, {"vxc", &c->vxc}, {"vyc", &c->vyc}, {"vzc", &c->vzc},
       {"ec", &c->ec}, {"ed", &c->ed}, {"vxd", &c->vxd}, {"vyd", &c->vyd}, {"vzd", &c->vzd}, {"pxm", &c->pxm}, {"pxp", &c->pxp},
       {"pym", &c->pym}, {"pyp", &c->pyp}, {"pzm", &c->pzm}, {"pzp", &c->pzp}, {"v0", &c->v0},
-      {"nshift", &c->nshift}, {"xi", &c->xi}};
+      {"nshift", &c->nshift}, {"xi", &c->xi},
+      {"bx", &c->bx}, {"by", &c->by}, {"bz", &c->bz}, {"emfx", &c->emfx}, {"emfy", &c->emfy}, {"emfz", &c->emfz}};
   auto it = m.find(name ? name : "");
   return it == m.end() ? nullptr : it->second;
 }

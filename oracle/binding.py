@@ -81,6 +81,10 @@ def lib(omp: bool = False):
             L.oracle_gas_force.argtypes = [vp, C.c_int, _DP]
             L.oracle_set_omega_frame.argtypes = [vp, C.c_double]
             L.oracle_diagnostics.argtypes = [vp, _DP]
+            L.oracle_set_bfield.argtypes = [vp, _DP, _DP, _DP, C.c_double, C.c_double, C.c_int]
+            L.oracle_get_bfield.argtypes = [vp, _DP, _DP, _DP]
+            L.oracle_max_divb.argtypes = [vp]
+            L.oracle_max_divb.restype = C.c_double
             L.oracle_vanleer_slopes.argtypes = [C.c_int, _DP, _DP, _DP]
             L.oracle_vanleer_slopes.restype = None
             L.oracle_vanleer_star.argtypes = [C.c_int, _DP, _DP, _DP, _DP, C.c_double, _DP]
@@ -173,6 +177,22 @@ class Oracle:
         t, dt, n = C.c_double(), C.c_double(), C.c_longlong()
         self._L.oracle_get_time(self._h, C.byref(t), C.byref(dt), C.byref(n))
         return t.value, dt.value, n.value
+
+    # ---- MHD (NEXT-4; Cartesian meshes) ----
+    def set_bfield(self, bx, by, bz, mu0: float = 1.0, eta: float = 0.0, passive: bool = False):
+        """Face-centred field, shape (nz, ny, nx) each (bx[k, j, i] on the lower X face of cell (i, j, k)); switches MHD on."""
+        b = [_f64(np.broadcast_to(a, self.shape)) for a in (bx, by, bz)]
+        if self._L.oracle_set_bfield(self._h, _p(b[0]), _p(b[1]), _p(b[2]), float(mu0), float(eta), 1 if passive else 0) != 0:
+            raise ValueError("oracle_set_bfield failed (MHD needs a Cartesian mesh without orbital advection)")
+
+    def get_bfield(self):
+        out = [np.empty(self.shape, dtype=np.float64) for _ in range(3)]
+        if self._L.oracle_get_bfield(self._h, *[_p(x) for x in out]) != 0:
+            raise RuntimeError("no magnetic field set")
+        return tuple(out)
+
+    def max_divb(self) -> float:
+        return float(self._L.oracle_max_divb(self._h))
 
     # ---- live planets (NEXT-2) ----
     def set_planets(self, gm, eps, pos, vel, force_mode: int = 1, gconst: float = 1.0):

@@ -62,6 +62,12 @@ int oracle_destroy(oracle_ctx* c);
 int oracle_set_fields(oracle_ctx* c, const double* rho, const double* e, const double* vx,
                       const double* vy, const double* vz);
 int oracle_get_fields(oracle_ctx* c, double* rho, double* e, double* vx, double* vy, double* vz);
+/* NEXT-4, MHD on Cartesian meshes (sections 3.6.1-3.6.2; mhd.cpp; readings G34-G36): the face-centred
+ * field (active cells; bx[i,j,k] on the LOWER X face of cell (i,j,k), like vx), mu0, the resistivity eta, and `passive`
+ * (the field is transported and diffused but exerts no force: the current-sheet test).  Switches the MHD substeps on. */
+int oracle_set_bfield(oracle_ctx* c, const double* bx, const double* by, const double* bz, double mu0, double eta, int passive);
+int oracle_get_bfield(oracle_ctx* c, double* bx, double* by, double* bz);
+double oracle_max_divb(oracle_ctx* c);
 int oracle_step(oracle_ctx* c, int n);
 int oracle_get_time(oracle_ctx* c, double* t, double* last_dt, long long* nsteps);
 

@@ -47,6 +47,12 @@ struct oracle_ctx {
   double pl_x[ORC_MAX_PLANETS][3], pl_v[ORC_MAX_PLANETS][3], pl_f[ORC_MAX_PLANETS][3];
   vec Vj;                              // 1 / invVj: V(j,k) = Vj[j] * syk[k] (Tab. 5)
 
+  // ---- MHD (NEXT-4, mhd.cpp): face-centred field, edge-centred electromotive forces and star values ----------
+  bool mhd = false, mhd_passive = false;   // passive: B is advected and diffused but exerts no force
+  double mu0 = 1.0, eta = 0.0;             // permeability, resistivity (Eq. 5)
+  vec bx, by, bz, emfx, emfy, emfz;
+  vec bstar[3][2];
+
   vec rho, e, vx, vy, vz;              // state
   vec phi;                             // potential at centres (cell 5)
   vec vxb, vyb, vzb;                   // after 7a
@@ -103,3 +109,11 @@ void orc_orbital_frac(oracle_ctx& c);
 void orc_orbital_shift(oracle_ctx& c);
 void orc_newvel(oracle_ctx& c);
 void orc_planets_update(oracle_ctx& c);   // planets.cpp, cell 5a
+// mhd.cpp (NEXT-4; Cartesian meshes)
+void orc_mhd_bc_fill(oracle_ctx& c);
+double orc_mhd_alfven2(const oracle_ctx& c, int i, int j, int k);
+void orc_mhd_source_a(oracle_ctx& c);
+void orc_mhd_emf(oracle_ctx& c);
+void orc_mhd_lorentz(oracle_ctx& c);
+void orc_mhd_ct(oracle_ctx& c);
+double orc_mhd_divb(const oracle_ctx& c, int i, int j, int k);

@@ -119,7 +119,8 @@ double orc_compute_dt(oracle_ctx& c, bool* clipped) {
       const double v0 = c.v0[c.rid(j, k)];
       for (int i = c.i0(); i < c.i1(); ++i) {
         const size_t l = c.id(i, j, k);
-        const double cs2 = (c.eos == ORC_ADIABATIC) ? (gg1 * c.e[l]) / c.rho[l] : c.e[l] * c.e[l];
+        double cs2 = (c.eos == ORC_ADIABATIC) ? (gg1 * c.e[l]) / c.rho[l] : c.e[l] * c.e[l];
+        if (c.mhd && !c.mhd_passive) cs2 = cs2 + orc_mhd_alfven2(c, i, j, k);   // item 1: C_w^2 = C_s^2 + v_A^2
         const double I1sq = cs2 * (ilmax * ilmax);
         double I2 = 0.0, I3 = 0.0;
         if (c.hasx) {
@@ -139,7 +140,11 @@ double orc_compute_dt(oracle_ctx& c, bool* clipped) {
         }
         I3 = c3 * I3;
         const double I4 = c4 * (ilmax * ilmax);
-        const double Isq = std::fma(I4, I4, std::fma(I3, I3, std::fma(I2, I2, I1sq)));
+        double Isq = std::fma(I4, I4, std::fma(I3, I3, std::fma(I2, I2, I1sq)));
+        if (c.mhd && c.eta != 0.0) {   // item 5: dt_5 = Delta^2 / (4 eta)
+          const double I5 = (4.0 * c.eta) * (ilmax * ilmax);
+          Isq = std::fma(I5, I5, Isq);
+        }
         M2 = std::max(M2, Isq);
       }
     }

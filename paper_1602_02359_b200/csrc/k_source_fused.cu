@@ -52,8 +52,10 @@ __device__ __forceinline__ T eos_p(const T gm1, const T e, const T rho) {   // E
 
 constexpr int SFW = 4;        // warps (consecutive rows) per block
 constexpr int SFIN = 60;      // cells stored per warp
-constexpr int SF_RD = 3;      // planes in flight
-constexpr int SF_RS = 6;      // ring slots (>= SF_RD + 3: planes n-2 .. n+SF_RD)
+// One plane in flight: the ring goes through L1 (cp.async.ca) and the neighbour rows are served by L1 as well, so a short
+// ring that leaves more of the 256 KB to L1 wins (three planes in flight: 2.89 ms at 512^3, one: 2.67 ms; profiles/r02a).
+constexpr int SF_RD = 1;             // planes in flight
+constexpr int SF_RS = SF_RD + 3;     // ring slots: planes n-2 .. n+SF_RD
 
 __device__ __forceinline__ void sf_cp_pair(unsigned dst, const double* src) {   // one pair of cells
   asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
@@ -336,24 +338,22 @@ static int launch_sf(const Dev<T>& d, const State<T>& st, const T* phi, const St
   const int ext = d.visc ? 1 : 0;   // 7d reads v_c one ghost layer out in Y and Z
   const int nyo = d.ny + 2 * ext, nzo = d.nz + 2 * ext;
   const int ntile = (d.nx + SFIN - 1) / SFIN, nrow = (nyo + SFW - 1) / SFW;
-  int nch = (148 * 12 + ntile * nrow - 1) / (ntile * nrow);
-  if (nch < 1) nch = 1;
-  int CH = (nzo + nch - 1) / nch;
-  if (CH < 16) CH = 16;   // shorter chunks on small meshes: the serial march, not the halo, is what costs there
-  if (CH > nzo) CH = nzo;
-  nch = (nzo + CH - 1) / CH;
-  dim3 b(32, SFW), g(ntile, nrow, nch);
   constexpr bool RING = GEO == GEO_CART || GEO == GEO_SHEAR;
   const size_t pair = 2 * sizeof(T);
-  if (d.has_pot) {
-    const int sm = RING ? (int)(SF_RS * 6 * 128 * pair) : 0;
-    if (RING) cudaFuncSetAttribute(k_source_fused<T, GEO, ADI, true, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-    k_source_fused<T, GEO, ADI, true, RING><<<g, b, sm, s>>>(d, st, phi, out, CH, ext);
-  } else {
-    const int sm = RING ? (int)(SF_RS * 5 * 128 * pair) : 0;
-    if (RING) cudaFuncSetAttribute(k_source_fused<T, GEO, ADI, false, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-    k_source_fused<T, GEO, ADI, false, RING><<<g, b, sm, s>>>(d, st, phi, out, CH, ext);
-  }
+  dim3 b(32, SFW);
+  // chunks of the Z march: equal blocks run in rounds of the resident slots; each chunk re-reads 4 planes
+  auto go = [&](auto kernel, const int sm) {
+    static int slots = 0;   // per instantiation
+    if (!slots) {
+      if (RING) cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+      slots = resident_slots(kernel, 32 * SFW, (size_t)sm);
+    }
+    const int CH = pick_chunk_len((long long)ntile * nrow, nzo, 4, slots, 16);
+    dim3 g(ntile, nrow, (nzo + CH - 1) / CH);
+    kernel<<<g, b, sm, s>>>(d, st, phi, out, CH, ext);
+  };
+  if (d.has_pot) go(k_source_fused<T, GEO, ADI, true, RING>, RING ? (int)(SF_RS * 6 * 128 * pair) : 0);
+  else go(k_source_fused<T, GEO, ADI, false, RING>, RING ? (int)(SF_RS * 5 * 128 * pair) : 0);
   return 1;
 }
 

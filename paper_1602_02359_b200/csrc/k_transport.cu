@@ -308,8 +308,12 @@ __global__ void __launch_bounds__(32 * X2W) k_sweep_x2(const Dev<T> d, const Swe
 #define FG_MBLOCKS 3
 #endif
 constexpr int MTHREADS = FG_MTHREADS;
-constexpr int RD = 5;            // rows in flight
-constexpr int RS = 8;            // ring slots (>= RD + 3), a power of two
+// Ring depth.  cp.async.ca passes through L1, and a line stays allocated there until its data has landed: the bytes a
+// SM can keep in flight are bounded by the L1 that the shared-memory carve-out leaves.  With three blocks of 8 x 9 KB
+// rings (221 KB) only 28 KB of L1 remain and the bare skeleton (no arithmetic) is capped at ~5.1 TB/s; with <= 196 KB of
+// rings (60 KB of L1) it moves 6.4 TB/s (profiles/r02a_marches.md).  So: as many slots as fit in
+// 64 KB per block, never more than 8; RS - 3 rows in flight (the ring also keeps rows r-1 and r-2).
+__host__ __device__ constexpr int ring_slots(int na) { return 64 / na < 8 ? 64 / na : 8; }   // na: 8-byte words per cell and row
 
 template <typename T> struct CpAsync;
 template <> struct CpAsync<double> {
@@ -335,6 +339,7 @@ template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.as
 template <typename T, int DIR, int NQ>
 __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T> d, const SweepArgs<T> A, const int CH) {
   constexpr int NA = NQ + 2;   // rho, NQ quantities, the face velocity
+  constexpr int RS = ring_slots(NA * (int)sizeof(T) / 8), RD = RS - 3;   // slots; rows in flight
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* const ring = reinterpret_cast<T*>(smem_raw) + threadIdx.x;   // element (slot, array) at (slot*NA + array)*MTHREADS
   if (d.ctl->done) return;
@@ -365,7 +370,7 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
       int r = c0 - 2 + n;
       r = r < 0 ? 0 : (r >= TL ? TL - 1 : r);
       const long long l = base + (long long)r * str;
-      const unsigned dst = ring_s + (unsigned)(((n & (RS - 1)) * NA) * MTHREADS * sizeof(T));
+      const unsigned dst = ring_s + (unsigned)(((n % RS) * NA) * MTHREADS * sizeof(T));
       CpAsync<T>::go(dst, A.srho + l);
 #pragma unroll
       for (int q = 0; q < NQ; ++q) CpAsync<T>::go(dst + (unsigned)((1 + q) * MTHREADS * sizeof(T)), A.sq[q] + l);
@@ -403,8 +408,8 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
     }
     fetch(n + RD);
     cp_wait<RD>();                                   // row n has landed
-    const T* cur = ring + ((n & (RS - 1)) * NA) * MTHREADS;
-    const T* old = ring + (((n - 2) & (RS - 1)) * NA) * MTHREADS;   // row r-2 (the cell being updated)
+    const T* cur = ring + ((n % RS) * NA) * MTHREADS;
+    const T* old = ring + (((n + RS - 2) % RS) * NA) * MTHREADS;   // row r-2 (the cell being updated)
     const T len0 = DIR == 1 ? cL : cL * gL;
     const T invd0 = DIR == 1 ? cD : cD * gD;
     const T S0 = DIR == 1 ? cS * gS : gS * cS;
@@ -477,17 +482,14 @@ static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cuda
     return 1;
   }
   const int TL = dir == 1 ? d.TY : d.TZ, lines = dir == 1 ? d.TZ : d.TY;
-  // chunk the sweep axis so that the grid fills the machine several times over, but keep chunks long
-  // (each one re-reads 4 rows of halo)
+  // chunk the sweep axis: equal blocks run in rounds of the resident slots; each chunk re-reads 4 rows of halo
   const long long cols = (long long)((d.TX + MTHREADS - 1) / MTHREADS) * lines;
-  int nch = (int)((148LL * 3 * 6 + cols - 1) / cols);
-  if (nch < 1) nch = 1;
-  int CH = (TL + nch - 1) / nch;
-  if (CH < 16) CH = 16;   // shorter chunks on small meshes: the serial march, not the halo, is what costs there
-  if (CH > TL) CH = TL;
-  nch = (TL + CH - 1) / CH;
+  const size_t sm = (size_t)ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * sizeof(T);
+  static int slots = 0;   // per instantiation (T, NQ): the two directions have the same resources
+  if (!slots) slots = resident_slots(k_sweep_ring<T, 1, NQ>, MTHREADS, sm);
+  const int CH = pick_chunk_len(cols, TL, 4, slots, 16);
+  const int nch = (TL + CH - 1) / CH;
   dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);
-  const size_t sm = (size_t)RS * (NQ + 2) * MTHREADS * sizeof(T);
   if (dir == 1) k_sweep_ring<T, 1, NQ><<<g, b, sm, s>>>(d, a, CH);
   else k_sweep_ring<T, 2, NQ><<<g, b, sm, s>>>(d, a, CH);
   return 1;
@@ -507,11 +509,12 @@ int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s
 }
 
 template <typename T, int NQ> static void ring_attr() {
-  const int sm = RS * (NQ + 2) * MTHREADS * (int)sizeof(T);
+  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T);
   cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-  cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  // 196 of 228 KB at most for the rings: the rest stays L1 for the cp.async.ca lines in flight (see ring_slots)
+  cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 86);
+  cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 86);
 }
 template <typename T> void sweep_setup() {
   ring_attr<T, 2>(); ring_attr<T, 3>(); ring_attr<T, 4>(); ring_attr<T, 5>(); ring_attr<T, 6>(); ring_attr<T, 7>();
@@ -615,6 +618,93 @@ __global__ void __launch_bounds__(128) k_newvel_dt(const Dev<T> d, const T* __re
   }
 }
 
+// The same with TWO cells per lane (even nx): 16-byte accesses, the X neighbours by shuffle (lanes 0 and 31 of a warp
+// load their outer neighbour), half the address arithmetic and twice the loads in flight per thread.  Every expression
+// is the one k_newvel_dt evaluates for the same face, so the results are bit-identical.
+template <typename T, bool ADI>
+__global__ void __launch_bounds__(128) k_newvel_dt2(const Dev<T> d, const T* __restrict__ rho, const T* __restrict__ en,
+                                                    const QSet<T> S, const State<T> st) {
+  if (d.ctl->done) return;
+  const int ia = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const bool live = ia < d.nx;
+  const int i = live ? ia : 0, j = d.ngy + blockIdx.y, k = d.ngz + blockIdx.z;
+  const int lane = threadIdx.x & 31;
+  const long long row = d.id(0, j, k), l = row + i;
+  const int jp = j + 1 == d.ngy + d.ny ? d.ngy : j + 1, kp = k + 1 == d.ngz + d.nz ? d.ngz : k + 1;
+  const long long lyp = d.id(i, jp, k), lzp = d.id(i, j, kp);
+  const bool wy = jp != j + 1, wz = kp != k + 1;   // uniform over the block
+  const T rx = d.Rx(j, k), rx2om = d.xmom_off(j, rx), irx = d.invRx(j, k), irz = d.invRzj[j];
+  T r0[2], xm[2], xp[2], ym[2], zm[2], e0[2];
+  ld_pair(rho + l, r0[0], r0[1]);
+  ld_pair(S.q[1] + l, xm[0], xm[1]);
+  ld_pair(S.q[2] + l, xp[0], xp[1]);
+  ld_pair(S.q[3] + l, ym[0], ym[1]);
+  ld_pair(S.q[5] + l, zm[0], zm[1]);
+  ld_pair(en + l, e0[0], e0[1]);
+  T ryl[2], ypl[2], rzl[2], zpl[2];              // lower neighbours in Y and Z
+  ld_pair(rho + l - d.pitch, ryl[0], ryl[1]);
+  ld_pair(S.q[4] + l - d.pitch, ypl[0], ypl[1]);
+  ld_pair(rho + l - d.plane, rzl[0], rzl[1]);
+  ld_pair(S.q[6] + l - d.plane, zpl[0], zpl[1]);
+  T ryu[2], ymu[2], ypc[2], ryc[2], rzu[2], zmu[2], zpc[2], rzc[2];   // upper faces: neighbour's own operands
+  ld_pair(rho + lyp, ryu[0], ryu[1]);
+  ld_pair(S.q[3] + lyp, ymu[0], ymu[1]);
+  ld_pair(rho + lzp, rzu[0], rzu[1]);
+  ld_pair(S.q[5] + lzp, zmu[0], zmu[1]);
+  if (wy) { ld_pair(S.q[4] + lyp - d.pitch, ypc[0], ypc[1]); ld_pair(rho + lyp - d.pitch, ryc[0], ryc[1]); }
+  else { ld_pair(S.q[4] + l, ypc[0], ypc[1]); ryc[0] = r0[0]; ryc[1] = r0[1]; }
+  if (wz) { ld_pair(S.q[6] + lzp - d.plane, zpc[0], zpc[1]); ld_pair(rho + lzp - d.plane, rzc[0], rzc[1]); }
+  else { ld_pair(S.q[6] + l, zpc[0], zpc[1]); rzc[0] = r0[0]; rzc[1] = r0[1]; }
+  // X neighbours: the pair to the left gives (rho, pxp) of cell i-1, the pair to the right (rho, pxm) of cell i+2
+  T rl = shfl_up1(r0[1]), pl = shfl_up1(xp[1]), rr = shfl_dn1(r0[0]), pr = shfl_dn1(xm[0]);
+  if (lane == 0 || i == 0) { const long long lm = row + (i == 0 ? d.nx - 1 : i - 1); rl = rho[lm]; pl = S.q[2][lm]; }
+  if (lane == 31 || i + 2 >= d.nx) { const long long lq = row + (i + 2 >= d.nx ? 0 : i + 2); rr = rho[lq]; pr = S.q[1][lq]; }
+  // Eq. 51 on the lower faces of both cells and on the upper X face of the second
+  const T ax0 = (rdiv(pl + xm[0], rl + r0[0]) - rx2om) * irx;
+  const T ax1 = (rdiv(xp[0] + xm[1], r0[0] + r0[1]) - rx2om) * irx;
+  const T ax2 = (rdiv(xp[1] + pr, r0[1] + rr) - rx2om) * irx;
+  T ay[2], az[2], by[2], bz[2];
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    ay[c] = rdiv(ypl[c] + ym[c], ryl[c] + r0[c]);
+    az[c] = rdiv(zpl[c] + zm[c], rzl[c] + r0[c]) * irz;
+    by[c] = rdiv(ypc[c] + ymu[c], ryc[c] + ryu[c]);
+    bz[c] = rdiv(zpc[c] + zmu[c], rzc[c] + rzu[c]) * irz;
+  }
+  if (live) { st_pair(st.vx + l, ax0, ax1); st_pair(st.vy + l, ay[0], ay[1]); st_pair(st.vz + l, az[0], az[1]); }
+  // Eq. 59 for the new state
+  const T ilx = d.invLX(j, k), ily = d.invLY[j], ilz = d.invLZ(j, k);
+  const T ilmax = rmax(rmax(rmax(T(0), ilx), ily), ilz);
+  const T il2 = ilmax * ilmax;
+  const T I4 = d.c4 * il2;
+  T m2 = T(0);
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    const T cs2 = ADI ? rdiv(d.gg1 * e0[c], r0[c]) : e0[c] * e0[c];
+    const T I1sq = cs2 * il2;
+    const T ax = c ? ax1 : ax0, bx = c ? ax2 : ax1;
+    T I2 = T(0), I3 = T(0);
+    I2 = rmax(I2, rabs(T(0.5) * (ax + bx)) * ilx);
+    I3 = rmax(I3, rabs(bx - ax) * ilx);
+    I2 = rmax(I2, rabs(T(0.5) * (ay[c] + by[c])) * ily);
+    I3 = rmax(I3, rabs(by[c] - ay[c]) * ily);
+    I2 = rmax(I2, rabs(T(0.5) * (az[c] + bz[c])) * ilz);
+    I3 = rmax(I3, rabs(bz[c] - az[c]) * ilz);
+    I3 = d.c3 * I3;
+    if (live) m2 = rmax(m2, rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq))));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+  __shared__ T sm[4];
+  if (lane == 0) sm[threadIdx.x >> 5] = m2;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    m2 = rmax(rmax(sm[0], sm[1]), rmax(sm[2], sm[3]));
+    const unsigned long long b = to_bits(m2);
+    if (b > *(volatile unsigned long long*)&d.ctl->m2bits) atomicMax(&d.ctl->m2bits, b);
+  }
+}
+
 template <typename T>
 bool newvel_dt_ok(const Dev<T>& d) {
   return d.hasx && d.hasy && d.hasz && d.xwrap && !d.fargo && d.bc[1][0] == BC_PERIODIC && d.bc[1][1] == BC_PERIODIC &&
@@ -623,6 +713,12 @@ bool newvel_dt_ok(const Dev<T>& d) {
 
 template <typename T>
 int launch_newvel_dt(const Dev<T>& d, const T* rho, const T* en, const QSet<T>& set, const State<T>& st, cudaStream_t s) {
+  if (d.nx % 2 == 0) {
+    dim3 b(128), g((d.nx / 2 + 127) / 128, d.ny, d.nz);
+    if (d.eos == EOS_ADI) k_newvel_dt2<T, true><<<g, b, 0, s>>>(d, rho, en, set, st);
+    else k_newvel_dt2<T, false><<<g, b, 0, s>>>(d, rho, en, set, st);
+    return 1;
+  }
   dim3 b(128), g((d.nx + 127) / 128, d.ny, d.nz);
   if (d.eos == EOS_ADI) k_newvel_dt<T, true><<<g, b, 0, s>>>(d, rho, en, set, st);
   else k_newvel_dt<T, false><<<g, b, 0, s>>>(d, rho, en, set, st);

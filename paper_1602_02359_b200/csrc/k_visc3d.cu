@@ -358,13 +358,10 @@ static int launch_v3f(const Dev<T>& d, const T* rho, const T* vx, const T* vy, c
                       cudaStream_t s) {
   // chunk the march so that the grid fills the machine a few times over; each chunk re-reads 2 planes
   const int ntile = (d.nx + V3IN - 1) / V3IN, nrow = (d.ny + V3W - 1) / V3W;
-  int nch = (148 * 12 + ntile * nrow - 1) / (ntile * nrow);
-  if (nch < 1) nch = 1;
-  int CH = (d.nz + nch - 1) / nch;
-  if (CH < 16) CH = 16;
-  if (CH > d.nz) CH = d.nz;
-  nch = (d.nz + CH - 1) / CH;
-  dim3 b(32, V3W), g(ntile, nrow, nch);
+  static int slots = 0;   // per instantiation
+  if (!slots) slots = resident_slots(k_visc3d_fused<T, GEO>, 32 * V3W, 0);
+  const int CH = pick_chunk_len((long long)ntile * nrow, d.nz, 4, slots, 16);
+  dim3 b(32, V3W), g(ntile, nrow, (d.nz + CH - 1) / CH);
   k_visc3d_fused<T, GEO><<<g, b, 0, s>>>(d, rho, vx, vy, vz, vxd, vyd, vzd, CH);
   return 1;
 }

@@ -1,0 +1,292 @@
+"""Pins of the MHD oracle (oracle/mhd.cpp; PAPER.md sections 3.6.1-3.6.2) against what the
+paper and the physics fix, not against itself:
+
+* Eq. 84 on uniform fields is v x B exactly (signs and the 1/2 of every term);
+* a uniform state with a uniform field is a fixed point;
+* constrained transport: div B and the mean field of a periodic box keep their values to rounding, also with
+  outflow boundaries and resistivity;
+* Alfven waves (Eqs. 78-82): phase speed B/sqrt(mu0 rho) against the closed form, convergence, and the SAME
+  numbers when the problem is turned onto each of the three axes (the cyclic permutations of P:534);
+* pure advection of a weak field by a uniform flow: translation at the flow speed (Eq. 101's sign of the CT update);
+* magnetic pressure: a pressure-balanced sheet stays at rest; tension (Eq. 86): the closed-form acceleration;
+* resistivity: the current-sheet test of section 5.2.2 against Eq. 115;
+* the advected field loop of section 5.2.5: the magnetic energy the paper prints at t = 2 (tests/golden/mhd_loop_paper.txt).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle.binding import Oracle
+from paper_1602_02359_b200 import workloads as W
+
+P, O = W.PERIODIC, W.OUTFLOW
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def box(nx, ny, nz, lx=1.0, ly=1.0, lz=1.0, bc=None, x0=0.0, y0=0.0, z0=0.0):
+    bc = bc or ((P, P), (P, P), (P, P))
+    return W.Mesh(nx, ny, nz, x0, x0 + lx, W.uedges(y0, y0 + ly, ny), W.uedges(z0, z0 + lz, nz), bc)
+
+
+def oracle(mesh, rho, e, v, b, gamma=5.0 / 3.0, eos=W.ADIABATIC, eta=0.0, passive=False, **kw):
+    prm = W.Params(gamma=gamma, **kw)
+    o = Oracle(mesh, W.CARTESIAN, eos, prm)
+    shape = (mesh.nz, mesh.ny, mesh.nx)
+    full = lambda a: np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=np.float64), shape))
+    o.set_fields(full(rho), full(e), full(v[0]), full(v[1]), full(v[2]))
+    o.set_bfield(full(b[0]), full(b[1]), full(b[2]), eta=eta, passive=passive)
+    return o
+
+
+def curl_a(ax, ay, az, dx, dy, dz):
+    """Face-centred B = curl A from edge-centred A (arrays [k, j, i]; A_d on the edge along d at the lower corner of the
+    cell in the two other directions), periodic: the discrete curl whose divergence vanishes identically."""
+    up = lambda a, axis: np.roll(a, -1, axis=axis)
+    bx = (up(az, 1) - az) / dy - (up(ay, 0) - ay) / dz
+    by = (up(ax, 0) - ax) / dz - (up(az, 2) - az) / dx
+    bz = (up(ay, 2) - ay) / dx - (up(ax, 1) - ax) / dy
+    return bx, by, bz
+
+
+# ---------------------------------------------------------------- Eq. 84 on uniform fields ---------------------------
+def test_emf_of_uniform_fields_is_v_cross_b():
+    m = box(8, 7, 6)
+    v, b = (0.3, -0.7, 0.45), (0.8, 0.25, -0.6)
+    o = oracle(m, 1.3, 2.0, v, b, dt_fixed=1e-3)
+    o.step(1)
+    vxb = np.cross(v, b)
+    for d, name in enumerate(("emfx", "emfy", "emfz")):
+        e = o.array(name)[3:-3, 3:-3, :]
+        assert np.allclose(e, vxb[d], rtol=0, atol=1e-15), (name, e.flat[0], vxb[d])
+    # and the state is a fixed point: nothing moves
+    for a, ref in zip(o.get_bfield(), b):
+        assert np.array_equal(a, np.full_like(a, ref))
+    rho, e, vx, vy, vz = o.get_fields()
+    assert np.allclose(vx, v[0], atol=1e-15) and np.allclose(vy, v[1], atol=1e-15) and np.allclose(vz, v[2], atol=1e-15)
+    assert np.allclose(rho, 1.3, atol=1e-15)
+
+
+# ---------------------------------------------------------------- constrained transport ------------------------------
+@pytest.mark.parametrize("bc,eta", [(((P, P), (P, P), (P, P)), 0.0), (((P, P), (O, O), (O, O)), 0.0), (((O, O), (P, P), (O, O)), 2e-3)],
+                         ids=["periodic", "outflow-yz", "outflow-xz-resistive"])
+def test_div_b_and_mean_field_are_kept_to_rounding(bc, eta):
+    nx, ny, nz = 12, 10, 9
+    m = box(nx, ny, nz, bc=bc)
+    r = np.random.default_rng(5)
+    shape = (nz, ny, nx)
+    ax, ay, az = (0.05 * r.standard_normal(shape) for _ in range(3))
+    bx, by, bz = curl_a(ax, ay, az, 1.0 / nx, 1.0 / ny, 1.0 / nz)
+    bx += 0.3; by -= 0.2; bz += 0.1
+    rho = 1.0 + 0.2 * r.uniform(-1, 1, shape)
+    e = 1.5 * (1.0 + 0.2 * r.uniform(-1, 1, shape))
+    v = [0.5 * r.uniform(-1, 1, shape) for _ in range(3)]
+    o = oracle(m, rho, e, v, (bx, by, bz), eta=eta)
+    bscale = float(np.sqrt(np.mean(bx ** 2 + by ** 2 + bz ** 2))) * max(nx, ny, nz)
+    periodic = all(b == (P, P) for b in bc)
+    if periodic:
+        assert o.max_divb() <= 1e-13 * bscale
+    d0 = o.max_divb()
+    mean0 = [float(np.mean(a)) for a in o.get_bfield()]
+    o.step(12)
+    assert o.time()[2] == 12
+    assert abs(o.max_divb() - d0) <= 2e-13 * bscale, (o.max_divb(), d0)
+    if periodic:   # the circulation of the EMF around a periodic box telescopes away: the mean field never changes
+        for a, m0 in zip(o.get_bfield(), mean0):
+            assert abs(float(np.mean(a)) - m0) <= 1e-15 * bscale
+    bnew = o.get_bfield()
+    assert all(np.isfinite(a).all() for a in bnew) and not np.array_equal(bnew[0], bx)   # something did happen
+
+
+# ---------------------------------------------------------------- Alfven waves ---------------------------------------
+def _alfven_run(axis, n, periods=1.0, amp=1e-5):
+    """A linearly polarised Alfven wave along `axis` (0, 1, 2) in a periodic box of n x 4 x 4 cells (a velocity component
+    along an ABSENT direction is not a variable of the update, as in the hydrodynamic step, so 1.5-D problems run on thin
+    3-D meshes); the transverse perturbation is along the next axis in cyclic order.  Returns (cells, initial transverse
+    field, final transverse field, final transverse velocity) along the line through the first cells."""
+    ext = [4, 4, 4]
+    ext[axis] = n
+    m = box(*ext)
+    shape = (ext[2], ext[1], ext[0])
+    t = (axis + 1) % 3                                     # direction of the perturbation
+    rho0, p0, b0 = 1.0, 0.6, 0.5
+    va = b0 / math.sqrt(rho0)
+    k = 2.0 * math.pi
+    xc = (np.arange(n) + 0.5) / n                          # centres along the axis: where transverse components live
+    shp = [1, 1, 1]
+    shp[2 - axis] = n
+    prof = amp * np.sin(k * xc).reshape(shp)
+    v = [np.zeros(shape) for _ in range(3)]
+    b = [np.zeros(shape) for _ in range(3)]
+    b[axis] = b[axis] + b0
+    v[t] = v[t] + prof                                     # psi_- = v - b = 0 ... a wave travelling along +axis has v = -b/sqrt(rho)
+    b[t] = b[t] - math.sqrt(rho0) * prof
+    o = oracle(m, rho0, p0 / (5.0 / 3.0 - 1.0), v, b, t_stop=periods / va)
+    o.step(100000)
+    assert o.time()[0] == periods / va
+    bt, vt = o.get_bfield()[t], o.get_fields()[2 + t]
+    line = lambda a: np.ravel(np.moveaxis(a, 2 - axis, 0)[:, 0, 0])
+    for a in (bt, vt):   # nothing varies across the thin directions
+        assert np.array_equal(a, np.broadcast_to(np.moveaxis(np.moveaxis(a, 2 - axis, 0)[:, :1, :1], 0, 2 - axis), a.shape))
+    return xc, line(np.broadcast_to(b[t], shape)), line(bt), line(vt)
+
+
+def _phase_and_amp(x, f):
+    c = np.sum(f * np.exp(-2j * math.pi * x)) * 2.0 / len(x)
+    return float(np.angle(c)), float(abs(c))
+
+
+def test_alfven_wave_speed_and_convergence():
+    errs = []
+    for n in (32, 64, 128):
+        x, b0, b1, _ = _alfven_run(0, n)
+        errs.append(float(np.max(np.abs(b1 - b0))) / float(np.max(np.abs(b0))))
+        ph0, a0 = _phase_and_amp(x, b0)
+        ph1, a1 = _phase_and_amp(x, b1)
+        lag = (ph1 - ph0 + math.pi) % (2 * math.pi) - math.pi   # phase error after one period of B/sqrt(mu0 rho)
+        assert abs(lag) <= 2 * math.pi * (0.01 if n >= 64 else 0.04), (n, lag)
+        # Eq. 84 pairs every time-centred star value with an upwind estimate taken at the beginning of the step, and
+        # in the printed order of Fig. 2 (8a-8c before 8d, reading G36) the EMFs see the velocities BEFORE the tension
+        # update: a forward-Euler component of first order in dt is left, +1.9 % of amplitude per period at 32 cells,
+        # +1.4 % at 64, +0.7 % at 128 (ZEUS's order, tension first, would damp instead)
+        assert abs(a1 / a0 - 1.0) <= 0.64 / n + 0.005, (n, a1 / a0)
+    assert errs[1] < 0.8 * errs[0] and errs[2] < 0.6 * errs[1] and errs[0] < 0.1, errs
+
+
+def test_alfven_wave_is_the_same_along_every_axis():
+    """The permutations X -> Y -> Z of P:534: the three runs must give the SAME numbers (same arithmetic, other indices)."""
+    ref = _alfven_run(0, 48, periods=0.5)
+    for axis in (1, 2):
+        got = _alfven_run(axis, 48, periods=0.5)
+        # (to rounding: the X spacing is (xmax - xmin)/nx, the Y and Z spacings are differences of edge coordinates)
+        assert np.allclose(got[2], ref[2], rtol=0, atol=1e-17) and np.allclose(got[3], ref[3], rtol=0, atol=1e-17), axis
+
+
+def test_a_wave_travelling_the_other_way_has_the_other_sign():
+    """v = +b/sqrt(rho) travels along -B: after a quarter period the two waves sit half a wavelength apart."""
+    n = 64
+    m = box(n, 4, 4)
+    xc = (np.arange(n) + 0.5) / n
+    prof = 1e-5 * np.sin(2 * math.pi * xc).reshape(1, 1, n) * np.ones((4, 4, 1))
+    z = np.zeros((4, 4, n))
+    outs = []
+    for sign in (-1.0, 1.0):
+        o = oracle(m, 1.0, 0.9, (z, prof, z), (z + 0.5, sign * prof, z), t_stop=0.25 / 0.5)
+        o.step(10000)
+        outs.append(_phase_and_amp(xc, o.get_fields()[3][0, 0, :])[0])
+    sep = (outs[0] - outs[1]) % (2 * math.pi)
+    assert abs(sep - math.pi) < 0.05, outs
+
+
+# ---------------------------------------------------------------- advection of a weak field (sign of the CT update) --
+def test_weak_field_is_carried_by_a_uniform_flow():
+    errs = []
+    for n in (32, 64):
+        m = box(n, 1, 1)
+        xc = (np.arange(n) + 0.5) / n
+        z = np.zeros((1, 1, n))
+        by0 = 1e-8 * np.sin(2 * math.pi * xc).reshape(1, 1, n)
+        o = oracle(m, 1.0, 1.0, (z + 0.8, z, z), (z, by0, z), t_stop=0.25)
+        o.step(10000)
+        exact = 1e-8 * np.sin(2 * math.pi * (xc - 0.8 * 0.25))
+        errs.append(float(np.max(np.abs(np.ravel(o.get_bfield()[1]) - exact))) / 1e-8)
+    assert errs[0] < 0.05 and errs[1] < 0.45 * errs[0], errs   # max norm: the limiter clips the two extrema
+
+
+# ---------------------------------------------------------------- magnetic pressure and tension ----------------------
+def test_pressure_balanced_sheet_stays_at_rest_and_unbalanced_one_accelerates():
+    """P + B_y^2/2 = const across x: no acceleration beyond the truncation error; with P uniform instead the face
+    velocity after one step is -dt (dB^2/2 / dx) / rho to second order."""
+    res = []
+    for n in (32, 64):
+        m = box(n, 1, 1)
+        xc = (np.arange(n) + 0.5) / n
+        z = np.zeros((1, 1, n))
+        by = (0.4 + 0.2 * np.sin(2 * math.pi * xc)).reshape(1, 1, n)
+        ptot = 1.0
+        p = ptot - 0.5 * by ** 2
+        gam = 5.0 / 3.0
+        dt = 1e-4
+        o = oracle(m, 1.0, p / (gam - 1.0), (z, z, z), (z, by, z), dt_fixed=dt)
+        o.step(1)
+        vbal = float(np.max(np.abs(o.get_fields()[2])))
+        o = oracle(m, 1.0, 1.0 / (gam - 1.0), (z, z, z), (z, by, z), dt_fixed=dt)
+        o.step(1)
+        xf = np.arange(n) / n                              # vx lives on the lower x face
+        byf = 0.4 + 0.2 * np.sin(2 * math.pi * xf)
+        exact = -dt * byf * (0.2 * 2 * math.pi * np.cos(2 * math.pi * xf))
+        err = float(np.max(np.abs(np.ravel(o.get_fields()[2]) - exact))) / float(np.max(np.abs(exact)))
+        res.append((vbal / float(np.max(np.abs(exact))), err))
+    assert res[0][0] < 1e-12 and res[1][0] < 1e-12, res   # zone-centred P + B^2/2 is uniform: balance to rounding
+    assert res[0][1] < 0.02 and res[1][1] < res[0][1] / 3.0, res
+
+
+def test_tension_gives_the_closed_form_acceleration():
+    """Eq. 86 with B_x = B0 and B_y = eps sin(kx): dv_y/dt = B0 dB_y/dx / (mu0 rho), second order; nothing else moves."""
+    errs = []
+    for n in (32, 64):
+        m = box(n, 4, 4)
+        xc = (np.arange(n) + 0.5) / n
+        z = np.zeros((4, 4, n))
+        eps, b0, rho, dt = 1e-6, 0.7, 1.6, 1e-5
+        by = eps * np.sin(2 * math.pi * xc).reshape(1, 1, n) + z
+        o = oracle(m, rho, 1.5, (z, z, z), (z + b0, by, z), dt_fixed=dt)
+        o.step(1)
+        assert float(np.max(np.abs(o.get_fields()[2]))) < 1e-3 * dt * eps and float(np.max(np.abs(o.get_fields()[4]))) == 0.0
+        vy = o.get_fields()[3][0, 0, :]
+        exact = dt * b0 * eps * 2 * math.pi * np.cos(2 * math.pi * xc) / rho
+        # mean error: van Leer's slope vanishes in the two zones that hold the extrema of B_y, a first-order error there
+        errs.append(float(np.mean(np.abs(vy - exact))) / float(np.max(np.abs(exact))))
+    assert errs[0] < 0.02 and errs[1] < errs[0] / 3.0, errs
+
+
+# ---------------------------------------------------------------- resistivity: section 5.2.2, Eq. 115 ----------------
+def test_current_sheet_diffusion_follows_eq_115():
+    """512 cells over -1 <= z <= 1, B_0 = 1, eta = 0.25, initial profile = Eq. 115 at t0 = (5 dz / 2)^2, the field passive
+    (P:887-897); compared at t = 30 t0 with B_0 erf(z / sqrt(4 eta (t0 + t)))."""
+    n = 512
+    m = box(1, 1, n, lz=2.0, z0=-1.0, bc=((P, P), (P, P), (O, O)))
+    dz = 2.0 / n
+    zc = -1.0 + (np.arange(n) + 0.5) * dz
+    eta, t0 = 0.25, (2.5 * dz) ** 2
+    erf = np.vectorize(math.erf)
+    by0 = erf(zc / math.sqrt(4 * eta * t0)).reshape(n, 1, 1)
+    z = np.zeros((n, 1, 1))
+    o = oracle(m, 1.0, 1.0 / (5.0 / 3.0 - 1.0), (z, z, z), (z, by0, z), eta=eta, passive=True, t_stop=29.0 * t0)
+    o.step(100000)
+    by = np.ravel(o.get_bfield()[1])
+    exact = erf(zc / math.sqrt(4 * eta * (30.0 * t0)))
+    assert float(np.max(np.abs(by - exact))) < 2e-3
+    assert float(np.max(np.abs(np.ravel(o.get_fields()[4])))) == 0.0      # passive: the fluid never moves
+    # the time step obeys item 5 of Eq. 59: dt <= C dz^2 / (4 eta)
+    assert o.time()[1] <= 0.44 * dz * dz / (4 * eta) * (1 + 1e-12)
+
+
+# ---------------------------------------------------------------- section 5.2.5: the advected field loop -------------
+def test_field_loop_magnetic_energy_matches_the_paper():
+    """128 x 64 cells on -1 <= y <= 1, -0.5 <= z <= 0.5, periodic; A_x = A0 (R - r) inside r < R = 0.3, A0 = 1e-3; rho = 1,
+    beta >> 1; v_y = sqrt(5)/2, v_z = 0.  The paper prints the mean magnetic energy at t = 2,
+    E_m ~ 1.235e-7 (against 1.225e-7 and 1.19e-7 for two Riemann solvers of Fromang et al. 2006)."""
+    with open(os.path.join(GOLD, "mhd_loop_paper.txt")) as f:
+        gold = float([ln for ln in f if not ln.startswith("#")][0].split()[0])
+    ny, nz = 128, 64
+    m = box(1, ny, nz, ly=2.0, lz=1.0, y0=-1.0, z0=-0.5)
+    dy, dz = 2.0 / ny, 1.0 / nz
+    ye = -1.0 + np.arange(ny) * dy                          # A_x lives on the edges along x: lower y, lower z corner
+    ze = -0.5 + np.arange(nz) * dz
+    r = np.sqrt(ye[None, :, None] ** 2 + ze[:, None, None] ** 2)
+    ax = np.where(r < 0.3, 1e-3 * (0.3 - r), 0.0)
+    zero = np.zeros_like(ax)
+    bx, by, bz = curl_a(ax, zero, zero, 1.0, dy, dz)
+    z = np.zeros((nz, ny, 1))
+    gam = 5.0 / 3.0
+    o = oracle(m, 1.0, 1.0 / (gam - 1.0), (z, z + math.sqrt(5.0) / 2.0, z), (bx, by, bz), gamma=gam, t_stop=2.0)
+    em0 = float(np.mean(by ** 2 + bz ** 2))
+    o.step(1000000)
+    assert o.time()[0] == 2.0
+    b = o.get_bfield()
+    em = float(np.mean(b[1] ** 2 + b[2] ** 2))
+    print("field loop: E_m(0) = %.4e, E_m(2) = %.4e (paper %.4e), %d updates" % (em0, em, gold, o.time()[2]))
+    assert o.max_divb() < 1e-13 * 1e-3 * 128          # |B| ~ 1e-3, 1/dy = 64: a few ulps of B / dy
+    assert abs(em - gold) <= 0.01 * gold, (em, gold)     # measured: 1.2370e-7, 0.16 % from the printed value

@@ -96,6 +96,8 @@ typedef struct fargo_params {
   int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (needs a non-default
                               cuda_stream; on the legacy default stream it falls back to plain launches);
                               0: plain stream launches */
+  int mhd;                 /* 1: reserve the arrays of the MHD substeps (NEXT-4: B, the EMFs and the star values, 12 arrays);
+                              they run once fargo_set_bfield has been called.  3-D Cartesian meshes without orbital advection */
   int kernel_plan;         /* 0 = the fused kernels wherever they apply (default).  Bit flags select the unfused
                               sequences instead, for measurements and for tests that compare the two (results are
                               bit-identical): FARGO_PLAN_UNFUSED_SOURCE, FARGO_PLAN_UNFUSED_VISC, FARGO_PLAN_UNFUSED_DT */
@@ -160,6 +162,20 @@ int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc)
  * the new rate is chosen: DESIGN.md reading G33).  Cylindrical and spherical meshes only: FARGO_EINVAL otherwise. */
 int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
 
+/* MHD (sections 3.6.1-3.6.2; readings G34-G36): method of characteristics +
+ * constrained transport on 3-D Cartesian meshes.  The context must have been created with fargo_params.mhd = 1.
+ * bx, by, bz: the face-centred field, HOST or DEVICE, nz*ny*nx elements of the context's precision each, ACTIVE cells,
+ * bx[i,j,k] on the LOWER X face of cell (i,j,k) like vx.  mu0 > 0; eta >= 0 is the resistivity of Eq. 5;
+ * passive != 0: the field is transported and diffused but exerts no force (the current-sheet test).  From then on
+ * every update also runs: the ghost fill of B (cell 2), C_w^2 = C_s^2 + v_A^2 and the resistive limit in Eq. 59 (cell 6),
+ * the magnetic pressure gradient (cell 7a), star values and electromotive forces (cells 8a-8c, Eqs. 80-84), the
+ * tension (cell 8d, Eq. 86) and the constrained-transport update (cell 10, Eq. 76), which keeps div B to rounding.
+ * The source step then runs as the kernel sequence 7a, 7b(c) (the magnetic pressure enters before 7b).
+ * fargo_get_bfield copies the active cells out (any pointer may be NULL).  Not with orbital advection (section 3.7), on
+ * sub-domains, or on curvilinear meshes (Eqs. 87-91): FARGO_EINVAL.  Errors: FARGO_EINVAL, FARGO_ESTATE, FARGO_ECUDA. */
+int fargo_set_bfield(fargo_ctx* ctx, const void* bx, const void* by, const void* bz, double mu0, double eta, int passive);
+int fargo_get_bfield(fargo_ctx* ctx, void* bx, void* by, void* bz);
+
 /* Domain decomposition in Y and Z (section 4.1: the mesh is split in Y and Z, never
  * in X; 3 ghost layers are exchanged at cells 2 and 9 of Fig. 2; the time step is the minimum over the sub-domains,
  * P:407).  A sub-domain is an ordinary context whose mesh holds a range of rows / planes and whose cut faces have the
@@ -199,7 +215,7 @@ int fargo_step_until(fargo_ctx* c, int stage);
 int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz);
 /* Copy a named ghost-inclusive array (TZ*TY*TX elements of the context's precision, X fastest,
  * unpadded; TZ*TY for "v0") to HOST memory.  Names: rho e vx vy vz phi vxb vyb vzb vxc vyc vzc ec ed
- * vxd vyd pxm pxp pym pyp pzm pzp trho te v0.  pxm..pzp, trho, te refer to the transported set written
+ * vxd vyd pxm pxp pym pyp pzm pzp trho te v0 (MHD: bx by bz emfx emfy emfz).  pxm..pzp, trho, te refer to the transported set written
  * by the most recent transport pass.  Which names hold defined data depends on the stage reached. */
 int fargo_get_array(fargo_ctx* c, const char* name, void* out);
 

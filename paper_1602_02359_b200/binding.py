@@ -22,7 +22,7 @@ EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fi
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
            "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div",
            "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics",
-           "fargo_update_phase", "fargo_halo_bytes", "fargo_halo", "fargo_dt_device_ptr"]
+           "fargo_update_phase", "fargo_halo_bytes", "fargo_halo", "fargo_dt_device_ptr", "fargo_set_bfield", "fargo_get_bfield"]
 
 
 class FargoMesh(C.Structure):
@@ -40,7 +40,7 @@ class FargoParams(C.Structure):
                 ("planet_r", C.c_double), ("planet_phi0", C.c_double), ("planet_omega", C.c_double),
                 ("planet_eps", C.c_double),
                 ("shear_c0", C.c_double), ("t_stop", C.c_double), ("dt_fixed", C.c_double), ("oort_a", C.c_double),
-                ("precision", C.c_int), ("use_graph", C.c_int), ("kernel_plan", C.c_int),
+                ("precision", C.c_int), ("use_graph", C.c_int), ("mhd", C.c_int), ("kernel_plan", C.c_int),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p)]
 
 
@@ -81,6 +81,8 @@ def load():
     L.fargo_get_planets.argtypes = [vp, _DP, _DP, _DP]
     L.fargo_set_omega_frame.argtypes = [vp, C.c_double]
     L.fargo_diagnostics.argtypes = [vp, _DP]
+    L.fargo_set_bfield.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, C.c_int]
+    L.fargo_get_bfield.argtypes = [vp, vp, vp, vp]
     L.fargo_update_phase.argtypes = [vp, C.c_int]
     L.fargo_halo_bytes.argtypes = [vp, C.c_int, C.c_int]
     L.fargo_halo_bytes.restype = C.c_size_t
@@ -110,7 +112,7 @@ class Fargo:
     """
 
     def __init__(self, mesh, geometry: int, eos: int, params, precision: int = 64, use_graph: bool = True,
-                 device: Optional[str] = None, kernel_plan: int = 0):
+                 device: Optional[str] = None, kernel_plan: int = 0, mhd: bool = False):
         import torch
         L = load()
         if not torch.cuda.is_available():
@@ -145,6 +147,7 @@ class Fargo:
             setattr(p, name, getattr(params, name))
         p.precision = precision
         p.use_graph = 1 if use_graph else 0
+        p.mhd = 1 if mhd else 0            # reserve the arrays of the MHD substeps (NEXT-4); set_bfield switches them on
         p.kernel_plan = int(kernel_plan)   # PLAN_* flags: the unfused kernel sequences (measurements, tests)
         nbytes = L.fargo_workspace_bytes(C.byref(m), geometry, eos, C.byref(p))
         if nbytes == 0:
@@ -252,6 +255,28 @@ class Fargo:
         class _View:
             __cuda_array_interface__ = {"shape": (1,), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
         return self._torch.as_tensor(_View(), device=self.device)
+
+    # -- MHD (NEXT-4; the context must have been created with mhd=True) ---------------------------------------
+    def set_bfield(self, bx, by, bz, mu0: float = 1.0, eta: float = 0.0, passive: bool = False):
+        """Face-centred field, shape (nz, ny, nx) each (bx[k, j, i] on the lower X face of cell (i, j, k))."""
+        arrs = []
+        for a in (bx, by, bz):
+            if isinstance(a, np.ndarray) or np.isscalar(a):
+                a = np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=self.dtype), self.shape))
+            else:
+                a = a.to(self.tdtype).contiguous()
+            arrs.append(a)
+        self._keep_b = arrs
+        with self._torch.cuda.device(self.device):
+            self._torch.cuda.current_stream(self.device).synchronize()
+            self._check(load().fargo_set_bfield(self._h, *[_ptr(a) for a in arrs], float(mu0), float(eta), 1 if passive else 0),
+                        "fargo_set_bfield")
+
+    def get_bfield(self):
+        out = [np.empty(self.shape, dtype=self.dtype) for _ in range(3)]
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_get_bfield(self._h, *[_ptr(a) for a in out]), "fargo_get_bfield")
+        return tuple(out)
 
     # -- live planets (NEXT-2) ------------------------------------------------------------------------
     def set_planets(self, gm, eps, pos, vel, force_mode: int = 1, gconst: float = 1.0):

@@ -40,6 +40,8 @@ struct CtxBase {
   virtual int get_planets(double*, double*, double*) = 0;
   virtual int set_omega_frame(double) = 0;
   virtual int diagnostics(double*) = 0;
+  virtual int set_bfield(const void*, const void*, const void*, double, double, int) = 0;
+  virtual int get_bfield(void*, void*, void*) = 0;
   virtual int profile(int enable) = 0;
   virtual int profile_report(char* buf, size_t len) = 0;
   long long launches = 0;
@@ -50,7 +52,7 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 struct Layout {   // sizes shared by fargo_workspace_bytes and fargo_init
   int nx, ny, nz, ngx, ngy, ngz, TX, TY, TZ;
   long long pitch, plane, narr;
-  bool xwrap, hasx, hasy, hasz, has_pot, visc, visc3d, fargo, adi;
+  bool xwrap, hasx, hasy, hasz, has_pot, visc, visc3d, fargo, adi, mhd;
   int n3d;             // number of 3-D arrays
   size_t table_elems;  // total 1-D table elements (each table padded to 32 elements)
   size_t bytes(size_t es) const {
@@ -101,7 +103,14 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.visc = L.visc3d || (p->nu > 0.0 && geometry == FARGO_CYLINDRICAL && L.hasx && L.hasy && !L.hasz && L.xwrap);
   L.fargo = p->fargo_on != 0;
   L.adi = eos == FARGO_ADIABATIC;
-  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4;   // state, Phi, two transport sets, the source step's output
+  L.mhd = p->mhd != 0;
+  if (L.mhd && !(cartesian_metric && geometry != FARGO_SHEARING_SHEET && L.hasx && L.hasy && L.hasz && !p->fargo_on)) {
+    err = "MHD: 3-D Cartesian meshes without orbital advection (1.5-D and 2.5-D problems run on thin 3-D meshes)"; return false;
+  }
+  for (int dd = 1; dd < 3 && L.mhd; ++dd)
+    for (int s = 0; s < 2; ++s)
+      if (m->bc[dd][s] == FARGO_EXTERNAL) { err = "MHD is not available on sub-domains"; return false; }
+  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4 + (L.mhd ? 12 : 0);   // state, Phi, two transport sets, the source step's output, MHD
   const size_t pad = 32;
   auto t1 = [&](int n) { return align_up((size_t)n, pad); };
   L.table_elems = 7 * t1(L.TY + 1) + 11 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 6 * t1(L.TZ + 1) + 2 * t1(L.TX);
@@ -122,6 +131,10 @@ struct Sim : CtxBase {
   int npl = 0, pl_mode = 0;
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
+  T *bfield[3] = {nullptr, nullptr, nullptr}, *emf[3], *bstar[6];   // MHD (NEXT-4): B on faces, EMFs and star values on edges
+  bool mhd_on = false;  // fargo_set_bfield was called
+  int mhd_passive = 0;
+  double mu0 = 1.0, eta = 0.0;
   int next_phase = 0;   // slab mode: the phase fargo_update_phase expects next
   State<T> s2m;         // slab mode: where e and v are after the source step (phase 2 -> phases 3, 4)
   bool fuse_source = false;
@@ -288,6 +301,11 @@ struct Sim : CtxBase {
     if (L.has_pot) phi = arr();
     for (int n = 0; n < 16; ++n) pool[n] = arr();
     for (int n = 0; n < 4; ++n) alt[n] = arr();
+    if (L.mhd) {
+      for (int n = 0; n < 3; ++n) bfield[n] = arr();
+      for (int n = 0; n < 3; ++n) emf[n] = arr();
+      for (int n = 0; n < 6; ++n) bstar[n] = arr();
+    }
     if (off > p->workspace_bytes) { err = "internal: workspace overflow"; return FARGO_ENOMEM; }
 
     if (!ck(cudaMemsetAsync(base, 0, off, stream), "cudaMemsetAsync(workspace)")) return FARGO_ECUDA;
@@ -532,6 +550,52 @@ struct Sim : CtxBase {
     return FARGO_OK;
   }
 
+  // ---- MHD (NEXT-4) ----------------------------------------------------------------------------------
+  int set_bfield(const void* bx, const void* by, const void* bz, double mu0_, double eta_, int passive) override {
+    if (!L.mhd) { err = "the context was created without fargo_params.mhd"; return FARGO_ESTATE; }
+    if (!bx || !by || !bz || !(mu0_ > 0.0) || eta_ < 0.0) { err = "bx, by, bz, mu0 > 0 and eta >= 0 are required"; return FARGO_EINVAL; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    const size_t nact = (size_t)L.nx * L.ny * L.nz;
+    const size_t arrb = align_up((size_t)L.narr * sizeof(T), 256);
+    if (!ck(cudaMemsetAsync(bfield[0], 0, 12 * arrb, stream), "cudaMemsetAsync(B)")) return FARGO_ECUDA;
+    const void* src[3] = {bx, by, bz};
+    T* staging = pool[15];   // dead between updates
+    for (int f = 0; f < 3; ++f) {
+      const T* dev = (const T*)src[f];
+      if (!on_device(src[f])) {
+        if (!ck(cudaMemcpyAsync(staging, src[f], nact * sizeof(T), cudaMemcpyHostToDevice, stream), "H2D field")) return FARGO_ECUDA;
+        dev = staging;
+      }
+      launches += launch_scatter<T>(d, dev, bfield[f], stream);
+    }
+    if (!ck(cudaMemsetAsync(staging, 0, (size_t)L.narr * sizeof(T), stream), "cudaMemsetAsync(staging)")) return FARGO_ECUDA;
+    launches += launch_bc_b<T>(d, bfield[0], bfield[1], bfield[2], stream);
+    if (!ck(cudaGetLastError(), "set_bfield launch")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "set_bfield sync")) return FARGO_ECUDA;
+    const bool changed = !mhd_on || passive != mhd_passive || mu0_ != mu0 || eta_ != eta;
+    mhd_on = true; mhd_passive = passive ? 1 : 0; mu0 = mu0_; eta = eta_;
+    dt_ready = false;
+    if (changed && gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }   // the kernel sequence and its arguments change
+    return FARGO_OK;
+  }
+
+  int get_bfield(void* bx, void* by, void* bz) override {
+    if (!mhd_on) { err = "no magnetic field set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    const size_t nact = (size_t)L.nx * L.ny * L.nz;
+    void* dstp[3] = {bx, by, bz};
+    for (int f = 0; f < 3; ++f) {
+      if (!dstp[f]) continue;
+      if (on_device(dstp[f])) { launches += launch_gather<T>(d, bfield[f], (T*)dstp[f], stream); continue; }
+      T* staging = pool[8 + f];   // set B is dead between updates
+      launches += launch_gather<T>(d, bfield[f], staging, stream);
+      if (!ck(cudaMemcpyAsync(dstp[f], staging, nact * sizeof(T), cudaMemcpyDeviceToHost, stream), "D2H field")) return FARGO_ECUDA;
+    }
+    if (!ck(cudaGetLastError(), "get_bfield launch")) return FARGO_ECUDA;
+    if (!ck(cudaStreamSynchronize(stream), "get_bfield sync")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
   int get_planets(double* pos, double* vel, double* gas_acc) override {
     PlanetsDev h;
     if (!ck(cudaMemcpyAsync(&h, pl, sizeof h, cudaMemcpyDeviceToHost, stream), "download planets")) return FARGO_ECUDA;
@@ -595,7 +659,9 @@ struct Sim : CtxBase {
     dbg.clear();
     dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
     dbg["phi"] = phi; dbg["v0"] = v0;
+    if (L.mhd) { dbg["bx"] = bfield[0]; dbg["by"] = bfield[1]; dbg["bz"] = bfield[2]; dbg["emfx"] = emf[0]; dbg["emfy"] = emf[1]; dbg["emfz"] = emf[2]; }
     n += timed("bc", [&] { return launch_bc<T>(d, st, field_mask(true, true), stream); });                        // cell 2
+    if (mhd_on) n += timed("bc_b", [&] { return launch_bc_b<T>(d, bfield[0], bfield[1], bfield[2], stream); });
     if (until == FARGO_ST_BC1 || phase == 0) return n;
   cell3:
     if (L.fargo) n += timed("vmean", [&] { return launch_vmean<T>(d, st.vx, v0, stream); });                         // cell 3
@@ -610,8 +676,9 @@ struct Sim : CtxBase {
     }
     if (until == FARGO_ST_POT) return n;
     {                                                                                // cell 6
-      const int mode = (fuse_dt && dt_ready) ? DT_FINISH : DT_BOTH;
-      n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream, mode); });
+      const int mode = (fuse_dt && !mhd_on && dt_ready) ? DT_FINISH : DT_BOTH;
+      const MhdDt<T> M{bfield[0], bfield[1], bfield[2], (T)mu0, (T)(4.0 * eta), mhd_passive};
+      n += timed("dt", [&] { return launch_dt<T>(d, st, v0p, stream, mode, mhd_on ? &M : nullptr); });
       dt_ready = false;   // k_dt_finish consumed and cleared the running max
     }
     if (until == FARGO_ST_DT) return n;
@@ -619,7 +686,7 @@ struct Sim : CtxBase {
       n += timed("planets", [&] { return launch_planets_update<T>(d, st.rho, pl, npl, pl_mode, pl_part, prm.gm_star, prm.omega_frame, stream); });
     if (phase == 1) return n;
   cell7:
-    if (fuse_source && (until < 0 || until == FARGO_ST_SRC_C || until == FARGO_ST_SRC_D)) {
+    if (fuse_source && !mhd_on && (until < 0 || until == FARGO_ST_SRC_C || until == FARGO_ST_SRC_D)) {
       // cells 7a-7c in one pass; it reads neighbours of the state, so its output goes to arrays of its own
       if (L.adi) s2.e = alt[0];
       s2.vx = alt[1]; s2.vy = alt[2]; s2.vz = alt[3];
@@ -638,6 +705,8 @@ struct Sim : CtxBase {
     // source step: intermediates live in transport set B (idle until the second pass)
       T *vxb = set_arr(1, 0), *vyb = set_arr(1, 1), *vzb = set_arr(1, 2), *ec = set_arr(1, 3);
       n += timed("source_a", [&] { return launch_source_a<T>(d, st, phi, vxb, vyb, vzb, stream); });                      // cell 7a
+      if (mhd_on && !mhd_passive)   // ... and the gradient of the magnetic pressure of the transverse components
+        n += timed("mhd_pressure", [&] { return launch_mhd_pressure<T>(d, st.rho, bfield[0], bfield[1], bfield[2], vxb, vyb, vzb, mu0, stream); });
       dbg["vxb"] = vxb; dbg["vyb"] = vyb; dbg["vzb"] = vzb;
       if (until == FARGO_ST_SRC_A) return n;
       T *vxc = st.vx, *vyc = st.vy, *vzc = st.vz;   // the state's velocities are dead after 7a (reading G18)
@@ -665,6 +734,13 @@ struct Sim : CtxBase {
       if (until == FARGO_ST_SRC_D) return n;
     }
     if (phase == 2) { s2m = s2; return n; }
+    if (mhd_on) {   // cells 8 and 10 (reading G34): the star values reach two zones out, so the ghosts of (e, v) are filled
+                    // before cell 8 as well as after it (8d changes the velocities)
+      n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });
+      n += timed("mhd_emf", [&] { return launch_mhd_emf<T>(d, st.rho, s2.vx, s2.vy, s2.vz, bfield[0], bfield[1], bfield[2], emf, bstar, mu0, eta, stream); });
+      if (!mhd_passive) n += timed("mhd_tension", [&] { return launch_mhd_tension<T>(d, st.rho, bfield, bstar, s2.vx, s2.vy, s2.vz, mu0, stream); });
+      n += timed("mhd_ct", [&] { return launch_mhd_ct<T>(d, emf, bfield[0], bfield[1], bfield[2], stream); });
+    }
   cell9:
     n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                      // cell 9
     if (until == FARGO_ST_BC2 || until == FARGO_ST_MOM || phase == 3) return n;
@@ -715,7 +791,7 @@ struct Sim : CtxBase {
     QSet<T> S;
     S.rho = st.rho;
     for (int q = 0; q < 7; ++q) S.q[q] = set_arr(ls, q);
-    if (fuse_dt) {                                                                   // cell 12d (+ cell 6 of the next update)
+    if (fuse_dt && !mhd_on) {                                                        // cell 12d (+ cell 6 of the next update)
       n += timed("newvel_dt", [&] { return launch_newvel_dt<T>(d, st.rho, st.e, S, st, stream); });
       dt_ready = true;
     } else {
@@ -735,7 +811,7 @@ struct Sim : CtxBase {
     // the legacy default stream cannot be captured: plain launches there
     const bool graph_ok = prm.use_graph && stream != nullptr && !prof;
     int s = 0;
-    if (graph_ok && fuse_dt && !dt_ready) {
+    if (graph_ok && fuse_dt && !mhd_on && !dt_ready) {
       // the captured sequence relies on the previous update's k_newvel_dt for the per-cell CFL rate: the first
       // update after fargo_set_fields gets it from the dt pass, after the ghost fill it reads through
       launches += launch_bc<T>(d, st, field_mask(true, true), stream);
@@ -786,6 +862,7 @@ struct Sim : CtxBase {
       dbg["rho"] = st.rho; dbg["e"] = st.e; dbg["vx"] = st.vx; dbg["vy"] = st.vy; dbg["vz"] = st.vz;
       dbg["phi"] = phi; dbg["v0"] = v0;
     }
+    if (L.mhd) { dbg["bx"] = bfield[0]; dbg["by"] = bfield[1]; dbg["bz"] = bfield[2]; dbg["emfx"] = emf[0]; dbg["emfy"] = emf[1]; dbg["emfz"] = emf[2]; }
     dbg["nshift"] = nshift;
     auto it = dbg.find(name);
     if (it == dbg.end() || !it->second) { err = std::string("array not available at this stage: ") + name; return FARGO_EINVAL; }
@@ -865,6 +942,10 @@ int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
 }
 int fargo_set_omega_frame(fargo_ctx* c, double omega_new) { return c ? c->impl->set_omega_frame(omega_new) : FARGO_EINVAL; }
 int fargo_diagnostics(fargo_ctx* c, double* out) { return c ? c->impl->diagnostics(out) : FARGO_EINVAL; }
+int fargo_set_bfield(fargo_ctx* c, const void* bx, const void* by, const void* bz, double mu0, double eta, int passive) {
+  return c ? c->impl->set_bfield(bx, by, bz, mu0, eta, passive) : FARGO_EINVAL;
+}
+int fargo_get_bfield(fargo_ctx* c, void* bx, void* by, void* bz) { return c ? c->impl->get_bfield(bx, by, bz) : FARGO_EINVAL; }
 int fargo_update_phase(fargo_ctx* c, int phase) { return c ? c->impl->update_phase(phase) : FARGO_EINVAL; }
 size_t fargo_halo_bytes(const fargo_ctx* c, int which, int dir) { return c ? c->impl->halo_bytes(which, dir) : 0; }
 int fargo_halo(fargo_ctx* c, int which, int dir, int side, int pack, void* device_buffer) {

@@ -68,7 +68,7 @@ int launch_potential(const Dev<T>& d, T* phi, T gm_star, T gm_planet, T xp, T yp
 // time step being the max over the directions present ("dt_i = min_j dt_ij").  max is exact,
 // so the block/grid reduction order does not matter: dt is bit-reproducible.
 template <typename T>
-__global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T> st, const T* __restrict__ v0) {
+__global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T> st, const T* __restrict__ v0, const MhdDt<T> M) {
   if (d.ctl->done) return;
   const int nrow = d.ny * d.nz;
   T m2 = T(0);
@@ -85,7 +85,13 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
     for (int ia = threadIdx.x; ia < d.nx; ia += blockDim.x) {
       const int i = d.ngx + ia;
       const long long l = d.id(i, j, k);
-      const T cs2 = (d.eos == EOS_ADI) ? rdiv(d.gg1 * st.e[l], st.rho[l]) : st.e[l] * st.e[l];
+      T cs2 = (d.eos == EOS_ADI) ? rdiv(d.gg1 * st.e[l], st.rho[l]) : st.e[l] * st.e[l];
+      if (M.bx && !M.passive) {   // item 1 of Eq. 59: C_w^2 = C_s^2 + v_A^2, B at the zone centre
+        const T cx = T(0.5) * (M.bx[l] + M.bx[d.id(d.xw(i + 1), j, k)]);
+        const T cy = T(0.5) * (M.by[l] + M.by[l + d.pitch]);
+        const T cz = T(0.5) * (M.bz[l] + M.bz[l + d.plane]);
+        cs2 = cs2 + rdiv(rfma(cz, cz, rfma(cy, cy, rfma(cx, cx, T(0)))), M.mu0 * st.rho[l]);
+      }
       const T I1sq = cs2 * il2;
       T I2 = T(0), I3 = T(0);
       if (d.hasx) {
@@ -104,7 +110,8 @@ __global__ void __launch_bounds__(256) k_dt_cells(const Dev<T> d, const State<T>
         I3 = rmax(I3, rabs(b - a) * ilz);
       }
       I3 = d.c3 * I3;
-      const T Isq = rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq)));
+      T Isq = rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq)));
+      if (M.bx && M.eta4 != T(0)) { const T I5 = M.eta4 * il2; Isq = rfma(I5, I5, Isq); }   // item 5: dt_5 = Delta^2 / (4 eta)
       m2 = rmax(m2, Isq);
     }
   }
@@ -236,19 +243,21 @@ __global__ void __launch_bounds__(1024) k_dt_finish(const Dev<T> d, const T* __r
 }
 
 template <typename T>
-int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode) {
+int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode, const MhdDt<T>* mhd) {
+  MhdDt<T> M{nullptr, nullptr, nullptr, T(1), T(0), 0};
+  if (mhd) M = *mhd;
   const int nrow = d.ny * d.nz;
   const int grid = nrow < 148 * 8 ? nrow : 148 * 8;
   if (mode == DT_FINISH) {   // the per-cell max was accumulated by k_newvel_dt at the end of the previous update
     k_dt_finish<T><<<1, 1024, 0, s>>>(d, v0);
     return 1;
   }
-  if (d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0) {
+  if (!M.bx && d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0) {
     const int g2 = nrow < 148 * 8 * 8 ? (nrow + 7) / 8 : 148 * 8;
     if (d.eos == EOS_ADI) k_dt_cells2<T, true><<<g2, 256, 0, s>>>(d, st, v0);
     else k_dt_cells2<T, false><<<g2, 256, 0, s>>>(d, st, v0);
   } else {
-    k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0);
+    k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0, M);
   }
   if (mode == DT_CELLS) return 1;
   k_dt_finish<T><<<1, 1024, 0, s>>>(d, v0);
@@ -292,7 +301,7 @@ int launch_selftest_div(const double* a, const double* b, double* out, long long
 #define INST(T)                                                                              \
   template int launch_vmean<T>(const Dev<T>&, const T*, T*, cudaStream_t);                   \
   template int launch_potential<T>(const Dev<T>&, T*, T, T, T, T, T, const T*, cudaStream_t);          \
-  template int launch_dt<T>(const Dev<T>&, const State<T>&, const T*, cudaStream_t, int);
+  template int launch_dt<T>(const Dev<T>&, const State<T>&, const T*, cudaStream_t, int, const MhdDt<T>*);
 INST(double)
 INST(float)
 #undef INST

@@ -1,0 +1,291 @@
+// k_mhd.cu -- SURVEY.md 8(f) NEXT-4: the MHD substeps of Fig. 2 on 3-D Cartesian meshes (sections 3.6.1-3.6.2):
+//   k_bc_b         cell 2    ghost fill of the face-centred field (the normal component keeps its boundary face)
+//   k_mhd_pressure cell 7a   gradient of the zone-centred magnetic pressure of the transverse components
+//   k_mhd_emf      cells 8a-8c  star values by the method of characteristics (Eqs. 80-83), electromotive forces (Eq. 84),
+//                            resistive term, and the "Lagrangian" star values of cell 8d (note 14)
+//   k_mhd_tension  cell 8d   magnetic tension on the velocities (Eq. 86)
+//   k_mhd_ct       cell 10   constrained transport (Eq. 76 with the signs of Eq. 101; reading G35)
+// and the Alfven speed for cell 6 (Eq. 59 item 1).  A first, plain version: one thread per edge / face, neighbours through
+// L1/L2; the expressions and their order are those of docs/ARITHMETIC.md ("MHD"), so the results agree with the CPU
+// oracle to rounding (bit for bit in fp64).  Product code: shares nothing with oracle/.
+// Directions 0, 1, 2 = X, Y, Z; (D1, D2, D3) cyclic; eps_D3 = v_D1 B_D2 - v_D2 B_D1 lives on the edge along D3 at the
+// lower-D1, lower-D2 corner of its cell; a component along D lives on the lower D face.
+#include "kernels.h"
+
+namespace fg {
+
+template <typename T> struct Cell { int n[3]; };
+
+template <typename T>
+__device__ __forceinline__ int ext_of(const Dev<T>& d, const int dir) { return dir == 0 ? d.TX : dir == 1 ? d.TY : d.TZ; }
+// the cell s steps along dir (X wraps when periodic)
+template <typename T>
+__device__ __forceinline__ Cell<T> mv(const Dev<T>& d, Cell<T> q, const int dir, const int s) {
+  int m = q.n[dir] + s;
+  if (dir == 0 && d.xwrap) { if (m < 0) m += d.nx; else if (m >= d.nx) m -= d.nx; }
+  q.n[dir] = m;
+  return q;
+}
+template <typename T>
+__device__ __forceinline__ long long at(const Dev<T>& d, const Cell<T>& q) { return d.id(q.n[0], q.n[1], q.n[2]); }
+template <typename T>
+__device__ __forceinline__ T width(const Dev<T>& d, const int dir, const int n) { return dir == 0 ? d.dx : dir == 1 ? d.LY[n] : d.dz[n]; }
+template <typename T>   // 1 / (centre n - centre n-1)
+__device__ __forceinline__ T invdist(const Dev<T>& d, const int dir, const int n) { return dir == 0 ? d.invdx : dir == 1 ? d.invDY[n] : d.invdzc[n]; }
+template <typename T>
+__device__ __forceinline__ bool fits(const Dev<T>& d, const int dir, const int n, const int lo, const int hi) {
+  if (dir == 0 && d.xwrap) return true;
+  return n - lo >= 0 && n + hi < ext_of(d, dir);
+}
+
+// van Leer slope along dir at cell q
+template <typename T>
+__device__ __forceinline__ T slope_at(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir) {
+  const T f0 = f[at(d, q)], fm = f[at(d, mv(d, q, dir, -1))], fp = f[at(d, mv(d, q, dir, +1))];
+  const T dm = (f0 - fm) * invdist(d, dir, q.n[dir]);
+  const T dp = (fp - f0) * invdist(d, dir, dir == 0 ? q.n[dir] : q.n[dir] + 1);
+  const T pr = dm * dp;
+  const bool flat = pr <= T(0);
+  const T a = rdiv(T(2) * pr, flat ? T(1) : dm + dp);
+  return flat ? T(0) : a;
+}
+// f on the lower dir face of cell q at half time step, carried at speed w (Eq. 48)
+template <typename T>
+__device__ __forceinline__ T star_at(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir, const T w, const T dt) {
+  if (w >= T(0)) {
+    const Cell<T> qm = mv(d, q, dir, -1);
+    return rfma(slope_at(d, f, qm, dir), rfma(-w, dt, width(d, dir, qm.n[dir])) * T(0.5), f[at(d, qm)]);
+  }
+  return rfma(-slope_at(d, f, q, dir), rfma(w, dt, width(d, dir, q.n[dir])) * T(0.5), f[at(d, q)]);
+}
+
+template <typename T> struct Vec3 { T* c[3]; };
+
+// ---- cell 2 ------------------------------------------------------------------------------------------------------------
+template <typename T, int DIR>
+__global__ void k_bc_b(const Dev<T> d, const Vec3<T> b) {
+  if (d.ctl->done) return;
+  const int N = DIR == 0 ? d.nx : DIR == 1 ? d.ny : d.nz;
+  const int ng = DIR == 0 ? d.ngx : DIR == 1 ? d.ngy : d.ngz;
+  const int P = DIR == 0 ? d.TY : d.TX, Q = DIR == 2 ? d.TY : d.TZ;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x, q = blockIdx.y;
+  if (p >= P || q >= Q) return;
+  const long long base = DIR == 0 ? d.id(0, p, q) : DIR == 1 ? d.id(p, 0, q) : d.id(p, q, 0);
+  const long long str = DIR == 0 ? 1 : DIR == 1 ? d.pitch : d.plane;
+  const int m0 = ng, m1 = ng + N, lo = d.bc[DIR][0], hi = d.bc[DIR][1];
+#pragma unroll
+  for (int f = 0; f < 3; ++f) {
+    T* a = b.c[f] + base;
+    const bool normal = f == DIR;
+    for (int g = 0; g < ng; ++g) {
+      if (lo == BC_PERIODIC) a[(m0 - 1 - g) * str] = a[(m1 - 1 - g) * str];
+      else if (lo == BC_OUTFLOW) a[(m0 - 1 - g) * str] = a[m0 * str];
+      else a[(m0 - 1 - g) * str] = normal ? a[(m0 + 1 + g) * str] : a[(m0 + g) * str];
+      if (hi == BC_PERIODIC) a[(m1 + g) * str] = a[(m0 + g) * str];
+      else if (normal) { if (g >= 1) a[(m1 + g) * str] = hi == BC_OUTFLOW ? a[m1 * str] : a[(m1 - g) * str]; }
+      else a[(m1 + g) * str] = hi == BC_OUTFLOW ? a[(m1 - 1) * str] : a[(m1 - 1 - g) * str];
+    }
+  }
+}
+
+template <typename T>
+int launch_bc_b(const Dev<T>& d, T* bx, T* by, T* bz, cudaStream_t s) {
+  Vec3<T> b{{bx, by, bz}};
+  int n = 0;
+  if (d.ngx > 0) { k_bc_b<T, 0><<<dim3((d.TY + 63) / 64, d.TZ), 64, 0, s>>>(d, b); ++n; }
+  if (d.ngy > 0) { k_bc_b<T, 1><<<dim3((d.TX + 127) / 128, d.TZ), 128, 0, s>>>(d, b); ++n; }
+  if (d.ngz > 0) { k_bc_b<T, 2><<<dim3((d.TX + 127) / 128, d.TY), 128, 0, s>>>(d, b); ++n; }
+  return n;
+}
+
+// ---- cell 7a: v_b -= dt * 2 / (rho + rho_-) * (Pm - Pm_-) / Delta, Pm = (B_a^2 + B_b^2) / (2 mu0) at the zone centre ------
+template <typename T>
+__device__ __forceinline__ T pmag(const Dev<T>& d, const Vec3<T>& b, const Cell<T>& q, const int dir, const T mu0) {
+  T s = T(0);
+#pragma unroll
+  for (int t = 1; t <= 2; ++t) {
+    const int a = (dir + t) % 3;
+    const T bc = T(0.5) * (b.c[a][at(d, q)] + b.c[a][at(d, mv(d, q, a, +1))]);
+    s = rfma(bc, bc, s);
+  }
+  return rdiv(s, T(2) * mu0);
+}
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_pressure(const Dev<T> d, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.TX) return;
+  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const T dt = (T)d.ctl->dt;
+#pragma unroll
+  for (int dir = 0; dir < 3; ++dir) {
+    const int da = (dir + 1) % 3, db = (dir + 2) % 3;
+    if (!fits(d, dir, q.n[dir], 1, 0) || !fits(d, da, q.n[da], 0, 1) || !fits(d, db, q.n[db], 0, 1)) continue;
+    const Cell<T> qm = mv(d, q, dir, -1);
+    const long long l = at(d, q);
+    const T wf = rdiv(T(2) * invdist(d, dir, q.n[dir]), rho[l] + rho[at(d, qm)]);
+    vb.c[dir][l] = rfma(-dt, wf * (pmag(d, b, q, dir, mu0) - pmag(d, b, qm, dir, mu0)), vb.c[dir][l]);
+  }
+}
+template <typename T>
+int launch_mhd_pressure(const Dev<T>& d, const T* rho, T* bx, T* by, T* bz, T* vxb, T* vyb, T* vzb, double mu0, cudaStream_t s) {
+  k_mhd_pressure<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0);
+  return 1;
+}
+
+// ---- cells 8a-8c (+ the star values of 8d): one thread per edge along D3 ----------------------------------------------
+template <typename T, int D3>
+__global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d, const T* __restrict__ rho, const Vec3<T> v, const Vec3<T> b,
+                                                 T* __restrict__ E, T* __restrict__ S1, T* __restrict__ S2, const T mu0, const T eta) {
+  constexpr int D1 = (D3 + 1) % 3, D2 = (D3 + 2) % 3;
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.TX) return;
+  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const long long l = at(d, q);
+  const T* __restrict__ V1 = v.c[D1];
+  const T* __restrict__ V2 = v.c[D2];
+  const T* __restrict__ B1 = b.c[D1];
+  const T* __restrict__ B2 = b.c[D2];
+  if (!fits(d, D1, q.n[D1], 2, 1) || !fits(d, D2, q.n[D2], 2, 1)) { E[l] = T(0); S1[l] = B1[l]; S2[l] = B2[l]; return; }
+  const T dt = (T)d.ctl->dt;
+  const Cell<T> q1 = mv(d, q, D1, -1), q2 = mv(d, q, D2, -1), q12 = mv(d, q1, D2, -1);
+  const long long l1 = at(d, q1), l2 = at(d, q2);
+  // density at the edge: the four zones around it
+  const T ro = T(0.25) * (((rho[l] + rho[l1]) + rho[l2]) + rho[at(d, q12)]);
+  const T sr = rsqrt_ieee(mu0 * ro);
+  // upwind estimates of the transverse fields (superscript u)
+  const T v2bar = T(0.5) * (V2[l] + V2[l1]);
+  const T v1bar = T(0.5) * (V1[l] + V1[l2]);
+  const T v1u = star_at(d, V1, q, D2, v2bar, dt), B1u = star_at(d, B1, q, D2, v2bar, dt);
+  const T v2u = star_at(d, V2, q, D1, v1bar, dt), B2u = star_at(d, B2, q, D1, v1bar, dt);
+  T v2s, B2s, v1s, B1s;
+  {   // (v_D2*, B_D2*): 1.5-D problem along D1 (Eqs. 80-83)
+    const T a = rdiv(B1u, sr);
+    const T Cp = v1u - a, Cm = v1u + a;
+    const T vp = star_at(d, V2, q, D1, Cp, dt), Bp = star_at(d, B2, q, D1, Cp, dt);
+    const T vm = star_at(d, V2, q, D1, Cm, dt), Bm = star_at(d, B2, q, D1, Cm, dt);
+    v2s = T(0.5) * ((vp + vm) + rdiv(Bp - Bm, sr));
+    B2s = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
+  }
+  {   // (v_D1*, B_D1*): 1.5-D problem along D2
+    const T a = rdiv(B2u, sr);
+    const T Cp = v2u - a, Cm = v2u + a;
+    const T vp = star_at(d, V1, q, D2, Cp, dt), Bp = star_at(d, B1, q, D2, Cp, dt);
+    const T vm = star_at(d, V1, q, D2, Cm, dt), Bm = star_at(d, B1, q, D2, Cm, dt);
+    v1s = T(0.5) * ((vp + vm) + rdiv(Bp - Bm, sr));
+    B1s = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
+  }
+  T emf = T(0.5) * (((v1s * B2u + B2s * v1u) - v2s * B1u) - B1s * v2u);   // Eq. 84
+  if (eta != T(0)) {   // cell 8c: - eta (curl B)_D3
+    T J = (B2[l] - B2[l1]) * invdist(d, D1, q.n[D1]);
+    J = J - (B1[l] - B1[l2]) * invdist(d, D2, q.n[D2]);
+    emf = rfma(-eta, J, emf);
+  }
+  E[l] = emf;
+  {   // cell 8d star values: characteristic speeds -+ B / sqrt(mu0 rho) only
+    const T a = rdiv(T(0.5) * (B2[l] + B2[l1]), sr);
+    const T vp = star_at(d, V1, q, D2, -a, dt), Bp = star_at(d, B1, q, D2, -a, dt);
+    const T vm = star_at(d, V1, q, D2, a, dt), Bm = star_at(d, B1, q, D2, a, dt);
+    S1[l] = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
+  }
+  {
+    const T a = rdiv(T(0.5) * (B1[l] + B1[l2]), sr);
+    const T vp = star_at(d, V2, q, D1, -a, dt), Bp = star_at(d, B2, q, D1, -a, dt);
+    const T vm = star_at(d, V2, q, D1, a, dt), Bm = star_at(d, B2, q, D1, a, dt);
+    S2[l] = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
+  }
+}
+
+template <typename T>
+int launch_mhd_emf(const Dev<T>& d, const T* rho, T* vx, T* vy, T* vz, T* bx, T* by, T* bz, T* const* emf, T* const* bstar,
+                   double mu0, double eta, cudaStream_t s) {
+  const Vec3<T> v{{vx, vy, vz}}, b{{bx, by, bz}};
+  dim3 g((d.TX + 127) / 128, d.TY, d.TZ);
+  k_mhd_emf<T, 0><<<g, 128, 0, s>>>(d, rho, v, b, emf[0], bstar[0], bstar[1], (T)mu0, (T)eta);
+  k_mhd_emf<T, 1><<<g, 128, 0, s>>>(d, rho, v, b, emf[1], bstar[2], bstar[3], (T)mu0, (T)eta);
+  k_mhd_emf<T, 2><<<g, 128, 0, s>>>(d, rho, v, b, emf[2], bstar[4], bstar[5], (T)mu0, (T)eta);
+  return 3;
+}
+
+// ---- cell 8d: Eq. 86; cell 10: Eq. 76 ---------------------------------------------------------------------------------------
+// bstar[2 D3 + 0] = B_D1* and bstar[2 D3 + 1] = B_D2* on the edges along D3.  For v_D (D, DA, DB cyclic): B_D* on the edges
+// along DB is bstar[2 DB + 0] (there D1 = D), on the edges along DA it is bstar[2 DA + 1] (there D2 = D).
+template <typename T>
+struct MhdArrays { const T* b[3]; const T* emf[3]; const T* bstar[6]; };
+
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d, const T* __restrict__ rho, const MhdArrays<T> A, const Vec3<T> v, const T mu0) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.TX) return;
+  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const long long l = at(d, q);
+  const T dt = (T)d.ctl->dt;
+#pragma unroll
+  for (int D = 0; D < 3; ++D) {
+    const int DA = (D + 1) % 3, DB = (D + 2) % 3;
+    if (!fits(d, D, q.n[D], 2, 1) || !fits(d, DA, q.n[DA], 2, 2) || !fits(d, DB, q.n[DB], 2, 2)) continue;
+    const T* __restrict__ Ba = A.b[DA];
+    const T* __restrict__ Bb = A.b[DB];
+    const T* __restrict__ Sa = A.bstar[2 * DB + 0];
+    const T* __restrict__ Sb = A.bstar[2 * DA + 1];
+    const Cell<T> qm = mv(d, q, D, -1), qa = mv(d, q, DA, +1), qb = mv(d, q, DB, +1);
+    const long long lm = at(d, qm), la = at(d, qa), lb = at(d, qb);
+    const T Bbar_a = T(0.25) * (((Ba[l] + Ba[la]) + Ba[lm]) + Ba[at(d, mv(d, qm, DA, +1))]);
+    const T Bbar_b = T(0.25) * (((Bb[l] + Bb[lb]) + Bb[lm]) + Bb[at(d, mv(d, qm, DB, +1))]);
+    T acc = Bbar_a * rdiv(Sa[la] - Sa[l], width(d, DA, q.n[DA]));
+    acc = rfma(Bbar_b, rdiv(Sb[lb] - Sb[l], width(d, DB, q.n[DB])), acc);
+    const T wf = rdiv(T(2), mu0 * (rho[l] + rho[lm]));
+    v.c[D][l] = rfma(dt, wf * acc, v.c[D][l]);
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_ct(const Dev<T> d, const MhdArrays<T> A, const Vec3<T> b) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.TX) return;
+  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const long long l = at(d, q);
+  const T dt = (T)d.ctl->dt;
+#pragma unroll
+  for (int D = 0; D < 3; ++D) {
+    const int DA = (D + 1) % 3, DB = (D + 2) % 3;
+    if (!fits(d, D, q.n[D], 2, 1) || !fits(d, DA, q.n[DA], 2, 2) || !fits(d, DB, q.n[DB], 2, 2)) continue;
+    const T* __restrict__ Eb = A.emf[DB];
+    const T* __restrict__ Ea = A.emf[DA];
+    T curl = rdiv(Eb[at(d, mv(d, q, DA, +1))] - Eb[l], width(d, DA, q.n[DA]));
+    curl = curl - rdiv(Ea[at(d, mv(d, q, DB, +1))] - Ea[l], width(d, DB, q.n[DB]));
+    b.c[D][l] = rfma(dt, curl, b.c[D][l]);
+  }
+}
+
+template <typename T>
+int launch_mhd_tension(const Dev<T>& d, const T* rho, T* const* b, T* const* bstar, T* vx, T* vy, T* vz, double mu0, cudaStream_t s) {
+  MhdArrays<T> A;
+  for (int n = 0; n < 3; ++n) { A.b[n] = b[n]; A.emf[n] = nullptr; }
+  for (int n = 0; n < 6; ++n) A.bstar[n] = bstar[n];
+  k_mhd_tension<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, A, Vec3<T>{{vx, vy, vz}}, (T)mu0);
+  return 1;
+}
+template <typename T>
+int launch_mhd_ct(const Dev<T>& d, T* const* emf, T* bx, T* by, T* bz, cudaStream_t s) {
+  MhdArrays<T> A;
+  for (int n = 0; n < 3; ++n) { A.b[n] = nullptr; A.emf[n] = emf[n]; }
+  for (int n = 0; n < 6; ++n) A.bstar[n] = nullptr;
+  k_mhd_ct<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, A, Vec3<T>{{bx, by, bz}});
+  return 1;
+}
+
+#define INST(T)                                                                                                          \
+  template int launch_bc_b<T>(const Dev<T>&, T*, T*, T*, cudaStream_t);                                                  \
+  template int launch_mhd_pressure<T>(const Dev<T>&, const T*, T*, T*, T*, T*, T*, T*, double, cudaStream_t);            \
+  template int launch_mhd_emf<T>(const Dev<T>&, const T*, T*, T*, T*, T*, T*, T*, T* const*, T* const*, double, double, cudaStream_t); \
+  template int launch_mhd_tension<T>(const Dev<T>&, const T*, T* const*, T* const*, T*, T*, T*, double, cudaStream_t);   \
+  template int launch_mhd_ct<T>(const Dev<T>&, T* const*, T*, T*, T*, cudaStream_t);
+INST(double)
+INST(float)
+#undef INST
+
+}  // namespace fg

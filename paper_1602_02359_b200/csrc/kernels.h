@@ -28,7 +28,10 @@ template <typename T> int launch_frame_change(const Dev<T>& d, T* vx, double dom
 template <typename T> int launch_diagnostics(const Dev<T>& d, const State<T>& st, double* part, cudaStream_t s);
 // cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
 enum { DT_BOTH = 0, DT_FINISH = 1, DT_CELLS = 2 };   // per-cell max + finish | finish only | per-cell max only
-template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode = DT_BOTH);
+// MHD (NEXT-4): the face-centred field for the fast magnetosonic speed, 4 eta for the resistive limit (bx = nullptr: off)
+template <typename T> struct MhdDt { const T *bx, *by, *bz; T mu0, eta4; int passive; };
+template <typename T> int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, int mode = DT_BOTH,
+                                    const MhdDt<T>* mhd = nullptr);
 // cell 7a: st -> vb[3]
 template <typename T> int launch_source_a(const Dev<T>& d, const State<T>& st, const T* phi, T* vxb, T* vyb, T* vzb,
                                           cudaStream_t s);
@@ -89,6 +92,17 @@ int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s);
 int launch_dt_sync(Ctl* ctl, double t_stop, bool single, cudaStream_t s);
 // out[n] = rdiv(a[n], b[n]): the kernels' branch-free division, exposed for its self-test
 int launch_selftest_div(const double* a, const double* b, double* out, long long n, cudaStream_t s);
+
+// MHD on 3-D Cartesian meshes (NEXT-4, k_mhd.cu): ghost fill of B; magnetic pressure in 7a (on v_b, in place); star values
+// and EMFs (emf[3]; bstar[6]: [2 d3] = B_d1*, [2 d3 + 1] = B_d2* on the edges along d3); tension (8d) and CT (10), in place
+template <typename T> int launch_bc_b(const Dev<T>& d, T* bx, T* by, T* bz, cudaStream_t s);
+template <typename T> int launch_mhd_pressure(const Dev<T>& d, const T* rho, T* bx, T* by, T* bz, T* vxb, T* vyb, T* vzb, double mu0,
+                                              cudaStream_t s);
+template <typename T> int launch_mhd_emf(const Dev<T>& d, const T* rho, T* vx, T* vy, T* vz, T* bx, T* by, T* bz, T* const* emf,
+                                         T* const* bstar, double mu0, double eta, cudaStream_t s);
+template <typename T> int launch_mhd_tension(const Dev<T>& d, const T* rho, T* const* b, T* const* bstar, T* vx, T* vy, T* vz,
+                                             double mu0, cudaStream_t s);
+template <typename T> int launch_mhd_ct(const Dev<T>& d, T* const* emf, T* bx, T* by, T* bz, cudaStream_t s);
 
 // active cells <-> ghosted, padded device layout
 template <typename T> int launch_scatter(const Dev<T>& d, const T* active, T* full, cudaStream_t s);

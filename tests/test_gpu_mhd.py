@@ -1,0 +1,140 @@
+"""GPU parity for the MHD substeps (sections 3.6.1-3.6.2; csrc/k_mhd.cu) against the CPU oracle
+(oracle/mhd.cpp) on the same seeded inputs, through the C ABI (fargo_set_bfield / fargo_step / fargo_get_bfield):
+fields and B within 1e-10 (fp64; bit-identical in practice), the clock bit-equal, the EMFs of the last update compared
+edge by edge, div B at rounding level.  The oracle itself is pinned in tests/test_oracle_mhd.py (among others to the
+field-loop energy the paper prints)."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle.binding import Oracle
+from paper_1602_02359_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+P, O, R = W.PERIODIC, W.OUTFLOW, W.REFLECTING
+TOL64, TOL32 = 1e-10, 1e-4
+
+
+def _box(nx, ny, nz, bc):
+    return W.Mesh(nx, ny, nz, 0.0, 1.0, W.uedges(0.0, 0.8, ny), W.uedges(-0.3, 0.4, nz), bc)
+
+
+def _curl_a(shape, dx, dy, dz, seed, amp):
+    r = np.random.default_rng(seed)
+    ax, ay, az = (amp * r.standard_normal(shape) for _ in range(3))
+    up = lambda a, axis: np.roll(a, -1, axis=axis)
+    return ((up(az, 1) - az) / dy - (up(ay, 0) - ay) / dz, (up(ax, 0) - ax) / dz - (up(az, 2) - az) / dx,
+            (up(ay, 2) - ay) / dx - (up(ax, 1) - ax) / dy)
+
+
+def _case(name):
+    r = np.random.default_rng(11)
+    if name == "brio_wu":          # section 5.2.1 on a thin 3-D mesh, 200 cells along z
+        n = 200
+        m = W.Mesh(4, 4, n, 0.0, 16.0, W.uedges(0.0, 16.0, 4), W.uedges(0.0, 800.0, n), ((P, P), (P, P), (O, O)))
+        shape = (n, 4, 4)
+        left = (np.arange(n) < n // 2)[:, None, None] * np.ones(shape, dtype=bool)
+        rho = np.where(left, 1.0, 0.1)
+        e = np.where(left, 1.0, 0.1) / (2.0 - 1.0)
+        z = np.zeros(shape)
+        return dict(mesh=m, eos=W.ADIABATIC, prm=W.Params(gamma=2.0), f=(rho, e, z, z, z), b=(z, np.where(left, 1.0, -1.0), z + 0.75),
+                    nsteps=60, eta=0.0, passive=False)
+    bcs = {"periodic": ((P, P), (P, P), (P, P)), "mixed": ((O, R), (R, O), (O, O)), "resistive": ((P, P), (O, O), (P, P)),
+           "passive": ((P, P), (P, P), (P, P)), "iso": ((P, P), (P, P), (R, R))}
+    nx, ny, nz = (34, 13, 11) if name != "mixed" else (21, 12, 14)
+    m = _box(nx, ny, nz, bcs[name])
+    shape = (nz, ny, nx)
+    bx, by, bz = _curl_a(shape, 1.0 / nx, 0.8 / ny, 0.7 / nz, 3, 0.02)
+    bx += 0.4; by -= 0.3; bz += 0.2
+    rho = 1.0 + 0.3 * r.uniform(-1, 1, shape)
+    eos = W.ISOTHERMAL if name == "iso" else W.ADIABATIC
+    e = 0.9 * (1.0 + 0.2 * r.uniform(-1, 1, shape)) if eos == W.ISOTHERMAL else 1.5 * (1.0 + 0.3 * r.uniform(-1, 1, shape))
+    v = tuple(0.6 * r.uniform(-1, 1, shape) for _ in range(3))
+    return dict(mesh=m, eos=eos, prm=W.Params(gamma=1.4), f=(rho, e) + v, b=(bx, by, bz), nsteps=6,
+                eta=3e-3 if name == "resistive" else 0.0, passive=name == "passive")
+
+
+def _pair(c, precision=64, use_graph=True):
+    from paper_1602_02359_b200 import Fargo
+    g = Fargo(c["mesh"], W.CARTESIAN, c["eos"], c["prm"], precision=precision, use_graph=use_graph, mhd=True)
+    g.set_fields(*c["f"])
+    g.set_bfield(*c["b"], eta=c["eta"], passive=c["passive"])
+    o = Oracle(c["mesh"], W.CARTESIAN, c["eos"], c["prm"])
+    o.set_fields(*c["f"])
+    o.set_bfield(*c["b"], eta=c["eta"], passive=c["passive"])
+    return g, o
+
+
+def _rel(a, b):
+    s = float(np.max(np.abs(b)))
+    d = float(np.max(np.abs(np.asarray(a, dtype=np.float64) - b)))
+    return d / s if s > 0 else d
+
+
+CASES = ["periodic", "mixed", "resistive", "passive", "iso", "brio_wu"]
+
+
+@pytest.mark.parametrize("name", CASES)
+@pytest.mark.parametrize("use_graph", [True, False], ids=["graph", "stream"])
+def test_mhd_updates_match_the_oracle(name, use_graph):
+    c = _case(name)
+    g, o = _pair(c, use_graph=use_graph)
+    g.step(c["nsteps"]); o.step(c["nsteps"])
+    assert g.time() == o.time(), (g.time(), o.time())
+    for nm, a, b in zip(("rho", "e", "vx", "vy", "vz"), g.get_fields(), o.get_fields()):
+        assert np.isfinite(a).all() and _rel(a, b) <= TOL64, (name, nm, _rel(a, b))
+    bg, bo = g.get_bfield(), o.get_bfield()
+    for nm, a, b in zip(("bx", "by", "bz"), bg, bo):
+        assert np.isfinite(a).all() and _rel(a, b) <= TOL64, (name, nm, _rel(a, b))
+        assert not np.array_equal(b, np.broadcast_to(c["b"]["xyz".index(nm[1])], b.shape)) or name == "brio_wu" and nm != "by"
+    # the electromotive forces of the last update, edge by edge, ghost zones included
+    for nm in ("emfx", "emfy", "emfz"):
+        a, b = g.array(nm), o.array(nm)
+        assert _rel(a, b) <= TOL64, (name, nm, _rel(a, b))
+    g.close(); o.close()
+
+
+def test_div_b_stays_at_rounding_level_on_the_gpu():
+    c = _case("periodic")
+    g, _ = _pair(c)
+    g.step(10)
+    bx, by, bz = g.get_bfield()
+    m = c["mesh"]
+    div = (np.roll(bx, -1, 2) - bx) * m.nx + (np.roll(by, -1, 1) - by) * (m.ny / 0.8) + (np.roll(bz, -1, 0) - bz) * (m.nz / 0.7)
+    scale = float(np.sqrt(np.mean(bx ** 2 + by ** 2 + bz ** 2))) * max(m.nx, m.ny / 0.8, m.nz / 0.7)
+    assert float(np.max(np.abs(div))) <= 1e-13 * scale
+    g.close()
+
+
+def test_mhd_fp32_build_is_close_to_the_fp64_oracle():
+    c = _case("periodic")
+    g, o = _pair(c, precision=32)
+    g.step(c["nsteps"]); o.step(c["nsteps"])
+    assert abs(g.time()[0] - o.time()[0]) <= 1e-5 * o.time()[0]
+    for a, b in zip(g.get_fields() + g.get_bfield(), o.get_fields() + o.get_bfield()):
+        assert a.dtype == np.float32 and _rel(a, b) <= TOL32, _rel(a, b)
+    g.close(); o.close()
+
+
+def test_mhd_argument_errors_and_second_set_bfield():
+    from paper_1602_02359_b200 import Fargo
+    c = _case("periodic")
+    g = Fargo(c["mesh"], W.CARTESIAN, c["eos"], c["prm"])          # created without mhd
+    g.set_fields(*c["f"])
+    with pytest.raises(RuntimeError):
+        g.set_bfield(*c["b"])
+    g.close()
+    with pytest.raises(ValueError):                                   # a 2-D mesh: thin 3-D meshes are the way
+        Fargo(W.Mesh(16, 16, 1, 0.0, 1.0, W.uedges(0, 1, 16), np.array([0.0, 1.0])), W.CARTESIAN, c["eos"], c["prm"], mhd=True)
+    g, o = _pair(c)
+    g.step(2); o.step(2)
+    for x in (g, o):                                                   # restart both from the same state with a new field
+        x.set_fields(*c["f"])
+        x.set_bfield(c["b"][0] * 0.5, c["b"][1], c["b"][2] * 2.0)
+    g.step(3); o.step(3)
+    assert g.time() == o.time()
+    for a, b in zip(g.get_bfield(), o.get_bfield()):
+        assert _rel(a, b) <= TOL64
+    g.close(); o.close()

@@ -49,6 +49,9 @@ def make_workload(name: str):
         n = int(name[5:])
         sample = W.noise_box(shape3=(n, min(n, 64), min(n, 64)))
         return W.noise_box(n), sample, "same recipe on a %dx%dx%d slab" % (n, min(n, 64), min(n, 64))
+    if name.startswith("mhd"):   # NEXT-4: the config-5 box threaded by a magnetic field (MOC + constrained transport)
+        n = int(name[3:])
+        return W.mhd_box(n), W.mhd_box(shape3=(n, min(n, 32), min(n, 32))), "same recipe on a %dx%dx%d slab" % (n, min(n, 32), min(n, 32))
     if name == "disk3d":
         return W.disk3d(), W.disk3d(1536, 32, 16), "same recipe on 1536x32x16 (full rings, fewer r and theta cells)"
     if name == "disk3dvisc":   # config 4 with a kinematic viscosity: the 3-D viscous stress of NEXT-1 (Eqs. B3, B6)
@@ -74,7 +77,7 @@ def make_workload(name: str):
 # roofline.traffic and the fp64-pipe figure are READ from the tracked raw ncu export of this workload
 # (profiles/ncu_raw_<workload>_<kernel source hash>.csv, see paper_1602_02359_b200/profiling.py); when the export was
 # captured on other kernel sources than the ones built here, traffic is null and the line says "stale".
-CONFIG_OF = {"sheet3d": "none (NEXT-1 workload)", "disk3dlive": "4 with a live planet (NEXT-2 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
+CONFIG_OF = {"mhd128": "5 with a magnetic field (NEXT-4 workload)", "mhd256": "5 with a magnetic field (NEXT-4 workload)", "mhd512": "5 with a magnetic field (NEXT-4 workload)", "sheet3d": "none (NEXT-1 workload)", "disk3dlive": "4 with a live planet (NEXT-2 workload)", "disk3dvisc": 4, "noise64": 5, "noise128": 5, "noise256": 5, "noise512": 5, "disk3d": 4, "disk2d": 3, "sound": 1, "sod": 2}
 
 
 def algorithmic_reals(w):
@@ -103,7 +106,12 @@ def algorithmic_reals(w):
         "potential": 1,     # live planets: Phi rewritten every update
         "planets": 1,       # gas force: rho read once per planet (ring served by L1 for the further ones)
         "newvel_dt": (1 + 2 * nd + (1 if adi else 0)) + nd,
+        # NEXT-4 (3-D): B joins the dt pass; pressure: rho, B, v_b -> v_b; emf (three kernels): rho, two v and two B
+        # components each -> eps and two star values; tension: rho, B, 6 star values, v -> v; ct: eps, B -> B
+        "mhd_pressure": (1 + 3 + 3) + 3, "mhd_emf": 3 * (1 + 2 + 2) + 9, "mhd_tension": (1 + 3 + 6 + 3) + 3, "mhd_ct": (3 + 3) + 3,
     }
+    if getattr(w, "bfield", None):
+        k["dt"] += 3
     if not adi:
         k["source_bc"] = 0
     else:
@@ -211,6 +219,8 @@ def oracle_rate(sample, steps, warmup):
     o.set_fields(*sample.fields())
     if sample.planets:
         o.set_planets(**sample.planets)
+    if sample.bfield:
+        o.set_bfield(**sample.bfield)
     o.step(warmup)
     t0 = time.perf_counter()
     o.step(steps)
@@ -264,7 +274,7 @@ def run_ours(args):
 
     w, sample, sample_desc = make_workload(args.workload)
     prec = 32 if args.fp32 else 64
-    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=prec)
+    g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=prec, mhd=w.bfield is not None)
     es = 8 if prec == 64 else 4
     ncell = w.mesh.ncells
     tdt = torch.float64 if prec == 64 else torch.float32
@@ -272,6 +282,8 @@ def run_ours(args):
     g.set_fields(*host_in)
     if w.planets:
         g.set_planets(**w.planets)
+    if w.bfield:
+        g.set_bfield(**w.bfield)
     K, Wm = args.steps, max(args.warmup, 3)
 
     # ---- region 1: device-resident throughput (graph replay) ----
@@ -312,7 +324,7 @@ def run_ours(args):
     for name, (nk, tms) in rep.items():
         key = "first_sweep" if name == first_sweep else ("sweep" if name.startswith("sweep") else name)
         r = reals.get(key, 0)
-        calls = K * (2 if name == "bc" else 1)
+        calls = K * ((3 if w.bfield else 2) if name == "bc" else 1)
         per_launch_ms = tms / calls
         gbs = (r * es * ncell / (per_launch_ms * 1e-3) / 1e9) if r else None
         kernels[name] = {"share": tms / total_ms, "ms_per_launch": per_launch_ms, "kernels": nk // calls,

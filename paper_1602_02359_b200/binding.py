@@ -112,7 +112,7 @@ class Fargo:
     """
 
     def __init__(self, mesh, geometry: int, eos: int, params, precision: int = 64, use_graph: bool = True,
-                 device: Optional[str] = None, kernel_plan: int = 0, mhd: bool = False):
+                 device: Optional[str] = None, kernel_plan: int = 0, mhd: bool = False, guard_bytes: int = 0):
         import torch
         L = load()
         if not torch.cuda.is_available():
@@ -158,10 +158,14 @@ class Fargo:
                 # the legacy default stream cannot be captured into a CUDA graph: give the context its own
                 self.stream = torch.cuda.Stream(self.device)
                 torch.cuda.current_stream(self.device).synchronize()
+            # guard_bytes > 0: a canary region before and after the workspace (check_guards(); compute-sanitizer is closed
+            # on this pool, so out-of-bounds writes next to the workspace are looked for this way)
+            self._guard = (int(guard_bytes) + 255) // 256 * 256
             with torch.cuda.stream(self.stream):   # the caching allocator ties the block to the stream that uses it
-                self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            base = self.workspace.data_ptr()
+                self.workspace = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr() + self._guard
             off = (-base) % 256
+            self._ws_off, self._ws_len = self._guard + off, nbytes
             p.workspace = base + off
             p.workspace_bytes = nbytes
             p.cuda_stream = self.stream.cuda_stream
@@ -190,6 +194,13 @@ class Fargo:
             self.close()
         except Exception:
             pass
+
+    def check_guards(self) -> bool:
+        """True when no byte of the canary regions around the workspace (guard_bytes) was written."""
+        self.stream.synchronize()
+        lo = self.workspace[:self._ws_off]                      # the guard and the alignment slack before the workspace
+        hi = self.workspace[self._ws_off + self._ws_len:]       # everything after it
+        return bool((lo == 0xA5).all().item()) and bool((hi == 0xA5).all().item())
 
     def _check(self, rc, what):
         if rc != 0:

@@ -5,8 +5,7 @@
 //                            resistive term, and the "Lagrangian" star values of cell 8d (note 14)
 //   k_mhd_tension  cell 8d   magnetic tension on the velocities (Eq. 86)
 //   k_mhd_ct       cell 10   constrained transport (Eq. 76 with the signs of Eq. 101; reading G35)
-// and the Alfven speed for cell 6 (Eq. 59 item 1).  A first, plain version: one thread per edge / face, neighbours through
-// L1/L2; the expressions and their order are those of docs/ARITHMETIC.md ("MHD"), so the results agree with the CPU
+// and the Alfven speed for cell 6 (Eq. 59 item 1).  One thread per edge / face, neighbours through L1/L2; the expressions and their order are those of docs/ARITHMETIC.md ("MHD"), so the results agree with the CPU
 // oracle to rounding (bit for bit in fp64).  Product code: shares nothing with oracle/.
 // Directions 0, 1, 2 = X, Y, Z; (D1, D2, D3) cyclic; eps_D3 = v_D1 B_D2 - v_D2 B_D1 lives on the edge along D3 at the
 // lower-D1, lower-D2 corner of its cell; a component along D lives on the lower D face.
@@ -38,25 +37,35 @@ __device__ __forceinline__ bool fits(const Dev<T>& d, const int dir, const int n
   return n - lo >= 0 && n + hi < ext_of(d, dir);
 }
 
-// van Leer slope along dir at cell q
-template <typename T>
-__device__ __forceinline__ T slope_at(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir) {
-  const T f0 = f[at(d, q)], fm = f[at(d, mv(d, q, dir, -1))], fp = f[at(d, mv(d, q, dir, +1))];
-  const T dm = (f0 - fm) * invdist(d, dir, q.n[dir]);
-  const T dp = (fp - f0) * invdist(d, dir, dir == 0 ? q.n[dir] : q.n[dir] + 1);
+// The linear reconstructions of f in the two zones next to the lower dir face of cell q: every star value on that face
+// (upwind estimate, the two feet of the characteristics, the Lagrangian ones: five per field) picks one of the two, so the
+// slopes -- a division each -- are formed once per field and face instead of once per star value.
+template <typename T> struct Recon {
+  T fm, f0, sm, s0, wm, w0;
+  __device__ __forceinline__ T star(const T w, const T dt) const {   // Eq. 48
+    return w >= T(0) ? rfma(sm, rfma(-w, dt, wm) * T(0.5), fm) : rfma(-s0, rfma(w, dt, w0) * T(0.5), f0);
+  }
+};
+template <typename T>   // van Leer slope
+__device__ __forceinline__ T slope3(const T fm, const T f0, const T fp, const T invd0, const T invdp) {
+  const T dm = (f0 - fm) * invd0, dp = (fp - f0) * invdp;
   const T pr = dm * dp;
   const bool flat = pr <= T(0);
   const T a = rdiv(T(2) * pr, flat ? T(1) : dm + dp);
   return flat ? T(0) : a;
 }
-// f on the lower dir face of cell q at half time step, carried at speed w (Eq. 48)
 template <typename T>
-__device__ __forceinline__ T star_at(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir, const T w, const T dt) {
-  if (w >= T(0)) {
-    const Cell<T> qm = mv(d, q, dir, -1);
-    return rfma(slope_at(d, f, qm, dir), rfma(-w, dt, width(d, dir, qm.n[dir])) * T(0.5), f[at(d, qm)]);
-  }
-  return rfma(-slope_at(d, f, q, dir), rfma(w, dt, width(d, dir, q.n[dir])) * T(0.5), f[at(d, q)]);
+__device__ __forceinline__ Recon<T> recon(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir) {
+  const Cell<T> qm = mv(d, q, dir, -1);
+  const T f2 = f[at(d, mv(d, qm, dir, -1))], f1 = f[at(d, qm)], f0 = f[at(d, q)], fp = f[at(d, mv(d, q, dir, +1))];
+  const int n = q.n[dir];
+  const T im = invdist(d, dir, dir == 0 ? n : n - 1), i0 = invdist(d, dir, n), ip = invdist(d, dir, dir == 0 ? n : n + 1);
+  Recon<T> r;
+  r.fm = f1; r.f0 = f0;
+  r.sm = slope3(f2, f1, f0, im, i0);
+  r.s0 = slope3(f1, f0, fp, i0, ip);
+  r.wm = width(d, dir, qm.n[dir]); r.w0 = width(d, dir, n);
+  return r;
 }
 
 template <typename T> struct Vec3 { T* c[3]; };
@@ -154,25 +163,25 @@ __global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d, const T* __rest
   // density at the edge: the four zones around it
   const T ro = T(0.25) * (((rho[l] + rho[l1]) + rho[l2]) + rho[at(d, q12)]);
   const T sr = rsqrt_ieee(mu0 * ro);
+  // the reconstructions every star value on this edge picks from: (v_D1, B_D1) along D2, (v_D2, B_D2) along D1
+  const Recon<T> rV1 = recon(d, V1, q, D2), rB1 = recon(d, B1, q, D2), rV2 = recon(d, V2, q, D1), rB2 = recon(d, B2, q, D1);
   // upwind estimates of the transverse fields (superscript u)
   const T v2bar = T(0.5) * (V2[l] + V2[l1]);
   const T v1bar = T(0.5) * (V1[l] + V1[l2]);
-  const T v1u = star_at(d, V1, q, D2, v2bar, dt), B1u = star_at(d, B1, q, D2, v2bar, dt);
-  const T v2u = star_at(d, V2, q, D1, v1bar, dt), B2u = star_at(d, B2, q, D1, v1bar, dt);
+  const T v1u = rV1.star(v2bar, dt), B1u = rB1.star(v2bar, dt);
+  const T v2u = rV2.star(v1bar, dt), B2u = rB2.star(v1bar, dt);
   T v2s, B2s, v1s, B1s;
   {   // (v_D2*, B_D2*): 1.5-D problem along D1 (Eqs. 80-83)
     const T a = rdiv(B1u, sr);
     const T Cp = v1u - a, Cm = v1u + a;
-    const T vp = star_at(d, V2, q, D1, Cp, dt), Bp = star_at(d, B2, q, D1, Cp, dt);
-    const T vm = star_at(d, V2, q, D1, Cm, dt), Bm = star_at(d, B2, q, D1, Cm, dt);
+    const T vp = rV2.star(Cp, dt), Bp = rB2.star(Cp, dt), vm = rV2.star(Cm, dt), Bm = rB2.star(Cm, dt);
     v2s = T(0.5) * ((vp + vm) + rdiv(Bp - Bm, sr));
     B2s = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
   }
   {   // (v_D1*, B_D1*): 1.5-D problem along D2
     const T a = rdiv(B2u, sr);
     const T Cp = v2u - a, Cm = v2u + a;
-    const T vp = star_at(d, V1, q, D2, Cp, dt), Bp = star_at(d, B1, q, D2, Cp, dt);
-    const T vm = star_at(d, V1, q, D2, Cm, dt), Bm = star_at(d, B1, q, D2, Cm, dt);
+    const T vp = rV1.star(Cp, dt), Bp = rB1.star(Cp, dt), vm = rV1.star(Cm, dt), Bm = rB1.star(Cm, dt);
     v1s = T(0.5) * ((vp + vm) + rdiv(Bp - Bm, sr));
     B1s = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
   }
@@ -185,14 +194,12 @@ __global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d, const T* __rest
   E[l] = emf;
   {   // cell 8d star values: characteristic speeds -+ B / sqrt(mu0 rho) only
     const T a = rdiv(T(0.5) * (B2[l] + B2[l1]), sr);
-    const T vp = star_at(d, V1, q, D2, -a, dt), Bp = star_at(d, B1, q, D2, -a, dt);
-    const T vm = star_at(d, V1, q, D2, a, dt), Bm = star_at(d, B1, q, D2, a, dt);
+    const T vp = rV1.star(-a, dt), Bp = rB1.star(-a, dt), vm = rV1.star(a, dt), Bm = rB1.star(a, dt);
     S1[l] = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
   }
   {
     const T a = rdiv(T(0.5) * (B1[l] + B1[l2]), sr);
-    const T vp = star_at(d, V2, q, D1, -a, dt), Bp = star_at(d, B2, q, D1, -a, dt);
-    const T vm = star_at(d, V2, q, D1, a, dt), Bm = star_at(d, B2, q, D1, a, dt);
+    const T vp = rV2.star(-a, dt), Bp = rB2.star(-a, dt), vm = rV2.star(a, dt), Bm = rB2.star(a, dt);
     S2[l] = T(0.5) * ((Bp + Bm) + sr * (vp - vm));
   }
 }

@@ -93,6 +93,7 @@ class Workload:
     vz: Optional[np.ndarray]
     nsteps: int
     planets: Optional[dict] = None   # live planets (NEXT-2): keyword arguments of set_planets, or None
+    bfield: Optional[dict] = None    # MHD (NEXT-4): keyword arguments of set_bfield (bx, by, bz, mu0, eta, passive), or None
 
     def fields(self):
         return self.rho, self.e, self.vx, self.vy, self.vz
@@ -264,3 +265,20 @@ def noise_box(n: int = 64, nsteps: int = 50, shape3: Optional[tuple] = None) -> 
     vz = (0.1 * uniform_pm1(4, m)).reshape(shape)
     return Workload("noise_box_%dx%dx%d" % (nx, ny, nz), mesh, CARTESIAN, ADIABATIC,
                     Params(gamma=gamma), rho, e, vx, vy, vz, nsteps)
+
+
+def mhd_box(n: int = 64, nsteps: int = 20, shape3: Optional[tuple] = None) -> Workload:
+    """NEXT-4: the noise box of config 5 threaded by a magnetic field: a uniform field (0.3, -0.2, 0.1) plus the discrete
+    curl of a seeded edge-centred vector potential (divergence-free to rounding), |B| ~ 0.4, beta ~ 10."""
+    w = noise_box(n, nsteps, shape3)
+    m = w.mesh
+    shape = (m.nz, m.ny, m.nx)
+    dx, dy, dz = m.dx, float(m.yedges[1] - m.yedges[0]), float(m.zedges[1] - m.zedges[0])
+    ax, ay, az = (0.02 * min(dx, dy, dz) * 8.0 * uniform_pm1(5 + f, m.ncells).reshape(shape) for f in range(3))
+    up = lambda a, axis: np.roll(a, -1, axis=axis)
+    bx = 0.3 + (up(az, 1) - az) / dy - (up(ay, 0) - ay) / dz
+    by = -0.2 + (up(ax, 0) - ax) / dz - (up(az, 2) - az) / dx
+    bz = 0.1 + (up(ay, 2) - ay) / dx - (up(ax, 1) - ax) / dy
+    w.name = w.name.replace("noise_box", "mhd_box")
+    w.bfield = dict(bx=bx, by=by, bz=bz, mu0=1.0, eta=0.0, passive=False)
+    return w

@@ -381,3 +381,27 @@ def test_division_is_correctly_rounded():
     bad = np.nonzero(got6 != ref6)[0]
     assert bad.size == 0, "rdiv6 first mismatch: %r / 6 -> gpu %r host %r (%d of %d)" % (
         a[bad[0]], got6[bad[0]], ref6[bad[0]], bad.size, n)
+
+
+GUARDED = [G.cart_adi_periodic_even, G.sph3d_iso_fargo, G.cart_adi_mixed_bc, G.cyl3d_visc_fargo, G.sheet3d_adi_fargo, G.sod_small,
+           G.yz_only_2d, G.sph3d_iso_fargo_odd]
+
+
+@pytest.mark.parametrize("make", GUARDED, ids=[m.__name__ for m in GUARDED])
+def test_nothing_is_written_outside_the_workspace(make):
+    """compute-sanitizer is closed on this GPU pool (profiles/r02b_final.md), so out-of-bounds writes are looked for with
+    1 MiB canary regions before and after the workspace: several updates through every kernel family (fused and
+    kernel-per-cell plans, both precisions), field I/O and the inspection calls must leave them untouched."""
+    from paper_1602_02359_b200 import Fargo
+    w = make()
+    for precision in (64, 32):
+        for plan in (0, 7):
+            g = Fargo(w.mesh, w.geometry, w.eos, w.params, precision=precision, kernel_plan=plan, guard_bytes=1 << 20)
+            g.set_fields(*w.fields())
+            g.step(3)
+            g.get_fields()
+            g.diagnostics()
+            g.step_until("SWEEP_X")
+            g.array("trho")
+            assert g.check_guards(), (w.name, precision, plan)
+            g.close()

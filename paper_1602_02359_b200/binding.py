@@ -162,10 +162,14 @@ class Fargo:
             # on this pool, so out-of-bounds writes next to the workspace are looked for this way)
             self._guard = (int(guard_bytes) + 255) // 256 * 256
             with torch.cuda.stream(self.stream):   # the caching allocator ties the block to the stream that uses it
-                self.workspace = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device)
+                self.workspace = torch.empty(nbytes + 256 + 2 * self._guard, dtype=torch.uint8, device=self.device)
             base = self.workspace.data_ptr() + self._guard
             off = (-base) % 256
             self._ws_off, self._ws_len = self._guard + off, nbytes
+            if self._guard:   # (a torch fill, on request only: no library kernel runs on the default path)
+                with torch.cuda.stream(self.stream):
+                    self.workspace[:self._ws_off].fill_(0xA5)
+                    self.workspace[self._ws_off + nbytes:].fill_(0xA5)
             p.workspace = base + off
             p.workspace_bytes = nbytes
             p.cuda_stream = self.stream.cuda_stream
@@ -197,6 +201,7 @@ class Fargo:
 
     def check_guards(self) -> bool:
         """True when no byte of the canary regions around the workspace (guard_bytes) was written."""
+        assert self._guard > 0, "the context was created without guard_bytes"
         self.stream.synchronize()
         lo = self.workspace[:self._ws_off]                      # the guard and the alignment slack before the workspace
         hi = self.workspace[self._ws_off + self._ws_len:]       # everything after it

@@ -68,11 +68,11 @@ extern "C" int oracle_set_fields(oracle_ctx* c, const double* rho, const double*
 }
 
 // NEXT-4: switch the MHD substeps on and load the face-centred field (active cells, like the velocities; a component of
-// an absent direction is uniform along it).  Cartesian meshes without orbital advection only.
+// an absent direction is uniform along it).  Cartesian meshes and the shearing sheet, with or without orbital advection.
 extern "C" int oracle_set_bfield(oracle_ctx* c, const double* bx, const double* by, const double* bz, double mu0,
                                  double eta, int passive) {
   if (!c || !bx || !by || !bz || !(mu0 > 0.0) || eta < 0.0) return -1;
-  if (c->geometry != ORC_CARTESIAN || c->shear || c->p.fargo_on) return -1;
+  if (c->geometry != ORC_CARTESIAN) return -1;   // (the shearing sheet has the Cartesian metric)
   for (vec* f : {&c->bx, &c->by, &c->bz, &c->emfx, &c->emfy, &c->emfz, &c->bstar[0][0], &c->bstar[0][1], &c->bstar[1][0],
                  &c->bstar[1][1], &c->bstar[2][0], &c->bstar[2][1]})
     f->assign(c->ncell(), 0.0);
@@ -137,6 +137,7 @@ static void full_update(oracle_ctx* c, int until) {
     orc_mhd_emf(o);                                                                                   // cells 8a-8c
     orc_mhd_lorentz(o);                                                                               // cell 8d
     orc_mhd_ct(o);                                                                                    // cell 10
+    orc_mhd_orbital(o);                                                                               // cell 11
   }
   orc_bc_fill(o, o.rho, o.e, o.vx, o.vy, o.vz);                 if (until == ORC_ST_BC2) return;      // cell 9
   orc_momenta(o);                                               if (until == ORC_ST_MOM) return;      // cell 12a
@@ -193,6 +194,20 @@ extern "C" int oracle_run_stage(oracle_ctx* c, int stage) {
     default: return -1;
   }
   c->midstep = true;
+  return 0;
+}
+// The same for the MHD substeps: 0 = ghost fill of B (cell 2), 1 = star values and EMFs (cells 8a-8c), 2 = tension (8d),
+// 3 = constrained transport (10), 4 = orbital advection of B (11; needs v0 of cell 3 and the current dt).
+extern "C" int oracle_run_mhd_stage(oracle_ctx* c, int which) {
+  if (!c || !c->mhd) return -1;
+  switch (which) {
+    case 0: orc_mhd_bc_fill(*c); break;
+    case 1: orc_mhd_emf(*c); break;
+    case 2: orc_mhd_lorentz(*c); break;
+    case 3: orc_mhd_ct(*c); break;
+    case 4: orc_mhd_orbital(*c); break;
+    default: return -1;
+  }
   return 0;
 }
 extern "C" int oracle_set_dt(oracle_ctx* c, double dt) { if (!c) return -1; c->dt = dt; return 0; }

@@ -83,6 +83,7 @@ def lib(omp: bool = False):
             L.oracle_diagnostics.argtypes = [vp, _DP]
             L.oracle_set_bfield.argtypes = [vp, _DP, _DP, _DP, C.c_double, C.c_double, C.c_int]
             L.oracle_get_bfield.argtypes = [vp, _DP, _DP, _DP]
+            L.oracle_run_mhd_stage.argtypes = [vp, C.c_int]
             L.oracle_max_divb.argtypes = [vp]
             L.oracle_max_divb.restype = C.c_double
             L.oracle_vanleer_slopes.argtypes = [C.c_int, _DP, _DP, _DP]
@@ -190,6 +191,11 @@ class Oracle:
         if self._L.oracle_get_bfield(self._h, *[_p(x) for x in out]) != 0:
             raise RuntimeError("no magnetic field set")
         return tuple(out)
+
+    def run_mhd_stage(self, name: str):
+        """One MHD substep on the arrays as they stand: BC_B, EMF, TENSION, CT or ORBITAL (cell 11)."""
+        if self._L.oracle_run_mhd_stage(self._h, ["BC_B", "EMF", "TENSION", "CT", "ORBITAL"].index(name)) != 0:
+            raise RuntimeError("oracle_run_mhd_stage failed")
 
     def max_divb(self) -> float:
         return float(self._L.oracle_max_divb(self._h))

@@ -68,6 +68,8 @@ int oracle_get_fields(oracle_ctx* c, double* rho, double* e, double* vx, double*
 int oracle_set_bfield(oracle_ctx* c, const double* bx, const double* by, const double* bz, double mu0, double eta, int passive);
 int oracle_get_bfield(oracle_ctx* c, double* bx, double* by, double* bz);
 double oracle_max_divb(oracle_ctx* c);
+/* one MHD substep on the arrays as they stand: 0 ghost fill of B, 1 EMFs, 2 tension, 3 CT, 4 orbital advection of B */
+int oracle_run_mhd_stage(oracle_ctx* c, int which);
 int oracle_step(oracle_ctx* c, int n);
 int oracle_get_time(oracle_ctx* c, double* t, double* last_dt, long long* nsteps);
 

@@ -7,7 +7,9 @@
 //   cell 8b  electromotive forces (Eq. 84)          cell 8c  resistive term (Eq. 74)
 //   cell 8d  magnetic tension on the velocities (Eq. 86) with the "Lagrangian" star values (note 14)
 //   cell 10  constrained transport (Eq. 76; signs fixed by Eq. 101 P:668 and by Faraday's law: reading G35)
-// Not here: curvilinear meshes (Eqs. 87-91), orbital advection of B (cell 11, section 3.7).
+//   cell 11  orbital advection of B by the upstream-averaged EMF (section 3.7, Eqs. 92-107), Cartesian meshes
+//            and the shearing sheet; the substeps of cell 8 then see the residual velocity v_X - v0 (reading G37)
+// Not here: curvilinear meshes (Eqs. 87-91).
 // CPU oracle, TEST INFRASTRUCTURE (see fargo_oracle.h): plain loops, one formula per line, the paper's notation.
 // Directions are numbered 0, 1, 2 = X, Y, Z; (d1, d2, d3) is always a cyclic permutation, eps_d3 = v_d1 B_d2 - v_d2 B_d1.
 // A field component along d lives on the LOWER d face of its cell; eps_d3 of cell q lives on the edge along d3
@@ -50,7 +52,7 @@ inline double star(const oracle_ctx& c, const vec& f, const Q& q, int d, double 
   return std::fma(-slope(c, f, q, d), std::fma(w, c.dt, width(c, d, q.n[d])) * 0.5, f[at(c, q)]);
 }
 
-inline vec& V(oracle_ctx& c, int d) { return d == 0 ? c.vx : d == 1 ? c.vy : c.vz; }
+inline vec& V(oracle_ctx& c, int d) { return d == 0 ? (c.p.fargo_on ? c.vxres : c.vx) : d == 1 ? c.vy : c.vz; }   // G37
 inline vec& B(oracle_ctx& c, int d) { return d == 0 ? c.bx : d == 1 ? c.by : c.bz; }
 inline vec& EMF(oracle_ctx& c, int d) { return d == 0 ? c.emfx : d == 1 ? c.emfy : c.emfz; }
 
@@ -133,6 +135,12 @@ void orc_mhd_source_a(oracle_ctx& c) {
 // the same edges: bstar[d3][0] = B_d1* from the 1.5-D problem along d2, bstar[d3][1] = B_d2* from the one along d1.
 void orc_mhd_emf(oracle_ctx& c) {
   const double mu0 = c.mu0, eta = c.eta;
+  if (c.p.fargo_on) {   // with orbital advection the MHD substeps see the residual velocity (reading G37)
+    c.vxres = c.vx;
+    for (int k = 0; k < c.TZ; ++k)
+      for (int j = 0; j < c.TY; ++j)
+        for (int i = 0; i < c.TX; ++i) c.vxres[c.id(i, j, k)] = c.vx[c.id(i, j, k)] - c.v0[c.rid(j, k)];
+  }
   for (int d3 = 0; d3 < 3; ++d3) {
     const int d1 = (d3 + 1) % 3, d2 = (d3 + 2) % 3;
     vec &V1 = V(c, d1), &V2 = V(c, d2), &B1 = B(c, d1), &B2 = B(c, d2), &E = EMF(c, d3);
@@ -209,7 +217,7 @@ void orc_mhd_lorentz(oracle_ctx& c) {
   for (int d = 0; d < 3; ++d) {
     if (!has(c, d)) continue;
     const int da = (d + 1) % 3, db = (d + 2) % 3;
-    vec& v = V(c, d);
+    vec& v = d == 0 ? c.vx : d == 1 ? c.vy : c.vz;
     const vec &Ba = B(c, da), &Bb = B(c, db);
     const vec &Sa = c.bstar[db][0];   // B_d* on the edges along db (d3 = db: d1 = d, d2 = da)
     const vec &Sb = c.bstar[da][1];   // B_d* on the edges along da (d3 = da: d1 = db, d2 = d)
@@ -266,4 +274,68 @@ double orc_mhd_divb(const oracle_ctx& c, int i, int j, int k) {
     s += (b[at(c, mv(c, q, d, +1))] - b[at(c, q)]) / width(c, d, q.n[d]);
   }
   return s;
+}
+
+// ---- cell 11: orbital advection of B (section 3.7).  d/dt B = curl (v0 x B) with v0 = v0(Y, Z) along X, integrated
+// over the whole step with the upstream average of the EMF (Eq. 96): the time integral of eps_Z at the edge
+// (i-1/2, j-1/2, k) is DX times the integral of B_Y over the arc of s = v0 dt / DX cells upstream of it, i.e. over
+// "as many zones as necessary" -- N = nint(s) whole zones, summed one after the other -- plus the residual
+// xi = s - N of a zone from the parabolic reconstruction of the orbital advection; v0 on a face is
+// the mean of the two zones next to it.  eps_Y = -v0 B_Z likewise on the edges (i-1/2, j, k-1/2); eps_X = 0.
+// The constrained-transport update with these integrals shifts B_Y and B_Z like zone-centred quantities (Eq. 103) and
+// gives B_X the shift plus the shear term (Eqs. 94, 104-107); div B keeps its value to rounding.
+// phi[i] of a row g = (integral of g over the arc upstream of the face i-1/2) / DX.
+static void arc_integrals(int n, const double* g, double s, double* phi) {
+  if (!std::isfinite(s) || std::fabs(s) > 4.0 * n) { for (int i = 0; i < n; ++i) phi[i] = s; return; }   // a blown-up run: no loop over ~inf zones
+  const double N = std::floor(s + 0.5), xi = s - N;   // reading G11
+  const int Ni = (int)N;
+  std::vector<double> gs(n);
+  oracle_ppa_star(n, g, xi, gs.data());                // gs[c]: mean of g over the part of the upwind zone that crosses face c+1/2
+  auto w = [n](int i) { int m = i % n; return m < 0 ? m + n : m; };
+  for (int i = 0; i < n; ++i) {                        // face i-1/2 = face (i-1)+1/2
+    double S = 0.0;
+    if (Ni > 0) for (int m = 0; m < Ni; ++m) S = S + g[w(i - 1 - m)];
+    if (Ni < 0) for (int m = 1; m <= -Ni; ++m) S = S - g[w(i - 1 + m)];
+    phi[i] = std::fma(xi, gs[w(i - 1 - Ni)], S);
+  }
+}
+void orc_mhd_orbital(oracle_ctx& c) {
+  if (!c.p.fargo_on) return;
+  const int n = c.TX;   // orbital advection needs a wrapped X axis: TX = nx
+  const double dt = c.dt, idx = 1.0 / c.dx;
+  vec &PZ = c.emfz, &PY = c.emfy;   // reused: the arc integrals on the Z edges (of B_Y) and on the Y edges (of B_Z)
+  std::vector<double> g(n), phi(n);
+  for (int k = 0; k < c.TZ; ++k)
+    for (int j = 0; j < c.TY; ++j) {
+      const size_t base = c.id(0, j, k);
+      for (int i = 0; i < n; ++i) { PZ[base + i] = 0.0; PY[base + i] = 0.0; }
+      if (!c.hasy || j >= 1) {   // Z edges of the Y face j-1/2: v0 = mean of the rings j-1 and j
+        const double v0f = c.hasy ? 0.5 * (c.v0[c.rid(j, k)] + c.v0[c.rid(j - 1, k)]) : c.v0[c.rid(j, k)];
+        for (int i = 0; i < n; ++i) g[i] = c.by[base + i];
+        arc_integrals(n, g.data(), (v0f * dt) * idx, phi.data());
+        for (int i = 0; i < n; ++i) PZ[base + i] = phi[i];
+      }
+      if (!c.hasz || k >= 1) {   // Y edges of the Z face k-1/2
+        const double v0f = c.hasz ? 0.5 * (c.v0[c.rid(j, k)] + c.v0[c.rid(j, k - 1)]) : c.v0[c.rid(j, k)];
+        for (int i = 0; i < n; ++i) g[i] = c.bz[base + i];
+        arc_integrals(n, g.data(), (v0f * dt) * idx, phi.data());
+        for (int i = 0; i < n; ++i) PY[base + i] = phi[i];
+      }
+    }
+  for (int k = 0; k < c.TZ; ++k)
+    for (int j = 0; j < c.TY; ++j) {
+      if ((c.hasy && (j < 1 || j + 1 >= c.TY)) || (c.hasz && (k < 1 || k + 1 >= c.TZ))) continue;
+      const size_t base = c.id(0, j, k);
+      for (int i = 0; i < n; ++i) {
+        const int ip = c.xw(i + 1);
+        const size_t l = base + i, lp = base + ip;
+        // B_X: DX [ (PZ(j+1) - PZ(j)) / DY + (PY(k+1) - PY(k)) / DZ ]   (Eq. 104 and its Z counterpart)
+        double d = 0.0;
+        if (c.hasy) d = (c.dx * (PZ[c.id(i, j + 1, k)] - PZ[l])) / c.LY[j];
+        if (c.hasz) d = d + (c.dx * (PY[c.id(i, j, k + 1)] - PY[l])) / c.dz[k];
+        c.bx[l] = c.bx[l] + d;
+        c.by[l] = c.by[l] - (PZ[lp] - PZ[l]);          // Eq. 101
+        c.bz[l] = c.bz[l] - (PY[lp] - PY[l]);
+      }
+    }
 }

@@ -52,6 +52,7 @@ struct oracle_ctx {
   double mu0 = 1.0, eta = 0.0;             // permeability, resistivity (Eq. 5)
   vec bx, by, bz, emfx, emfy, emfz;
   vec bstar[3][2];
+  vec vxres;                               // v_X - v0: what cell 8 sees under orbital advection (reading G37)
 
   vec rho, e, vx, vy, vz;              // state
   vec phi;                             // potential at centres (cell 5)
@@ -116,4 +117,5 @@ void orc_mhd_source_a(oracle_ctx& c);
 void orc_mhd_emf(oracle_ctx& c);
 void orc_mhd_lorentz(oracle_ctx& c);
 void orc_mhd_ct(oracle_ctx& c);
+void orc_mhd_orbital(oracle_ctx& c);
 double orc_mhd_divb(const oracle_ctx& c, int i, int j, int k);

@@ -96,8 +96,8 @@ typedef struct fargo_params {
   int use_graph;           /* 1: fargo_step replays one captured CUDA graph per update (needs a non-default
                               cuda_stream; on the legacy default stream it falls back to plain launches);
                               0: plain stream launches */
-  int mhd;                 /* 1: reserve the arrays of the MHD substeps (NEXT-4: B, the EMFs and the star values, 12 arrays);
-                              they run once fargo_set_bfield has been called.  3-D Cartesian meshes without orbital advection */
+  int mhd;                 /* 1: reserve the arrays of the MHD substeps (NEXT-4: B, the EMFs, the star values, v_X - v0: 13 arrays);
+                              they run once fargo_set_bfield has been called.  3-D Cartesian meshes and shearing sheets */
   int kernel_plan;         /* 0 = the fused kernels wherever they apply (default).  Bit flags select the unfused
                               sequences instead, for measurements and for tests that compare the two (results are
                               bit-identical): FARGO_PLAN_UNFUSED_SOURCE, FARGO_PLAN_UNFUSED_VISC, FARGO_PLAN_UNFUSED_DT */
@@ -169,10 +169,12 @@ int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
  * passive != 0: the field is transported and diffused but exerts no force (the current-sheet test).  From then on
  * every update also runs: the ghost fill of B (cell 2), C_w^2 = C_s^2 + v_A^2 and the resistive limit in Eq. 59 (cell 6),
  * the magnetic pressure gradient (cell 7a), star values and electromotive forces (cells 8a-8c, Eqs. 80-84), the
- * tension (cell 8d, Eq. 86) and the constrained-transport update (cell 10, Eq. 76), which keeps div B to rounding.
+ * tension (cell 8d, Eq. 86), the constrained-transport update (cell 10, Eq. 76), which keeps div B to rounding, and, with
+ * orbital advection on, the orbital advection of B by the upstream-averaged EMF (cell 11, section 3.7, Eqs. 92-107; the
+ * substeps of cell 8 then see the residual velocity v_X - v0).
  * The source step then runs as the kernel sequence 7a, 7b(c) (the magnetic pressure enters before 7b).
- * fargo_get_bfield copies the active cells out (any pointer may be NULL).  Not with orbital advection (section 3.7), on
- * sub-domains, or on curvilinear meshes (Eqs. 87-91): FARGO_EINVAL.  Errors: FARGO_EINVAL, FARGO_ESTATE, FARGO_ECUDA. */
+ * fargo_get_bfield copies the active cells out (any pointer may be NULL).  Cartesian meshes and the shearing sheet; not on
+ * sub-domains or on curvilinear meshes (Eqs. 87-91): FARGO_EINVAL.  Errors: FARGO_EINVAL, FARGO_ESTATE, FARGO_ECUDA. */
 int fargo_set_bfield(fargo_ctx* ctx, const void* bx, const void* by, const void* bz, double mu0, double eta, int passive);
 int fargo_get_bfield(fargo_ctx* ctx, void* bx, void* by, void* bz);
 

@@ -104,13 +104,13 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.fargo = p->fargo_on != 0;
   L.adi = eos == FARGO_ADIABATIC;
   L.mhd = p->mhd != 0;
-  if (L.mhd && !(cartesian_metric && geometry != FARGO_SHEARING_SHEET && L.hasx && L.hasy && L.hasz && !p->fargo_on)) {
-    err = "MHD: 3-D Cartesian meshes without orbital advection (1.5-D and 2.5-D problems run on thin 3-D meshes)"; return false;
+  if (L.mhd && !(cartesian_metric && L.hasx && L.hasy && L.hasz)) {
+    err = "MHD: 3-D Cartesian meshes and shearing sheets (1.5-D and 2.5-D problems run on thin 3-D meshes)"; return false;
   }
   for (int dd = 1; dd < 3 && L.mhd; ++dd)
     for (int s = 0; s < 2; ++s)
       if (m->bc[dd][s] == FARGO_EXTERNAL) { err = "MHD is not available on sub-domains"; return false; }
-  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4 + (L.mhd ? 12 : 0);   // state, Phi, two transport sets, the source step's output, MHD
+  L.n3d = 5 + (L.has_pot ? 1 : 0) + 16 + 4 + (L.mhd ? 13 : 0);   // state, Phi, two transport sets, the source step's output, MHD
   const size_t pad = 32;
   auto t1 = [&](int n) { return align_up((size_t)n, pad); };
   L.table_elems = 7 * t1(L.TY + 1) + 11 * t1(L.TY + 1) + 10 * t1(L.TZ + 1) + 6 * t1(L.TZ + 1) + 2 * t1(L.TX);
@@ -131,7 +131,7 @@ struct Sim : CtxBase {
   int npl = 0, pl_mode = 0;
   T* pool[16];
   T* alt[4];            // e, vx, vy, vz written by the fused source step (the state stays intact while it is read)
-  T *bfield[3] = {nullptr, nullptr, nullptr}, *emf[3], *bstar[6];   // MHD (NEXT-4): B on faces, EMFs and star values on edges
+  T *bfield[3] = {nullptr, nullptr, nullptr}, *emf[3], *bstar[6], *vxres = nullptr;   // MHD (NEXT-4): B on faces, EMFs and star values on edges
   bool mhd_on = false;  // fargo_set_bfield was called
   int mhd_passive = 0;
   double mu0 = 1.0, eta = 0.0;
@@ -305,6 +305,7 @@ struct Sim : CtxBase {
       for (int n = 0; n < 3; ++n) bfield[n] = arr();
       for (int n = 0; n < 3; ++n) emf[n] = arr();
       for (int n = 0; n < 6; ++n) bstar[n] = arr();
+      vxres = arr();   // v_X - v0: what cell 8 sees under orbital advection
     }
     if (off > p->workspace_bytes) { err = "internal: workspace overflow"; return FARGO_ENOMEM; }
 
@@ -557,7 +558,7 @@ struct Sim : CtxBase {
     if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
     const size_t nact = (size_t)L.nx * L.ny * L.nz;
     const size_t arrb = align_up((size_t)L.narr * sizeof(T), 256);
-    if (!ck(cudaMemsetAsync(bfield[0], 0, 12 * arrb, stream), "cudaMemsetAsync(B)")) return FARGO_ECUDA;
+    if (!ck(cudaMemsetAsync(bfield[0], 0, 13 * arrb, stream), "cudaMemsetAsync(B)")) return FARGO_ECUDA;
     const void* src[3] = {bx, by, bz};
     T* staging = pool[15];   // dead between updates
     for (int f = 0; f < 3; ++f) {
@@ -737,9 +738,13 @@ struct Sim : CtxBase {
     if (mhd_on) {   // cells 8 and 10 (reading G34): the star values reach two zones out, so the ghosts of (e, v) are filled
                     // before cell 8 as well as after it (8d changes the velocities)
       n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });
-      n += timed("mhd_emf", [&] { return launch_mhd_emf<T>(d, st.rho, s2.vx, s2.vy, s2.vz, bfield[0], bfield[1], bfield[2], emf, bstar, mu0, eta, stream); });
+      T* vx8 = s2.vx;   // with orbital advection cell 8 sees the residual velocity (reading G37)
+      if (L.fargo) { n += timed("mhd_resid", [&] { return launch_mhd_resid<T>(d, s2.vx, v0, vxres, stream); }); vx8 = vxres; }
+      n += timed("mhd_emf", [&] { return launch_mhd_emf<T>(d, st.rho, vx8, s2.vy, s2.vz, bfield[0], bfield[1], bfield[2], emf, bstar, mu0, eta, stream); });
       if (!mhd_passive) n += timed("mhd_tension", [&] { return launch_mhd_tension<T>(d, st.rho, bfield, bstar, s2.vx, s2.vy, s2.vz, mu0, stream); });
       n += timed("mhd_ct", [&] { return launch_mhd_ct<T>(d, emf, bfield[0], bfield[1], bfield[2], stream); });
+      if (L.fargo)   // cell 11: orbital advection of B (the arc integrals reuse the arrays of eps_Z and eps_Y)
+        n += timed("mhd_orbital", [&] { return launch_mhd_orbital<T>(d, v0, bfield[0], bfield[1], bfield[2], emf[2], emf[1], stream); });
     }
   cell9:
     n += timed("bc", [&] { return launch_bc<T>(d, s2, field_mask(false, L.adi), stream); });                      // cell 9

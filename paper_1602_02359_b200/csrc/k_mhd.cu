@@ -5,6 +5,7 @@
 //                            resistive term, and the "Lagrangian" star values of cell 8d (note 14)
 //   k_mhd_tension  cell 8d   magnetic tension on the velocities (Eq. 86)
 //   k_mhd_ct       cell 10   constrained transport (Eq. 76 with the signs of Eq. 101; reading G35)
+//   k_mhd_resid, k_mhd_arc, k_mhd_orbital   cell 11: orbital advection of B by the upstream-averaged EMF (section 3.7)
 // and the Alfven speed for cell 6 (Eq. 59 item 1).  One thread per edge / face, neighbours through L1/L2; the expressions and their order are those of docs/ARITHMETIC.md ("MHD"), so the results agree with the CPU
 // oracle to rounding (bit for bit in fp64).  Product code: shares nothing with oracle/.
 // Directions 0, 1, 2 = X, Y, Z; (D1, D2, D3) cyclic; eps_D3 = v_D1 B_D2 - v_D2 B_D1 lives on the edge along D3 at the
@@ -285,7 +286,105 @@ int launch_mhd_ct(const Dev<T>& d, T* const* emf, T* bx, T* by, T* bz, cudaStrea
   return 1;
 }
 
+// ---- cell 11: orbital advection of B (section 3.7, Eqs. 92-107) -------------------------------------------------------------
+// With orbital advection the substeps of cell 8 see the residual velocity v_X - v0 (reading G37).
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_resid(const Dev<T> d, const T* __restrict__ vx, const T* __restrict__ v0, T* __restrict__ vres) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= d.TX) return;
+  const long long l = d.id(i, j, k);
+  vres[l] = vx[l] - v0[d.rid(j, k)];
+}
+
+// Monotonised parabola of zone u of a periodic row: its left and right interface values
+template <typename T>
+__device__ __forceinline__ T ppa_dm(const T fm, const T f0, const T fp) {
+  const T a = f0 - fm, b = fp - f0, dd = T(0.5) * (fp - fm);
+  if (a * b <= T(0)) return T(0);
+  const T m = rmin(rmin(T(2) * rabs(a), T(2) * rabs(b)), rabs(dd));
+  return dd < T(0) ? -m : m;
+}
+template <typename T>
+__device__ __forceinline__ void ppa_zone(const T f2m, const T f1m, const T f0, const T f1p, const T f2p, T& fl, T& fr) {
+  const T dmm = ppa_dm(f2m, f1m, f0), dm0 = ppa_dm(f1m, f0, f1p), dmp = ppa_dm(f0, f1p, f2p);
+  fr = rfma(T(0.5), f1p - f0, f0) - rdiv6(dmp - dm0);      // Eq. 71
+  fl = rfma(T(0.5), f0 - f1m, f1m) - rdiv6(dm0 - dmm);
+  const T a = f0 - f1m, b = f1p - f0;
+  if (a * b <= T(0)) { fl = f0; fr = f0; return; }
+  const T D = fr - fl;
+  const T C = rfma(T(-0.5), fl + fr, f0);
+  const T DC = D * C, D26 = rdiv6(D * D);
+  if (DC > D26) fl = rfma(T(3), f0, -(T(2) * fr));
+  else if (-D26 > DC) fr = rfma(T(3), f0, -(T(2) * fl));
+}
+// (integral of g over the arc of s zones upstream of the face i-1/2) / DX, g a periodic row of n zones (Eq. 96):
+// the whole zones one after the other, then the residual fraction from the parabola of the zone it falls in
+template <typename T>
+__device__ __forceinline__ T arc_integral(const T* __restrict__ g, const int n, const int i, const T s) {
+  const T N = floor(s + T(0.5)), xi = s - N;
+  const int Ni = (int)N;
+  auto w = [n](int m) { m %= n; return m < 0 ? m + n : m; };
+  const int c = w(i - 1 - Ni);                         // the star value sits on the face c+1/2
+  const int u = xi >= T(0) ? c : w(c + 1);             // its upwind zone
+  T fl, fr;
+  const T fu = g[u];
+  ppa_zone(g[w(u - 2)], g[w(u - 1)], fu, g[w(u + 1)], g[w(u + 2)], fl, fr);
+  const T x = rabs(xi), x1x = x * (T(1) - x);
+  const T edge = xi >= T(0) ? fr : fl;
+  const T gs = rfma(x1x, rfma(T(2), fu, -fr) - fl, rfma(x, fu - edge, edge));
+  T S = T(0);
+  if (Ni > 0) for (int m = 0; m < Ni; ++m) S = S + g[w(i - 1 - m)];
+  if (Ni < 0) for (int m = 1; m <= -Ni; ++m) S = S - g[w(i - 1 + m)];
+  return rfma(xi, gs, S);
+}
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_arc(const Dev<T> d, const T* __restrict__ by, const T* __restrict__ bz,
+                                                 const T* __restrict__ v0, T* __restrict__ PZ, T* __restrict__ PY) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= d.TX) return;
+  const long long row = d.id(0, j, k), l = row + i;
+  const T dt = (T)d.ctl->dt;
+  T pz = T(0), py = T(0);
+  if (j >= 1) {   // Z edges of the Y face j-1/2: it moves with the mean of the rings j-1 and j
+    const T v0f = T(0.5) * (v0[d.rid(j, k)] + v0[d.rid(j - 1, k)]);
+    pz = arc_integral(by + row, d.nx, i, (v0f * dt) * d.invdx);
+  }
+  if (k >= 1) {   // Y edges of the Z face k-1/2
+    const T v0f = T(0.5) * (v0[d.rid(j, k)] + v0[d.rid(j, k - 1)]);
+    py = arc_integral(bz + row, d.nx, i, (v0f * dt) * d.invdx);
+  }
+  PZ[l] = pz; PY[l] = py;
+}
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_orbital(const Dev<T> d, const T* __restrict__ PZ, const T* __restrict__ PY, const Vec3<T> b) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= d.TX || j < 1 || j + 1 >= d.TY || k < 1 || k + 1 >= d.TZ) return;
+  const long long l = d.id(i, j, k), lp = d.id(d.xw(i + 1), j, k);
+  T dd = rdiv(d.dx * (PZ[l + d.pitch] - PZ[l]), d.LY[j]);              // Eq. 104 ...
+  dd = dd + rdiv(d.dx * (PY[l + d.plane] - PY[l]), d.dz[k]);            // ... and its Z counterpart
+  b.c[0][l] = b.c[0][l] + dd;
+  b.c[1][l] = b.c[1][l] - (PZ[lp] - PZ[l]);                             // Eq. 101
+  b.c[2][l] = b.c[2][l] - (PY[lp] - PY[l]);
+}
+template <typename T>
+int launch_mhd_resid(const Dev<T>& d, const T* vx, const T* v0, T* vres, cudaStream_t s) {
+  k_mhd_resid<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, vx, v0, vres);
+  return 1;
+}
+template <typename T>
+int launch_mhd_orbital(const Dev<T>& d, const T* v0, T* bx, T* by, T* bz, T* PZ, T* PY, cudaStream_t s) {
+  dim3 g((d.TX + 127) / 128, d.TY, d.TZ);
+  k_mhd_arc<T><<<g, 128, 0, s>>>(d, by, bz, v0, PZ, PY);
+  k_mhd_orbital<T><<<g, 128, 0, s>>>(d, PZ, PY, Vec3<T>{{bx, by, bz}});
+  return 2;
+}
+
 #define INST(T)                                                                                                          \
+  template int launch_mhd_resid<T>(const Dev<T>&, const T*, const T*, T*, cudaStream_t);                                 \
+  template int launch_mhd_orbital<T>(const Dev<T>&, const T*, T*, T*, T*, T*, T*, cudaStream_t);                         \
   template int launch_bc_b<T>(const Dev<T>&, T*, T*, T*, cudaStream_t);                                                  \
   template int launch_mhd_pressure<T>(const Dev<T>&, const T*, T*, T*, T*, T*, T*, T*, double, cudaStream_t);            \
   template int launch_mhd_emf<T>(const Dev<T>&, const T*, T*, T*, T*, T*, T*, T*, T* const*, T* const*, double, double, cudaStream_t); \

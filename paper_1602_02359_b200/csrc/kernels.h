@@ -103,6 +103,9 @@ template <typename T> int launch_mhd_emf(const Dev<T>& d, const T* rho, T* vx, T
 template <typename T> int launch_mhd_tension(const Dev<T>& d, const T* rho, T* const* b, T* const* bstar, T* vx, T* vy, T* vz,
                                              double mu0, cudaStream_t s);
 template <typename T> int launch_mhd_ct(const Dev<T>& d, T* const* emf, T* bx, T* by, T* bz, cudaStream_t s);
+// cell 11 (section 3.7): vres = vx - v0 for cell 8; arc integrals of B_Y, B_Z (into PZ, PY) and the CT update with them
+template <typename T> int launch_mhd_resid(const Dev<T>& d, const T* vx, const T* v0, T* vres, cudaStream_t s);
+template <typename T> int launch_mhd_orbital(const Dev<T>& d, const T* v0, T* bx, T* by, T* bz, T* PZ, T* PY, cudaStream_t s);
 
 // active cells <-> ghosted, padded device layout
 template <typename T> int launch_scatter(const Dev<T>& d, const T* active, T* full, cudaStream_t s);

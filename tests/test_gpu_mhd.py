@@ -41,6 +41,22 @@ def _case(name):
         z = np.zeros(shape)
         return dict(mesh=m, eos=W.ADIABATIC, prm=W.Params(gamma=2.0), f=(rho, e, z, z, z), b=(z, np.where(left, 1.0, -1.0), z + 0.75),
                     nsteps=60, eta=0.0, passive=False)
+    if name in ("fargo", "sheet"):   # section 3.7: orbital advection of B; the sheet adds Eq. 29 and Tab. 2's X momentum
+        nx, ny, nz = 66, 14, 9
+        sheet = name == "sheet"
+        bc = ((P, P), (R, R), (P, P)) if sheet else ((P, P), (P, P), (P, P))
+        m = W.Mesh(nx, ny, nz, 0.0, 2.0, W.uedges(-0.5, 0.5, ny), W.uedges(-0.2, 0.2, nz), bc)
+        shape = (nz, ny, nx)
+        y = m.yc()[None, :, None] * np.ones(shape)
+        bx, by, bz = _curl_a(shape, 2.0 / nx, 1.0 / ny, 0.4 / nz, 5, 0.01)
+        bx += 0.05; by += 0.3; bz -= 0.1
+        rho = 1.0 + 0.2 * r.uniform(-1, 1, shape)
+        e = 0.9 * (1.0 + 0.2 * r.uniform(-1, 1, shape))
+        shear = -24.0 * y if sheet else 15.0 * np.sin(2 * math.pi * y)          # arcs of up to two zones per update, both signs
+        v = (shear + 0.2 * r.uniform(-1, 1, shape), 0.2 * r.uniform(-1, 1, shape), 0.2 * r.uniform(-1, 1, shape))
+        prm = W.Params(gamma=1.4, fargo_on=1, omega_frame=1.0 if sheet else 0.0, oort_a=-0.75 if sheet else 0.0)
+        return dict(mesh=m, eos=W.ADIABATIC, prm=prm, f=(rho, e) + v, b=(bx, by, bz), nsteps=6, eta=0.0, passive=False,
+                    geometry=W.SHEARING_SHEET if sheet else W.CARTESIAN)
     bcs = {"periodic": ((P, P), (P, P), (P, P)), "mixed": ((O, R), (R, O), (O, O)), "resistive": ((P, P), (O, O), (P, P)),
            "passive": ((P, P), (P, P), (P, P)), "iso": ((P, P), (P, P), (R, R))}
     nx, ny, nz = (34, 13, 11) if name != "mixed" else (21, 12, 14)
@@ -58,10 +74,11 @@ def _case(name):
 
 def _pair(c, precision=64, use_graph=True):
     from paper_1602_02359_b200 import Fargo
-    g = Fargo(c["mesh"], W.CARTESIAN, c["eos"], c["prm"], precision=precision, use_graph=use_graph, mhd=True)
+    geo = c.get("geometry", W.CARTESIAN)
+    g = Fargo(c["mesh"], geo, c["eos"], c["prm"], precision=precision, use_graph=use_graph, mhd=True)
     g.set_fields(*c["f"])
     g.set_bfield(*c["b"], eta=c["eta"], passive=c["passive"])
-    o = Oracle(c["mesh"], W.CARTESIAN, c["eos"], c["prm"])
+    o = Oracle(c["mesh"], geo, c["eos"], c["prm"])
     o.set_fields(*c["f"])
     o.set_bfield(*c["b"], eta=c["eta"], passive=c["passive"])
     return g, o
@@ -73,7 +90,7 @@ def _rel(a, b):
     return d / s if s > 0 else d
 
 
-CASES = ["periodic", "mixed", "resistive", "passive", "iso", "brio_wu"]
+CASES = ["periodic", "mixed", "resistive", "passive", "iso", "brio_wu", "fargo", "sheet"]
 
 
 @pytest.mark.parametrize("name", CASES)

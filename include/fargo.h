@@ -194,7 +194,8 @@ int fargo_get_bfield(fargo_ctx* ctx, void* bx, void* by, void* bz);
  * next to the face into buf, pack == 0 copies buf into the 3 GHOST layers beyond it.  buf is DEVICE memory of
  * fargo_halo_bytes(which, dir) bytes, caller-owned; what was packed on the lower side of a sub-domain is unpacked on the
  * upper side of the one below it, and vice versa (over NCCL, peer copies, or directly when both live on one device).
- * Everything is enqueued on the context's stream; no host synchronisation.  The result is bit-identical to the
+ * Everything is enqueued on the context's stream; no host synchronisation; with use_graph the kernels of each phase are
+ * captured once and replayed.  The result is bit-identical to the
  * undivided mesh (tests/test_gpu_slabs.py).  Not with live planets.  Errors: FARGO_EINVAL, FARGO_ESTATE (phases out of
  * order), FARGO_ECUDA. */
 int fargo_update_phase(fargo_ctx* ctx, int phase);
@@ -202,6 +203,9 @@ size_t fargo_halo_bytes(const fargo_ctx* ctx, int which, int dir);
 int fargo_halo(fargo_ctx* ctx, int which, int dir, int side, int pack, void* device_buffer);
 /* DEVICE address of the current time step (one double): all-reduce it in place (min) between phases 0 and 1. */
 void* fargo_dt_device_ptr(fargo_ctx* ctx);
+/* Sub-domains that live on ONE device: dt of this context <- min(dt, *other_dt_device_ptr), one tiny kernel on the context's
+ * stream (the caller runs it pairwise over its sub-domains instead of an all-reduce; both contexts must share the stream). */
+int fargo_dt_min_with(fargo_ctx* ctx, const void* other_dt_device_ptr);
 
 /* Diagnostics, the sum reductions of P:787 ("the mass or angular momentum"): out[5] (HOST) = total mass, the X, Y and Z
  * momenta of Tab. 2 (per cell the mean of its left and right momenta, Eqs. 49-50; X is the angular

@@ -14,6 +14,11 @@
  * Shearing sheet (geometry 3; Tab. 1/2 P:115; Eqs. 28-30; reading G32): pinned by the steady
  * shear flow, the epicyclic frequency and amplitude ratio, conservation of Tab. 2's X momentum and the exact
  * integer shift (tests/test_oracle_shearing_sheet.py).
+ * MHD (NEXT-4; sections 3.6.1-3.7; mhd.cpp; readings G34-G37): pinned by v x B on uniform fields, div B and the mean
+ * field to rounding, the Alfven phase speed along each axis, advection with the flow, pressure balance, the closed-form
+ * pressure and tension accelerations, Eq. 115 (current sheet), the field-loop energy the paper prints at t = 2, and for
+ * cell 11 the exact circular shift, the hydrodynamic orbital routine on B_Y and Eq. 94 (tests/test_oracle_mhd.py).
+ * PARITY UNPINNED there: the ghost fill of B, the order inside cell 8 (G36), the extra ghost fill before it (G34).
  *
  * Layout of every field passed through this interface: nz*ny*nx doubles, X (i) fastest, ACTIVE
  * cells only; velocities on the LOWER face of the cell in their own direction.

@@ -22,7 +22,7 @@ EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fi
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
            "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div",
            "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics",
-           "fargo_update_phase", "fargo_halo_bytes", "fargo_halo", "fargo_dt_device_ptr", "fargo_set_bfield", "fargo_get_bfield"]
+           "fargo_update_phase", "fargo_halo_bytes", "fargo_halo", "fargo_dt_device_ptr", "fargo_set_bfield", "fargo_get_bfield", "fargo_dt_min_with"]
 
 
 class FargoMesh(C.Structure):
@@ -87,6 +87,7 @@ def load():
     L.fargo_halo_bytes.argtypes = [vp, C.c_int, C.c_int]
     L.fargo_halo_bytes.restype = C.c_size_t
     L.fargo_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]
+    L.fargo_dt_min_with.argtypes = [vp, vp]
     L.fargo_dt_device_ptr.argtypes = [vp]
     L.fargo_dt_device_ptr.restype = vp
     L.fargo_selftest_div.argtypes = [vp, vp, vp, C.c_longlong, vp]
@@ -263,6 +264,14 @@ class Fargo:
         assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.halo_bytes(which, direction)
         with self._torch.cuda.device(self.device):
             self._check(load().fargo_halo(self._h, which, direction, side, 1 if pack else 0, buf.data_ptr()), "fargo_halo")
+
+    def dt_device_ptr(self) -> int:
+        return int(load().fargo_dt_device_ptr(self._h))
+
+    def dt_min_with(self, other: "Fargo"):
+        """dt <- min(dt, other's dt): one tiny kernel on this context's stream (sub-domains on one device)."""
+        with self._torch.cuda.device(self.device):
+            self._check(load().fargo_dt_min_with(self._h, other.dt_device_ptr()), "fargo_dt_min_with")
 
     def dt_tensor(self):
         """The device-resident time step as a 1-element float64 tensor VIEW (for an in-place all-reduce)."""

@@ -36,6 +36,7 @@ struct CtxBase {
   virtual int halo(int, int, int, int, void*) = 0;
   virtual size_t halo_bytes(int, int) const = 0;
   virtual void* dt_ptr() = 0;
+  virtual int dt_min_with(const void*) = 0;
   virtual int set_planets(int, const double*, const double*, const double*, const double*, int, double) = 0;
   virtual int get_planets(double*, double*, double*) = 0;
   virtual int set_omega_frame(double) = 0;
@@ -146,6 +147,12 @@ struct Sim : CtxBase {
   int geometry, eos;
   cudaStream_t stream = nullptr;
   cudaGraphExec_t gexec = nullptr;
+  cudaGraphExec_t gphase[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // sub-domains: one captured graph per phase
+  int gphase_launches[5] = {0, 0, 0, 0, 0};
+  void drop_graphs() {
+    if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
+    for (auto& g : gphase) if (g) { cudaGraphExecDestroy(g); g = nullptr; }
+  }
   int launches_per_step = 0;
   bool midstep = false, have_fields = false, pot_static = true, pot_valid = false;
   std::map<std::string, T*> dbg;
@@ -159,7 +166,7 @@ struct Sim : CtxBase {
 
   ~Sim() override {
     cudaStreamSynchronize(stream);   // nothing of this context may still be running when the caller frees the workspace
-    if (gexec) cudaGraphExecDestroy(gexec);
+    drop_graphs();
     if (hclock) cudaFreeHost(hclock);
     for (auto& sp : spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   }
@@ -440,7 +447,23 @@ struct Sim : CtxBase {
     if (phase < 0 || phase > 4) { err = "phase must be 0 .. 4"; return FARGO_EINVAL; }
     if (phase != next_phase) { err = "phases run in the order 0, 1, 2, 3, 4"; return FARGO_ESTATE; }
     if (npl > 0) { err = "live planets are not supported on slabs (the gas force is a sum over the whole mesh)"; return FARGO_EINVAL; }
-    launches += enqueue_update(-1, false, phase);
+    // the kernels of a phase are a fixed sequence too: captured once per phase and replayed (the halo copies and the
+    // all-reduce of dt between the phases stay with the caller)
+    if (prm.use_graph && stream != nullptr && !prof) {
+      if (phase == 1 && L.has_pot && !pot_valid && npl == 0 && pot_static) { launches += potential(0.0); pot_valid = true; }
+      if (!gphase[phase]) {
+        cudaGraph_t g = nullptr;
+        if (!ck(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal), "begin capture")) return FARGO_ECUDA;
+        gphase_launches[phase] = enqueue_update(-1, true, phase);
+        if (!ck(cudaStreamEndCapture(stream, &g), "end capture")) return FARGO_ECUDA;
+        if (!ck(cudaGraphInstantiate(&gphase[phase], g, 0), "graph instantiate")) { cudaGraphDestroy(g); return FARGO_ECUDA; }
+        cudaGraphDestroy(g);
+      }
+      if (!ck(cudaGraphLaunch(gphase[phase], stream), "graph launch")) return FARGO_ECUDA;
+      launches += gphase_launches[phase];
+    } else {
+      launches += enqueue_update(-1, false, phase);
+    }
     next_phase = (phase + 1) % 5;
     if (!ck(cudaGetLastError(), "phase launch")) return FARGO_ECUDA;
     return FARGO_OK;
@@ -486,6 +509,12 @@ struct Sim : CtxBase {
   }
 
   void* dt_ptr() override { return &ctl->dt; }
+  int dt_min_with(const void* other) override {
+    if (!other) { err = "null pointer"; return FARGO_EINVAL; }
+    launches += launch_dt_min(ctl, (const double*)other, stream);
+    if (!ck(cudaGetLastError(), "dt_min launch")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
 
   // ---- live planets (NEXT-2) ---------------------------------------------------------------------------
   int set_planets(int n, const double* gm, const double* eps, const double* pos, const double* vel, int mode, double gconst) override {
@@ -504,7 +533,7 @@ struct Sim : CtxBase {
     if (!ck(cudaMemcpyAsync(pl, &h, sizeof h, cudaMemcpyHostToDevice, stream), "upload planets")) return FARGO_ECUDA;
     if (!ck(cudaStreamSynchronize(stream), "set_planets sync")) return FARGO_ECUDA;
     if ((n > 0) != (npl > 0) || n != npl || mode != pl_mode) {   // the kernel sequence changes: capture it again
-      if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
+      drop_graphs();
     }
     npl = n; pl_mode = mode;
     pot_valid = false;
@@ -527,7 +556,7 @@ struct Sim : CtxBase {
     d.omega = (T)omega_new; d.om_eff = (T)omega_new;
     pot_static = !(L.has_pot && prm.planet_mass != 0.0 && prm.planet_omega != prm.omega_frame);
     pot_valid = false;
-    if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }   // Omega_f is a kernel argument: capture again
+    drop_graphs();   // Omega_f is a kernel argument: capture again
     if (!ck(cudaGetLastError(), "frame change launch")) return FARGO_ECUDA;
     return FARGO_OK;
   }
@@ -576,7 +605,7 @@ struct Sim : CtxBase {
     const bool changed = !mhd_on || passive != mhd_passive || mu0_ != mu0 || eta_ != eta;
     mhd_on = true; mhd_passive = passive ? 1 : 0; mu0 = mu0_; eta = eta_;
     dt_ready = false;
-    if (changed && gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }   // the kernel sequence and its arguments change
+    if (changed) drop_graphs();   // the kernel sequence and its arguments change
     return FARGO_OK;
   }
 
@@ -957,6 +986,7 @@ int fargo_halo(fargo_ctx* c, int which, int dir, int side, int pack, void* devic
   return c ? c->impl->halo(which, dir, side, pack, device_buffer) : FARGO_EINVAL;
 }
 void* fargo_dt_device_ptr(fargo_ctx* c) { return c ? c->impl->dt_ptr() : nullptr; }
+int fargo_dt_min_with(fargo_ctx* c, const void* other_dt_device_ptr) { return c ? c->impl->dt_min_with(other_dt_device_ptr) : FARGO_EINVAL; }
 int fargo_step_until(fargo_ctx* c, int stage) { return c ? c->impl->step_until(stage) : FARGO_EINVAL; }
 int fargo_dims(const fargo_ctx* c, int* tx, int* ty, int* tz, int* ngx, int* ngy, int* ngz) {
   if (!c) return FARGO_EINVAL;

@@ -279,6 +279,16 @@ __global__ void k_dt_sync(Ctl* c, const double t_stop, const int single) {
   const double rest = single ? (double)(float)(t_stop - c->t) : t_stop - c->t;
   c->clipped = (t_stop > 0.0 && (c->t + c->dt >= t_stop || c->dt == rest)) ? 1 : 0;
 }
+// Sub-domains on one device: dt <- min(dt, *other), the all-reduce (min) of P:407 done pairwise by the caller
+__global__ void k_dt_min(Ctl* c, const double* __restrict__ other) {
+  if (c->done) return;
+  const double o = *other;
+  if (o < c->dt) c->dt = o;
+}
+int launch_dt_min(Ctl* ctl, const double* other, cudaStream_t s) {
+  k_dt_min<<<1, 1, 0, s>>>(ctl, other);
+  return 1;
+}
 int launch_dt_sync(Ctl* ctl, double t_stop, bool single, cudaStream_t s) {
   k_dt_sync<<<1, 1, 0, s>>>(ctl, t_stop, single ? 1 : 0);
   return 1;

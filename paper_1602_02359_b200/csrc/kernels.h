@@ -90,6 +90,7 @@ template <typename T> int launch_copy(const Dev<T>& d, const T* src, T* dst, cud
 int launch_advance(Ctl* ctl, double t_stop, cudaStream_t s);
 // slabs: retake the t_stop clip flag after ctl->dt was all-reduced (min) over the slabs
 int launch_dt_sync(Ctl* ctl, double t_stop, bool single, cudaStream_t s);
+int launch_dt_min(Ctl* ctl, const double* other, cudaStream_t s);   // ctl->dt = min(ctl->dt, *other)
 // out[n] = rdiv(a[n], b[n]): the kernels' branch-free division, exposed for its self-test
 int launch_selftest_div(const double* a, const double* b, double* out, long long n, cudaStream_t s);
 

@@ -136,7 +136,7 @@ class SlabRun:
                 sub, (rows, planes) = slab_mesh(mesh, r, self.grid)
                 # the last sub-domain of a periodic Y axis: its upper cut is the seam, no ring pair of Eq. 73 across it
                 seam = self.periodic[1] and self.grid[0] > 1 and grid_coords(r, self.grid)[0] == self.grid[0] - 1
-                self.ctx[r] = Fargo(sub, geometry, eos, prm, precision=precision, use_graph=False,
+                self.ctx[r] = Fargo(sub, geometry, eos, prm, precision=precision, use_graph=True,   # one graph per phase
                                     kernel_plan=PLAN_SEAM_ABOVE if seam else 0)
                 self.rows[r], self.planes[r] = rows, planes
         self._buf = {}
@@ -202,13 +202,14 @@ class SlabRun:
             self.ctx[r].halo(which, direction, side, False, b["recv"][side])
 
     def _reduce_dt(self):
-        views = [self.ctx[r].dt_tensor() for r in self.ranks]
-        if self.group is None:
-            m = self._torch.stack(views).min(dim=0).values
-            for v in views:
-                v.copy_(m)
+        if self.group is None:   # one device, one stream: pairwise min into the first sub-domain, then back out (our own kernel)
+            first = self.ctx[self.ranks[0]]
+            for r in self.ranks[1:]:
+                first.dt_min_with(self.ctx[r])
+            for r in self.ranks[1:]:
+                self.ctx[r].dt_min_with(first)
         else:
-            self._dist.all_reduce(views[0], op=self._dist.ReduceOp.MIN, group=self.group)
+            self._dist.all_reduce(self.ctx[self.ranks[0]].dt_tensor(), op=self._dist.ReduceOp.MIN, group=self.group)
 
     def _phase(self, p):
         for r in self.ranks:

@@ -412,3 +412,42 @@ def test_field_loop_carried_by_orbital_advection_does_not_diffuse():
     o.step(nx // 2)
     bb = o.get_bfield()
     assert abs(float(np.mean(bb[0] ** 2 + bb[1] ** 2)) - em0) <= 1e-3 * em0     # measured 4e-4
+
+
+# ---------------------------------------------------------------- section 5.2.1: the MHD Riemann problem -------------
+def test_brio_wu_wave_fronts_travel_at_the_fast_magnetosonic_speeds():
+    """P:871-877 (Brio & Wu): P = 1 | 0.1, rho = 1 | 0.1, B_z = 0.75 on both sides, B_y = +1 | -1, gamma = 2, along z.  Half
+    the paper's size (400 zones over 0 <= z <= 400, t = 40: the solution is self-similar).  What the equations fix in
+    closed form: the normal field never changes; nothing moves ahead of the two fast rarefactions, whose heads travel at
+    the fast speeds of the undisturbed states, c_f^2 = (a^2 + b^2 + sqrt((a^2 + b^2)^2 - 4 a^2 b_n^2)) / 2; B_y changes sign
+    through the compound wave and the slow shock; mass is conserved."""
+    n, t_end = 400, 40.0
+    m = W.Mesh(4, 4, n, 0.0, 4.0, W.uedges(0.0, 4.0, 4), W.uedges(0.0, 400.0, n), ((P, P), (P, P), (O, O)))
+    shape = (n, 4, 4)
+    left = (np.arange(n) < n // 2)[:, None, None] * np.ones(shape, dtype=bool)
+    rho0 = np.where(left, 1.0, 0.1)
+    z = np.zeros(shape)
+    o = oracle(m, rho0, np.where(left, 1.0, 0.1) / (2.0 - 1.0), (z, z, z), (z, np.where(left, 1.0, -1.0), z + 0.75), gamma=2.0, t_stop=t_end)
+    o.step(100000)
+    assert o.time()[0] == t_end
+    rho, e, vx, vy, vz = (a[:, 0, 0] for a in o.get_fields())
+    bx, by, bz = (a[:, 0, 0] for a in o.get_bfield())
+    zc = np.arange(n) + 0.5
+    assert np.array_equal(o.get_bfield()[2], z + 0.75)                    # div B = 0 in one dimension
+    for a in o.get_fields() + o.get_bfield():                             # nothing varies across the thin directions
+        assert np.array_equal(a, np.broadcast_to(a[:, :1, :1], a.shape))
+
+    def cfast(p, r, byv, bn, gam=2.0):
+        a2, b2, bn2 = gam * p / r, (byv * byv + bn * bn) / r, bn * bn / r
+        return math.sqrt(0.5 * (a2 + b2 + math.sqrt((a2 + b2) ** 2 - 4.0 * a2 * bn2)))
+    head_l = 200.0 - cfast(1.0, 1.0, 1.0, 0.75) * t_end                   # 128.3
+    head_r = 200.0 + cfast(0.1, 0.1, -1.0, 0.75) * t_end                  # 364.7
+    moved = np.abs(rho / rho0[:, 0, 0] - 1.0) > 2e-3
+    first, last = zc[moved][0], zc[moved][-1]
+    assert abs(first - head_l) <= 4.0 and abs(last - head_r) <= 6.0, (first, head_l, last, head_r)
+    # (the fronts are smeared over a few zones; ten zones ahead of them the gas is still at rest)
+    assert np.all(np.abs(vz[zc < head_l - 10]) < 1e-5) and np.all(np.abs(vz[zc > head_r + 10]) < 1e-5)
+    assert abs(float(np.sum(rho)) - float(np.sum(rho0[:, 0, 0]))) <= 1e-10 * n          # outflow ends are still at rest
+    assert 0.08 < rho.min() < 0.1 and rho.max() < 1.0 + 2e-3             # the right fast rarefaction thins the gas behind it
+    assert by[10] == 1.0 and by[-10] == -1.0 and np.sum(np.diff(np.sign(by)) != 0) == 1   # one sign change
+    assert float(np.max(np.abs(vy))) > 0.5                                # the rotational part of the jump sets v_y going

@@ -72,7 +72,8 @@ extern "C" int oracle_set_fields(oracle_ctx* c, const double* rho, const double*
 extern "C" int oracle_set_bfield(oracle_ctx* c, const double* bx, const double* by, const double* bz, double mu0,
                                  double eta, int passive) {
   if (!c || !bx || !by || !bz || !(mu0 > 0.0) || eta < 0.0) return -1;
-  if (c->geometry != ORC_CARTESIAN) return -1;   // (the shearing sheet has the Cartesian metric)
+  if (c->geometry != ORC_CARTESIAN && eta != 0.0) return -1;   // the resistive term is built for the Cartesian metric only
+  if (c->geometry == ORC_SPHERICAL && c->p.fargo_on) return -1;  // cell 11 is built for Cartesian and cylindrical meshes (G38)
   for (vec* f : {&c->bx, &c->by, &c->bz, &c->emfx, &c->emfy, &c->emfz, &c->bstar[0][0], &c->bstar[0][1], &c->bstar[1][0],
                  &c->bstar[1][1], &c->bstar[2][0], &c->bstar[2][1]})
     f->assign(c->ncell(), 0.0);
@@ -124,7 +125,7 @@ static void full_update(oracle_ctx* c, int until) {
   o.dt = orc_compute_dt(o, &clipped);                           if (until == ORC_ST_DT) return;       // cell 6
   orc_planets_update(o);                                                                              // cell 5a (G33)
   orc_source_a(o);                                                                                    // cell 7a
-  if (o.mhd) orc_mhd_source_a(o);
+  if (o.mhd) { orc_mhd_source_a(o); orc_mhd_source_curv(o); }
   if (until == ORC_ST_SRC_A) return;
   orc_source_b(o);                                              if (until == ORC_ST_SRC_B) return;    // cell 7b
   orc_source_c(o);                                              if (until == ORC_ST_SRC_C) return;    // cell 7c

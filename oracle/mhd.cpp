@@ -1,5 +1,5 @@
-// mhd.cpp -- SURVEY.md 8(f) NEXT-4: the MHD substeps of Fig. 2 (cells 8, 10; sections 3.6.1-3.6.2) on
-// CARTESIAN meshes: method of characteristics + constrained transport (MOCCT).
+// mhd.cpp -- SURVEY.md 8(f) NEXT-4: the MHD substeps of Fig. 2 (cells 8, 10, 11; sections 3.6.1-3.7): method of
+// characteristics + constrained transport (MOCCT) on Cartesian, cylindrical and spherical meshes and the shearing sheet.
 //   cell 2   ghost fill of the face-centred field B (kinds of G22; the normal component keeps its boundary face)
 //   cell 6   fast magnetosonic speed C_w^2 = C_s^2 + v_A^2 and the resistive limit in Eq. 59 (items 1 and 5)
 //   cell 7a  gradient of the zone-centred magnetic pressure of the transverse components
@@ -9,7 +9,10 @@
 //   cell 10  constrained transport (Eq. 76; signs fixed by Eq. 101 P:668 and by Faraday's law: reading G35)
 //   cell 11  orbital advection of B by the upstream-averaged EMF (section 3.7, Eqs. 92-107), Cartesian meshes
 //            and the shearing sheet; the substeps of cell 8 then see the residual velocity v_X - v0 (reading G37)
-// Not here: curvilinear meshes (Eqs. 87-91).
+// Curvilinear meshes (reading G38): every length is the physical one at the place where it is used -- R_x = 1 | r | r sin(theta)
+// and R_z = 1 | 1 | r taken at the zone centre or at the lower Y / Z face according to where the interpolated quantity
+// lives --, Eq. 76 is applied with the edge lengths and the face areas of Tab. 5, and cell 7a gets the geometric terms of
+// Eqs. 87-91.  On a Cartesian mesh every R is 1.0 and the arithmetic is bit for bit what it was.
 // CPU oracle, TEST INFRASTRUCTURE (see fargo_oracle.h): plain loops, one formula per line, the paper's notation.
 // Directions are numbered 0, 1, 2 = X, Y, Z; (d1, d2, d3) is always a cyclic permutation, eps_d3 = v_d1 B_d2 - v_d2 B_d1.
 // A field component along d lives on the LOWER d face of its cell; eps_d3 of cell q lives on the edge along d3
@@ -28,8 +31,22 @@ inline Q mv(const oracle_ctx& c, Q q, int d, int s) {
   return q;
 }
 inline size_t at(const oracle_ctx& c, const Q& q) { return c.id(q.n[0], q.n[1], q.n[2]); }
-inline double width(const oracle_ctx& c, int d, int n) { return d == 0 ? c.dx : d == 1 ? c.LY[n] : c.dz[n]; }           // Delta_d of cell n
-inline double invdist(const oracle_ctx& c, int d, int n) { return d == 0 ? 1.0 / c.dx : d == 1 ? c.invDY[n] : c.invdzc[n]; }   // 1 / (centre n - centre n-1)
+// R_x = 1 | r | r sin(theta) and R_z = 1 | 1 | r (Tab. 1) where a quantity that lives on the lower f face of cell q sits
+// (f = 1: at the lower Y edge; f = 2: at the lower Z edge; else at the zone centre), and their reciprocals
+inline double RxJ(const oracle_ctx& c, const Q& q, int f) { return c.geometry == ORC_CARTESIAN ? 1.0 : (f == 1 ? c.ye[q.n[1]] : c.yc[q.n[1]]); }
+inline double RxK(const oracle_ctx& c, const Q& q, int f) { return c.geometry == ORC_SPHERICAL ? (f == 2 ? c.sin_ze[q.n[2]] : c.sin_zc[q.n[2]]) : 1.0; }
+inline double RzJ(const oracle_ctx& c, const Q& q, int f) { return c.geometry == ORC_SPHERICAL ? (f == 1 ? c.ye[q.n[1]] : c.yc[q.n[1]]) : 1.0; }
+inline double iRxJ(const oracle_ctx& c, const Q& q, int f) { return c.geometry == ORC_CARTESIAN ? 1.0 : (f == 1 ? c.inv_ye[q.n[1]] : c.inv_yc[q.n[1]]); }
+inline double iRxK(const oracle_ctx& c, const Q& q, int f) { return c.geometry == ORC_SPHERICAL ? (f == 2 ? c.inv_sin_ze[q.n[2]] : c.invRxk[q.n[2]]) : 1.0; }
+inline double iRzJ(const oracle_ctx& c, const Q& q, int f) { return c.geometry == ORC_SPHERICAL ? (f == 1 ? c.inv_ye[q.n[1]] : c.inv_yc[q.n[1]]) : 1.0; }
+// physical width of cell q along d, and 1 / (distance of its centre from the centre of the zone below), for a quantity
+// on the lower f face (f != d; f = d or f < 0: a zone-centred position in the two other directions)
+inline double width(const oracle_ctx& c, int d, const Q& q, int f) {
+  return d == 0 ? (c.dx * RxJ(c, q, f)) * RxK(c, q, f) : d == 1 ? c.LY[q.n[1]] : c.dz[q.n[2]] * RzJ(c, q, f);
+}
+inline double invdist(const oracle_ctx& c, int d, const Q& q, int f) {
+  return d == 0 ? ((1.0 / c.dx) * iRxJ(c, q, f)) * iRxK(c, q, f) : d == 1 ? c.invDY[q.n[1]] : c.invdzc[q.n[2]] * iRzJ(c, q, f);
+}
 // can cell index n along d reach s_lo cells down and s_hi cells up?
 inline bool fits(const oracle_ctx& c, int d, int n, int s_lo, int s_hi) {
   if (!has(c, d) || (d == 0 && c.xwrap)) return true;
@@ -37,19 +54,21 @@ inline bool fits(const oracle_ctx& c, int d, int n, int s_lo, int s_hi) {
 }
 
 // van Leer slope of f along d at cell q (readings G4, G5)
-inline double slope(const oracle_ctx& c, const vec& f, const Q& q, int d) {
-  const double f0 = f[at(c, q)], fm = f[at(c, mv(c, q, d, -1))], fp = f[at(c, mv(c, q, d, +1))];
-  const double dm = (f0 - fm) * invdist(c, d, q.n[d]);
-  const double dp = (fp - f0) * invdist(c, d, d == 0 ? q.n[d] : q.n[d] + 1);   // X is uniform
+inline double slope(const oracle_ctx& c, const vec& f, const Q& q, int d, int fc) {
+  const Q qp = mv(c, q, d, +1);
+  const double f0 = f[at(c, q)], fm = f[at(c, mv(c, q, d, -1))], fp = f[at(c, qp)];
+  const double dm = (f0 - fm) * invdist(c, d, q, fc);
+  const double dp = (fp - f0) * invdist(c, d, d == 0 ? q : qp, fc);   // X is uniform
   return (dm * dp <= 0.0) ? 0.0 : (2.0 * (dm * dp)) / (dm + dp);
 }
 // f at the lower d face of cell q at half time step, carried at speed w: Eq. 48 -- the upwind cell's value plus
 // its slope times the distance to the foot of the characteristic (readings G2, G3, G6)
-inline double star(const oracle_ctx& c, const vec& f, const Q& q, int d, double w) {
+// (fc: the direction of the faces f lives on, which fixes the lengths on a curvilinear mesh)
+inline double star(const oracle_ctx& c, const vec& f, const Q& q, int d, double w, int fc) {
   if (!has(c, d)) return f[at(c, q)];
   const Q qm = mv(c, q, d, -1);
-  if (w >= 0.0) return std::fma(slope(c, f, qm, d), std::fma(-w, c.dt, width(c, d, qm.n[d])) * 0.5, f[at(c, qm)]);
-  return std::fma(-slope(c, f, q, d), std::fma(w, c.dt, width(c, d, q.n[d])) * 0.5, f[at(c, q)]);
+  if (w >= 0.0) return std::fma(slope(c, f, qm, d, fc), std::fma(-w, c.dt, width(c, d, qm, fc)) * 0.5, f[at(c, qm)]);
+  return std::fma(-slope(c, f, q, d, fc), std::fma(w, c.dt, width(c, d, q, fc)) * 0.5, f[at(c, q)]);
 }
 
 inline vec& V(oracle_ctx& c, int d) { return d == 0 ? (c.p.fargo_on ? c.vxres : c.vx) : d == 1 ? c.vy : c.vz; }   // G37
@@ -124,10 +143,53 @@ void orc_mhd_source_a(oracle_ctx& c) {
           const Q q = {{i, j, k}};
           if (!fits(c, d, q.n[d], 1, 0) || !fits(c, (d + 1) % 3, q.n[(d + 1) % 3], 0, 1) || !fits(c, (d + 2) % 3, q.n[(d + 2) % 3], 0, 1)) continue;
           const Q qm = mv(c, q, d, -1);
-          const double wf = (2.0 * invdist(c, d, q.n[d])) / (c.rho[at(c, q)] + c.rho[at(c, qm)]);
+          const double il = d == 0 ? c.invLX(j, k) : d == 1 ? c.invDY[j] : c.invDZ(j, k);   // as the pressure gradient of 7a
+          const double wf = (2.0 * il) / (c.rho[at(c, q)] + c.rho[at(c, qm)]);
           vb[at(c, q)] = std::fma(-dt, wf * (pm(q, d) - pm(qm, d)), vb[at(c, q)]);
         }
   }
+}
+
+// ---- cell 7a, geometric terms of B.grad B on curvilinear meshes (Eqs. 87-91), applied to v_b like the others.
+// Each component of B is brought to the face of the velocity by the mean of the (two or four) face values next to it; the
+// density on the face is the arithmetic mean; r, cot(theta) are those of the face.
+void orc_mhd_source_curv(oracle_ctx& c) {
+  if (c.mhd_passive || c.geometry == ORC_CARTESIAN) return;
+  const bool sph = c.geometry == ORC_SPHERICAL;
+  const double dt = c.dt, imu = 1.0 / c.mu0;
+  auto avg4 = [&](const vec& b, const Q& q, int da, int db) {   // mean over q, q+e_da, q-e_db, q+e_da-e_db
+    const Q qm = mv(c, q, db, -1);
+    return 0.25 * (((b[at(c, q)] + b[at(c, mv(c, q, da, +1))]) + b[at(c, qm)]) + b[at(c, mv(c, qm, da, +1))]);
+  };
+  vec vxb = c.vxb, vyb = c.vyb, vzb = c.vzb;
+  for (int k = 0; k < c.TZ; ++k)
+    for (int j = 0; j < c.TY; ++j)
+      for (int i = 0; i < c.TX; ++i) {
+        const Q q = {{i, j, k}};
+        const size_t l = at(c, q);
+        const bool zok = !(sph && c.hasz) || fits(c, 2, k, 1, 1);
+        if (c.hasx && fits(c, 0, i, 1, 0) && fits(c, 1, j, 0, 1) && zok) {   // v_phi on the face (i-1/2, j, k): Eqs. 87, 89
+          const double wf = (2.0 * imu) / (c.rho[l] + c.rho[at(c, mv(c, q, 0, -1))]);
+          const double bphi = c.bx[l], br = avg4(c.by, q, 1, 0);
+          double g = br * bphi;
+          if (sph && c.hasz) g = std::fma(avg4(c.bz, q, 2, 0) * bphi, c.cot_zc[k], g);
+          vxb[l] = std::fma(dt, (wf * g) * c.inv_yc[j], c.vxb[l]);
+        }
+        if (c.hasy && fits(c, 1, j, 1, 0) && fits(c, 0, i, 0, 1) && zok) {    // v_r on the face (i, j-1/2, k): Eqs. 88, 90
+          const double wf = (2.0 * imu) / (c.rho[l] + c.rho[at(c, mv(c, q, 1, -1))]);
+          const double bphi = avg4(c.bx, q, 0, 1);
+          double g = bphi * bphi;
+          if (sph && c.hasz) { const double bth = avg4(c.bz, q, 2, 1); g = std::fma(bth, bth, g); }
+          vyb[l] = std::fma(-dt, (wf * g) * c.inv_ye[j], c.vyb[l]);
+        }
+        if (sph && c.hasz && fits(c, 2, k, 1, 0) && fits(c, 0, i, 0, 1) && fits(c, 1, j, 0, 1)) {   // v_theta: Eq. 91
+          const double wf = (2.0 * imu) / (c.rho[l] + c.rho[at(c, mv(c, q, 2, -1))]);
+          const double bth = c.bz[l], br = avg4(c.by, q, 1, 2), bphi = avg4(c.bx, q, 0, 2);
+          const double g = std::fma(-(bphi * bphi), c.cot_ze[k], br * bth);
+          vzb[l] = std::fma(dt, (wf * g) * c.inv_yc[j], c.vzb[l]);
+        }
+      }
+  c.vxb = vxb; c.vyb = vyb; c.vzb = vzb;
 }
 
 // ---- cells 8a-8c: star values and electromotive forces on every edge whose stencil fits ------------------------------------
@@ -161,21 +223,21 @@ void orc_mhd_emf(oracle_ctx& c) {
           // v_d2 of the two faces next to the edge, and vice versa
           const double v2bar = 0.5 * (V2[l] + V2[at(c, q1)]);
           const double v1bar = 0.5 * (V1[l] + V1[at(c, q2)]);
-          const double v1u = star(c, V1, q, d2, v2bar), B1u = star(c, B1, q, d2, v2bar);
-          const double v2u = star(c, V2, q, d1, v1bar), B2u = star(c, B2, q, d1, v1bar);
+          const double v1u = star(c, V1, q, d2, v2bar, d1), B1u = star(c, B1, q, d2, v2bar, d1);
+          const double v2u = star(c, V2, q, d1, v1bar, d2), B2u = star(c, B2, q, d1, v1bar, d2);
           // (v_d2*, B_d2*): 1.5-D problem along d1, C+- = v_d1 -+ B_d1 / sqrt(mu0 rho) (Eq. 81), psi+- = v_d2 +- B_d2 / sqrt(mu0 rho)
           double v2s, B2s, v1s, B1s;
           {
             const double Cp = v1u - B1u / sr, Cm = v1u + B1u / sr;
-            const double vp = star(c, V2, q, d1, Cp), Bp = star(c, B2, q, d1, Cp);
-            const double vm = star(c, V2, q, d1, Cm), Bm = star(c, B2, q, d1, Cm);
+            const double vp = star(c, V2, q, d1, Cp, d2), Bp = star(c, B2, q, d1, Cp, d2);
+            const double vm = star(c, V2, q, d1, Cm, d2), Bm = star(c, B2, q, d1, Cm, d2);
             v2s = 0.5 * ((vp + vm) + (Bp - Bm) / sr);     // Eq. 83
             B2s = 0.5 * ((Bp + Bm) + sr * (vp - vm));
           }
           {   // (v_d1*, B_d1*): 1.5-D problem along d2
             const double Cp = v2u - B2u / sr, Cm = v2u + B2u / sr;
-            const double vp = star(c, V1, q, d2, Cp), Bp = star(c, B1, q, d2, Cp);
-            const double vm = star(c, V1, q, d2, Cm), Bm = star(c, B1, q, d2, Cm);
+            const double vp = star(c, V1, q, d2, Cp, d1), Bp = star(c, B1, q, d2, Cp, d1);
+            const double vm = star(c, V1, q, d2, Cm, d1), Bm = star(c, B1, q, d2, Cm, d1);
             v1s = 0.5 * ((vp + vm) + (Bp - Bm) / sr);
             B1s = 0.5 * ((Bp + Bm) + sr * (vp - vm));
           }
@@ -184,8 +246,8 @@ void orc_mhd_emf(oracle_ctx& c) {
           // cell 8c: - eta (curl B)_d3, plain differences
           if (eta != 0.0) {
             double J = 0.0;   // (curl B)_d3 = d(B_d2)/d(X_d1) - d(B_d1)/d(X_d2) at the edge
-            if (has(c, d1)) J = (B2[l] - B2[at(c, q1)]) * invdist(c, d1, q.n[d1]);
-            if (has(c, d2)) J = J - (B1[l] - B1[at(c, q2)]) * invdist(c, d2, q.n[d2]);
+            if (has(c, d1)) J = (B2[l] - B2[at(c, q1)]) * invdist(c, d1, q, d2);
+            if (has(c, d2)) J = J - (B1[l] - B1[at(c, q2)]) * invdist(c, d2, q, d1);
             emf = std::fma(-eta, J, emf);
           }
           E[l] = emf;
@@ -193,14 +255,14 @@ void orc_mhd_emf(oracle_ctx& c) {
           // of the characteristic speed; B along the characteristic = mean of the two faces next to the edge
           {
             const double a = (0.5 * (B2[l] + B2[at(c, q1)])) / sr;      // B_d2 / sqrt(mu0 rho) at the edge
-            const double vp = star(c, V1, q, d2, -a), Bp = star(c, B1, q, d2, -a);
-            const double vm = star(c, V1, q, d2, a), Bm = star(c, B1, q, d2, a);
+            const double vp = star(c, V1, q, d2, -a, d1), Bp = star(c, B1, q, d2, -a, d1);
+            const double vm = star(c, V1, q, d2, a, d1), Bm = star(c, B1, q, d2, a, d1);
             S1[l] = 0.5 * ((Bp + Bm) + sr * (vp - vm));
           }
           {
             const double a = (0.5 * (B1[l] + B1[at(c, q2)])) / sr;
-            const double vp = star(c, V2, q, d1, -a), Bp = star(c, B2, q, d1, -a);
-            const double vm = star(c, V2, q, d1, a), Bm = star(c, B2, q, d1, a);
+            const double vp = star(c, V2, q, d1, -a, d2), Bp = star(c, B2, q, d1, -a, d2);
+            const double vm = star(c, V2, q, d1, a, d2), Bm = star(c, B2, q, d1, a, d2);
             S2[l] = 0.5 * ((Bp + Bm) + sr * (vp - vm));
           }
         }
@@ -232,8 +294,8 @@ void orc_mhd_lorentz(oracle_ctx& c) {
           const double Bbar_a = 0.25 * (((Ba[l] + Ba[at(c, qa)]) + Ba[at(c, qm)]) + Ba[at(c, mv(c, qm, da, +1))]);
           const double Bbar_b = 0.25 * (((Bb[l] + Bb[at(c, qb)]) + Bb[at(c, qm)]) + Bb[at(c, mv(c, qm, db, +1))]);
           double acc = 0.0;
-          if (has(c, da)) acc = Bbar_a * ((Sa[at(c, qa)] - Sa[l]) / width(c, da, q.n[da]));
-          if (has(c, db)) acc = std::fma(Bbar_b, (Sb[at(c, qb)] - Sb[l]) / width(c, db, q.n[db]), acc);
+          if (has(c, da)) acc = Bbar_a * ((Sa[at(c, qa)] - Sa[l]) / width(c, da, q, d));
+          if (has(c, db)) acc = std::fma(Bbar_b, (Sb[at(c, qb)] - Sb[l]) / width(c, db, q, d), acc);
           const double wf = 2.0 / (c.mu0 * (c.rho[l] + c.rho[at(c, qm)]));
           out[l] = std::fma(dt, wf * acc, v[l]);
         }
@@ -246,6 +308,40 @@ void orc_mhd_lorentz(oracle_ctx& c) {
 // Every edge value enters two faces of a cell with opposite signs: div B keeps its value to rounding.
 void orc_mhd_ct(oracle_ctx& c) {
   const double dt = c.dt;
+  if (c.geometry != ORC_CARTESIAN) {
+    // Eq. 76 proper: d(B S)/dt = circulation of eps around the face, with the physical edge lengths and Tab. 5's areas.
+    //   Z edge at (i-1/2, j-1/2, k): lZ = dz R_z(edge j);  X edge at (i, j-1/2, k-1/2): lX = dx R_x(edge j, edge k);  Y edge: LY[j]
+    auto lZ = [&](int j, int k) { return c.dz[k] * (c.geometry == ORC_SPHERICAL ? c.ye[j] : 1.0); };
+    auto lX = [&](int j, int k) { return (c.dx * c.ye[j]) * (c.geometry == ORC_SPHERICAL ? c.sin_ze[k] : 1.0); };
+    vec bx = c.bx, by = c.by, bz = c.bz;
+    for (int k = 0; k < c.TZ; ++k)
+      for (int j = 0; j < c.TY; ++j)
+        for (int i = 0; i < c.TX; ++i) {
+          const Q q = {{i, j, k}};
+          const size_t l = at(c, q);
+          const size_t li = at(c, mv(c, q, 0, +1)), lj = at(c, mv(c, q, 1, +1)), lk = at(c, mv(c, q, 2, +1));
+          if (fits(c, 0, i, 2, 1) && fits(c, 1, j, 2, 2) && fits(c, 2, k, 2, 2)) {
+            double circ = 0.0;
+            if (c.hasy) circ = c.emfz[lj] * lZ(j + 1, k) - c.emfz[l] * lZ(j, k);
+            if (c.hasz) circ = circ - (c.emfy[lk] - c.emfy[l]) * c.LY[j];
+            bx[l] = std::fma(dt, circ / c.Sx(j, k), c.bx[l]);
+          }
+          if (fits(c, 1, j, 2, 1) && fits(c, 2, k, 2, 2) && fits(c, 0, i, 2, 2)) {
+            double circ = 0.0;
+            if (c.hasz) circ = c.emfx[lk] * lX(j, k + 1) - c.emfx[l] * lX(j, k);
+            if (c.hasx) circ = circ - (c.emfz[li] - c.emfz[l]) * lZ(j, k);
+            by[l] = std::fma(dt, circ / c.Sy(j, k), c.by[l]);
+          }
+          if (fits(c, 2, k, 2, 1) && fits(c, 0, i, 2, 2) && fits(c, 1, j, 2, 2)) {
+            double circ = 0.0;
+            if (c.hasx) circ = (c.emfy[li] - c.emfy[l]) * c.LY[j];
+            if (c.hasy) circ = circ - (c.emfx[lj] * lX(j + 1, k) - c.emfx[l] * lX(j, k));
+            bz[l] = std::fma(dt, circ / c.Sz(j, k), c.bz[l]);
+          }
+        }
+    c.bx = bx; c.by = by; c.bz = bz;
+    return;
+  }
   for (int d = 0; d < 3; ++d) {
     const int da = (d + 1) % 3, db = (d + 2) % 3;
     vec& b = B(c, d);
@@ -257,8 +353,8 @@ void orc_mhd_ct(oracle_ctx& c) {
           if (!fits(c, d, q.n[d], 2, 1) || !fits(c, da, q.n[da], 2, 2) || !fits(c, db, q.n[db], 2, 2)) continue;
           const size_t l = at(c, q);
           double curl = 0.0;
-          if (has(c, da)) curl = (Eb[at(c, mv(c, q, da, +1))] - Eb[l]) / width(c, da, q.n[da]);
-          if (has(c, db)) curl = curl - (Ea[at(c, mv(c, q, db, +1))] - Ea[l]) / width(c, db, q.n[db]);
+          if (has(c, da)) curl = (Eb[at(c, mv(c, q, da, +1))] - Eb[l]) / width(c, da, q, d);
+          if (has(c, db)) curl = curl - (Ea[at(c, mv(c, q, db, +1))] - Ea[l]) / width(c, db, q, d);
           b[l] = std::fma(dt, curl, b[l]);
         }
   }
@@ -267,11 +363,18 @@ void orc_mhd_ct(oracle_ctx& c) {
 // div B of a cell (Eq. 75 summed over its six faces, divided by the volume): the CT invariant
 double orc_mhd_divb(const oracle_ctx& c, int i, int j, int k) {
   const Q q = {{i, j, k}};
+  if (c.geometry != ORC_CARTESIAN) {   // (sum of B S over the six faces) / V with Tab. 5's areas and volume
+    double s = 0.0;
+    if (c.hasx) s += (c.bx[at(c, mv(c, q, 0, +1))] - c.bx[at(c, q)]) * c.Sx(j, k);
+    if (c.hasy) s += c.by[at(c, mv(c, q, 1, +1))] * c.Sy(j + 1, k) - c.by[at(c, q)] * c.Sy(j, k);
+    if (c.hasz) s += c.bz[at(c, mv(c, q, 2, +1))] * c.Sz(j, k + 1) - c.bz[at(c, q)] * c.Sz(j, k);
+    return s * c.invV(j, k);
+  }
   double s = 0.0;
   for (int d = 0; d < 3; ++d) {
     if (!has(c, d)) continue;
     const vec& b = d == 0 ? c.bx : d == 1 ? c.by : c.bz;
-    s += (b[at(c, mv(c, q, d, +1))] - b[at(c, q)]) / width(c, d, q.n[d]);
+    s += (b[at(c, mv(c, q, d, +1))] - b[at(c, q)]) / width(c, d, q, d);
   }
   return s;
 }
@@ -302,7 +405,8 @@ static void arc_integrals(int n, const double* g, double s, double* phi) {
 void orc_mhd_orbital(oracle_ctx& c) {
   if (!c.p.fargo_on) return;
   const int n = c.TX;   // orbital advection needs a wrapped X axis: TX = nx
-  const double dt = c.dt, idx = 1.0 / c.dx;
+  const double dt = c.dt;
+  const bool cart = c.geometry == ORC_CARTESIAN;
   vec &PZ = c.emfz, &PY = c.emfy;   // reused: the arc integrals on the Z edges (of B_Y) and on the Y edges (of B_Z)
   std::vector<double> g(n), phi(n);
   for (int k = 0; k < c.TZ; ++k)
@@ -312,13 +416,13 @@ void orc_mhd_orbital(oracle_ctx& c) {
       if (!c.hasy || j >= 1) {   // Z edges of the Y face j-1/2: v0 = mean of the rings j-1 and j
         const double v0f = c.hasy ? 0.5 * (c.v0[c.rid(j, k)] + c.v0[c.rid(j - 1, k)]) : c.v0[c.rid(j, k)];
         for (int i = 0; i < n; ++i) g[i] = c.by[base + i];
-        arc_integrals(n, g.data(), (v0f * dt) * idx, phi.data());
+        arc_integrals(n, g.data(), (v0f * dt) * invdist(c, 0, Q{{0, j, k}}, 1), phi.data());   // zones of the Y face's own arc length
         for (int i = 0; i < n; ++i) PZ[base + i] = phi[i];
       }
       if (!c.hasz || k >= 1) {   // Y edges of the Z face k-1/2
         const double v0f = c.hasz ? 0.5 * (c.v0[c.rid(j, k)] + c.v0[c.rid(j, k - 1)]) : c.v0[c.rid(j, k)];
         for (int i = 0; i < n; ++i) g[i] = c.bz[base + i];
-        arc_integrals(n, g.data(), (v0f * dt) * idx, phi.data());
+        arc_integrals(n, g.data(), (v0f * dt) * invdist(c, 0, Q{{0, j, k}}, 2), phi.data());
         for (int i = 0; i < n; ++i) PY[base + i] = phi[i];
       }
     }
@@ -331,8 +435,15 @@ void orc_mhd_orbital(oracle_ctx& c) {
         const size_t l = base + i, lp = base + ip;
         // B_X: DX [ (PZ(j+1) - PZ(j)) / DY + (PY(k+1) - PY(k)) / DZ ]   (Eq. 104 and its Z counterpart)
         double d = 0.0;
-        if (c.hasy) d = (c.dx * (PZ[c.id(i, j + 1, k)] - PZ[l])) / c.LY[j];
-        if (c.hasz) d = d + (c.dx * (PY[c.id(i, j, k + 1)] - PY[l])) / c.dz[k];
+        if (cart) {
+          if (c.hasy) d = (c.dx * (PZ[c.id(i, j + 1, k)] - PZ[l])) / c.LY[j];
+          if (c.hasz) d = d + (c.dx * (PY[c.id(i, j, k + 1)] - PY[l])) / c.dz[k];
+        } else {   // cylindrical: the same circulation with each edge's own arc length (Eq. 105), over the area of the face
+          const Q q = {{i, j, k}}, qj = {{i, j + 1, k}}, qk = {{i, j, k + 1}};
+          if (c.hasy) d = (width(c, 0, qj, 1) * PZ[c.id(i, j + 1, k)]) * c.dz[k] - (width(c, 0, q, 1) * PZ[l]) * c.dz[k];
+          if (c.hasz) d = d + (width(c, 0, qk, 2) * PY[c.id(i, j, k + 1)] - width(c, 0, q, 2) * PY[l]) * c.LY[j];
+          d = d / c.Sx(j, k);
+        }
         c.bx[l] = c.bx[l] + d;
         c.by[l] = c.by[l] - (PZ[lp] - PZ[l]);          // Eq. 101
         c.bz[l] = c.bz[l] - (PY[lp] - PY[l]);

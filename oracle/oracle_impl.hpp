@@ -114,6 +114,7 @@ void orc_planets_update(oracle_ctx& c);   // planets.cpp, cell 5a
 void orc_mhd_bc_fill(oracle_ctx& c);
 double orc_mhd_alfven2(const oracle_ctx& c, int i, int j, int k);
 void orc_mhd_source_a(oracle_ctx& c);
+void orc_mhd_source_curv(oracle_ctx& c);
 void orc_mhd_emf(oracle_ctx& c);
 void orc_mhd_lorentz(oracle_ctx& c);
 void orc_mhd_ct(oracle_ctx& c);

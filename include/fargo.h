@@ -97,7 +97,7 @@ typedef struct fargo_params {
                               cuda_stream; on the legacy default stream it falls back to plain launches);
                               0: plain stream launches */
   int mhd;                 /* 1: reserve the arrays of the MHD substeps (NEXT-4: B, the EMFs, the star values, v_X - v0: 13 arrays);
-                              they run once fargo_set_bfield has been called.  3-D Cartesian meshes and shearing sheets */
+                              they run once fargo_set_bfield has been called.  3-D meshes */
   int kernel_plan;         /* 0 = the fused kernels wherever they apply (default).  Bit flags select the unfused
                               sequences instead, for measurements and for tests that compare the two (results are
                               bit-identical): FARGO_PLAN_UNFUSED_SOURCE, FARGO_PLAN_UNFUSED_VISC, FARGO_PLAN_UNFUSED_DT */
@@ -163,7 +163,7 @@ int fargo_get_planets(fargo_ctx* ctx, double* pos, double* vel, double* gas_acc)
 int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
 
 /* MHD (sections 3.6.1-3.6.2; readings G34-G36): method of characteristics +
- * constrained transport on 3-D Cartesian meshes.  The context must have been created with fargo_params.mhd = 1.
+ * constrained transport on 3-D meshes.  The context must have been created with fargo_params.mhd = 1.
  * bx, by, bz: the face-centred field, HOST or DEVICE, nz*ny*nx elements of the context's precision each, ACTIVE cells,
  * bx[i,j,k] on the LOWER X face of cell (i,j,k) like vx.  mu0 > 0; eta >= 0 is the resistivity of Eq. 5;
  * passive != 0: the field is transported and diffused but exerts no force (the current-sheet test).  From then on
@@ -173,8 +173,10 @@ int fargo_set_omega_frame(fargo_ctx* ctx, double omega_new);
  * orbital advection on, the orbital advection of B by the upstream-averaged EMF (cell 11, section 3.7, Eqs. 92-107; the
  * substeps of cell 8 then see the residual velocity v_X - v0).
  * The source step then runs as the kernel sequence 7a, 7b(c) (the magnetic pressure enters before 7b).
- * fargo_get_bfield copies the active cells out (any pointer may be NULL).  Cartesian meshes and the shearing sheet; not on
- * sub-domains or on curvilinear meshes (Eqs. 87-91): FARGO_EINVAL.  Errors: FARGO_EINVAL, FARGO_ESTATE, FARGO_ECUDA. */
+ * On cylindrical and spherical meshes every length is the physical one at the place where it is used, Eq. 76 is applied with
+ * the edge lengths and face areas of Tab. 5, and cell 7a gets the geometric terms of Eqs. 87-91 (reading G38).
+ * fargo_get_bfield copies the active cells out (any pointer may be NULL).  Not on sub-domains; the resistive term on Cartesian
+ * meshes only; the orbital advection of B not on spherical meshes: FARGO_EINVAL.  Errors: FARGO_EINVAL, FARGO_ESTATE, FARGO_ECUDA. */
 int fargo_set_bfield(fargo_ctx* ctx, const void* bx, const void* by, const void* bz, double mu0, double eta, int passive);
 int fargo_get_bfield(fargo_ctx* ctx, void* bx, void* by, void* bz);
 

@@ -105,8 +105,11 @@ static bool make_layout(Layout& L, const fargo_mesh* m, int geometry, int eos, c
   L.fargo = p->fargo_on != 0;
   L.adi = eos == FARGO_ADIABATIC;
   L.mhd = p->mhd != 0;
-  if (L.mhd && !(cartesian_metric && L.hasx && L.hasy && L.hasz)) {
-    err = "MHD: 3-D Cartesian meshes and shearing sheets (1.5-D and 2.5-D problems run on thin 3-D meshes)"; return false;
+  if (L.mhd && !(L.hasx && L.hasy && L.hasz)) {
+    err = "MHD: 3-D meshes (1.5-D and 2.5-D problems run on thin 3-D meshes)"; return false;
+  }
+  if (L.mhd && geometry == FARGO_SPHERICAL && p->fargo_on) {
+    err = "MHD: the orbital advection of B (cell 11) is built for Cartesian and cylindrical meshes (DESIGN.md G38)"; return false;
   }
   for (int dd = 1; dd < 3 && L.mhd; ++dd)
     for (int s = 0; s < 2; ++s)
@@ -584,6 +587,7 @@ struct Sim : CtxBase {
   int set_bfield(const void* bx, const void* by, const void* bz, double mu0_, double eta_, int passive) override {
     if (!L.mhd) { err = "the context was created without fargo_params.mhd"; return FARGO_ESTATE; }
     if (!bx || !by || !bz || !(mu0_ > 0.0) || eta_ < 0.0) { err = "bx, by, bz, mu0 > 0 and eta >= 0 are required"; return FARGO_EINVAL; }
+    if (eta_ != 0.0 && d.geometry != GEO_CART) { err = "the resistive term is built for the Cartesian metric only"; return FARGO_EINVAL; }
     if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
     const size_t nact = (size_t)L.nx * L.ny * L.nz;
     const size_t arrb = align_up((size_t)L.narr * sizeof(T), 256);

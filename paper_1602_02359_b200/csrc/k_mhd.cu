@@ -28,10 +28,24 @@ __device__ __forceinline__ Cell<T> mv(const Dev<T>& d, Cell<T> q, const int dir,
 }
 template <typename T>
 __device__ __forceinline__ long long at(const Dev<T>& d, const Cell<T>& q) { return d.id(q.n[0], q.n[1], q.n[2]); }
+// R_x = 1 | r | r sin(theta), R_z = 1 | 1 | r (Tab. 1) where a quantity on the lower f face of cell q sits (f = 1: at the
+// lower Y edge, f = 2: at the lower Z edge, else at the zone centre), and their reciprocals (host tables).  On a Cartesian
+// mesh every factor is 1.0 and the products below are exact (reading G38).
+template <typename T> __device__ __forceinline__ T RxJ(const Dev<T>& d, const Cell<T>& q, const int f) { return d.geometry == GEO_CART ? T(1) : (f == 1 ? d.ye[q.n[1]] : d.yc[q.n[1]]); }
+template <typename T> __device__ __forceinline__ T RxK(const Dev<T>& d, const Cell<T>& q, const int f) { return d.geometry == GEO_SPH ? (f == 2 ? d.sin_ze[q.n[2]] : d.sin_zc[q.n[2]]) : T(1); }
+template <typename T> __device__ __forceinline__ T RzJ(const Dev<T>& d, const Cell<T>& q, const int f) { return d.geometry == GEO_SPH ? (f == 1 ? d.ye[q.n[1]] : d.yc[q.n[1]]) : T(1); }
+template <typename T> __device__ __forceinline__ T iRxJ(const Dev<T>& d, const Cell<T>& q, const int f) { return d.geometry == GEO_CART ? T(1) : (f == 1 ? d.inv_ye[q.n[1]] : d.inv_yc[q.n[1]]); }
+template <typename T> __device__ __forceinline__ T iRxK(const Dev<T>& d, const Cell<T>& q, const int f) { return d.geometry == GEO_SPH ? (f == 2 ? d.inv_sin_ze[q.n[2]] : d.invRxk[q.n[2]]) : T(1); }
+template <typename T> __device__ __forceinline__ T iRzJ(const Dev<T>& d, const Cell<T>& q, const int f) { return d.geometry == GEO_SPH ? (f == 1 ? d.inv_ye[q.n[1]] : d.inv_yc[q.n[1]]) : T(1); }
+// physical width of cell q along dir and 1 / (distance of its centre from the centre below), for a quantity on the lower f face
 template <typename T>
-__device__ __forceinline__ T width(const Dev<T>& d, const int dir, const int n) { return dir == 0 ? d.dx : dir == 1 ? d.LY[n] : d.dz[n]; }
-template <typename T>   // 1 / (centre n - centre n-1)
-__device__ __forceinline__ T invdist(const Dev<T>& d, const int dir, const int n) { return dir == 0 ? d.invdx : dir == 1 ? d.invDY[n] : d.invdzc[n]; }
+__device__ __forceinline__ T width(const Dev<T>& d, const int dir, const Cell<T>& q, const int f) {
+  return dir == 0 ? (d.dx * RxJ(d, q, f)) * RxK(d, q, f) : dir == 1 ? d.LY[q.n[1]] : d.dz[q.n[2]] * RzJ(d, q, f);
+}
+template <typename T>
+__device__ __forceinline__ T invdist(const Dev<T>& d, const int dir, const Cell<T>& q, const int f) {
+  return dir == 0 ? (d.invdx * iRxJ(d, q, f)) * iRxK(d, q, f) : dir == 1 ? d.invDY[q.n[1]] : d.invdzc[q.n[2]] * iRzJ(d, q, f);
+}
 template <typename T>
 __device__ __forceinline__ bool fits(const Dev<T>& d, const int dir, const int n, const int lo, const int hi) {
   if (dir == 0 && d.xwrap) return true;
@@ -55,21 +69,21 @@ __device__ __forceinline__ T slope3(const T fm, const T f0, const T fp, const T 
   const T a = rdiv(T(2) * pr, flat ? T(1) : dm + dp);
   return flat ? T(0) : a;
 }
-template <typename T>
-__device__ __forceinline__ Recon<T> recon(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir) {
-  const Cell<T> qm = mv(d, q, dir, -1);
-  const T f2 = f[at(d, mv(d, qm, dir, -1))], f1 = f[at(d, qm)], f0 = f[at(d, q)], fp = f[at(d, mv(d, q, dir, +1))];
-  const int n = q.n[dir];
-  const T im = invdist(d, dir, dir == 0 ? n : n - 1), i0 = invdist(d, dir, n), ip = invdist(d, dir, dir == 0 ? n : n + 1);
+template <typename T>   // fc: the direction of the faces f lives on (it fixes the lengths on a curvilinear mesh)
+__device__ __forceinline__ Recon<T> recon(const Dev<T>& d, const T* __restrict__ f, const Cell<T>& q, const int dir, const int fc) {
+  const Cell<T> qm = mv(d, q, dir, -1), qp = mv(d, q, dir, +1);
+  const T f2 = f[at(d, mv(d, qm, dir, -1))], f1 = f[at(d, qm)], f0 = f[at(d, q)], fp = f[at(d, qp)];
+  const T im = invdist(d, dir, dir == 0 ? q : qm, fc), i0 = invdist(d, dir, q, fc), ip = invdist(d, dir, dir == 0 ? q : qp, fc);
   Recon<T> r;
   r.fm = f1; r.f0 = f0;
   r.sm = slope3(f2, f1, f0, im, i0);
   r.s0 = slope3(f1, f0, fp, i0, ip);
-  r.wm = width(d, dir, qm.n[dir]); r.w0 = width(d, dir, n);
+  r.wm = width(d, dir, qm, fc); r.w0 = width(d, dir, q, fc);
   return r;
 }
 
 template <typename T> struct Vec3 { T* c[3]; };
+template <typename T> __global__ void k_mhd_curv(const Dev<T> d, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0);
 
 // ---- cell 2 ------------------------------------------------------------------------------------------------------------
 template <typename T, int DIR>
@@ -133,14 +147,17 @@ __global__ void __launch_bounds__(128) k_mhd_pressure(const Dev<T> d, const T* _
     if (!fits(d, dir, q.n[dir], 1, 0) || !fits(d, da, q.n[da], 0, 1) || !fits(d, db, q.n[db], 0, 1)) continue;
     const Cell<T> qm = mv(d, q, dir, -1);
     const long long l = at(d, q);
-    const T wf = rdiv(T(2) * invdist(d, dir, q.n[dir]), rho[l] + rho[at(d, qm)]);
+    const T il = dir == 0 ? d.invLX(q.n[1], q.n[2]) : dir == 1 ? d.invDY[q.n[1]] : d.invDZ(q.n[1], q.n[2]);   // as 7a's pressure gradient
+    const T wf = rdiv(T(2) * il, rho[l] + rho[at(d, qm)]);
     vb.c[dir][l] = rfma(-dt, wf * (pmag(d, b, q, dir, mu0) - pmag(d, b, qm, dir, mu0)), vb.c[dir][l]);
   }
 }
 template <typename T>
 int launch_mhd_pressure(const Dev<T>& d, const T* rho, T* bx, T* by, T* bz, T* vxb, T* vyb, T* vzb, double mu0, cudaStream_t s) {
   k_mhd_pressure<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0);
-  return 1;
+  if (d.geometry == GEO_CART) return 1;
+  k_mhd_curv<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0);
+  return 2;
 }
 
 // ---- cells 8a-8c (+ the star values of 8d): one thread per edge along D3 ----------------------------------------------
@@ -165,7 +182,7 @@ __global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d, const T* __rest
   const T ro = T(0.25) * (((rho[l] + rho[l1]) + rho[l2]) + rho[at(d, q12)]);
   const T sr = rsqrt_ieee(mu0 * ro);
   // the reconstructions every star value on this edge picks from: (v_D1, B_D1) along D2, (v_D2, B_D2) along D1
-  const Recon<T> rV1 = recon(d, V1, q, D2), rB1 = recon(d, B1, q, D2), rV2 = recon(d, V2, q, D1), rB2 = recon(d, B2, q, D1);
+  const Recon<T> rV1 = recon(d, V1, q, D2, D1), rB1 = recon(d, B1, q, D2, D1), rV2 = recon(d, V2, q, D1, D2), rB2 = recon(d, B2, q, D1, D2);
   // upwind estimates of the transverse fields (superscript u)
   const T v2bar = T(0.5) * (V2[l] + V2[l1]);
   const T v1bar = T(0.5) * (V1[l] + V1[l2]);
@@ -188,8 +205,8 @@ __global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d, const T* __rest
   }
   T emf = T(0.5) * (((v1s * B2u + B2s * v1u) - v2s * B1u) - B1s * v2u);   // Eq. 84
   if (eta != T(0)) {   // cell 8c: - eta (curl B)_D3
-    T J = (B2[l] - B2[l1]) * invdist(d, D1, q.n[D1]);
-    J = J - (B1[l] - B1[l2]) * invdist(d, D2, q.n[D2]);
+    T J = (B2[l] - B2[l1]) * invdist(d, D1, q, D2);
+    J = J - (B1[l] - B1[l2]) * invdist(d, D2, q, D1);
     emf = rfma(-eta, J, emf);
   }
   E[l] = emf;
@@ -242,8 +259,8 @@ __global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d, const T* __
     const long long lm = at(d, qm), la = at(d, qa), lb = at(d, qb);
     const T Bbar_a = T(0.25) * (((Ba[l] + Ba[la]) + Ba[lm]) + Ba[at(d, mv(d, qm, DA, +1))]);
     const T Bbar_b = T(0.25) * (((Bb[l] + Bb[lb]) + Bb[lm]) + Bb[at(d, mv(d, qm, DB, +1))]);
-    T acc = Bbar_a * rdiv(Sa[la] - Sa[l], width(d, DA, q.n[DA]));
-    acc = rfma(Bbar_b, rdiv(Sb[lb] - Sb[l], width(d, DB, q.n[DB])), acc);
+    T acc = Bbar_a * rdiv(Sa[la] - Sa[l], width(d, DA, q, D));
+    acc = rfma(Bbar_b, rdiv(Sb[lb] - Sb[l], width(d, DB, q, D)), acc);
     const T wf = rdiv(T(2), mu0 * (rho[l] + rho[lm]));
     v.c[D][l] = rfma(dt, wf * acc, v.c[D][l]);
   }
@@ -257,15 +274,83 @@ __global__ void __launch_bounds__(128) k_mhd_ct(const Dev<T> d, const MhdArrays<
   const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
   const long long l = at(d, q);
   const T dt = (T)d.ctl->dt;
+  if (d.geometry != GEO_CART) {
+    // Eq. 76 proper: d(B S)/dt = circulation of eps around the face with the physical edge lengths, over Tab. 5's area:
+    // Z edge at (i-1/2, j-1/2, k): lZ = dz R_z(edge j); X edge at (i, j-1/2, k-1/2): lX = dx R_x(edge j, edge k); Y edge: LY[j]
+    const int j = q.n[1], k = q.n[2];
+    const bool sph = d.geometry == GEO_SPH;
+    auto lZ = [&](const int jj) { return d.dz[k] * (sph ? d.ye[jj] : T(1)); };
+    auto lX = [&](const int jj, const int kk) { return (d.dx * d.ye[jj]) * (sph ? d.sin_ze[kk] : T(1)); };
+    const long long li = at(d, mv(d, q, 0, +1)), lj = l + d.pitch, lk = l + d.plane;
+    const T* __restrict__ EX = A.emf[0];
+    const T* __restrict__ EY = A.emf[1];
+    const T* __restrict__ EZ = A.emf[2];
+    if (fits(d, 0, i, 2, 1) && fits(d, 1, j, 2, 2) && fits(d, 2, k, 2, 2)) {
+      T circ = EZ[lj] * lZ(j + 1) - EZ[l] * lZ(j);
+      circ = circ - (EY[lk] - EY[l]) * d.LY[j];
+      b.c[0][l] = rfma(dt, rdiv(circ, d.Sx(j, k)), b.c[0][l]);
+    }
+    if (fits(d, 1, j, 2, 1) && fits(d, 2, k, 2, 2) && fits(d, 0, i, 2, 2)) {
+      T circ = EX[lk] * lX(j, k + 1) - EX[l] * lX(j, k);
+      circ = circ - (EZ[li] - EZ[l]) * lZ(j);
+      b.c[1][l] = rfma(dt, rdiv(circ, d.Sy(j, k)), b.c[1][l]);
+    }
+    if (fits(d, 2, k, 2, 1) && fits(d, 0, i, 2, 2) && fits(d, 1, j, 2, 2)) {
+      T circ = (EY[li] - EY[l]) * d.LY[j];
+      circ = circ - (EX[lj] * lX(j + 1, k) - EX[l] * lX(j, k));
+      b.c[2][l] = rfma(dt, rdiv(circ, d.Sz(j, k)), b.c[2][l]);
+    }
+    return;
+  }
 #pragma unroll
   for (int D = 0; D < 3; ++D) {
     const int DA = (D + 1) % 3, DB = (D + 2) % 3;
     if (!fits(d, D, q.n[D], 2, 1) || !fits(d, DA, q.n[DA], 2, 2) || !fits(d, DB, q.n[DB], 2, 2)) continue;
     const T* __restrict__ Eb = A.emf[DB];
     const T* __restrict__ Ea = A.emf[DA];
-    T curl = rdiv(Eb[at(d, mv(d, q, DA, +1))] - Eb[l], width(d, DA, q.n[DA]));
-    curl = curl - rdiv(Ea[at(d, mv(d, q, DB, +1))] - Ea[l], width(d, DB, q.n[DB]));
+    T curl = rdiv(Eb[at(d, mv(d, q, DA, +1))] - Eb[l], width(d, DA, q, D));
+    curl = curl - rdiv(Ea[at(d, mv(d, q, DB, +1))] - Ea[l], width(d, DB, q, D));
     b.c[D][l] = rfma(dt, curl, b.c[D][l]);
+  }
+}
+
+// ---- cell 7a, geometric terms of B.grad B on curvilinear meshes (Eqs. 87-91), applied to v_b in place --------------------
+template <typename T>
+__device__ __forceinline__ T avg4(const Dev<T>& d, const T* __restrict__ b, const Cell<T>& q, const int da, const int db) {
+  const Cell<T> qm = mv(d, q, db, -1);
+  return T(0.25) * (((b[at(d, q)] + b[at(d, mv(d, q, da, +1))]) + b[at(d, qm)]) + b[at(d, mv(d, qm, da, +1))]);
+}
+template <typename T>
+__global__ void __launch_bounds__(128) k_mhd_curv(const Dev<T> d, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0) {
+  if (d.ctl->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.TX) return;
+  const int j = blockIdx.y, k = blockIdx.z;
+  const Cell<T> q{{i, j, k}};
+  const long long l = at(d, q);
+  const bool sph = d.geometry == GEO_SPH;
+  const T dt = (T)d.ctl->dt, imu = rdiv(T(1), mu0);
+  const bool zok = !sph || fits(d, 2, k, 1, 1);
+  // all three read B only: the in-place update of v_b is safe
+  if (fits(d, 0, i, 1, 0) && fits(d, 1, j, 0, 1) && zok) {   // v_phi: Eqs. 87, 89
+    const T wf = rdiv(T(2) * imu, rho[l] + rho[at(d, mv(d, q, 0, -1))]);
+    const T bphi = b.c[0][l], br = avg4(d, b.c[1], q, 1, 0);
+    T g = br * bphi;
+    if (sph) g = rfma(avg4(d, b.c[2], q, 2, 0) * bphi, d.cot_zc[k], g);
+    vb.c[0][l] = rfma(dt, (wf * g) * d.inv_yc[j], vb.c[0][l]);
+  }
+  if (fits(d, 1, j, 1, 0) && fits(d, 0, i, 0, 1) && zok) {    // v_r: Eqs. 88, 90
+    const T wf = rdiv(T(2) * imu, rho[l] + rho[at(d, mv(d, q, 1, -1))]);
+    const T bphi = avg4(d, b.c[0], q, 0, 1);
+    T g = bphi * bphi;
+    if (sph) { const T bth = avg4(d, b.c[2], q, 2, 1); g = rfma(bth, bth, g); }
+    vb.c[1][l] = rfma(-dt, (wf * g) * d.inv_ye[j], vb.c[1][l]);
+  }
+  if (sph && fits(d, 2, k, 1, 0) && fits(d, 0, i, 0, 1) && fits(d, 1, j, 0, 1)) {   // v_theta: Eq. 91
+    const T wf = rdiv(T(2) * imu, rho[l] + rho[at(d, mv(d, q, 2, -1))]);
+    const T bth = b.c[2][l], br = avg4(d, b.c[1], q, 1, 2), bphi = avg4(d, b.c[0], q, 0, 2);
+    const T g = rfma(-(bphi * bphi), d.cot_ze[k], br * bth);
+    vb.c[2][l] = rfma(dt, (wf * g) * d.inv_yc[j], vb.c[2][l]);
   }
 }
 
@@ -349,11 +434,11 @@ __global__ void __launch_bounds__(128) k_mhd_arc(const Dev<T> d, const T* __rest
   T pz = T(0), py = T(0);
   if (j >= 1) {   // Z edges of the Y face j-1/2: it moves with the mean of the rings j-1 and j
     const T v0f = T(0.5) * (v0[d.rid(j, k)] + v0[d.rid(j - 1, k)]);
-    pz = arc_integral(by + row, d.nx, i, (v0f * dt) * d.invdx);
+    pz = arc_integral(by + row, d.nx, i, (v0f * dt) * invdist(d, 0, Cell<T>{{0, j, k}}, 1));   // zones of the face's own arc length
   }
   if (k >= 1) {   // Y edges of the Z face k-1/2
     const T v0f = T(0.5) * (v0[d.rid(j, k)] + v0[d.rid(j, k - 1)]);
-    py = arc_integral(bz + row, d.nx, i, (v0f * dt) * d.invdx);
+    py = arc_integral(bz + row, d.nx, i, (v0f * dt) * invdist(d, 0, Cell<T>{{0, j, k}}, 2));
   }
   PZ[l] = pz; PY[l] = py;
 }
@@ -363,8 +448,16 @@ __global__ void __launch_bounds__(128) k_mhd_orbital(const Dev<T> d, const T* __
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
   if (i >= d.TX || j < 1 || j + 1 >= d.TY || k < 1 || k + 1 >= d.TZ) return;
   const long long l = d.id(i, j, k), lp = d.id(d.xw(i + 1), j, k);
-  T dd = rdiv(d.dx * (PZ[l + d.pitch] - PZ[l]), d.LY[j]);              // Eq. 104 ...
-  dd = dd + rdiv(d.dx * (PY[l + d.plane] - PY[l]), d.dz[k]);            // ... and its Z counterpart
+  T dd;
+  if (d.geometry == GEO_CART) {
+    dd = rdiv(d.dx * (PZ[l + d.pitch] - PZ[l]), d.LY[j]);              // Eq. 104 ...
+    dd = dd + rdiv(d.dx * (PY[l + d.plane] - PY[l]), d.dz[k]);          // ... and its Z counterpart
+  } else {   // cylindrical: the same circulation with each edge's own arc length (Eq. 105), over the area of the face
+    const Cell<T> q{{i, j, k}}, qj{{i, j + 1, k}}, qk{{i, j, k + 1}};
+    dd = (width(d, 0, qj, 1) * PZ[l + d.pitch]) * d.dz[k] - (width(d, 0, q, 1) * PZ[l]) * d.dz[k];
+    dd = dd + (width(d, 0, qk, 2) * PY[l + d.plane] - width(d, 0, q, 2) * PY[l]) * d.LY[j];
+    dd = rdiv(dd, d.Sx(j, k));
+  }
   b.c[0][l] = b.c[0][l] + dd;
   b.c[1][l] = b.c[1][l] - (PZ[lp] - PZ[l]);                             // Eq. 101
   b.c[2][l] = b.c[2][l] - (PY[lp] - PY[l]);

@@ -57,6 +57,22 @@ def _case(name):
         prm = W.Params(gamma=1.4, fargo_on=1, omega_frame=1.0 if sheet else 0.0, oort_a=-0.75 if sheet else 0.0)
         return dict(mesh=m, eos=W.ADIABATIC, prm=prm, f=(rho, e) + v, b=(bx, by, bz), nsteps=6, eta=0.0, passive=False,
                     geometry=W.SHEARING_SHEET if sheet else W.CARTESIAN)
+    if name in ("cyl", "cyl_fargo", "sph"):   # curvilinear meshes (reading G38): a magnetised Keplerian disk with noise
+        sphc = name == "sph"
+        nx, ny, nz = (192 if name == "cyl_fargo" else 48), 18, 10   # cyl_fargo: arcs of more than one zone at the inner edge
+        zed = W.uedges(0.5 * math.pi - 0.25, 0.5 * math.pi + 0.25, nz) if sphc else W.uedges(-0.3, 0.3, nz)
+        m = W.Mesh(nx, ny, nz, 0.0, 2.0 * math.pi, W.uedges(0.6, 1.8, ny), zed, ((P, P), (R, O), (O, R) if sphc else (P, P)))
+        shape = (nz, ny, nx)
+        rr = m.yc()[None, :, None] * np.ones(shape)
+        om = 0.0 if name == "cyl_fargo" else 0.5                        # inertial frame: the planet also moves in the frame
+        prm = W.Params(gamma=1.4, fargo_on=1 if name == "cyl_fargo" else 0, omega_frame=om, gm_star=1.0, planet_mass=1e-3, planet_r=1.1,
+                       planet_phi0=0.3, planet_omega=0.5, planet_eps=0.05)
+        rho = rr ** -1.0 * (1.0 + 0.1 * r.uniform(-1, 1, shape))
+        e = rho * (0.1 ** 2 / rr) / 0.4 * (1.0 + 0.1 * r.uniform(-1, 1, shape))
+        v = (rr ** -0.5 - rr * om + 0.03 * r.uniform(-1, 1, shape), 0.03 * r.uniform(-1, 1, shape), 0.03 * r.uniform(-1, 1, shape))
+        b = tuple(0.05 * r.uniform(-1, 1, shape) + s0 for s0 in (0.02, 0.01, 0.05))
+        return dict(mesh=m, eos=W.ADIABATIC, prm=prm, f=(rho, e) + v, b=b, nsteps=6, eta=0.0, passive=False,
+                    geometry=W.SPHERICAL if sphc else W.CYLINDRICAL)
     bcs = {"periodic": ((P, P), (P, P), (P, P)), "mixed": ((O, R), (R, O), (O, O)), "resistive": ((P, P), (O, O), (P, P)),
            "passive": ((P, P), (P, P), (P, P)), "iso": ((P, P), (P, P), (R, R))}
     nx, ny, nz = (34, 13, 11) if name != "mixed" else (21, 12, 14)
@@ -90,7 +106,7 @@ def _rel(a, b):
     return d / s if s > 0 else d
 
 
-CASES = ["periodic", "mixed", "resistive", "passive", "iso", "brio_wu", "fargo", "sheet"]
+CASES = ["periodic", "mixed", "resistive", "passive", "iso", "brio_wu", "fargo", "sheet", "cyl", "cyl_fargo", "sph"]
 
 
 @pytest.mark.parametrize("name", CASES)
@@ -143,6 +159,11 @@ def test_mhd_argument_errors_and_second_set_bfield():
     with pytest.raises(RuntimeError):
         g.set_bfield(*c["b"])
     g.close()
+    sp = _case("sph")
+    with pytest.raises(RuntimeError):                                 # the resistive term: Cartesian metric only
+        gs = Fargo(sp["mesh"], W.SPHERICAL, sp["eos"], sp["prm"], mhd=True)
+        gs.set_fields(*sp["f"])
+        gs.set_bfield(*sp["b"], eta=1e-3)
     with pytest.raises(ValueError):                                   # a 2-D mesh: thin 3-D meshes are the way
         Fargo(W.Mesh(16, 16, 1, 0.0, 1.0, W.uedges(0, 1, 16), np.array([0.0, 1.0])), W.CARTESIAN, c["eos"], c["prm"], mhd=True)
     g, o = _pair(c)

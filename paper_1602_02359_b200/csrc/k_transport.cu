@@ -313,7 +313,7 @@ constexpr int MTHREADS = FG_MTHREADS;
 // rings (221 KB) only 28 KB of L1 remain and the bare skeleton (no arithmetic) is capped at ~5.1 TB/s; with <= 196 KB of
 // rings (60 KB of L1) it moves 6.4 TB/s (profiles/r02a_marches.md).  So: as many slots as fit in
 // 64 KB per block, never more than 8; RS - 3 rows in flight (the ring also keeps rows r-1 and r-2).
-__host__ __device__ constexpr int ring_slots(int na) { return 64 / na < 8 ? 64 / na : 8; }   // na: 8-byte words per cell and row
+__host__ __device__ constexpr int ring_slots(int na) { return (196 / FG_MBLOCKS) / na < 8 ? (196 / FG_MBLOCKS) / na : 8; }   // na: 8-byte words per cell and row
 
 template <typename T> struct CpAsync;
 template <> struct CpAsync<double> {
@@ -388,24 +388,21 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
   for (int q = 0; q <= NQ; ++q) { fA[q] = fB[q] = a2[q] = F2[q] = T(0); }
   T len2 = T(0), len1 = T(0), invd1 = T(0), w1 = T(0), S1 = T(0), dtiv2 = T(0), dtiv1 = T(0);
 
-  T nL, nD, nS, nV;   // table entries of the next row to be reduced
-  {
-    const int r0 = c0 - 2;
+  // the geometry of the chunk's rows (Tab. 5 factors along the sweep axis), staged once in shared memory behind the ring:
+  // a global load per row and table kept an LDG scoreboard busy in every row (ncu: a third of the long-scoreboard
+  // stalls sat on the first FMA after it, profiles/r02b_final.md); a broadcast LDS has none of that
+  T* const tab = reinterpret_cast<T*>(smem_raw) + (size_t)RS * NA * MTHREADS;   // [4][nrow]
+  for (int n = threadIdx.x; n < nrow; n += MTHREADS) {
+    const int r0 = c0 - 2 + n;
     const int rc = r0 < 0 ? 0 : (r0 >= TL ? TL - 1 : r0);
-    nL = tL[rc]; nD = tD[rc]; nS = tS[rc]; nV = tV[rc];
+    tab[n] = tL[rc]; tab[nrow + n] = tD[rc]; tab[2 * nrow + n] = tS[rc]; tab[3 * nrow + n] = tV[rc];
   }
+  __syncthreads();
 
   // one row: f2 (in: q of row r-2; out: q of row r), f1 (q of row r-1)
   auto row_step = [&](const int n, T (&f2)[NQ + 1], T (&f1)[NQ + 1]) {
     const int r = c0 - 2 + n;
-    // geometry of row r was fetched one row ago (a load consumed in the row it is issued in costs a full L1
-    // round trip per row: profiles/r01e); row r+1's is fetched here, pinned ahead of the wait below
-    const T cL = nL, cD = nD, cS = nS, cV = nV;
-    {
-      const int rn = r + 1;
-      const int rc = rn < 0 ? 0 : (rn >= TL ? TL - 1 : rn);
-      nL = ld_pinned(tL + rc); nD = ld_pinned(tD + rc); nS = ld_pinned(tS + rc); nV = ld_pinned(tV + rc);
-    }
+    const T cL = tab[n], cD = tab[nrow + n], cS = tab[2 * nrow + n], cV = tab[3 * nrow + n];
     fetch(n + RD);
     cp_wait<RD>();                                   // row n has landed
     const T* cur = ring + ((n % RS) * NA) * MTHREADS;
@@ -484,11 +481,13 @@ static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cuda
   const int TL = dir == 1 ? d.TY : d.TZ, lines = dir == 1 ? d.TZ : d.TY;
   // chunk the sweep axis: equal blocks run in rounds of the resident slots; each chunk re-reads 4 rows of halo
   const long long cols = (long long)((d.TX + MTHREADS - 1) / MTHREADS) * lines;
-  const size_t sm = (size_t)ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * sizeof(T);
+  const size_t ring = (size_t)ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * sizeof(T);
   static int slots = 0;   // per instantiation (T, NQ): the two directions have the same resources
-  if (!slots) slots = resident_slots(k_sweep_ring<T, 1, NQ>, MTHREADS, sm);
-  const int CH = pick_chunk_len(cols, TL, 4, slots, 16);
+  if (!slots) slots = resident_slots(k_sweep_ring<T, 1, NQ>, MTHREADS, ring + 4096);
+  int CH = pick_chunk_len(cols, TL, 4, slots, 16);
+  if (CH > 508) CH = 508;                                   // the chunk's geometry tables sit behind the ring: 4 x (CH + 4) reals, <= 16 KB
   const int nch = (TL + CH - 1) / CH;
+  const size_t sm = ring + (size_t)4 * (CH + 4) * sizeof(T);
   dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);
   if (dir == 1) k_sweep_ring<T, 1, NQ><<<g, b, sm, s>>>(d, a, CH);
   else k_sweep_ring<T, 2, NQ><<<g, b, sm, s>>>(d, a, CH);
@@ -509,7 +508,7 @@ int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s
 }
 
 template <typename T, int NQ> static void ring_attr() {
-  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T);
+  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T) + 4 * 512 * (int)sizeof(T);
   cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   // 196 of 228 KB at most for the rings: the rest stays L1 for the cp.async.ca lines in flight (see ring_slots)

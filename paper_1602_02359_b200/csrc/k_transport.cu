@@ -311,9 +311,11 @@ constexpr int MTHREADS = FG_MTHREADS;
 // Ring depth.  cp.async.ca passes through L1, and a line stays allocated there until its data has landed: the bytes a
 // SM can keep in flight are bounded by the L1 that the shared-memory carve-out leaves.  With three blocks of 8 x 9 KB
 // rings (221 KB) only 28 KB of L1 remain and the bare skeleton (no arithmetic) is capped at ~5.1 TB/s; with <= 196 KB of
-// rings (60 KB of L1) it moves 6.4 TB/s (profiles/r02a_marches.md).  So: as many slots as fit in
-// 64 KB per block, never more than 8; RS - 3 rows in flight (the ring also keeps rows r-1 and r-2).
-__host__ __device__ constexpr int ring_slots(int na) { return (196 / FG_MBLOCKS) / na < 8 ? (196 / FG_MBLOCKS) / na : 8; }   // na: 8-byte words per cell and row
+// shared memory per SM (60 KB of L1) it moves 6.4 TB/s (profiles/r02a_marches.md).  So: as many slots as fit in
+// 196 KB / blocks per SM, never more than 8; RS - 3 rows in flight (the ring also keeps rows r-1 and r-2).
+__host__ __device__ constexpr int ring_slots(int na) {   // na: 8-byte words per cell and row; 8 KB per block go to the tables
+  return (196 / FG_MBLOCKS - 8) / na < 8 ? (196 / FG_MBLOCKS - 8) / na : 8;
+}
 
 template <typename T> struct CpAsync;
 template <> struct CpAsync<double> {
@@ -485,7 +487,7 @@ static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cuda
   static int slots = 0;   // per instantiation (T, NQ): the two directions have the same resources
   if (!slots) slots = resident_slots(k_sweep_ring<T, 1, NQ>, MTHREADS, ring + 4096);
   int CH = pick_chunk_len(cols, TL, 4, slots, 16);
-  if (CH > 508) CH = 508;                                   // the chunk's geometry tables sit behind the ring: 4 x (CH + 4) reals, <= 16 KB
+  if (CH > 216) CH = 216;                                   // the chunk's geometry tables sit behind the ring: 4 x (CH + 4) reals, <= 7 KB
   const int nch = (TL + CH - 1) / CH;
   const size_t sm = ring + (size_t)4 * (CH + 4) * sizeof(T);
   dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);
@@ -508,12 +510,11 @@ int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s
 }
 
 template <typename T, int NQ> static void ring_attr() {
-  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T) + 4 * 512 * (int)sizeof(T);
+  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T) + 4 * 220 * (int)sizeof(T);
   cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-  // 196 of 228 KB at most for the rings: the rest stays L1 for the cp.async.ca lines in flight (see ring_slots)
-  cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 86);
-  cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributePreferredSharedMemoryCarveout, 86);
+  // no carve-out request: the driver then picks the smallest shared-memory configuration that holds the resident blocks
+  // (196 KB here) and L1 keeps the rest; asking for 86 % or 100 % was measured to select the 228 KB one (see ring_slots)
 }
 template <typename T> void sweep_setup() {
   ring_attr<T, 2>(); ring_attr<T, 3>(); ring_attr<T, 4>(); ring_attr<T, 5>(); ring_attr<T, 6>(); ring_attr<T, 7>();

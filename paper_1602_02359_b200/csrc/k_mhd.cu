@@ -134,8 +134,10 @@ __device__ __forceinline__ T pmag(const Dev<T>& d, const Vec3<T>& b, const Cell<
   }
   return rdiv(s, T(2) * mu0);
 }
-template <typename T>
-__global__ void __launch_bounds__(128) k_mhd_pressure(const Dev<T> d, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0) {
+template <typename T, int GEO>
+__global__ void __launch_bounds__(128) k_mhd_pressure(const Dev<T> d_in, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0) {
+  Dev<T> d = d_in;
+  if (GEO == GEO_CART) d.geometry = GEO_CART;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
@@ -147,24 +149,31 @@ __global__ void __launch_bounds__(128) k_mhd_pressure(const Dev<T> d, const T* _
     if (!fits(d, dir, q.n[dir], 1, 0) || !fits(d, da, q.n[da], 0, 1) || !fits(d, db, q.n[db], 0, 1)) continue;
     const Cell<T> qm = mv(d, q, dir, -1);
     const long long l = at(d, q);
-    const T il = dir == 0 ? d.invLX(q.n[1], q.n[2]) : dir == 1 ? d.invDY[q.n[1]] : d.invDZ(q.n[1], q.n[2]);   // as 7a's pressure gradient
+    // as 7a's pressure gradient (on a Cartesian mesh invLX = 1/dx and invDZ = invdzc: the table factors are 1.0)
+    const T il = GEO == GEO_CART ? (dir == 0 ? d.invdx : dir == 1 ? d.invDY[q.n[1]] : d.invdzc[q.n[2]])
+                                 : (dir == 0 ? d.invLX(q.n[1], q.n[2]) : dir == 1 ? d.invDY[q.n[1]] : d.invDZ(q.n[1], q.n[2]));
     const T wf = rdiv(T(2) * il, rho[l] + rho[at(d, qm)]);
     vb.c[dir][l] = rfma(-dt, wf * (pmag(d, b, q, dir, mu0) - pmag(d, b, qm, dir, mu0)), vb.c[dir][l]);
   }
 }
 template <typename T>
 int launch_mhd_pressure(const Dev<T>& d, const T* rho, T* bx, T* by, T* bz, T* vxb, T* vyb, T* vzb, double mu0, cudaStream_t s) {
-  k_mhd_pressure<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0);
-  if (d.geometry == GEO_CART) return 1;
+  const dim3 g((d.TX + 127) / 128, d.TY, d.TZ);
+  if (d.geometry == GEO_CART) { k_mhd_pressure<T, GEO_CART><<<g, 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0); return 1; }
+  k_mhd_pressure<T, GEO_CYL><<<g, 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0);   // (any curvilinear tag: tables are read)
   k_mhd_curv<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, Vec3<T>{{bx, by, bz}}, Vec3<T>{{vxb, vyb, vzb}}, (T)mu0);
   return 2;
 }
 
 // ---- cells 8a-8c (+ the star values of 8d): one thread per edge along D3 ----------------------------------------------
-template <typename T, int D3>
-__global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d, const T* __restrict__ rho, const Vec3<T> v, const Vec3<T> b,
+// GEO is the mesh geometry as a compile-time constant: on a Cartesian mesh every metric factor folds to 1.0 and its table
+// loads disappear (the run-time test cost a third of the kernel's time at 512^3)
+template <typename T, int D3, int GEO>
+__global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d_in, const T* __restrict__ rho, const Vec3<T> v, const Vec3<T> b,
                                                  T* __restrict__ E, T* __restrict__ S1, T* __restrict__ S2, const T mu0, const T eta) {
   constexpr int D1 = (D3 + 1) % 3, D2 = (D3 + 2) % 3;
+  Dev<T> d = d_in;
+  d.geometry = GEO;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
@@ -227,9 +236,14 @@ int launch_mhd_emf(const Dev<T>& d, const T* rho, T* vx, T* vy, T* vz, T* bx, T*
                    double mu0, double eta, cudaStream_t s) {
   const Vec3<T> v{{vx, vy, vz}}, b{{bx, by, bz}};
   dim3 g((d.TX + 127) / 128, d.TY, d.TZ);
-  k_mhd_emf<T, 0><<<g, 128, 0, s>>>(d, rho, v, b, emf[0], bstar[0], bstar[1], (T)mu0, (T)eta);
-  k_mhd_emf<T, 1><<<g, 128, 0, s>>>(d, rho, v, b, emf[1], bstar[2], bstar[3], (T)mu0, (T)eta);
-  k_mhd_emf<T, 2><<<g, 128, 0, s>>>(d, rho, v, b, emf[2], bstar[4], bstar[5], (T)mu0, (T)eta);
+#define FG_EMF(GEO)                                                                                     \
+  k_mhd_emf<T, 0, GEO><<<g, 128, 0, s>>>(d, rho, v, b, emf[0], bstar[0], bstar[1], (T)mu0, (T)eta);      \
+  k_mhd_emf<T, 1, GEO><<<g, 128, 0, s>>>(d, rho, v, b, emf[1], bstar[2], bstar[3], (T)mu0, (T)eta);      \
+  k_mhd_emf<T, 2, GEO><<<g, 128, 0, s>>>(d, rho, v, b, emf[2], bstar[4], bstar[5], (T)mu0, (T)eta);
+  if (d.geometry == GEO_CART) { FG_EMF(GEO_CART) }
+  else if (d.geometry == GEO_CYL) { FG_EMF(GEO_CYL) }
+  else { FG_EMF(GEO_SPH) }
+#undef FG_EMF
   return 3;
 }
 
@@ -239,8 +253,10 @@ int launch_mhd_emf(const Dev<T>& d, const T* rho, T* vx, T* vy, T* vz, T* bx, T*
 template <typename T>
 struct MhdArrays { const T* b[3]; const T* emf[3]; const T* bstar[6]; };
 
-template <typename T>
-__global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d, const T* __restrict__ rho, const MhdArrays<T> A, const Vec3<T> v, const T mu0) {
+template <typename T, bool CART>
+__global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d_in, const T* __restrict__ rho, const MhdArrays<T> A, const Vec3<T> v, const T mu0) {
+  Dev<T> d = d_in;
+  if (CART) d.geometry = GEO_CART;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
@@ -266,8 +282,10 @@ __global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d, const T* __
   }
 }
 
-template <typename T>
-__global__ void __launch_bounds__(128) k_mhd_ct(const Dev<T> d, const MhdArrays<T> A, const Vec3<T> b) {
+template <typename T, bool CART>
+__global__ void __launch_bounds__(128) k_mhd_ct(const Dev<T> d_in, const MhdArrays<T> A, const Vec3<T> b) {
+  Dev<T> d = d_in;
+  if (CART) d.geometry = GEO_CART;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
@@ -359,7 +377,8 @@ int launch_mhd_tension(const Dev<T>& d, const T* rho, T* const* b, T* const* bst
   MhdArrays<T> A;
   for (int n = 0; n < 3; ++n) { A.b[n] = b[n]; A.emf[n] = nullptr; }
   for (int n = 0; n < 6; ++n) A.bstar[n] = bstar[n];
-  k_mhd_tension<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, A, Vec3<T>{{vx, vy, vz}}, (T)mu0);
+  if (d.geometry == GEO_CART) k_mhd_tension<T, true><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, A, Vec3<T>{{vx, vy, vz}}, (T)mu0);
+  else k_mhd_tension<T, false><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, rho, A, Vec3<T>{{vx, vy, vz}}, (T)mu0);
   return 1;
 }
 template <typename T>
@@ -367,7 +386,8 @@ int launch_mhd_ct(const Dev<T>& d, T* const* emf, T* bx, T* by, T* bz, cudaStrea
   MhdArrays<T> A;
   for (int n = 0; n < 3; ++n) { A.b[n] = nullptr; A.emf[n] = emf[n]; }
   for (int n = 0; n < 6; ++n) A.bstar[n] = nullptr;
-  k_mhd_ct<T><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, A, Vec3<T>{{bx, by, bz}});
+  if (d.geometry == GEO_CART) k_mhd_ct<T, true><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, A, Vec3<T>{{bx, by, bz}});
+  else k_mhd_ct<T, false><<<dim3((d.TX + 127) / 128, d.TY, d.TZ), 128, 0, s>>>(d, A, Vec3<T>{{bx, by, bz}});
   return 1;
 }
 

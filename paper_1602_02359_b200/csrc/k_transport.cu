@@ -165,7 +165,7 @@ template <typename T> struct Pair;
 template <> struct Pair<double> { using type = double2; };
 template <> struct Pair<float> { using type = float2; };
 
-constexpr int X2W = 4;          // warps (rows) per block
+constexpr int X2W = 2;          // warps (rows) per block
 constexpr int X2IN = 60;        // interior cells per warp
 
 template <typename T>
@@ -621,8 +621,13 @@ __global__ void __launch_bounds__(128) k_newvel_dt(const Dev<T> d, const T* __re
 // The same with TWO cells per lane (even nx): 16-byte accesses, the X neighbours by shuffle (lanes 0 and 31 of a warp
 // load their outer neighbour), half the address arithmetic and twice the loads in flight per thread.  Every expression
 // is the one k_newvel_dt evaluates for the same face, so the results are bit-identical.
+// Blocks of 64 threads (128 cells) and no register cap: at 512^3 that is 2.30 ms against 2.61 with 128 threads (66
+// registers), 2.62 with 96, and 3.1-3.4 ms for every variant whose registers were capped by a minimum block count
+// (ptxas then sinks half of the loads behind the arithmetic); tiles of 2-8 rows x 64 cells cost 2.9-3.4 ms
+// (profiles/r02b_final.md).
+constexpr int NVT = 64;
 template <typename T, bool ADI>
-__global__ void __launch_bounds__(128) k_newvel_dt2(const Dev<T> d, const T* __restrict__ rho, const T* __restrict__ en,
+__global__ void __launch_bounds__(NVT) k_newvel_dt2(const Dev<T> d, const T* __restrict__ rho, const T* __restrict__ en,
                                                     const QSet<T> S, const State<T> st) {
   if (d.ctl->done) return;
   const int ia = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
@@ -695,11 +700,12 @@ __global__ void __launch_bounds__(128) k_newvel_dt2(const Dev<T> d, const T* __r
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) m2 = rmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
-  __shared__ T sm[4];
+  __shared__ T sm[NVT / 32];
   if (lane == 0) sm[threadIdx.x >> 5] = m2;
   __syncthreads();
   if (threadIdx.x == 0) {
-    m2 = rmax(rmax(sm[0], sm[1]), rmax(sm[2], sm[3]));
+#pragma unroll
+    for (int n = 1; n < NVT / 32; ++n) m2 = rmax(m2, sm[n]);
     const unsigned long long b = to_bits(m2);
     if (b > *(volatile unsigned long long*)&d.ctl->m2bits) atomicMax(&d.ctl->m2bits, b);
   }
@@ -714,7 +720,7 @@ bool newvel_dt_ok(const Dev<T>& d) {
 template <typename T>
 int launch_newvel_dt(const Dev<T>& d, const T* rho, const T* en, const QSet<T>& set, const State<T>& st, cudaStream_t s) {
   if (d.nx % 2 == 0) {
-    dim3 b(128), g((d.nx / 2 + 127) / 128, d.ny, d.nz);
+    dim3 b(NVT), g((d.nx / 2 + NVT - 1) / NVT, d.ny, d.nz);
     if (d.eos == EOS_ADI) k_newvel_dt2<T, true><<<g, b, 0, s>>>(d, rho, en, set, st);
     else k_newvel_dt2<T, false><<<g, b, 0, s>>>(d, rho, en, set, st);
     return 1;

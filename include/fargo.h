@@ -215,6 +215,18 @@ int fargo_dt_min_with(fargo_ctx* ctx, const void* other_dt_device_ptr);
  * active cells with the volumes of Tab. 5.  Applies the ghost fill of cell 2 first (the next update starts with the
  * same fill); synchronises the stream.  Reduced on the device in a fixed-shape tree: reproducible. */
 int fargo_diagnostics(fargo_ctx* ctx, double* out);
+/* The same sums for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): out_device[5] is a DEVICE address the caller owns; the call enqueues the ghost fill of cell 2, the
+ * reduction kernel and a finishing kernel on the context's stream and returns WITHOUT synchronising (read out_device
+ * after the stream has run).  It calls no cudaMalloc / cudaFree and no allocating routine: the per-block partial sums
+ * live in a file-scope device array of the library (65536 x 5 doubles = 2.5 MiB, held by every device that loads the
+ * library until exit), and are added on the device in block order, the order fargo_diagnostics adds them on the host.
+ * Limit: ny * nz <= 524288 (8 rows along X per block); a larger mesh returns FARGO_EINVAL with a message and launches
+ * nothing.  All contexts of a device share the array: calls that overlap on the GPU (different streams, no
+ * dependency) race on it -- order them; the array's previous contents are never read.  The first call on a device
+ * looks the array's address up (cudaGetSymbolAddress, which may load the module): make it once before a capture.
+ * The device that holds the context's workspace must be current, as for every call. */
+int fargo_diagnostics_noalloc(fargo_ctx* ctx, double* out_device);
 
 /* Run the NEXT update up to and including `stage`; the state is then mid-step (only
  * fargo_get_array / fargo_dims / fargo_destroy / fargo_set_fields are valid afterwards). */

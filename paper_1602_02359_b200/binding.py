@@ -21,7 +21,7 @@ STAGES = ["BC1", "VMEAN", "POT", "DT", "SRC_A", "SRC_B", "SRC_C", "SRC_D", "BC2"
 EXPORTS = ["fargo_workspace_bytes", "fargo_init", "fargo_destroy", "fargo_set_fields", "fargo_get_fields",
            "fargo_step", "fargo_get_time", "fargo_kernel_launches", "fargo_step_until", "fargo_dims",
            "fargo_get_array", "fargo_last_error", "fargo_profile", "fargo_profile_report", "fargo_selftest_div",
-           "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics",
+           "fargo_set_planets", "fargo_get_planets", "fargo_set_omega_frame", "fargo_diagnostics", "fargo_diagnostics_noalloc",
            "fargo_update_phase", "fargo_halo_bytes", "fargo_halo", "fargo_dt_device_ptr", "fargo_set_bfield", "fargo_get_bfield", "fargo_dt_min_with"]
 
 
@@ -81,6 +81,7 @@ def load():
     L.fargo_get_planets.argtypes = [vp, _DP, _DP, _DP]
     L.fargo_set_omega_frame.argtypes = [vp, C.c_double]
     L.fargo_diagnostics.argtypes = [vp, _DP]
+    L.fargo_diagnostics_noalloc.argtypes = [vp, vp]
     L.fargo_set_bfield.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, C.c_int]
     L.fargo_get_bfield.argtypes = [vp, vp, vp, vp]
     L.fargo_update_phase.argtypes = [vp, C.c_int]
@@ -319,6 +320,16 @@ class Fargo:
         out = np.zeros(5)
         with self._torch.cuda.device(self.device):
             self._check(load().fargo_diagnostics(self._h, out.ctypes.data_as(_DP)), "fargo_diagnostics")
+        return out
+
+    def diagnostics_noalloc(self, out):
+        """fargo_diagnostics_noalloc: the same five sums into `out` (a CUDA float64 tensor of 5 elements on this device),
+        asynchronously on the context's stream; allocates nothing (ny * nz <= 524288).  Returns `out`."""
+        t = self._torch
+        if not (isinstance(out, t.Tensor) and out.is_cuda and out.dtype == t.float64 and out.numel() >= 5 and out.is_contiguous()):
+            raise ValueError("out: a contiguous CUDA float64 tensor of at least 5 elements")
+        with t.cuda.device(self.device):
+            self._check(load().fargo_diagnostics_noalloc(self._h, C.c_void_p(out.data_ptr())), "fargo_diagnostics_noalloc")
         return out
 
     def set_omega_frame(self, omega_new: float):

@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfargo_b200.so")
-SOURCES = ["api.cu", "k_bc.cu", "k_dt.cu", "k_source.cu", "k_source_fused.cu", "k_visc3d.cu", "k_transport.cu", "k_orbital.cu", "k_planets.cu", "k_mhd.cu", "tables.cpp"]
+SOURCES = ["api.cu", "k_bc.cu", "k_dt.cu", "k_source.cu", "k_source_fused.cu", "k_visc3d.cu", "k_transport.cu", "k_orbital.cu", "k_planets.cu", "k_noalloc.cu", "k_mhd.cu", "tables.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "-Xptxas", "-v"]
 

@@ -41,6 +41,7 @@ struct CtxBase {
   virtual int get_planets(double*, double*, double*) = 0;
   virtual int set_omega_frame(double) = 0;
   virtual int diagnostics(double*) = 0;
+  virtual int diagnostics_noalloc(double*) = 0;
   virtual int set_bfield(const void*, const void*, const void*, double, double, int) = 0;
   virtual int get_bfield(void*, void*, void*) = 0;
   virtual int profile(int enable) = 0;
@@ -583,6 +584,30 @@ struct Sim : CtxBase {
     return FARGO_OK;
   }
 
+  // the same without any allocation: partials in the static device array of k_noalloc.cu, sums added on the device
+  // into out_device[5]; asynchronous on the context's stream
+  int diagnostics_noalloc(double* out_device) override {
+    if (!out_device) { err = "null argument"; return FARGO_EINVAL; }
+    if (!have_fields) { err = "no fields set"; return FARGO_ESTATE; }
+    if (midstep) { err = "context is mid-step"; return FARGO_ESTATE; }
+    cudaPointerAttributes at;
+    if (!ck(cudaPointerGetAttributes(&at, out_device), "cudaPointerGetAttributes(out_device)")) return FARGO_ECUDA;
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) { err = "out_device is not device memory"; return FARGO_EINVAL; }
+    if ((long long)L.ny * L.nz > diagnostics_noalloc_max_rings()) {   // before anything is launched
+      std::string e;
+      launch_diagnostics_noalloc<T>(d, st, out_device, stream, e);
+      err = e;
+      return FARGO_EINVAL;
+    }
+    launches += launch_bc<T>(d, st, field_mask(true, true), stream);
+    std::string e;
+    const int n = launch_diagnostics_noalloc<T>(d, st, out_device, stream, e);
+    if (n < 0) { err = e; return n == -1 ? FARGO_EINVAL : FARGO_ECUDA; }
+    launches += n;
+    if (!ck(cudaGetLastError(), "diagnostics_noalloc launch")) return FARGO_ECUDA;
+    return FARGO_OK;
+  }
+
   // ---- MHD (NEXT-4) ----------------------------------------------------------------------------------
   int set_bfield(const void* bx, const void* by, const void* bz, double mu0_, double eta_, int passive) override {
     if (!L.mhd) { err = "the context was created without fargo_params.mhd"; return FARGO_ESTATE; }
@@ -980,6 +1005,7 @@ int fargo_get_planets(fargo_ctx* c, double* pos, double* vel, double* gas_acc) {
 }
 int fargo_set_omega_frame(fargo_ctx* c, double omega_new) { return c ? c->impl->set_omega_frame(omega_new) : FARGO_EINVAL; }
 int fargo_diagnostics(fargo_ctx* c, double* out) { return c ? c->impl->diagnostics(out) : FARGO_EINVAL; }
+int fargo_diagnostics_noalloc(fargo_ctx* c, double* out_device) { return c ? c->impl->diagnostics_noalloc(out_device) : FARGO_EINVAL; }
 int fargo_set_bfield(fargo_ctx* c, const void* bx, const void* by, const void* bz, double mu0, double eta, int passive) {
   return c ? c->impl->set_bfield(bx, by, bz, mu0, eta, passive) : FARGO_EINVAL;
 }

@@ -2,6 +2,7 @@
 // on the arithmetic type, instantiated for double and float in the k_*.cu files).
 // Every launcher enqueues on `s` and returns the number of kernels it launched.
 #pragma once
+#include <string>
 #include "common.cuh"
 
 namespace fg {
@@ -26,6 +27,11 @@ template <typename T> int launch_planets_update(const Dev<T>& d, const T* rho, P
 template <typename T> int launch_frame_change(const Dev<T>& d, T* vx, double dom, PlanetsDev* pl, int npl, cudaStream_t s);
 // diagnostics: per-block partial sums of mass, Tab. 2 momenta and internal energy: part[planets_blocks()][5]
 template <typename T> int launch_diagnostics(const Dev<T>& d, const State<T>& st, double* part, cudaStream_t s);
+// the same with the partials in a file-scope device array and the final sums added on the device into out_device[5]
+// (k_noalloc.cu: no allocation, no synchronisation); launches, or -1 (mesh beyond the array) / -2 (CUDA error) + err
+template <typename T> int launch_diagnostics_noalloc(const Dev<T>& d, const State<T>& st, double* out_device, cudaStream_t s,
+                                                     std::string& err);
+long long diagnostics_noalloc_max_rings();
 // cell 6: Eq. 59 + Eq. 73 -> ctl->dt (device resident)
 enum { DT_BOTH = 0, DT_FINISH = 1, DT_CELLS = 2 };   // per-cell max + finish | finish only | per-cell max only
 // MHD (NEXT-4): the face-centred field for the fast magnetosonic speed, 4 eta for the resistive limit (bx = nullptr: off)

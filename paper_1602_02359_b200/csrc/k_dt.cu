@@ -136,8 +136,9 @@ template <typename T> struct DPair;
 template <> struct DPair<double> { using type = double2; };
 template <> struct DPair<float> { using type = float2; };
 
-template <typename T, bool ADI>
-__global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T> st, const T* __restrict__ v0) {
+// MHD = true: C_w^2 = C_s^2 + v_A^2 with B averaged to the zone centre and the resistive item 5, as in k_dt_cells.
+template <typename T, bool ADI, bool MHD>
+__global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T> st, const T* __restrict__ v0, const MhdDt<T> M) {
   if (d.ctl->done) return;
   using P2 = typename DPair<T>::type;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -164,11 +165,31 @@ __global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T
       const P2 az = *reinterpret_cast<const P2*>(st.vz + l);
       const P2 bz = *reinterpret_cast<const P2*>(st.vz + l + d.plane);
       T nxt = __shfl_down_sync(0xffffffffu, ax.x, 1);
-      if (lane == 31 || i + 2 >= nx) { const int ip = i + 2 >= nx ? i + 2 - nx : i + 2; nxt = st.vx[base + (live ? ip : 0)]; }
+      const bool edge = lane == 31 || i + 2 >= nx;
+      const int ip = i + 2 >= nx ? i + 2 - nx : i + 2;
+      if (edge) nxt = st.vx[base + (live ? ip : 0)];
+      P2 fx = {T(0), T(0)}, fy0 = fx, fy1 = fx, fz0 = fx, fz1 = fx;
+      T fxn = T(0);
+      const bool alfven = MHD && !M.passive;
+      if (alfven) {
+        fx = *reinterpret_cast<const P2*>(M.bx + l);
+        fy0 = *reinterpret_cast<const P2*>(M.by + l);
+        fy1 = *reinterpret_cast<const P2*>(M.by + l + d.pitch);
+        fz0 = *reinterpret_cast<const P2*>(M.bz + l);
+        fz1 = *reinterpret_cast<const P2*>(M.bz + l + d.plane);
+        fxn = __shfl_down_sync(0xffffffffu, fx.x, 1);
+        if (edge) fxn = M.bx[base + (live ? ip : 0)];
+      }
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
         const T rho = c ? r.y : r.x, en = c ? e.y : e.x;
-        const T cs2 = ADI ? rdiv(d.gg1 * en, rho) : en * en;
+        T cs2 = ADI ? rdiv(d.gg1 * en, rho) : en * en;
+        if (alfven) {
+          const T cx = T(0.5) * ((c ? fx.y : fx.x) + (c ? fxn : fx.y));
+          const T cy = T(0.5) * ((c ? fy0.y : fy0.x) + (c ? fy1.y : fy1.x));
+          const T cz = T(0.5) * ((c ? fz0.y : fz0.x) + (c ? fz1.y : fz1.x));
+          cs2 = cs2 + rdiv(rfma(cz, cz, rfma(cy, cy, rfma(cx, cx, T(0)))), M.mu0 * rho);
+        }
         const T I1sq = cs2 * il2;
         T I2 = T(0), I3 = T(0);
         {
@@ -187,7 +208,8 @@ __global__ void __launch_bounds__(256) k_dt_cells2(const Dev<T> d, const State<T
           I3 = rmax(I3, rabs(b - a) * ilz);
         }
         I3 = d.c3 * I3;
-        const T Isq = rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq)));
+        T Isq = rfma(I4, I4, rfma(I3, I3, rfma(I2, I2, I1sq)));
+        if (MHD && M.eta4 != T(0)) { const T I5 = M.eta4 * il2; Isq = rfma(I5, I5, Isq); }
         if (live) m2 = rmax(m2, Isq);
       }
     }
@@ -252,10 +274,13 @@ int launch_dt(const Dev<T>& d, const State<T>& st, const T* v0, cudaStream_t s, 
     k_dt_finish<T><<<1, 1024, 0, s>>>(d, v0);
     return 1;
   }
-  if (!M.bx && d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0) {
+  if (d.hasx && d.hasy && d.hasz && d.xwrap && d.nx % 2 == 0) {
     const int g2 = nrow < 148 * 8 * 8 ? (nrow + 7) / 8 : 148 * 8;
-    if (d.eos == EOS_ADI) k_dt_cells2<T, true><<<g2, 256, 0, s>>>(d, st, v0);
-    else k_dt_cells2<T, false><<<g2, 256, 0, s>>>(d, st, v0);
+    if (M.bx) {
+      if (d.eos == EOS_ADI) k_dt_cells2<T, true, true><<<g2, 256, 0, s>>>(d, st, v0, M);
+      else k_dt_cells2<T, false, true><<<g2, 256, 0, s>>>(d, st, v0, M);
+    } else if (d.eos == EOS_ADI) k_dt_cells2<T, true, false><<<g2, 256, 0, s>>>(d, st, v0, M);
+    else k_dt_cells2<T, false, false><<<g2, 256, 0, s>>>(d, st, v0, M);
   } else {
     k_dt_cells<T><<<grid, 256, 0, s>>>(d, st, v0, M);
   }

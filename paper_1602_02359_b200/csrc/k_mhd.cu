@@ -14,7 +14,10 @@
 
 namespace fg {
 
-template <typename T> struct Cell { int n[3]; };
+// a cell and its linear index (kept along by mv: a neighbour costs an addition, not an index product)
+template <typename T> struct Cell { int n[3]; long long l; };
+template <typename T>
+__device__ __forceinline__ Cell<T> cell(const Dev<T>& d, const int i, const int j, const int k) { return Cell<T>{{i, j, k}, d.id(i, j, k)}; }
 
 template <typename T>
 __device__ __forceinline__ int ext_of(const Dev<T>& d, const int dir) { return dir == 0 ? d.TX : dir == 1 ? d.TY : d.TZ; }
@@ -23,11 +26,12 @@ template <typename T>
 __device__ __forceinline__ Cell<T> mv(const Dev<T>& d, Cell<T> q, const int dir, const int s) {
   int m = q.n[dir] + s;
   if (dir == 0 && d.xwrap) { if (m < 0) m += d.nx; else if (m >= d.nx) m -= d.nx; }
+  q.l += dir == 0 ? (long long)(m - q.n[0]) : dir == 1 ? s * d.pitch : s * d.plane;
   q.n[dir] = m;
   return q;
 }
 template <typename T>
-__device__ __forceinline__ long long at(const Dev<T>& d, const Cell<T>& q) { return d.id(q.n[0], q.n[1], q.n[2]); }
+__device__ __forceinline__ long long at(const Dev<T>&, const Cell<T>& q) { return q.l; }
 // R_x = 1 | r | r sin(theta), R_z = 1 | 1 | r (Tab. 1) where a quantity on the lower f face of cell q sits (f = 1: at the
 // lower Y edge, f = 2: at the lower Z edge, else at the zone centre), and their reciprocals (host tables).  On a Cartesian
 // mesh every factor is 1.0 and the products below are exact (reading G38).
@@ -135,13 +139,13 @@ __device__ __forceinline__ T pmag(const Dev<T>& d, const Vec3<T>& b, const Cell<
   return rdiv(s, T(2) * mu0);
 }
 template <typename T, int GEO>
-__global__ void __launch_bounds__(128) k_mhd_pressure(const Dev<T> d_in, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0) {
+__global__ void __launch_bounds__(128, 16) k_mhd_pressure(const Dev<T> d_in, const T* __restrict__ rho, const Vec3<T> b, const Vec3<T> vb, const T mu0) {
   Dev<T> d = d_in;
   if (GEO == GEO_CART) d.geometry = GEO_CART;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
-  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const Cell<T> q = cell(d, i, (int)blockIdx.y, (int)blockIdx.z);
   const T dt = (T)d.ctl->dt;
 #pragma unroll
   for (int dir = 0; dir < 3; ++dir) {
@@ -177,7 +181,7 @@ __global__ void __launch_bounds__(128) k_mhd_emf(const Dev<T> d_in, const T* __r
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
-  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const Cell<T> q = cell(d, i, (int)blockIdx.y, (int)blockIdx.z);
   const long long l = at(d, q);
   const T* __restrict__ V1 = v.c[D1];
   const T* __restrict__ V2 = v.c[D2];
@@ -254,13 +258,13 @@ template <typename T>
 struct MhdArrays { const T* b[3]; const T* emf[3]; const T* bstar[6]; };
 
 template <typename T, bool CART>
-__global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d_in, const T* __restrict__ rho, const MhdArrays<T> A, const Vec3<T> v, const T mu0) {
+__global__ void __launch_bounds__(128, 16) k_mhd_tension(const Dev<T> d_in, const T* __restrict__ rho, const MhdArrays<T> A, const Vec3<T> v, const T mu0) {
   Dev<T> d = d_in;
   if (CART) d.geometry = GEO_CART;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
-  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const Cell<T> q = cell(d, i, (int)blockIdx.y, (int)blockIdx.z);
   const long long l = at(d, q);
   const T dt = (T)d.ctl->dt;
 #pragma unroll
@@ -283,13 +287,13 @@ __global__ void __launch_bounds__(128) k_mhd_tension(const Dev<T> d_in, const T*
 }
 
 template <typename T, bool CART>
-__global__ void __launch_bounds__(128) k_mhd_ct(const Dev<T> d_in, const MhdArrays<T> A, const Vec3<T> b) {
+__global__ void __launch_bounds__(128, 16) k_mhd_ct(const Dev<T> d_in, const MhdArrays<T> A, const Vec3<T> b) {
   Dev<T> d = d_in;
   if (CART) d.geometry = GEO_CART;
   if (d.ctl->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
-  const Cell<T> q{{i, (int)blockIdx.y, (int)blockIdx.z}};
+  const Cell<T> q = cell(d, i, (int)blockIdx.y, (int)blockIdx.z);
   const long long l = at(d, q);
   const T dt = (T)d.ctl->dt;
   if (d.geometry != GEO_CART) {
@@ -344,7 +348,7 @@ __global__ void __launch_bounds__(128) k_mhd_curv(const Dev<T> d, const T* __res
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.TX) return;
   const int j = blockIdx.y, k = blockIdx.z;
-  const Cell<T> q{{i, j, k}};
+  const Cell<T> q = cell(d, i, j, k);
   const long long l = at(d, q);
   const bool sph = d.geometry == GEO_SPH;
   const T dt = (T)d.ctl->dt, imu = rdiv(T(1), mu0);
@@ -454,11 +458,11 @@ __global__ void __launch_bounds__(128) k_mhd_arc(const Dev<T> d, const T* __rest
   T pz = T(0), py = T(0);
   if (j >= 1) {   // Z edges of the Y face j-1/2: it moves with the mean of the rings j-1 and j
     const T v0f = T(0.5) * (v0[d.rid(j, k)] + v0[d.rid(j - 1, k)]);
-    pz = arc_integral(by + row, d.nx, i, (v0f * dt) * invdist(d, 0, Cell<T>{{0, j, k}}, 1));   // zones of the face's own arc length
+    pz = arc_integral(by + row, d.nx, i, (v0f * dt) * invdist(d, 0, cell(d, 0, j, k), 1));   // zones of the face's own arc length
   }
   if (k >= 1) {   // Y edges of the Z face k-1/2
     const T v0f = T(0.5) * (v0[d.rid(j, k)] + v0[d.rid(j, k - 1)]);
-    py = arc_integral(bz + row, d.nx, i, (v0f * dt) * invdist(d, 0, Cell<T>{{0, j, k}}, 2));
+    py = arc_integral(bz + row, d.nx, i, (v0f * dt) * invdist(d, 0, cell(d, 0, j, k), 2));
   }
   PZ[l] = pz; PY[l] = py;
 }
@@ -473,7 +477,7 @@ __global__ void __launch_bounds__(128) k_mhd_orbital(const Dev<T> d, const T* __
     dd = rdiv(d.dx * (PZ[l + d.pitch] - PZ[l]), d.LY[j]);              // Eq. 104 ...
     dd = dd + rdiv(d.dx * (PY[l + d.plane] - PY[l]), d.dz[k]);          // ... and its Z counterpart
   } else {   // cylindrical: the same circulation with each edge's own arc length (Eq. 105), over the area of the face
-    const Cell<T> q{{i, j, k}}, qj{{i, j + 1, k}}, qk{{i, j, k + 1}};
+    const Cell<T> q = cell(d, i, j, k), qj = cell(d, i, j + 1, k), qk = cell(d, i, j, k + 1);
     dd = (width(d, 0, qj, 1) * PZ[l + d.pitch]) * d.dz[k] - (width(d, 0, q, 1) * PZ[l]) * d.dz[k];
     dd = dd + (width(d, 0, qk, 2) * PY[l + d.plane] - width(d, 0, q, 2) * PY[l]) * d.LY[j];
     dd = rdiv(dd, d.Sx(j, k));

@@ -339,6 +339,9 @@ def run_ours(args):
             upd = e["launches"] / per
             kernels[name]["ncu_dram_bytes_per_cell"] = None if ncu_stale else e["dram_bytes"] / upd / ncell
             kernels[name]["ncu_fp64_pipe_pct"] = None if (ncu_stale or not e["fp64"]) else sum(e["fp64"]) / len(e["fp64"])
+            # thread-level instructions per cell and update, and instructions issued per cycle and SM (of 4)
+            kernels[name]["ncu_inst_per_cell"] = None if (ncu_stale or not e["inst"]) else 32.0 * e["inst"] / upd / ncell
+            kernels[name]["ncu_ipc_per_sm"] = None if (ncu_stale or not e["ipc"]) else sum(e["ipc"]) / len(e["ipc"])
     dom_ncu = kernels[dom].get("ncu_dram_bytes_per_cell")
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kernels[dom]["frac"],
@@ -368,6 +371,9 @@ def run_ours(args):
                      "frac_of_nominal_8TBs_as_built": built_gbs / 8000.0,
                      "ncu_dram_bytes_per_cell_update": ncu_step,
                      "frac_of_nominal_8TBs_ncu_dram": (ncu_step * ncell / (ms / K * 1e-3) / 1e9 / 8000.0) if ncu_step else None,
+                     # the bound the update actually reaches: instructions per cell and update
+                     "ncu_inst_per_cell_update": (sum(k.get("ncu_inst_per_cell") or 0.0 for k in kernels.values()) or None)
+                     if (ncu and not ncu_stale) else None,
                      "ms_per_step_profiled": ms_prof / K}
 
     # ---- region 3: end to end through the public API with pinned host buffers ----

@@ -104,7 +104,8 @@ def ncu_table(workload: str):
         name = launcher_of(kname)
         if name is None:
             continue
-        e = acc.setdefault(name, {"launches": 0, "dram_bytes": 0.0, "ms": 0.0, "fp64": [], "regs": [], "kernels": set()})
+        e = acc.setdefault(name, {"launches": 0, "dram_bytes": 0.0, "ms": 0.0, "fp64": [], "regs": [], "kernels": set(),
+                                  "inst": 0.0, "ipc": []})
         e["launches"] += 1
         e["kernels"].add(kname)
         rd, wr = _val(row, "dram__bytes_read.sum"), _val(row, "dram__bytes_write.sum")
@@ -113,8 +114,11 @@ def ncu_table(workload: str):
         t = _val(row, "gpu__time_duration.sum")
         if t is not None:
             e["ms"] += t
+        ni = _val(row, "smsp__inst_executed.sum")   # warp-level instructions
+        if ni is not None:
+            e["inst"] += ni
         for key, dst in (("sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active", "fp64"),
-                         ("launch__registers_per_thread", "regs")):
+                         ("launch__registers_per_thread", "regs"), ("sm__inst_executed.avg.per_cycle_active", "ipc")):
             x = _val(row, key)
             if x is not None:
                 e[dst].append(x)

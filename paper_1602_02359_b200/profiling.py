@@ -31,6 +31,7 @@ LAUNCHER_OF = [
     (r"k_bc_b", "bc_b"), (r"k_mhd_pressure|k_mhd_curv", "mhd_pressure"), (r"k_mhd_emf", "mhd_emf"), (r"k_mhd_tension", "mhd_tension"),
     (r"k_mhd_ct", "mhd_ct"), (r"k_mhd_resid", "mhd_resid"), (r"k_mhd_arc|k_mhd_orbital", "mhd_orbital"),
     (r"k_source_fused|k_source_tile", "source"), (r"k_visc3d_fused", "source_d"), (r"k_visc3d_(tensor|force)", "source_d"),
+    (r"k_momenta", "momenta"), (r"k_visc_(tensor|force)", "source_d"), (r"k_source_c\b", "source_c"),
     (r"k_source_a\b", "source_a"), (r"k_source_bc\b", "source_bc"), (r"k_source_b\b", "source_b"),
     (r"k_sweep_x", "sweep_x"), (r"k_sweep_ring<\w+, *\(?int\)?1|k_sweep_ring<\w+, *1", "sweep_y"),
     (r"k_sweep_ring<\w+, *\(?int\)?2|k_sweep_ring<\w+, *2", "sweep_z"), (r"k_sweep_last", "sweep_last"),

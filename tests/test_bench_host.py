@@ -116,3 +116,29 @@ def test_ncu_exports_are_keyed_by_the_kernel_source_hash(tmp_path, monkeypatch):
     (tmp_path / ("ncu_raw_other_0123456789.csv")).write_text(head + rows)
     assert P.ncu_table("other")[2] is True
     assert P.ncu_table("absent") == ({}, None, None)
+
+
+def test_every_update_kernel_of_the_build_maps_to_a_launcher():
+    """profiling.launcher_of joins ncu's kernel names with the launcher names of fargo_profile_report: a kernel of the
+    update that maps to nothing would drop out of roofline.traffic silently.  Kernel names come from the tracked SASS
+    digest; the exceptions are kernels that run outside an update (field I/O, halo packing, diagnostics, self-test)."""
+    import glob
+    import re
+    sys.path.insert(0, ROOT)
+    from paper_1602_02359_b200 import profiling as P
+    outside = {"k_copy", "k_gather", "k_scatter", "k_unpad", "k_pad", "k_diagnostics", "k_diag_finish", "k_frame_change",
+               "k_selftest_div", "k_halo_pack", "k_halo_unpack", "k_fill"}
+    digests = glob.glob(os.path.join(ROOT, "profiles", "sass_digest_*.md"))
+    assert digests
+    names = set()
+    for path in digests:
+        for ln in open(path):
+            m = re.match(r"\| (k_\w+)(<[^|]*>)? \|", ln)
+            if m:
+                names.add((m.group(1), (m.group(2) or "").replace("f64", "double").replace("f32", "float")))
+    assert len(names) > 40
+    unmapped = sorted({n for n, targs in names if n not in outside and P.launcher_of(n + targs) is None})
+    assert not unmapped, unmapped
+    assert P.launcher_of("void fg::k_sweep_ring<double, (int)1, (int)7>(fg::Dev<double>)") == "sweep_y"
+    assert P.launcher_of("void fg::k_mhd_emf<double, (int)2, (int)0>(...)") == "mhd_emf"
+    assert P.launcher_of("void fg::k_bc_b<double, (int)1>(...)") == "bc_b" and P.launcher_of("void fg::k_bc<double, (int)1>(...)") == "bc"

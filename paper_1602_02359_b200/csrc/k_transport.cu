@@ -367,8 +367,11 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
 
   const unsigned ring_s = (unsigned)__cvta_generic_to_shared(ring);
   const int nrow = (c1 - c0) + 4;                    // rows c0-2 .. c1+1, numbered n = 0 .. nrow-1
+  // rows are taken in pairs without a test in between (a conditional second step costs ~60 register moves per pair where
+  // the two paths merge): an odd chunk runs one row more, fetched like the others, which stores nothing
+  const int nrow2 = (nrow + 1) & ~1;
   auto fetch = [&](const int n) {                    // row n -> slot n & (RS-1); rows off the array are clamped
-    if (n < nrow) {
+    if (n < nrow2) {
       int r = c0 - 2 + n;
       r = r < 0 ? 0 : (r >= TL ? TL - 1 : r);
       const long long l = base + (long long)r * str;
@@ -393,18 +396,18 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
   // the geometry of the chunk's rows (Tab. 5 factors along the sweep axis), staged once in shared memory behind the ring:
   // a global load per row and table kept an LDG scoreboard busy in every row (ncu: a third of the long-scoreboard
   // stalls sat on the first FMA after it, profiles/r02b_final.md); a broadcast LDS has none of that
-  T* const tab = reinterpret_cast<T*>(smem_raw) + (size_t)RS * NA * MTHREADS;   // [4][nrow]
-  for (int n = threadIdx.x; n < nrow; n += MTHREADS) {
+  T* const tab = reinterpret_cast<T*>(smem_raw) + (size_t)RS * NA * MTHREADS;   // [4][nrow2]
+  for (int n = threadIdx.x; n < nrow2; n += MTHREADS) {
     const int r0 = c0 - 2 + n;
     const int rc = r0 < 0 ? 0 : (r0 >= TL ? TL - 1 : r0);
-    tab[n] = tL[rc]; tab[nrow + n] = tD[rc]; tab[2 * nrow + n] = tS[rc]; tab[3 * nrow + n] = tV[rc];
+    tab[n] = tL[rc]; tab[nrow2 + n] = tD[rc]; tab[2 * nrow2 + n] = tS[rc]; tab[3 * nrow2 + n] = tV[rc];
   }
   __syncthreads();
 
   // one row: f2 (in: q of row r-2; out: q of row r), f1 (q of row r-1)
   auto row_step = [&](const int n, T (&f2)[NQ + 1], T (&f1)[NQ + 1]) {
     const int r = c0 - 2 + n;
-    const T cL = tab[n], cD = tab[nrow + n], cS = tab[2 * nrow + n], cV = tab[3 * nrow + n];
+    const T cL = tab[n], cD = tab[nrow2 + n], cS = tab[2 * nrow2 + n], cV = tab[3 * nrow2 + n];
     fetch(n + RD);
     cp_wait<RD>();                                   // row n has landed
     const T* cur = ring + ((n % RS) * NA) * MTHREADS;
@@ -420,7 +423,7 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
     const bool up = w1 >= T(0);
     const T hup = rfma(-w1, dt, len2) * T(0.5), hdn = rfma(w1, dt, len1) * T(0.5);
     const int m = r - 2;
-    const bool wr = n >= 4 && live;
+    const bool wr = n >= 4 && n < nrow && live;
     const bool upd = m >= 2 && m < TL - 2;
     const long long lo = base + (long long)m * str;
     T Fr;
@@ -444,9 +447,9 @@ __global__ void __launch_bounds__(MTHREADS, FG_MBLOCKS) k_sweep_ring(const Dev<T
     len2 = len1; len1 = len0; invd1 = invd0; w1 = w0; S1 = S0; dtiv2 = dtiv1; dtiv1 = dtiv0;
   };
 #pragma unroll 1
-  for (int n = 0; n < nrow; n += 2) {
+  for (int n = 0; n < nrow2; n += 2) {
     row_step(n, fA, fB);
-    if (n + 1 < nrow) row_step(n + 1, fB, fA);
+    row_step(n + 1, fB, fA);
   }
   cp_wait<0>();
 }
@@ -487,9 +490,9 @@ static int launch_sweep_nq(const Dev<T>& d, const SweepArgs<T>& a, int dir, cuda
   static int slots = 0;   // per instantiation (T, NQ): the two directions have the same resources
   if (!slots) slots = resident_slots(k_sweep_ring<T, 1, NQ>, MTHREADS, ring + 4096);
   int CH = pick_chunk_len(cols, TL, 4, slots, 16);
-  if (CH > 216) CH = 216;                                   // the chunk's geometry tables sit behind the ring: 4 x (CH + 4) reals, <= 7 KB
+  if (CH > 216) CH = 216;                                   // the chunk's geometry tables sit behind the ring: 4 x (CH + 5) reals, <= 7 KB
   const int nch = (TL + CH - 1) / CH;
-  const size_t sm = ring + (size_t)4 * (CH + 4) * sizeof(T);
+  const size_t sm = ring + (size_t)4 * (CH + 5) * sizeof(T);
   dim3 b(MTHREADS), g((d.TX + MTHREADS - 1) / MTHREADS, lines, nch);
   if (dir == 1) k_sweep_ring<T, 1, NQ><<<g, b, sm, s>>>(d, a, CH);
   else k_sweep_ring<T, 2, NQ><<<g, b, sm, s>>>(d, a, CH);
@@ -510,7 +513,7 @@ int launch_sweep(const Dev<T>& d, const SweepArgs<T>& a, int dir, cudaStream_t s
 }
 
 template <typename T, int NQ> static void ring_attr() {
-  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T) + 4 * 220 * (int)sizeof(T);
+  const int sm = ring_slots((NQ + 2) * (int)sizeof(T) / 8) * (NQ + 2) * MTHREADS * (int)sizeof(T) + 4 * 221 * (int)sizeof(T);
   cudaFuncSetAttribute(k_sweep_ring<T, 1, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   cudaFuncSetAttribute(k_sweep_ring<T, 2, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
   // no carve-out request: the driver then picks the smallest shared-memory configuration that holds the resident blocks
